@@ -1,0 +1,193 @@
+/*
+ * maestro_mac.h -- C ABI of the B200-native MAC projection of MAESTROeX (arXiv:1910.12979).
+ *
+ * The library solves, on a uniform 3-D cell-centred grid and entirely on one GPU (fp64),
+ *
+ *        D( (beta0/rho) G phi ) = D( beta0 U_edge ) - beta0 S                         (*)
+ *        U <- U_edge - (1/rho_face) G phi
+ *
+ * so that the corrected face velocities satisfy the low Mach number divergence constraint
+ *        div(beta0 U) = beta0 (S - (1/(Gamma1bar p0)) dp0/dt)      PAPER.md:49  (Sec. 2, Eq. 6)
+ * (the dp0/dt term is folded into S by the caller).  The coefficient beta0/rho is the weighting of
+ * the pressure term (beta0/rho) grad(pi/beta0) of PAPER.md:35 (Sec. 2, Eq. 2); beta0, rho0 are the
+ * one-dimensional base state of PAPER.md:29,39,45 (Eq. 4-5); (*) is solved by geometric multigrid
+ * V-cycles ("multigrid linear solvers for the pressure projection steps", "second order projection
+ * method", Sec. 3).  The paper gives no discretisation; the one used here is stated in
+ * DESIGN.md ("Readings") and SURVEY.md Sec. 8(c): 7-point variable-coefficient operator, arithmetic
+ * face densities, red-black Gauss-Seidel V(nu_pre,nu_post), 8-cell-mean restriction, cell-centred
+ * trilinear prolongation, BiCGStab on the coarsest level, max-norm stopping test.
+ *
+ * LAYOUT (all arrays x-fastest, fp64, DEVICE memory unless stated otherwise)
+ *   cells  rho, S, phi :  idx = i + nx*(j + ny*k)                      nx*ny*nz entries
+ *   u (x-faces i-1/2)  :  idx = i + (nx+1)*(j + ny*k),  i in [0,nx]    (nx+1)*ny*nz
+ *   v (y-faces j-1/2)  :  idx = i + nx*(j + (ny+1)*k),  j in [0,ny]    nx*(ny+1)*nz
+ *   w (z-faces k-1/2)  :  idx = i + nx*(j + ny*k),      k in [0,nz]    nx*ny*(nz+1)
+ *   beta0, rho0        :  nr samples at radius r_m = (m + 1/2) dr; planar geometry: r = z,
+ *                         spherical: r = |x - center|.  Evaluated by linear interpolation, held
+ *                         constant beyond the first and last sample.
+ *   On a periodic axis the face array still has n+1 entries: entry n is ignored on input and
+ *   written equal to entry 0 on output.
+ *
+ * OWNERSHIP  Every device array and the workspace belong to the caller; the library allocates no
+ *   device memory.  The handle (host memory, a few pinned host words, CUDA events) belongs to the
+ *   library until maestro_mac_free().  The base-state profiles are device pointers: they never
+ *   round-trip through the host (the lesson of PAPER.md:111-113).
+ *
+ * ERRORS  Return codes only; the library never prints, throws or exits.
+ */
+#ifndef MAESTRO_MAC_H
+#define MAESTRO_MAC_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct maestro_mac_handle maestro_mac_handle; /* opaque */
+
+enum { MAESTRO_MAC_PERIODIC = 0, MAESTRO_MAC_WALL = 1, MAESTRO_MAC_OUTFLOW = 2 }; /* bc */
+enum { MAESTRO_MAC_PLANAR = 0, MAESTRO_MAC_SPHERICAL = 1 };                        /* geometry */
+enum {
+    MAESTRO_MAC_OK = 0,
+    MAESTRO_MAC_NOT_CONVERGED = 1, /* max_cycles reached; u,v,w,phi hold the last iterate */
+    MAESTRO_MAC_ERR_ARG = -1,      /* null pointer, non-positive size/spacing, periodic on one side
+                                      only, unknown enum, struct_bytes mismatch */
+    MAESTRO_MAC_ERR_UNSUPPORTED = -2, /* hierarchy ends above 4096 bottom unknowns */
+    MAESTRO_MAC_ERR_WORKSPACE = -3,   /* workspace NULL or too small (workspace_needed is written) */
+    MAESTRO_MAC_ERR_CUDA = -4,        /* a CUDA call failed */
+    MAESTRO_MAC_ERR_NONFINITE = -5    /* ||rhs||inf is NaN/Inf, or some rho <= 0 / non-finite */
+};
+
+typedef struct {
+    int struct_bytes;         /* = sizeof(maestro_mac_desc), for versioning */
+    int nx, ny, nz;           /* cells */
+    double dx[3];             /* grid spacing */
+    int bc_lo[3], bc_hi[3];   /* periodic must be set on both sides of an axis */
+    int geometry;             /* planar: r = z.  spherical: r = |x - center| */
+    int nr;                   /* base-state samples */
+    double dr;                /* sample spacing; samples at (m + 1/2) dr */
+    double center[3];         /* spherical only */
+    int nu_pre, nu_post;      /* RBGS sweeps per level, default 2, 2 (0 = default) */
+    int max_cycles;           /* default 100 (0 = default), at most 128 are recorded in stats */
+    double rel_tol;           /* on ||r||inf / ||rhs||inf ; < 0 = default 1e-10 ; 0 = run exactly
+                                 max_cycles cycles without a stop test */
+    int coarsest_n;           /* default 4 (0 = default) */
+    int bottom_max_iter;      /* BiCGStab iterations, default 100 (0 = default) */
+    double bottom_rel_tol;    /* on ||r||2 / ||f||2, default 1e-8 (<= 0 = default) */
+    int prolongation;         /* 0 = cell-centred trilinear (default), 1 = piecewise constant */
+    int host_staging;         /* 1 = reserve device staging in the workspace so that
+                                 maestro_mac_project_host() can be used */
+    int smoother;             /* 0 = default (fused red+black single pass), 1 = reference two-pass
+                                 (one kernel per colour).  Same arithmetic, same results. */
+} maestro_mac_desc;
+
+typedef struct {
+    int cycles, bottom_iters_total, singular, levels;
+    double rhs_norm_inf;      /* after mean removal */
+    double res_norm_inf;      /* ||rhs - L phi||inf after the last cycle */
+    double rhs_mean_removed;  /* singular problems: mean(rhs) that was subtracted, else 0 */
+    double res_history[128];  /* ||r||inf / ||rhs||inf after each cycle */
+    float ms_setup_kernels;   /* coefficients, coarsening, rhs */
+    float ms_vcycles;         /* all cycles including the stop tests */
+    float ms_correct;         /* mean shift, velocity correction, phi copy-out */
+    int gpu_launches;         /* kernels launched by this call */
+} maestro_mac_stats;
+
+/* Fill *desc with defaults for an nx*ny*nz unit-spacing periodic planar problem. */
+void maestro_mac_default_desc(maestro_mac_desc *desc);
+
+/*
+ * maestro_mac_setup: validate the descriptor, build the level hierarchy (level l+1 exists while
+ * every dimension of level l is even and its half is >= coarsest_n), carve `workspace` into the
+ * per-level arrays.  Host-only apart from creating CUDA events; no device->host traffic.
+ *   workspace        device memory owned by the caller, 256-byte aligned, kept alive and untouched
+ *                    by the caller until maestro_mac_free().  May be NULL to query the size.
+ *   workspace_needed always written when non-NULL (also on ERR_WORKSPACE).
+ *   out              receives the handle on success.
+ * Errors: ERR_ARG, ERR_UNSUPPORTED, ERR_WORKSPACE, ERR_CUDA.
+ */
+int maestro_mac_setup(const maestro_mac_desc *desc, void *workspace, size_t workspace_bytes,
+                      size_t *workspace_needed, maestro_mac_handle **out);
+
+/*
+ * maestro_mac_project: the whole hot path on `cuda_stream` (a cudaStream_t, NULL = default stream):
+ *   face coefficients beta0/rho_face -> coarsening to all levels -> rhs = D(beta0 U_edge) - beta0 S
+ *   (minus its mean when no side is OUTFLOW) -> V-cycles from phi = 0 until
+ *   ||rhs - L phi||inf <= rel_tol ||rhs||inf -> (singular: phi -= mean phi) ->
+ *   U -= (1/rho_face) G phi.
+ *   beta0, rho0  device [nr].
+ *   rho          device [nx*ny*nz], or NULL: then rho := rho0 evaluated at cell centres
+ *                (base-state-only projection).  Otherwise rho0 is accepted and unused.
+ *   u, v, w      device, in/out.  WALL faces are left unchanged.
+ *   S            device [nx*ny*nz] or NULL (= 0).
+ *   phi          device [nx*ny*nz], out, or NULL.
+ *   stats        HOST, out, or NULL.
+ * u, v, w, phi, rho, S must not overlap each other or the workspace.  One in-flight call per
+ * handle.  The call synchronises the stream (it reads the stop test after every cycle) unless
+ * rel_tol == 0.  rhs == 0 returns OK with cycles = 0, phi = 0 and the velocities untouched.
+ * Returns OK, NOT_CONVERGED, ERR_ARG, ERR_CUDA or ERR_NONFINITE.
+ */
+int maestro_mac_project(maestro_mac_handle *h, const double *beta0, const double *rho0,
+                        const double *rho, double *u, double *v, double *w, const double *S,
+                        double *phi, maestro_mac_stats *stats, void *cuda_stream);
+
+/*
+ * maestro_mac_project_host: the same call with HOST buffers (pinned memory recommended): copies
+ * the inputs to the staging area reserved by desc.host_staging = 1, projects, copies u, v, w
+ * (and phi when non-NULL) back, and synchronises the stream.  Same layouts and NULL conventions as
+ * above.  Returns ERR_ARG if the handle was set up without host_staging.
+ */
+int maestro_mac_project_host(maestro_mac_handle *h, const double *beta0, const double *rho0,
+                             const double *rho, double *u, double *v, double *w, const double *S,
+                             double *phi, maestro_mac_stats *stats, void *cuda_stream);
+
+/* Release the handle (host memory, pinned words, events).  NULL is a no-op.  Returns OK. */
+int maestro_mac_free(maestro_mac_handle *h);
+
+/* ------------------------------------------------------------------------------------------------
+ * Step API: the individual kernels of the path, for per-kernel parity tests and timing.  They act
+ * on the handle's internal level arrays.  `level` 0 is the finest.  All are asynchronous on
+ * `cuda_stream` unless they return a scalar to the host.
+ * ---------------------------------------------------------------------------------------------- */
+
+enum { MAESTRO_MAC_ARR_PHI = 0, MAESTRO_MAC_ARR_RHS = 1, MAESTRO_MAC_ARR_BX = 2,
+       MAESTRO_MAC_ARR_BY = 3, MAESTRO_MAC_ARR_BZ = 4 };
+
+int maestro_mac_num_levels(const maestro_mac_handle *h);
+/* n[3] cells and h[3] spacing of a level */
+int maestro_mac_level_dims(const maestro_mac_handle *h, int level, int n[3], double hh[3]);
+/* Copy a level array to / from a caller DEVICE buffer in the public layout (cells, or the face
+ * layout of u/v/w for BX/BY/BZ).  Coefficients are returned as b = beta0/rho_face (the internal
+ * pre-scaling by 1/h^2 and the folding of boundary types are undone on WALL/OUTFLOW faces only
+ * as far as recoverable: WALL faces read back as 0). */
+int maestro_mac_level_get(maestro_mac_handle *h, int level, int which, double *dst, void *cuda_stream);
+int maestro_mac_level_set(maestro_mac_handle *h, int level, int which, const double *src, void *cuda_stream);
+
+/* a2 + a3: face coefficients on level 0 and coarsening to every level */
+int maestro_mac_step_coefficients(maestro_mac_handle *h, const double *beta0, const double *rho0,
+                                  const double *rho, void *cuda_stream);
+/* a4: rhs on level 0 (mean removed if singular); host outputs may be NULL; synchronises */
+int maestro_mac_step_rhs(maestro_mac_handle *h, const double *beta0, const double *u,
+                         const double *v, const double *w, const double *S,
+                         double *rhs_norm_inf, double *mean_removed, void *cuda_stream);
+/* a5: nsweeps red-black Gauss-Seidel sweeps on a level */
+int maestro_mac_step_smooth(maestro_mac_handle *h, int level, int nsweeps, void *cuda_stream);
+/* a6: rhs[level+1] = restrict(rhs[level] - L phi[level]);  phi[level+1] = 0 */
+int maestro_mac_step_residual_restrict(maestro_mac_handle *h, int level, void *cuda_stream);
+/* a7: phi[level] += P phi[level+1] */
+int maestro_mac_step_prolong(maestro_mac_handle *h, int level, void *cuda_stream);
+/* a8: BiCGStab on the coarsest level: phi = L^-1 rhs */
+int maestro_mac_step_bottom(maestro_mac_handle *h, void *cuda_stream);
+/* one V-cycle from level 0 */
+int maestro_mac_step_vcycle(maestro_mac_handle *h, void *cuda_stream);
+/* a9: ||rhs - L phi||inf on a level; synchronises */
+int maestro_mac_step_residual_norm(maestro_mac_handle *h, int level, double *norm_inf, void *cuda_stream);
+/* a10: velocity correction from the level-0 phi */
+int maestro_mac_step_correct(maestro_mac_handle *h, const double *rho0, const double *rho,
+                             double *u, double *v, double *w, void *cuda_stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

@@ -1,0 +1,581 @@
+// mac_kernels.cuh -- the pointwise / transfer / bottom kernels of the MAC projection (sm_100a).
+// Hot smoother kernels live in mac_smoother.cuh.  Step names (a2..a11) follow SURVEY.md Sec. 8(a).
+#pragma once
+#include "mac_common.cuh"
+
+// ------------------------------------------------------------------------------------------------
+// a1/a2  face coefficients  a_f = c_f * beta0(face centre) / (0.5 (rho_L + rho_R)) / h^2
+// (Eq. 2: the factor beta0/rho of the pressure term.)  One thread per index of the
+// extended (nx+1, ny+1, nz+1) space writes the low x, y and z face of that index.
+// ------------------------------------------------------------------------------------------------
+
+__device__ __forceinline__ double rho_cell(const GeoDev& G, const double* __restrict__ rho,
+                                           const double* __restrict__ rho0, int i, int j, int k)
+{
+    if (rho) return __ldg(rho + ((size_t)i + (size_t)G.nx * ((size_t)j + (size_t)G.ny * (size_t)k)));
+    return profile_eval(rho0, G.nr, G.dr, radius(G, (i + 0.5) * G.dx, (j + 0.5) * G.dy, (k + 0.5) * G.dz));
+}
+
+// density on face f of axis d through cell (i,j,k)'s row (O2), and the folding weight c_f (O5)
+template <int D>
+__device__ __forceinline__ void face_rho_weight(const GeoDev& G, const double* __restrict__ rho,
+                                                const double* __restrict__ rho0, int i, int j, int k,
+                                                double& rf, double& cf, int& fpos)
+{
+    const int n = D == 0 ? G.nx : (D == 1 ? G.ny : G.nz);
+    const int f = D == 0 ? i : (D == 1 ? j : k);
+    const bool per = G.bclo[D] == MAC_PERIODIC;
+    int lo, hi;
+    cf = 1.0;
+    fpos = f;
+    if (f == 0 || f == n) {
+        if (per) {
+            lo = n - 1; hi = 0; fpos = 0;              // face n is face 0 (reading A18)
+        } else if (f == 0) {
+            lo = hi = 0; cf = G.bclo[D] == MAC_WALL ? 0.0 : 2.0;
+        } else {
+            lo = hi = n - 1; cf = G.bchi[D] == MAC_WALL ? 0.0 : 2.0;
+        }
+    } else {
+        lo = f - 1; hi = f;
+    }
+    double rl = rho_cell(G, rho, rho0, D == 0 ? lo : i, D == 1 ? lo : j, D == 2 ? lo : k);
+    double rr = rho_cell(G, rho, rho0, D == 0 ? hi : i, D == 1 ? hi : j, D == 2 ? hi : k);
+    rf = 0.5 * (rl + rr);
+}
+
+__global__ void __launch_bounds__(256)
+k_face_coeff(GeoDev G, LevelDev L, const double* __restrict__ beta0, const double* __restrict__ rho,
+             const double* __restrict__ rho0, int* __restrict__ flags)
+{
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    int j = blockIdx.y * blockDim.y + threadIdx.y;
+    int k = blockIdx.z;
+    if (i > G.nx || j > G.ny) return;
+    const bool ci = i < G.nx, cj = j < G.ny, ck = k < G.nz;
+    if (ci && cj && ck) {
+        double r = rho_cell(G, rho, rho0, i, j, k);
+        if (!(r > 0.0) || !(r <= 1.79769313486231570e308)) atomicOr(flags, 1);
+    }
+    double rf, cf;
+    int fp;
+    if (cj && ck) {
+        face_rho_weight<0>(G, rho, rho0, i, j, k, rf, cf, fp);
+        double b = profile_eval(beta0, G.nr, G.dr, radius(G, fp * G.dx, (j + 0.5) * G.dy, (k + 0.5) * G.dz));
+        L.ax[axidx(L, i, j, k)] = cf * (b / rf) / (G.dx * G.dx);
+    }
+    if (ci && ck) {
+        face_rho_weight<1>(G, rho, rho0, i, j, k, rf, cf, fp);
+        double b = profile_eval(beta0, G.nr, G.dr, radius(G, (i + 0.5) * G.dx, fp * G.dy, (k + 0.5) * G.dz));
+        L.ay[ayidx(L, i, j, k)] = cf * (b / rf) / (G.dy * G.dy);
+    }
+    if (ci && cj) {
+        face_rho_weight<2>(G, rho, rho0, i, j, k, rf, cf, fp);
+        double b = profile_eval(beta0, G.nr, G.dr, radius(G, (i + 0.5) * G.dx, (j + 0.5) * G.dy, fp * G.dz));
+        L.az[azidx(L, i, j, k)] = cf * (b / rf) / (G.dz * G.dz);
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// a3  coefficient coarsening: coarse face = mean of the 4 fine faces that tile it (reading A11);
+// with the 1/h^2 pre-scaling that is  a_c = (1/16) * sum of the 4 fine a_f.
+// ------------------------------------------------------------------------------------------------
+
+__global__ void __launch_bounds__(256)
+k_coarsen_coeff(LevelDev F, LevelDev C)
+{
+    int I = blockIdx.x * blockDim.x + threadIdx.x;
+    int J = blockIdx.y * blockDim.y + threadIdx.y;
+    int K = blockIdx.z;
+    if (I > C.nx || J > C.ny) return;
+    const bool ci = I < C.nx, cj = J < C.ny, ck = K < C.nz;
+    if (cj && ck) {
+        double s = F.ax[axidx(F, 2 * I, 2 * J, 2 * K)] + F.ax[axidx(F, 2 * I, 2 * J + 1, 2 * K)] +
+                   F.ax[axidx(F, 2 * I, 2 * J, 2 * K + 1)] + F.ax[axidx(F, 2 * I, 2 * J + 1, 2 * K + 1)];
+        C.ax[axidx(C, I, J, K)] = 0.0625 * s;
+    }
+    if (ci && ck) {
+        double s = F.ay[ayidx(F, 2 * I, 2 * J, 2 * K)] + F.ay[ayidx(F, 2 * I + 1, 2 * J, 2 * K)] +
+                   F.ay[ayidx(F, 2 * I, 2 * J, 2 * K + 1)] + F.ay[ayidx(F, 2 * I + 1, 2 * J, 2 * K + 1)];
+        C.ay[ayidx(C, I, J, K)] = 0.0625 * s;
+    }
+    if (ci && cj) {
+        double s = F.az[azidx(F, 2 * I, 2 * J, 2 * K)] + F.az[azidx(F, 2 * I + 1, 2 * J, 2 * K)] +
+                   F.az[azidx(F, 2 * I, 2 * J + 1, 2 * K)] + F.az[azidx(F, 2 * I + 1, 2 * J + 1, 2 * K)];
+        C.az[azidx(C, I, J, K)] = 0.0625 * s;
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// block-level deterministic reductions: every block writes one partial (sum, nanmax) pair; a
+// single-block kernel folds the partials in a fixed order.
+// ------------------------------------------------------------------------------------------------
+
+__device__ __forceinline__ void block_reduce_store(double s, double m, double* __restrict__ part_sum,
+                                                   double* __restrict__ part_max, int slot)
+{
+    __shared__ double sh_s[32], sh_m[32];
+    const int tid = threadIdx.x + blockDim.x * threadIdx.y;
+    const int nthr = blockDim.x * blockDim.y;
+    s = warp_sum(s);
+    m = warp_nanmax(m);
+    if ((tid & 31) == 0) { sh_s[tid >> 5] = s; sh_m[tid >> 5] = m; }
+    __syncthreads();
+    if (tid < 32) {
+        int nw = (nthr + 31) >> 5;
+        s = tid < nw ? sh_s[tid] : 0.0;
+        m = tid < nw ? sh_m[tid] : 0.0;
+        s = warp_sum(s);
+        m = warp_nanmax(m);
+        if (tid == 0) { part_sum[slot] = s; part_max[slot] = m; }
+    }
+}
+
+// out[0] = sum of part_sum, out[1] = nanmax of part_max
+__global__ void __launch_bounds__(1024)
+k_reduce_final(const double* __restrict__ part_sum, const double* __restrict__ part_max, int n,
+               double* __restrict__ out)
+{
+    double s = 0.0, m = 0.0;
+    for (int q = threadIdx.x; q < n; q += blockDim.x) { s += part_sum[q]; m = nanmax(m, part_max[q]); }
+    __shared__ double sh_s[32], sh_m[32];
+    s = warp_sum(s);
+    m = warp_nanmax(m);
+    if ((threadIdx.x & 31) == 0) { sh_s[threadIdx.x >> 5] = s; sh_m[threadIdx.x >> 5] = m; }
+    __syncthreads();
+    if (threadIdx.x < 32) {
+        s = sh_s[threadIdx.x];
+        m = sh_m[threadIdx.x];
+        s = warp_sum(s);
+        m = warp_nanmax(m);
+        if (threadIdx.x == 0) { out[0] = s; out[1] = m; }
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// a4  rhs = D(beta0_face U_edge) - beta0_cell S    (Eq. 6), partial sum and max|rhs|.
+// Blocks walk rows (j,k) grid-stride; threads walk i.
+// ------------------------------------------------------------------------------------------------
+
+__device__ __forceinline__ double beta_at(const GeoDev& G, const double* __restrict__ beta0,
+                                          double x, double y, double z)
+{
+    return profile_eval(beta0, G.nr, G.dr, radius(G, x, y, z));
+}
+
+__global__ void __launch_bounds__(256)
+k_rhs(GeoDev G, const double* __restrict__ beta0, const double* __restrict__ u,
+      const double* __restrict__ v, const double* __restrict__ w, const double* __restrict__ S,
+      double* __restrict__ rhs, double* __restrict__ part_sum, double* __restrict__ part_max)
+{
+    const int nrows = G.ny * G.nz;
+    const bool px = G.bclo[0] == MAC_PERIODIC, py = G.bclo[1] == MAC_PERIODIC, pz = G.bclo[2] == MAC_PERIODIC;
+    double s = 0.0, m = 0.0;
+    for (int row = blockIdx.x; row < nrows; row += gridDim.x) {
+        const int j = row % G.ny, k = row / G.ny;
+        const double yc = (j + 0.5) * G.dy, zc = (k + 0.5) * G.dz;
+        const int jh = (py && j + 1 == G.ny) ? 0 : j + 1;     // periodic: face n reads entry 0
+        const int kh = (pz && k + 1 == G.nz) ? 0 : k + 1;
+        for (int i = threadIdx.x; i < G.nx; i += blockDim.x) {
+            const double xc = (i + 0.5) * G.dx;
+            const int ih = (px && i + 1 == G.nx) ? 0 : i + 1;
+            const size_t ub = (size_t)(G.nx + 1) * ((size_t)j + (size_t)G.ny * k);
+            double fxl = beta_at(G, beta0, i * G.dx, yc, zc) * u[ub + i];
+            double fxh = beta_at(G, beta0, ih * G.dx, yc, zc) * u[ub + ih];
+            double fyl = beta_at(G, beta0, xc, j * G.dy, zc) * v[(size_t)i + (size_t)G.nx * ((size_t)j + (size_t)(G.ny + 1) * k)];
+            double fyh = beta_at(G, beta0, xc, jh * G.dy, zc) * v[(size_t)i + (size_t)G.nx * ((size_t)jh + (size_t)(G.ny + 1) * k)];
+            double fzl = beta_at(G, beta0, xc, yc, k * G.dz) * w[(size_t)i + (size_t)G.nx * ((size_t)j + (size_t)G.ny * k)];
+            double fzh = beta_at(G, beta0, xc, yc, kh * G.dz) * w[(size_t)i + (size_t)G.nx * ((size_t)j + (size_t)G.ny * kh)];
+            double r = (fxh - fxl) / G.dx + (fyh - fyl) / G.dy + (fzh - fzl) / G.dz;
+            const size_t c = (size_t)i + (size_t)G.nx * ((size_t)j + (size_t)G.ny * k);
+            if (S) r -= beta_at(G, beta0, xc, yc, zc) * S[c];
+            rhs[c] = r;
+            s += r;
+            m = nanmax(m, fabs(r));
+        }
+    }
+    block_reduce_store(s, m, part_sum, part_max, blockIdx.x);
+}
+
+// a -= scal[0]/count  (mean removal), with partial sum / max of the shifted values
+__global__ void __launch_bounds__(256)
+k_shift_mean(double* __restrict__ a, size_t n, const double* __restrict__ scal, double inv_count,
+             double* __restrict__ part_sum, double* __restrict__ part_max)
+{
+    const double c = scal[0] * inv_count;
+    double s = 0.0, m = 0.0;
+    for (size_t q = (size_t)blockIdx.x * blockDim.x + threadIdx.x; q < n; q += (size_t)gridDim.x * blockDim.x) {
+        double v = a[q] - c;
+        a[q] = v;
+        s += v;
+        m = nanmax(m, fabs(v));
+    }
+    block_reduce_store(s, m, part_sum, part_max, blockIdx.x);
+}
+
+__global__ void __launch_bounds__(256)
+k_sum(const double* __restrict__ a, size_t n, double* __restrict__ part_sum, double* __restrict__ part_max)
+{
+    double s = 0.0, m = 0.0;
+    for (size_t q = (size_t)blockIdx.x * blockDim.x + threadIdx.x; q < n; q += (size_t)gridDim.x * blockDim.x) {
+        double v = a[q];
+        s += v;
+        m = nanmax(m, fabs(v));
+    }
+    block_reduce_store(s, m, part_sum, part_max, blockIdx.x);
+}
+
+// ------------------------------------------------------------------------------------------------
+// operator pieces shared by the reference smoother, residual and bottom solver
+// ------------------------------------------------------------------------------------------------
+
+// phi at a neighbour index that may be one outside along axis D: wrapped if periodic, else 0
+template <int D>
+__device__ __forceinline__ double nb_val(const LevelDev& L, const double* __restrict__ p, int i, int j, int k)
+{
+    const int n = D == 0 ? L.nx : (D == 1 ? L.ny : L.nz);
+    int f = D == 0 ? i : (D == 1 ? j : k);
+    if (f < 0) {
+        if (L.bclo[D] != MAC_PERIODIC) return 0.0;
+        f += n;
+    } else if (f >= n) {
+        if (L.bchi[D] != MAC_PERIODIC) return 0.0;
+        f -= n;
+    }
+    return p[cidx(L, D == 0 ? f : i, D == 1 ? f : j, D == 2 ? f : k)];
+}
+
+// off = sum_f a_f phi_nb, dg = sum_f a_f
+__device__ __forceinline__ void stencil_sums(const LevelDev& L, const double* __restrict__ p, int i, int j,
+                                             int k, double& off, double& dg)
+{
+    const double axl = L.ax[axidx(L, i, j, k)], axh = L.ax[axidx(L, i + 1, j, k)];
+    const double ayl = L.ay[ayidx(L, i, j, k)], ayh = L.ay[ayidx(L, i, j + 1, k)];
+    const double azl = L.az[azidx(L, i, j, k)], azh = L.az[azidx(L, i, j, k + 1)];
+    off = axl * nb_val<0>(L, p, i - 1, j, k) + axh * nb_val<0>(L, p, i + 1, j, k) +
+          ayl * nb_val<1>(L, p, i, j - 1, k) + ayh * nb_val<1>(L, p, i, j + 1, k) +
+          azl * nb_val<2>(L, p, i, j, k - 1) + azh * nb_val<2>(L, p, i, j, k + 1);
+    dg = ((axl + axh) + (ayl + ayh)) + (azl + azh);
+}
+
+// ------------------------------------------------------------------------------------------------
+// a5 (reference form)  one colour of red-black Gauss-Seidel, in place:
+//   phi_0 <- phi_0 + (rhs_0 - (L phi)_0)/L_diag  ==  (sum_f a_f phi_nb - rhs_0) / sum_f a_f
+// One thread per cell pair along x; the pair holds exactly one cell of each colour.
+// ------------------------------------------------------------------------------------------------
+
+__global__ void __launch_bounds__(256)
+k_rbgs_color(LevelDev L, int color)
+{
+    const int p = blockIdx.x * blockDim.x + threadIdx.x;
+    const int j = blockIdx.y * blockDim.y + threadIdx.y;
+    const int k = blockIdx.z;
+    if (j >= L.ny) return;
+    const int i = 2 * p + ((j + k + color) & 1);
+    if (i >= L.nx) return;
+    double off, dg;
+    stencil_sums(L, L.phi, i, j, k, off, dg);
+    const size_t c = cidx(L, i, j, k);
+    L.phi[c] = (off - L.rhs[c]) / dg;
+}
+
+// ------------------------------------------------------------------------------------------------
+// a6 (reference form)  coarse rhs = mean over the 8 children of (rhs - L phi); coarse phi = 0
+// ------------------------------------------------------------------------------------------------
+
+__global__ void __launch_bounds__(256)
+k_residual_restrict(LevelDev F, LevelDev C)
+{
+    const int I = blockIdx.x * blockDim.x + threadIdx.x;
+    const int J = blockIdx.y * blockDim.y + threadIdx.y;
+    const int K = blockIdx.z;
+    if (I >= C.nx || J >= C.ny) return;
+    double s = 0.0;
+#pragma unroll
+    for (int dk = 0; dk < 2; ++dk)
+#pragma unroll
+        for (int dj = 0; dj < 2; ++dj)
+#pragma unroll
+            for (int di = 0; di < 2; ++di) {
+                const int i = 2 * I + di, j = 2 * J + dj, k = 2 * K + dk;
+                double off, dg;
+                stencil_sums(F, F.phi, i, j, k, off, dg);
+                const size_t c = cidx(F, i, j, k);
+                s += F.rhs[c] - (off - F.phi[c] * dg);
+            }
+    const size_t cc = cidx(C, I, J, K);
+    C.rhs[cc] = 0.125 * s;
+    C.phi[cc] = 0.0;
+}
+
+// ------------------------------------------------------------------------------------------------
+// a7  phi_f += P e_c : cell-centred trilinear (3/4 parent, 1/4 neighbour on the child's side per
+// axis); coarse neighbours outside the grid follow the ghost rule (periodic wrap, WALL +e_0,
+// OUTFLOW -e_0).  prolongation == 1: piecewise constant.
+// ------------------------------------------------------------------------------------------------
+
+__device__ __forceinline__ int ghost_index(int f, int n, int lo, int hi, double& sign)
+{
+    if (f < 0) {
+        if (lo == MAC_PERIODIC) return f + n;
+        if (lo == MAC_OUTFLOW) sign = -sign;
+        return -1 - f;
+    }
+    if (f >= n) {
+        if (hi == MAC_PERIODIC) return f - n;
+        if (hi == MAC_OUTFLOW) sign = -sign;
+        return 2 * n - 1 - f;
+    }
+    return f;
+}
+
+__global__ void __launch_bounds__(256)
+k_prolong_add(LevelDev F, LevelDev C, int prolongation)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    const int j = blockIdx.y * blockDim.y + threadIdx.y;
+    const int k = blockIdx.z;
+    if (i >= F.nx || j >= F.ny) return;
+    const int I = i >> 1, J = j >> 1, K = k >> 1;
+    double val;
+    if (prolongation == 1) {
+        val = C.phi[cidx(C, I, J, K)];
+    } else {
+        double sx = 1.0, sy = 1.0, sz = 1.0;
+        const int I2 = ghost_index(I + ((i & 1) ? 1 : -1), C.nx, C.bclo[0], C.bchi[0], sx);
+        const int J2 = ghost_index(J + ((j & 1) ? 1 : -1), C.ny, C.bclo[1], C.bchi[1], sy);
+        const int K2 = ghost_index(K + ((k & 1) ? 1 : -1), C.nz, C.bclo[2], C.bchi[2], sz);
+        const double* __restrict__ e = C.phi;
+        const double wx0 = 0.75, wx1 = 0.25 * sx, wy0 = 0.75, wy1 = 0.25 * sy, wz0 = 0.75, wz1 = 0.25 * sz;
+        val = wz0 * (wy0 * (wx0 * e[cidx(C, I, J, K)] + wx1 * e[cidx(C, I2, J, K)]) +
+                     wy1 * (wx0 * e[cidx(C, I, J2, K)] + wx1 * e[cidx(C, I2, J2, K)])) +
+              wz1 * (wy0 * (wx0 * e[cidx(C, I, J, K2)] + wx1 * e[cidx(C, I2, J, K2)]) +
+                     wy1 * (wx0 * e[cidx(C, I, J2, K2)] + wx1 * e[cidx(C, I2, J2, K2)]));
+    }
+    F.phi[cidx(F, i, j, k)] += val;
+}
+
+// ------------------------------------------------------------------------------------------------
+// a9  ||rhs - L phi||inf  (block partial maxima; folded by k_reduce_final)
+// ------------------------------------------------------------------------------------------------
+
+__global__ void __launch_bounds__(256)
+k_residual_norm(LevelDev L, double* __restrict__ part_sum, double* __restrict__ part_max)
+{
+    const int nrows = L.ny * L.nz;
+    double m = 0.0;
+    for (int row = blockIdx.x; row < nrows; row += gridDim.x) {
+        const int j = row % L.ny, k = row / L.ny;
+        for (int i = threadIdx.x; i < L.nx; i += blockDim.x) {
+            double off, dg;
+            stencil_sums(L, L.phi, i, j, k, off, dg);
+            const size_t c = cidx(L, i, j, k);
+            m = nanmax(m, fabs(L.rhs[c] - (off - L.phi[c] * dg)));
+        }
+    }
+    block_reduce_store(0.0, m, part_sum, part_max, blockIdx.x);
+}
+
+// out = rhs - L phi on a level (used by level_get-style diagnostics / tests)
+__global__ void __launch_bounds__(256)
+k_residual(LevelDev L, double* __restrict__ out)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    const int j = blockIdx.y * blockDim.y + threadIdx.y;
+    const int k = blockIdx.z;
+    if (i >= L.nx || j >= L.ny) return;
+    double off, dg;
+    stencil_sums(L, L.phi, i, j, k, off, dg);
+    const size_t c = cidx(L, i, j, k);
+    out[c] = L.rhs[c] - (off - L.phi[c] * dg);
+}
+
+// ------------------------------------------------------------------------------------------------
+// a8  bottom solve: unpreconditioned BiCGStab, x0 = 0, rhat = r0, one thread block; dot products
+// by warp shuffles + one shared-memory stage (deterministic).  Stops at ||r||2 <= tol ||f||2,
+// maxit iterations, or breakdown (the current iterate is kept) -- reading A15.
+// Singular problems: f is projected to zero mean first and x to zero mean last.
+// Vectors r, rhat, p, v, s, t live in `vecs` (6 * nb doubles, cache resident).
+// ------------------------------------------------------------------------------------------------
+
+struct Dot2 { double a, b; };
+
+__device__ __forceinline__ Dot2 block_dot2(double a, double b, double* sh)
+{
+    a = warp_sum(a);
+    b = warp_sum(b);
+    const int w = threadIdx.x >> 5, l = threadIdx.x & 31, nw = (blockDim.x + 31) >> 5;
+    __syncthreads();                      // protect sh from the previous use
+    if (l == 0) { sh[2 * w] = a; sh[2 * w + 1] = b; }
+    __syncthreads();
+    a = l < nw ? sh[2 * l] : 0.0;
+    b = l < nw ? sh[2 * l + 1] : 0.0;
+    Dot2 r;
+    r.a = warp_sum(a);
+    r.b = warp_sum(b);
+    return r;
+}
+
+__device__ __forceinline__ double bottom_matvec_at(const LevelDev& L, const double* __restrict__ x, int c)
+{
+    const int i = c % L.nx, j = (c / L.nx) % L.ny, k = c / (L.nx * L.ny);
+    double off, dg;
+    stencil_sums(L, x, i, j, k, off, dg);
+    return off - x[c] * dg;
+}
+
+__global__ void __launch_bounds__(1024)
+k_bottom_bicgstab(LevelDev L, double* __restrict__ vecs, int maxit, double tol, int singular,
+                  int* __restrict__ iters_accum)
+{
+    __shared__ double sh[64];
+    const int nb = L.nx * L.ny * L.nz;
+    double* __restrict__ x = L.phi;
+    const double* __restrict__ f = L.rhs;
+    double* r = vecs;
+    double* rhat = vecs + nb;
+    double* p = vecs + 2 * (size_t)nb;
+    double* v = vecs + 3 * (size_t)nb;
+    double* s = vecs + 4 * (size_t)nb;
+    double* t = vecs + 5 * (size_t)nb;
+    const int tid = threadIdx.x, nt = blockDim.x;
+
+    double fm = 0.0;
+    if (singular) {
+        double a = 0.0;
+        for (int c = tid; c < nb; c += nt) a += f[c];
+        fm = block_dot2(a, 0.0, sh).a / (double)nb;
+    }
+    double rr = 0.0;
+    for (int c = tid; c < nb; c += nt) {
+        double fv = f[c] - fm;
+        r[c] = fv; rhat[c] = fv; p[c] = 0.0; v[c] = 0.0; x[c] = 0.0;
+        rr += fv * fv;
+    }
+    rr = block_dot2(rr, 0.0, sh).a;            // (r,r) = (rhat,r)
+    const double bnorm2 = rr;
+    int it = 0;
+    if (bnorm2 > 0.0 && bnorm2 == bnorm2) {
+        const double stop2 = tol * tol * bnorm2;
+        double rho = rr, rho_old = 1.0, alpha = 1.0, omega = 1.0;
+        while (it < maxit && rr > stop2) {
+            if (rho == 0.0) break;                                   // breakdown
+            const double beta = it == 0 ? 0.0 : (rho / rho_old) * (alpha / omega);
+            for (int c = tid; c < nb; c += nt) p[c] = r[c] + beta * (p[c] - omega * v[c]);
+            __syncthreads();
+            double d = 0.0;
+            for (int c = tid; c < nb; c += nt) { double y = bottom_matvec_at(L, p, c); v[c] = y; d += rhat[c] * y; }
+            d = block_dot2(d, 0.0, sh).a;
+            if (d == 0.0) break;
+            alpha = rho / d;
+            double ss = 0.0;
+            for (int c = tid; c < nb; c += nt) { double y = r[c] - alpha * v[c]; s[c] = y; ss += y * y; }
+            ss = block_dot2(ss, 0.0, sh).a;                          // also makes s visible
+            ++it;
+            if (ss <= stop2) {
+                for (int c = tid; c < nb; c += nt) x[c] += alpha * p[c];
+                rr = ss;
+                break;
+            }
+            double ts = 0.0, tt = 0.0;
+            for (int c = tid; c < nb; c += nt) { double y = bottom_matvec_at(L, s, c); t[c] = y; ts += y * s[c]; tt += y * y; }
+            Dot2 q = block_dot2(ts, tt, sh);
+            if (q.b == 0.0) {
+                for (int c = tid; c < nb; c += nt) x[c] += alpha * p[c];
+                break;
+            }
+            omega = q.a / q.b;
+            double r2 = 0.0, hr = 0.0;
+            for (int c = tid; c < nb; c += nt) {
+                x[c] += alpha * p[c] + omega * s[c];
+                double y = s[c] - omega * t[c];
+                r[c] = y;
+                r2 += y * y;
+                hr += rhat[c] * y;
+            }
+            q = block_dot2(r2, hr, sh);
+            rr = q.a;
+            rho_old = rho;
+            rho = q.b;
+            if (omega == 0.0) break;
+        }
+    }
+    if (singular) {
+        __syncthreads();
+        double a = 0.0;
+        for (int c = tid; c < nb; c += nt) a += x[c];
+        const double xm = block_dot2(a, 0.0, sh).a / (double)nb;
+        for (int c = tid; c < nb; c += nt) x[c] -= xm;
+    }
+    if (tid == 0 && iters_accum) *iters_accum += it;
+}
+
+// ------------------------------------------------------------------------------------------------
+// a10  U <- U_edge - (1/rho_face) G phi  (Eq. 2).  WALL faces unchanged; OUTFLOW faces
+// use the ghost -phi_0; periodic: entry n written equal to entry 0.
+// ------------------------------------------------------------------------------------------------
+
+template <int D>
+__device__ __forceinline__ void correct_face(const GeoDev& G, const double* __restrict__ phi,
+                                             const double* __restrict__ rho, const double* __restrict__ rho0,
+                                             double* __restrict__ vel, int i, int j, int k)
+{
+    const int n = D == 0 ? G.nx : (D == 1 ? G.ny : G.nz);
+    const double h = D == 0 ? G.dx : (D == 1 ? G.dy : G.dz);
+    const int f = D == 0 ? i : (D == 1 ? j : k);
+    const bool per = G.bclo[D] == MAC_PERIODIC;
+    const size_t sx = G.nx + (D == 0), sy = G.ny + (D == 1);
+    const size_t fi = (size_t)i + sx * ((size_t)j + sy * (size_t)k);
+    if (f == n && per) return;                       // written by the thread of face 0
+    int lo = f - 1, hi = f;
+    double glo = 1.0, ghi = 1.0;                     // multipliers of phi[lo], phi[hi]
+    if (f == 0) {
+        if (per) lo = n - 1;
+        else { if (G.bclo[D] == MAC_WALL) return; lo = 0; glo = -1.0; }     // ghost = -phi_0
+    } else if (f == n) {
+        if (G.bchi[D] == MAC_WALL) return;
+        hi = n - 1; ghi = -1.0;
+    }
+    auto cell = [&](int q) -> size_t {
+        return (size_t)(D == 0 ? q : i) + (size_t)G.nx * ((size_t)(D == 1 ? q : j) + (size_t)G.ny * (size_t)(D == 2 ? q : k));
+    };
+    const double grad = (ghi * phi[cell(hi)] - glo * phi[cell(lo)]) / h;
+    const double rf = 0.5 * (rho_cell(G, rho, rho0, D == 0 ? lo : i, D == 1 ? lo : j, D == 2 ? lo : k) +
+                             rho_cell(G, rho, rho0, D == 0 ? hi : i, D == 1 ? hi : j, D == 2 ? hi : k));
+    const double nv = vel[fi] - grad / rf;
+    vel[fi] = nv;
+    if (f == 0 && per) {
+        const size_t fn = (size_t)(D == 0 ? n : i) + sx * ((size_t)(D == 1 ? n : j) + sy * (size_t)(D == 2 ? n : k));
+        vel[fn] = nv;
+    }
+}
+
+__global__ void __launch_bounds__(256)
+k_correct(GeoDev G, const double* __restrict__ phi, const double* __restrict__ rho,
+          const double* __restrict__ rho0, double* __restrict__ u, double* __restrict__ v,
+          double* __restrict__ w)
+{
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    int j = blockIdx.y * blockDim.y + threadIdx.y;
+    int k = blockIdx.z;
+    if (i > G.nx || j > G.ny) return;
+    const bool ci = i < G.nx, cj = j < G.ny, ck = k < G.nz;
+    if (cj && ck) correct_face<0>(G, phi, rho, rho0, u, i, j, k);
+    if (ci && ck) correct_face<1>(G, phi, rho, rho0, v, i, j, k);
+    if (ci && cj) correct_face<2>(G, phi, rho, rho0, w, i, j, k);
+}
+
+// ------------------------------------------------------------------------------------------------
+// layout conversion for the step API: public face layout <-> internal (pitched) ax
+// ------------------------------------------------------------------------------------------------
+
+__global__ void k_copy_ax(LevelDev L, double* pub, int to_public)
+{
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    int j = blockIdx.y * blockDim.y + threadIdx.y;
+    int k = blockIdx.z;
+    if (i > L.nx || j >= L.ny) return;
+    size_t a = axidx(L, i, j, k), b = (size_t)i + (size_t)(L.nx + 1) * ((size_t)j + (size_t)L.ny * k);
+    if (to_public) pub[b] = L.ax[a];
+    else L.ax[a] = pub[b];
+}

@@ -1,0 +1,641 @@
+// maestro_mac.cu -- host side of the C ABI declared in include/maestro_mac.h.
+// Validates descriptors, builds the level hierarchy, carves the caller's workspace, and drives the
+// kernels of mac_kernels.cuh / mac_smoother.cuh on the caller's stream.  No device allocation here.
+#include "maestro_mac.h"
+
+#include <cuda_runtime.h>
+
+#include <cmath>
+#include <cstdlib>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "mac_kernels.cuh"
+#include "mac_smoother.cuh"
+
+namespace {
+
+constexpr int kMaxLevels = 32;
+constexpr int kRedBlocks = 148 * 8;       // blocks of the row-walking reduction kernels
+constexpr int kBottomMax = 4096;          // largest coarsest level (unknowns)
+
+struct Level {
+    int n[3];
+    double h[3];
+    int px;
+    size_t ncell, nax, nay, naz;
+    double *phi, *phi2, *rhs, *ax, *ay, *az;
+};
+
+struct Staging {
+    double *beta0, *rho0, *rho, *u, *v, *w, *S, *phi;
+};
+
+}  // namespace
+
+struct maestro_mac_handle {
+    maestro_mac_desc d;
+    int nlev;
+    Level lev[kMaxLevels];
+    int singular;
+    // scratch carved from the workspace
+    double *part_sum, *part_max;   // kRedBlocks each
+    double *scal;                  // device scalars: [0] sum, [1] max (k_reduce_final output) ...
+    double *bottom_vecs;           // 6 * bottom unknowns
+    int *flags;                    // [0] bad rho, [1] bottom iterations
+    Staging st;
+    bool has_staging;
+    // host side
+    double *host_scal;             // pinned, 8 doubles
+    int *host_flags;               // pinned, 4 ints
+    cudaEvent_t ev[4];
+    int launches;
+};
+
+namespace {
+
+inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
+
+bool valid_bc(int b) { return b == MAESTRO_MAC_PERIODIC || b == MAESTRO_MAC_WALL || b == MAESTRO_MAC_OUTFLOW; }
+
+int validate_and_default(const maestro_mac_desc* in, maestro_mac_desc* d)
+{
+    if (!in || in->struct_bytes != (int)sizeof(maestro_mac_desc)) return MAESTRO_MAC_ERR_ARG;
+    *d = *in;
+    if (d->nx <= 0 || d->ny <= 0 || d->nz <= 0) return MAESTRO_MAC_ERR_ARG;
+    if (d->nx > 65535 || d->ny > 65535 || d->nz > 65535) return MAESTRO_MAC_ERR_UNSUPPORTED;
+    for (int a = 0; a < 3; ++a) {
+        if (!(d->dx[a] > 0.0) || !std::isfinite(d->dx[a])) return MAESTRO_MAC_ERR_ARG;
+        if (!valid_bc(d->bc_lo[a]) || !valid_bc(d->bc_hi[a])) return MAESTRO_MAC_ERR_ARG;
+        if ((d->bc_lo[a] == MAESTRO_MAC_PERIODIC) != (d->bc_hi[a] == MAESTRO_MAC_PERIODIC)) return MAESTRO_MAC_ERR_ARG;
+    }
+    if (d->geometry != MAESTRO_MAC_PLANAR && d->geometry != MAESTRO_MAC_SPHERICAL) return MAESTRO_MAC_ERR_ARG;
+    if (d->nr <= 0 || !(d->dr > 0.0) || !std::isfinite(d->dr)) return MAESTRO_MAC_ERR_ARG;
+    if (d->nu_pre < 0 || d->nu_post < 0 || d->max_cycles < 0 || d->coarsest_n < 0 || d->bottom_max_iter < 0)
+        return MAESTRO_MAC_ERR_ARG;
+    if (d->nu_pre == 0 && d->nu_post == 0) { d->nu_pre = 2; d->nu_post = 2; }
+    if (d->max_cycles == 0) d->max_cycles = 100;
+    if (d->rel_tol < 0.0) d->rel_tol = 1e-10;
+    if (!std::isfinite(d->rel_tol)) return MAESTRO_MAC_ERR_ARG;
+    if (d->coarsest_n == 0) d->coarsest_n = 4;
+    if (d->bottom_max_iter == 0) d->bottom_max_iter = 100;
+    if (!(d->bottom_rel_tol > 0.0)) d->bottom_rel_tol = 1e-8;
+    if (d->prolongation != 0 && d->prolongation != 1) return MAESTRO_MAC_ERR_ARG;
+    if (d->host_staging != 0 && d->host_staging != 1) return MAESTRO_MAC_ERR_ARG;
+    if (d->smoother != 0 && d->smoother != 1) return MAESTRO_MAC_ERR_ARG;
+    return MAESTRO_MAC_OK;
+}
+
+// Build level geometry; returns OK or UNSUPPORTED.
+int build_levels(const maestro_mac_desc& d, Level* lev, int* nlev)
+{
+    int n[3] = {d.nx, d.ny, d.nz};
+    double h[3] = {d.dx[0], d.dx[1], d.dx[2]};
+    int l = 0;
+    for (;;) {
+        Level& L = lev[l];
+        for (int a = 0; a < 3; ++a) { L.n[a] = n[a]; L.h[a] = h[a]; }
+        L.px = (int)align_up((size_t)n[0] + 1, 4);
+        L.ncell = (size_t)n[0] * n[1] * n[2];
+        L.nax = (size_t)L.px * n[1] * n[2];
+        L.nay = (size_t)n[0] * (n[1] + 1) * n[2];
+        L.naz = (size_t)n[0] * n[1] * (n[2] + 1);
+        ++l;
+        bool can = l < kMaxLevels;
+        for (int a = 0; a < 3; ++a)
+            if ((n[a] & 1) || n[a] / 2 < d.coarsest_n) can = false;
+        if (!can) break;
+        for (int a = 0; a < 3; ++a) { n[a] /= 2; h[a] *= 2.0; }
+    }
+    *nlev = l;
+    if (lev[l - 1].ncell > (size_t)kBottomMax) return MAESTRO_MAC_ERR_UNSUPPORTED;
+    return MAESTRO_MAC_OK;
+}
+
+// Carve (or just size) the workspace.  base may be NULL when only sizing.
+size_t carve(maestro_mac_handle* H, char* base)
+{
+    size_t off = 0;
+    auto take = [&](size_t count, size_t elem) -> void* {
+        off = align_up(off, 256);
+        void* p = base ? (void*)(base + off) : nullptr;
+        off += count * elem;
+        return p;
+    };
+    for (int l = 0; l < H->nlev; ++l) {
+        Level& L = H->lev[l];
+        L.phi = (double*)take(L.ncell, 8);
+        L.phi2 = (double*)take(L.ncell, 8);
+        L.rhs = (double*)take(L.ncell, 8);
+        L.ax = (double*)take(L.nax, 8);
+        L.ay = (double*)take(L.nay, 8);
+        L.az = (double*)take(L.naz, 8);
+    }
+    H->part_sum = (double*)take(kRedBlocks, 8);
+    H->part_max = (double*)take(kRedBlocks, 8);
+    H->scal = (double*)take(16, 8);
+    H->bottom_vecs = (double*)take(6 * H->lev[H->nlev - 1].ncell, 8);
+    H->flags = (int*)take(16, 4);
+    H->has_staging = H->d.host_staging == 1;
+    if (H->has_staging) {
+        const maestro_mac_desc& d = H->d;
+        size_t nc = (size_t)d.nx * d.ny * d.nz;
+        H->st.beta0 = (double*)take(d.nr, 8);
+        H->st.rho0 = (double*)take(d.nr, 8);
+        H->st.rho = (double*)take(nc, 8);
+        H->st.S = (double*)take(nc, 8);
+        H->st.phi = (double*)take(nc, 8);
+        H->st.u = (double*)take((size_t)(d.nx + 1) * d.ny * d.nz, 8);
+        H->st.v = (double*)take((size_t)d.nx * (d.ny + 1) * d.nz, 8);
+        H->st.w = (double*)take((size_t)d.nx * d.ny * (d.nz + 1), 8);
+    }
+    return align_up(off, 256);
+}
+
+LevelDev dev_level(const maestro_mac_handle* H, int l)
+{
+    const Level& L = H->lev[l];
+    LevelDev D;
+    D.nx = L.n[0]; D.ny = L.n[1]; D.nz = L.n[2]; D.px = L.px;
+    for (int a = 0; a < 3; ++a) { D.bclo[a] = H->d.bc_lo[a]; D.bchi[a] = H->d.bc_hi[a]; }
+    D.phi = L.phi; D.phi2 = L.phi2; D.rhs = L.rhs; D.ax = L.ax; D.ay = L.ay; D.az = L.az;
+    return D;
+}
+
+GeoDev dev_geo(const maestro_mac_handle* H)
+{
+    const maestro_mac_desc& d = H->d;
+    GeoDev G;
+    G.nx = d.nx; G.ny = d.ny; G.nz = d.nz;
+    G.dx = d.dx[0]; G.dy = d.dx[1]; G.dz = d.dx[2];
+    for (int a = 0; a < 3; ++a) { G.bclo[a] = d.bc_lo[a]; G.bchi[a] = d.bc_hi[a]; }
+    G.geometry = d.geometry; G.nr = d.nr; G.dr = d.dr;
+    G.cx = d.center[0]; G.cy = d.center[1]; G.cz = d.center[2];
+    return G;
+}
+
+// block (bx, by) with bx*by = 256 and grid covering (ex, ey, ez)
+void dims3(int ex, int ey, int ez, dim3* grid, dim3* block)
+{
+    int bx = 32;
+    while (bx < 128 && bx < ex) bx *= 2;
+    int by = 256 / bx;
+    *block = dim3(bx, by, 1);
+    *grid = dim3((ex + bx - 1) / bx, (ey + by - 1) / by, ez);
+}
+
+#define CUDA_OK(call) do { if ((call) != cudaSuccess) return MAESTRO_MAC_ERR_CUDA; } while (0)
+#define LAUNCHED(H) do { ++(H)->launches; if (cudaPeekAtLastError() != cudaSuccess) return MAESTRO_MAC_ERR_CUDA; } while (0)
+
+int red_blocks(int rows) { return rows < kRedBlocks ? rows : kRedBlocks; }
+
+// ---- individual steps ------------------------------------------------------------------------
+
+int do_coefficients(maestro_mac_handle* H, const double* beta0, const double* rho0, const double* rho, cudaStream_t s)
+{
+    GeoDev G = dev_geo(H);
+    dim3 g, b;
+    dims3(G.nx + 1, G.ny + 1, G.nz + 1, &g, &b);
+    CUDA_OK(cudaMemsetAsync(H->flags, 0, 16 * sizeof(int), s));
+    k_face_coeff<<<g, b, 0, s>>>(G, dev_level(H, 0), beta0, rho, rho0, H->flags);
+    LAUNCHED(H);
+    for (int l = 0; l + 1 < H->nlev; ++l) {
+        LevelDev C = dev_level(H, l + 1);
+        dims3(C.nx + 1, C.ny + 1, C.nz + 1, &g, &b);
+        k_coarsen_coeff<<<g, b, 0, s>>>(dev_level(H, l), C);
+        LAUNCHED(H);
+    }
+    return MAESTRO_MAC_OK;
+}
+
+// rhs on level 0; leaves sum/max of the final rhs in scal[0..1] and the removed sum in scal[2]
+int do_rhs(maestro_mac_handle* H, const double* beta0, const double* u, const double* v, const double* w,
+           const double* S, cudaStream_t s)
+{
+    GeoDev G = dev_geo(H);
+    Level& L0 = H->lev[0];
+    int rows = G.ny * G.nz;
+    int nb = red_blocks(rows);
+    int bt = G.nx >= 256 ? 256 : (G.nx >= 128 ? 128 : 64);
+    k_rhs<<<nb, bt, 0, s>>>(G, beta0, u, v, w, S, L0.rhs, H->part_sum, H->part_max);
+    LAUNCHED(H);
+    k_reduce_final<<<1, 1024, 0, s>>>(H->part_sum, H->part_max, nb, H->scal);
+    LAUNCHED(H);
+    if (H->singular) {
+        CUDA_OK(cudaMemcpyAsync(H->scal + 2, H->scal, sizeof(double), cudaMemcpyDeviceToDevice, s));
+        k_shift_mean<<<kRedBlocks, 256, 0, s>>>(L0.rhs, L0.ncell, H->scal + 2, 1.0 / (double)L0.ncell, H->part_sum, H->part_max);
+        LAUNCHED(H);
+        k_reduce_final<<<1, 1024, 0, s>>>(H->part_sum, H->part_max, kRedBlocks, H->scal);
+        LAUNCHED(H);
+    } else {
+        CUDA_OK(cudaMemsetAsync(H->scal + 2, 0, sizeof(double), s));
+    }
+    return MAESTRO_MAC_OK;
+}
+
+int do_smooth(maestro_mac_handle* H, int l, int nsweeps, cudaStream_t s)
+{
+    LevelDev L = dev_level(H, l);
+    for (int sw = 0; sw < nsweeps; ++sw) {
+        if (H->d.smoother == 0 && fused_sweep_supported(L)) {
+            int rc = launch_fused_sweep(H->lev[l].phi, H->lev[l].phi2, L, s);
+            if (rc != 0) return MAESTRO_MAC_ERR_CUDA;
+            ++H->launches;
+            // the fused sweep ping-pongs: result is in phi2; swap the level's buffers
+            double* t = H->lev[l].phi; H->lev[l].phi = H->lev[l].phi2; H->lev[l].phi2 = t;
+            L = dev_level(H, l);
+        } else {
+            dim3 g, b;
+            dims3((L.nx + 1) / 2, L.ny, L.nz, &g, &b);
+            k_rbgs_color<<<g, b, 0, s>>>(L, 0);
+            LAUNCHED(H);
+            k_rbgs_color<<<g, b, 0, s>>>(L, 1);
+            LAUNCHED(H);
+        }
+    }
+    return MAESTRO_MAC_OK;
+}
+
+int do_residual_restrict(maestro_mac_handle* H, int l, cudaStream_t s)
+{
+    LevelDev C = dev_level(H, l + 1);
+    dim3 g, b;
+    dims3(C.nx, C.ny, C.nz, &g, &b);
+    k_residual_restrict<<<g, b, 0, s>>>(dev_level(H, l), C);
+    LAUNCHED(H);
+    return MAESTRO_MAC_OK;
+}
+
+int do_prolong(maestro_mac_handle* H, int l, cudaStream_t s)
+{
+    LevelDev F = dev_level(H, l);
+    dim3 g, b;
+    dims3(F.nx, F.ny, F.nz, &g, &b);
+    k_prolong_add<<<g, b, 0, s>>>(F, dev_level(H, l + 1), H->d.prolongation);
+    LAUNCHED(H);
+    return MAESTRO_MAC_OK;
+}
+
+int do_bottom(maestro_mac_handle* H, cudaStream_t s)
+{
+    int l = H->nlev - 1;
+    int nb = (int)H->lev[l].ncell;
+    int threads = nb >= 1024 ? 1024 : ((nb + 31) / 32) * 32;
+    k_bottom_bicgstab<<<1, threads, 0, s>>>(dev_level(H, l), H->bottom_vecs, H->d.bottom_max_iter,
+                                            H->d.bottom_rel_tol, H->singular, H->flags + 1);
+    LAUNCHED(H);
+    return MAESTRO_MAC_OK;
+}
+
+int do_vcycle(maestro_mac_handle* H, cudaStream_t s)
+{
+    int rc;
+    for (int l = 0; l + 1 < H->nlev; ++l) {
+        if ((rc = do_smooth(H, l, H->d.nu_pre, s)) != 0) return rc;
+        if ((rc = do_residual_restrict(H, l, s)) != 0) return rc;
+    }
+    if ((rc = do_bottom(H, s)) != 0) return rc;
+    for (int l = H->nlev - 2; l >= 0; --l) {
+        if ((rc = do_prolong(H, l, s)) != 0) return rc;
+        if ((rc = do_smooth(H, l, H->d.nu_post, s)) != 0) return rc;
+    }
+    return MAESTRO_MAC_OK;
+}
+
+// max-norm of the residual of a level into scal[4]
+int do_residual_norm(maestro_mac_handle* H, int l, cudaStream_t s)
+{
+    LevelDev L = dev_level(H, l);
+    int rows = L.ny * L.nz;
+    int nb = red_blocks(rows);
+    int bt = L.nx >= 256 ? 256 : (L.nx >= 128 ? 128 : 64);
+    k_residual_norm<<<nb, bt, 0, s>>>(L, H->part_sum, H->part_max);
+    LAUNCHED(H);
+    k_reduce_final<<<1, 1024, 0, s>>>(H->part_sum, H->part_max, nb, H->scal + 3);
+    LAUNCHED(H);
+    return MAESTRO_MAC_OK;
+}
+
+int do_correct(maestro_mac_handle* H, const double* phi, const double* rho0, const double* rho,
+               double* u, double* v, double* w, cudaStream_t s)
+{
+    GeoDev G = dev_geo(H);
+    dim3 g, b;
+    dims3(G.nx + 1, G.ny + 1, G.nz + 1, &g, &b);
+    k_correct<<<g, b, 0, s>>>(G, phi, rho, rho0, u, v, w);
+    LAUNCHED(H);
+    return MAESTRO_MAC_OK;
+}
+
+}  // namespace
+
+// ================================================================================================
+// C ABI
+// ================================================================================================
+
+extern "C" void maestro_mac_default_desc(maestro_mac_desc* d)
+{
+    if (!d) return;
+    std::memset(d, 0, sizeof(*d));
+    d->struct_bytes = (int)sizeof(maestro_mac_desc);
+    d->nx = d->ny = d->nz = 32;
+    for (int a = 0; a < 3; ++a) { d->dx[a] = 1.0; d->bc_lo[a] = d->bc_hi[a] = MAESTRO_MAC_PERIODIC; }
+    d->geometry = MAESTRO_MAC_PLANAR;
+    d->nr = 32;
+    d->dr = 1.0;
+    d->nu_pre = d->nu_post = 2;
+    d->max_cycles = 100;
+    d->rel_tol = 1e-10;
+    d->coarsest_n = 4;
+    d->bottom_max_iter = 100;
+    d->bottom_rel_tol = 1e-8;
+}
+
+extern "C" int maestro_mac_setup(const maestro_mac_desc* desc, void* workspace, size_t workspace_bytes,
+                                 size_t* workspace_needed, maestro_mac_handle** out)
+{
+    if (out) *out = nullptr;
+    maestro_mac_handle tmp;
+    std::memset(&tmp, 0, sizeof(tmp));
+    int rc = validate_and_default(desc, &tmp.d);
+    if (rc != MAESTRO_MAC_OK) return rc;
+    rc = build_levels(tmp.d, tmp.lev, &tmp.nlev);
+    if (rc != MAESTRO_MAC_OK) return rc;
+    size_t need = carve(&tmp, nullptr);
+    if (workspace_needed) *workspace_needed = need;
+    if (!workspace || workspace_bytes < need) return MAESTRO_MAC_ERR_WORKSPACE;
+    if (!out) return MAESTRO_MAC_ERR_ARG;
+    if (((uintptr_t)workspace & 255u) != 0) return MAESTRO_MAC_ERR_ARG;
+
+    maestro_mac_handle* H = new (std::nothrow) maestro_mac_handle;
+    if (!H) return MAESTRO_MAC_ERR_ARG;
+    *H = tmp;
+    carve(H, (char*)workspace);
+    H->singular = 1;
+    for (int a = 0; a < 3; ++a)
+        if (H->d.bc_lo[a] == MAESTRO_MAC_OUTFLOW || H->d.bc_hi[a] == MAESTRO_MAC_OUTFLOW) H->singular = 0;
+    H->host_scal = nullptr;
+    H->host_flags = nullptr;
+    for (int e = 0; e < 4; ++e) H->ev[e] = nullptr;
+    bool ok = cudaMallocHost((void**)&H->host_scal, 8 * sizeof(double)) == cudaSuccess &&
+              cudaMallocHost((void**)&H->host_flags, 4 * sizeof(int)) == cudaSuccess;
+    for (int e = 0; ok && e < 4; ++e) ok = cudaEventCreate(&H->ev[e]) == cudaSuccess;
+    if (ok) ok = smoother_configure() == 0;
+    if (!ok) {
+        maestro_mac_free(H);
+        return MAESTRO_MAC_ERR_CUDA;
+    }
+    *out = H;
+    return MAESTRO_MAC_OK;
+}
+
+extern "C" int maestro_mac_free(maestro_mac_handle* H)
+{
+    if (!H) return MAESTRO_MAC_OK;
+    if (H->host_scal) cudaFreeHost(H->host_scal);
+    if (H->host_flags) cudaFreeHost(H->host_flags);
+    for (int e = 0; e < 4; ++e)
+        if (H->ev[e]) cudaEventDestroy(H->ev[e]);
+    delete H;
+    return MAESTRO_MAC_OK;
+}
+
+extern "C" int maestro_mac_project(maestro_mac_handle* H, const double* beta0, const double* rho0,
+                                   const double* rho, double* u, double* v, double* w, const double* S,
+                                   double* phi, maestro_mac_stats* stats, void* cuda_stream)
+{
+    if (!H || !beta0 || !u || !v || !w) return MAESTRO_MAC_ERR_ARG;
+    if (!rho && !rho0) return MAESTRO_MAC_ERR_ARG;
+    if (u == v || u == w || v == w || (phi && (phi == u || phi == v || phi == w || phi == rho || phi == S)))
+        return MAESTRO_MAC_ERR_ARG;
+    cudaStream_t s = (cudaStream_t)cuda_stream;
+    const maestro_mac_desc& d = H->d;
+    maestro_mac_stats st;
+    std::memset(&st, 0, sizeof(st));
+    st.singular = H->singular;
+    st.levels = H->nlev;
+    H->launches = 0;
+    int rc;
+    int result = MAESTRO_MAC_OK;
+    Level& L0 = H->lev[0];
+
+    CUDA_OK(cudaEventRecord(H->ev[0], s));
+    if ((rc = do_coefficients(H, beta0, rho0, rho, s)) != 0) return rc;
+    if ((rc = do_rhs(H, beta0, u, v, w, S, s)) != 0) return rc;
+    CUDA_OK(cudaMemcpyAsync(H->host_scal, H->scal, 3 * sizeof(double), cudaMemcpyDeviceToHost, s));
+    CUDA_OK(cudaMemcpyAsync(H->host_flags, H->flags, sizeof(int), cudaMemcpyDeviceToHost, s));
+    CUDA_OK(cudaMemsetAsync(L0.phi, 0, L0.ncell * sizeof(double), s));   // A16: phi = 0
+    CUDA_OK(cudaEventRecord(H->ev[1], s));
+    CUDA_OK(cudaStreamSynchronize(s));
+    st.rhs_norm_inf = H->host_scal[1];
+    st.rhs_mean_removed = H->singular ? H->host_scal[2] / (double)L0.ncell : 0.0;
+    const bool bad = H->host_flags[0] != 0 || !std::isfinite(st.rhs_norm_inf) || !std::isfinite(H->host_scal[0]);
+    if (bad) {
+        if (stats) *stats = st;
+        return MAESTRO_MAC_ERR_NONFINITE;
+    }
+    const bool trivial = st.rhs_norm_inf == 0.0;
+    if (!trivial) {
+        result = d.rel_tol > 0.0 ? MAESTRO_MAC_NOT_CONVERGED : MAESTRO_MAC_OK;
+        if (d.rel_tol > 0.0) {
+            while (st.cycles < d.max_cycles) {
+                if ((rc = do_vcycle(H, s)) != 0) return rc;
+                if ((rc = do_residual_norm(H, 0, s)) != 0) return rc;
+                CUDA_OK(cudaMemcpyAsync(H->host_scal + 4, H->scal + 4, sizeof(double), cudaMemcpyDeviceToHost, s));
+                CUDA_OK(cudaStreamSynchronize(s));
+                st.res_norm_inf = H->host_scal[4];
+                const double rel = st.res_norm_inf / st.rhs_norm_inf;
+                if (st.cycles < 128) st.res_history[st.cycles] = rel;
+                ++st.cycles;
+                if (rel != rel) { result = MAESTRO_MAC_ERR_NONFINITE; break; }
+                if (rel <= d.rel_tol) { result = MAESTRO_MAC_OK; break; }
+            }
+        } else {
+            for (; st.cycles < d.max_cycles; ++st.cycles)
+                if ((rc = do_vcycle(H, s)) != 0) return rc;
+        }
+    }
+    CUDA_OK(cudaEventRecord(H->ev[2], s));
+    if (!trivial && result != MAESTRO_MAC_ERR_NONFINITE) {
+        if (H->singular) {   // A10: zero-mean phi
+            k_sum<<<kRedBlocks, 256, 0, s>>>(H->lev[0].phi, L0.ncell, H->part_sum, H->part_max);
+            LAUNCHED(H);
+            k_reduce_final<<<1, 1024, 0, s>>>(H->part_sum, H->part_max, kRedBlocks, H->scal + 6);
+            LAUNCHED(H);
+            k_shift_mean<<<kRedBlocks, 256, 0, s>>>(H->lev[0].phi, L0.ncell, H->scal + 6, 1.0 / (double)L0.ncell, H->part_sum, H->part_max);
+            LAUNCHED(H);
+        }
+        if ((rc = do_correct(H, H->lev[0].phi, rho0, rho, u, v, w, s)) != 0) return rc;
+    }
+    if (phi) CUDA_OK(cudaMemcpyAsync(phi, H->lev[0].phi, L0.ncell * sizeof(double), cudaMemcpyDeviceToDevice, s));
+    CUDA_OK(cudaEventRecord(H->ev[3], s));
+    if (stats || d.rel_tol > 0.0) {
+        CUDA_OK(cudaMemcpyAsync(H->host_flags + 1, H->flags + 1, sizeof(int), cudaMemcpyDeviceToHost, s));
+        CUDA_OK(cudaStreamSynchronize(s));
+        st.bottom_iters_total = H->host_flags[1];
+        cudaEventElapsedTime(&st.ms_setup_kernels, H->ev[0], H->ev[1]);
+        cudaEventElapsedTime(&st.ms_vcycles, H->ev[1], H->ev[2]);
+        cudaEventElapsedTime(&st.ms_correct, H->ev[2], H->ev[3]);
+        if (d.rel_tol == 0.0 && !trivial) {   // fixed-cycle run: report the final residual too
+            if ((rc = do_residual_norm(H, 0, s)) != 0) return rc;
+            CUDA_OK(cudaMemcpyAsync(H->host_scal + 4, H->scal + 4, sizeof(double), cudaMemcpyDeviceToHost, s));
+            CUDA_OK(cudaStreamSynchronize(s));
+            st.res_norm_inf = H->host_scal[4];
+        }
+    }
+    st.gpu_launches = H->launches;
+    if (stats) *stats = st;
+    return result;
+}
+
+extern "C" int maestro_mac_project_host(maestro_mac_handle* H, const double* beta0, const double* rho0,
+                                        const double* rho, double* u, double* v, double* w, const double* S,
+                                        double* phi, maestro_mac_stats* stats, void* cuda_stream)
+{
+    if (!H || !H->has_staging || !beta0 || !u || !v || !w || (!rho && !rho0)) return MAESTRO_MAC_ERR_ARG;
+    cudaStream_t s = (cudaStream_t)cuda_stream;
+    const maestro_mac_desc& d = H->d;
+    const size_t nc = (size_t)d.nx * d.ny * d.nz;
+    const size_t nu = (size_t)(d.nx + 1) * d.ny * d.nz, nv = (size_t)d.nx * (d.ny + 1) * d.nz, nw = (size_t)d.nx * d.ny * (d.nz + 1);
+    Staging& T = H->st;
+    CUDA_OK(cudaMemcpyAsync(T.beta0, beta0, d.nr * sizeof(double), cudaMemcpyHostToDevice, s));
+    if (rho0) CUDA_OK(cudaMemcpyAsync(T.rho0, rho0, d.nr * sizeof(double), cudaMemcpyHostToDevice, s));
+    if (rho) CUDA_OK(cudaMemcpyAsync(T.rho, rho, nc * sizeof(double), cudaMemcpyHostToDevice, s));
+    if (S) CUDA_OK(cudaMemcpyAsync(T.S, S, nc * sizeof(double), cudaMemcpyHostToDevice, s));
+    CUDA_OK(cudaMemcpyAsync(T.u, u, nu * sizeof(double), cudaMemcpyHostToDevice, s));
+    CUDA_OK(cudaMemcpyAsync(T.v, v, nv * sizeof(double), cudaMemcpyHostToDevice, s));
+    CUDA_OK(cudaMemcpyAsync(T.w, w, nw * sizeof(double), cudaMemcpyHostToDevice, s));
+    int rc = maestro_mac_project(H, T.beta0, rho0 ? T.rho0 : nullptr, rho ? T.rho : nullptr, T.u, T.v, T.w,
+                                 S ? T.S : nullptr, phi ? T.phi : nullptr, stats, cuda_stream);
+    if (rc < 0) return rc;
+    CUDA_OK(cudaMemcpyAsync(u, T.u, nu * sizeof(double), cudaMemcpyDeviceToHost, s));
+    CUDA_OK(cudaMemcpyAsync(v, T.v, nv * sizeof(double), cudaMemcpyDeviceToHost, s));
+    CUDA_OK(cudaMemcpyAsync(w, T.w, nw * sizeof(double), cudaMemcpyDeviceToHost, s));
+    if (phi) CUDA_OK(cudaMemcpyAsync(phi, T.phi, nc * sizeof(double), cudaMemcpyDeviceToHost, s));
+    CUDA_OK(cudaStreamSynchronize(s));
+    return rc;
+}
+
+// ---- step API ----------------------------------------------------------------------------------
+
+extern "C" int maestro_mac_num_levels(const maestro_mac_handle* H) { return H ? H->nlev : MAESTRO_MAC_ERR_ARG; }
+
+extern "C" int maestro_mac_level_dims(const maestro_mac_handle* H, int level, int n[3], double hh[3])
+{
+    if (!H || level < 0 || level >= H->nlev) return MAESTRO_MAC_ERR_ARG;
+    for (int a = 0; a < 3; ++a) {
+        if (n) n[a] = H->lev[level].n[a];
+        if (hh) hh[a] = H->lev[level].h[a];
+    }
+    return MAESTRO_MAC_OK;
+}
+
+static int level_copy(maestro_mac_handle* H, int level, int which, double* pub, int to_public, cudaStream_t s)
+{
+    if (!H || !pub || level < 0 || level >= H->nlev) return MAESTRO_MAC_ERR_ARG;
+    Level& L = H->lev[level];
+    double* internal = nullptr;
+    size_t count = 0;
+    switch (which) {
+        case MAESTRO_MAC_ARR_PHI: internal = L.phi; count = L.ncell; break;
+        case MAESTRO_MAC_ARR_RHS: internal = L.rhs; count = L.ncell; break;
+        case MAESTRO_MAC_ARR_BY: internal = L.ay; count = L.nay; break;
+        case MAESTRO_MAC_ARR_BZ: internal = L.az; count = L.naz; break;
+        case MAESTRO_MAC_ARR_BX: {
+            LevelDev D = dev_level(H, level);
+            dim3 g, b;
+            dims3(D.nx + 1, D.ny, D.nz, &g, &b);
+            k_copy_ax<<<g, b, 0, s>>>(D, pub, to_public);
+            LAUNCHED(H);
+            return MAESTRO_MAC_OK;
+        }
+        default: return MAESTRO_MAC_ERR_ARG;
+    }
+    if (to_public) CUDA_OK(cudaMemcpyAsync(pub, internal, count * sizeof(double), cudaMemcpyDeviceToDevice, s));
+    else CUDA_OK(cudaMemcpyAsync(internal, pub, count * sizeof(double), cudaMemcpyDeviceToDevice, s));
+    return MAESTRO_MAC_OK;
+}
+
+extern "C" int maestro_mac_level_get(maestro_mac_handle* H, int level, int which, double* dst, void* cuda_stream)
+{
+    return level_copy(H, level, which, dst, 1, (cudaStream_t)cuda_stream);
+}
+
+extern "C" int maestro_mac_level_set(maestro_mac_handle* H, int level, int which, const double* src, void* cuda_stream)
+{
+    return level_copy(H, level, which, const_cast<double*>(src), 0, (cudaStream_t)cuda_stream);
+}
+
+extern "C" int maestro_mac_step_coefficients(maestro_mac_handle* H, const double* beta0, const double* rho0,
+                                             const double* rho, void* cuda_stream)
+{
+    if (!H || !beta0 || (!rho && !rho0)) return MAESTRO_MAC_ERR_ARG;
+    return do_coefficients(H, beta0, rho0, rho, (cudaStream_t)cuda_stream);
+}
+
+extern "C" int maestro_mac_step_rhs(maestro_mac_handle* H, const double* beta0, const double* u, const double* v,
+                                    const double* w, const double* S, double* rhs_norm_inf, double* mean_removed,
+                                    void* cuda_stream)
+{
+    if (!H || !beta0 || !u || !v || !w) return MAESTRO_MAC_ERR_ARG;
+    cudaStream_t s = (cudaStream_t)cuda_stream;
+    int rc = do_rhs(H, beta0, u, v, w, S, s);
+    if (rc != 0) return rc;
+    CUDA_OK(cudaMemcpyAsync(H->host_scal, H->scal, 3 * sizeof(double), cudaMemcpyDeviceToHost, s));
+    CUDA_OK(cudaStreamSynchronize(s));
+    if (rhs_norm_inf) *rhs_norm_inf = H->host_scal[1];
+    if (mean_removed) *mean_removed = H->singular ? H->host_scal[2] / (double)H->lev[0].ncell : 0.0;
+    return MAESTRO_MAC_OK;
+}
+
+extern "C" int maestro_mac_step_smooth(maestro_mac_handle* H, int level, int nsweeps, void* cuda_stream)
+{
+    if (!H || level < 0 || level >= H->nlev || nsweeps < 0) return MAESTRO_MAC_ERR_ARG;
+    for (int a = 0; a < 3; ++a)   // red-black needs even periodic extents (always true above the bottom)
+        if (H->d.bc_lo[a] == MAESTRO_MAC_PERIODIC && (H->lev[level].n[a] & 1)) return MAESTRO_MAC_ERR_UNSUPPORTED;
+    return do_smooth(H, level, nsweeps, (cudaStream_t)cuda_stream);
+}
+
+extern "C" int maestro_mac_step_residual_restrict(maestro_mac_handle* H, int level, void* cuda_stream)
+{
+    if (!H || level < 0 || level + 1 >= H->nlev) return MAESTRO_MAC_ERR_ARG;
+    return do_residual_restrict(H, level, (cudaStream_t)cuda_stream);
+}
+
+extern "C" int maestro_mac_step_prolong(maestro_mac_handle* H, int level, void* cuda_stream)
+{
+    if (!H || level < 0 || level + 1 >= H->nlev) return MAESTRO_MAC_ERR_ARG;
+    return do_prolong(H, level, (cudaStream_t)cuda_stream);
+}
+
+extern "C" int maestro_mac_step_bottom(maestro_mac_handle* H, void* cuda_stream)
+{
+    if (!H) return MAESTRO_MAC_ERR_ARG;
+    return do_bottom(H, (cudaStream_t)cuda_stream);
+}
+
+extern "C" int maestro_mac_step_vcycle(maestro_mac_handle* H, void* cuda_stream)
+{
+    if (!H) return MAESTRO_MAC_ERR_ARG;
+    return do_vcycle(H, (cudaStream_t)cuda_stream);
+}
+
+extern "C" int maestro_mac_step_residual_norm(maestro_mac_handle* H, int level, double* norm_inf, void* cuda_stream)
+{
+    if (!H || level < 0 || level >= H->nlev || !norm_inf) return MAESTRO_MAC_ERR_ARG;
+    cudaStream_t s = (cudaStream_t)cuda_stream;
+    int rc = do_residual_norm(H, level, s);
+    if (rc != 0) return rc;
+    CUDA_OK(cudaMemcpyAsync(H->host_scal + 4, H->scal + 4, sizeof(double), cudaMemcpyDeviceToHost, s));
+    CUDA_OK(cudaStreamSynchronize(s));
+    *norm_inf = H->host_scal[4];
+    return MAESTRO_MAC_OK;
+}
+
+extern "C" int maestro_mac_step_correct(maestro_mac_handle* H, const double* rho0, const double* rho, double* u,
+                                        double* v, double* w, void* cuda_stream)
+{
+    if (!H || !u || !v || !w || (!rho && !rho0)) return MAESTRO_MAC_ERR_ARG;
+    return do_correct(H, H->lev[0].phi, rho0, rho, u, v, w, (cudaStream_t)cuda_stream);
+}

@@ -1,0 +1,270 @@
+"""GPU-vs-oracle parity through the C ABI (SURVEY.md Sec. 8(d) "Parity protocol").
+
+Per-kernel parity uses the step API with a 1e-13 relative bar (reading A24: FMA contraction and
+evaluation order are not part of the contract); end-to-end parity uses the north_star bar of
+1e-10 relative L2 in phi and in u, v, w on the same seeded inputs, with the same cycle count.
+"""
+import numpy as np
+import pytest
+
+from helpers import oracle_project, oracle_structs, rel_l2
+from paper_1910_12979_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+PER, WALL, OUT = W.PERIODIC, W.WALL, W.OUTFLOW
+KERNEL_TOL = 1e-13
+E2E_TOL = 1e-10
+
+
+@pytest.fixture(scope="module")
+def mac():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    from paper_1910_12979_b200 import build, mac
+    build.build()
+    return mac
+
+
+def tt(a):
+    import torch
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def small_cases():
+    return [
+        W.mixed_bc_case(n=(16, 8, 12)),
+        W.mixed_bc_case(n=(16, 8, 12), geometry=W.SPHERICAL, seed=11),
+        W.mixed_bc_case(n=(24, 20, 8), bc_lo=(PER, WALL, OUT), bc_hi=(PER, WALL, WALL), seed=12),
+        W.mixed_bc_case(n=(8, 8, 40), bc_lo=(WALL, PER, PER), bc_hi=(OUT, PER, PER), seed=13),
+        W.config1(N=16), W.config2(N=16), W.config3(N=16, variant="N"), W.config3(N=16, variant="D"),
+    ]
+
+
+def folded(O, g, bfaces):
+    """internal coefficient a = c_f b / h^2 from the oracle's b (c_f: 1 interior/periodic, 0 WALL, 2 OUTFLOW)."""
+    out = []
+    for d in range(3):
+        a = bfaces[d] / g.h[d] ** 2
+        ax = 2 - d
+        lo = [slice(None)] * 3; hi = [slice(None)] * 3
+        lo[ax] = 0; hi[ax] = a.shape[ax] - 1
+        if g.bc_lo[d] != PER:
+            a[tuple(lo)] *= 0.0 if g.bc_lo[d] == WALL else 2.0
+            a[tuple(hi)] *= 0.0 if g.bc_hi[d] == WALL else 2.0
+        out.append(a)
+    return out
+
+
+def close(a, b, tol=KERNEL_TOL):
+    a = a.cpu().numpy() if hasattr(a, "cpu") else a
+    scale = max(np.abs(b).max(), 1e-300)
+    return np.abs(a - b).max() <= tol * scale
+
+
+@pytest.mark.parametrize("case", range(8))
+@pytest.mark.parametrize("smoother", [0, 1])
+def test_per_kernel_parity(oracle, mac, case, smoother):
+    import torch
+    O = oracle
+    wl = small_cases()[case]
+    g, b, mg = oracle_structs(O, wl)
+    P = mac.MacProjector(mac.desc_from_workload(wl, smoother=smoother))
+    dv = mac.to_device(wl)
+    nlev = P.num_levels
+
+    # a2 + a3: coefficients on every level
+    P.step_coefficients(dv["beta0"], dv["rho0"], dv["rho"])
+    bf = O.face_coeff(g, b, wl.beta0, wl.rho)
+    grids, coeffs = [g], [bf]
+    while O.can_coarsen(grids[-1], 4):
+        gc, cbx, cby, cbz = O.coarsen_coeff(grids[-1], *coeffs[-1])
+        grids.append(gc); coeffs.append((cbx, cby, cbz))
+    assert nlev == len(grids)
+    for l in range(nlev):
+        n, h = P.level_dims(l)
+        assert list(n) == list(grids[l].n) and np.allclose(h, list(grids[l].h), rtol=1e-15)
+        exp = folded(O, grids[l], [c.copy() for c in coeffs[l]])
+        for which, e in zip((mac.ARR_BX, mac.ARR_BY, mac.ARR_BZ), exp):
+            assert close(P.level_get(l, which), e), (l, which)
+
+    # a4: rhs, its max-norm and the removed mean
+    nrm, mean = P.step_rhs(dv["beta0"], dv["u"], dv["v"], dv["w"], dv["S"])
+    rhs = O.rhs(g, b, wl.beta0, wl.u, wl.v, wl.w, wl.S)
+    m = O.mean(rhs) if O.is_singular(g) else 0.0
+    rhs = rhs - m
+    assert close(P.level_get(0, mac.ARR_RHS), rhs)
+    assert nrm == pytest.approx(np.abs(rhs).max(), rel=1e-12)
+    assert mean == pytest.approx(m, abs=1e-13 * np.abs(rhs).max())
+
+    rng = np.random.default_rng(100 + case)
+    for l in range(nlev):
+        gl, cl = grids[l], coeffs[l]
+        shape = O.cell_shape(gl)
+        phi = rng.standard_normal(shape)
+        f = rng.standard_normal(shape)
+        P.level_set(l, mac.ARR_PHI, tt(phi)); P.level_set(l, mac.ARR_RHS, tt(f))
+        # a9: residual norm
+        assert P.step_residual_norm(l) == pytest.approx(np.abs(O.residual(gl, *cl, phi, f)).max(), rel=1e-12)
+        if l + 1 < nlev:
+            # a5: two sweeps
+            P.step_smooth(l, 2)
+            ref = phi.copy(); O.rbgs_sweep(gl, *cl, f, ref); O.rbgs_sweep(gl, *cl, f, ref)
+            assert close(P.level_get(l, mac.ARR_PHI), ref), l
+            # a6: residual + restriction (and the zeroed coarse phi)
+            P.step_residual_restrict(l)
+            assert close(P.level_get(l + 1, mac.ARR_RHS), O.restrict(gl, O.residual(gl, *cl, ref, f))), l
+            assert float(P.level_get(l + 1, mac.ARR_PHI).abs().max()) == 0.0
+            # a7: prolongation
+            ec = rng.standard_normal(O.cell_shape(grids[l + 1]))
+            P.level_set(l + 1, mac.ARR_PHI, tt(ec))
+            P.step_prolong(l)
+            O.prolong_add(gl, ec, ref, 0)
+            assert close(P.level_get(l, mac.ARR_PHI), ref), l
+        else:
+            # a8: bottom solve vs the dense solve (BiCGStab stops at 1e-8 by default)
+            P.step_bottom()
+            e = O.bottom_solve(gl, *cl, f)
+            assert rel_l2(P.level_get(l, mac.ARR_PHI).cpu().numpy(), e) <= 1e-6
+
+    # one whole V-cycle from a random state on level 0
+    phi = rng.standard_normal(O.cell_shape(g)); f = rng.standard_normal(O.cell_shape(g))
+    if O.is_singular(g):
+        f -= f.mean()
+    P.level_set(0, mac.ARR_PHI, tt(phi)); P.level_set(0, mac.ARR_RHS, tt(f))
+    P.step_vcycle()
+    ref = phi.copy(); O.vcycle(g, *bf, f, ref, mg)
+    assert rel_l2(P.level_get(0, mac.ARR_PHI).cpu().numpy(), ref) <= 1e-9
+
+    # a10: correction from a given phi
+    P.level_set(0, mac.ARR_PHI, tt(phi))
+    u, v, w = tt(wl.u), tt(wl.v), tt(wl.w)
+    P.step_correct(dv["rho0"], dv["rho"], u, v, w)
+    ru, rv, rw = wl.u.copy(), wl.v.copy(), wl.w.copy()
+    O.correct(g, wl.rho, phi, ru, rv, rw)
+    assert close(u, ru) and close(v, rv) and close(w, rw)
+    torch.cuda.synchronize()
+    P.close()
+
+
+E2E_CASES = [("1", 32), ("2", 32), ("3N", 32), ("3D", 32), ("4N", 32), ("4D", 64), ("5", 32),
+             ("2", 64), ("3N", 64), ("mixed", 0), ("mixed_sph", 0)]
+
+
+def get_case(name, N):
+    if name == "mixed":
+        return W.mixed_bc_case(n=(32, 16, 24))
+    if name == "mixed_sph":
+        return W.mixed_bc_case(n=(16, 48, 32), geometry=W.SPHERICAL, seed=21)
+    return W.by_name(name, N)
+
+
+def gpu_project(mac, wl, **over):
+    import torch
+    P = mac.MacProjector(mac.desc_from_workload(wl, **over))
+    dv = mac.to_device(wl)
+    phi = torch.full((wl.n[2], wl.n[1], wl.n[0]), float("nan"), dtype=torch.float64, device="cuda")
+    rc, st = P.project(dv["beta0"], dv["rho0"], dv["rho"], dv["u"], dv["v"], dv["w"], dv["S"], phi)
+    out = dict(status=rc, stats=st, phi=phi.cpu().numpy(), u=dv["u"].cpu().numpy(),
+               v=dv["v"].cpu().numpy(), w=dv["w"].cpu().numpy())
+    P.close()
+    return out
+
+
+@pytest.mark.parametrize("name,N", E2E_CASES)
+@pytest.mark.parametrize("smoother", [0, 1])
+def test_end_to_end_parity(oracle, mac, name, N, smoother):
+    O = oracle
+    wl = get_case(name, N)
+    ref = oracle_project(O, wl)
+    K = ref["stats"]["cycles"]
+    got = gpu_project(mac, wl, smoother=smoother)
+    if got["stats"]["cycles"] != K:            # knife-edge on the stop test: rerun in lockstep
+        got = gpu_project(mac, wl, smoother=smoother, rel_tol=0.0, max_cycles=K)
+    assert got["status"] == ref["status"] == 0
+    assert got["stats"]["cycles"] == K
+    assert got["stats"]["singular"] == ref["stats"]["singular"]
+    assert got["stats"]["levels"] == ref["stats"]["levels"]
+    for key in ("phi", "u", "v", "w"):
+        assert rel_l2(got[key], ref[key]) <= E2E_TOL, key
+    # same residual reduction
+    hist_g, hist_o = got["stats"]["res_history"], ref["stats"]["res_history"]
+    if hist_g:
+        assert np.allclose(hist_g, hist_o[:len(hist_g)], rtol=1e-3)
+        assert hist_g[-1] <= wl.rel_tol
+    assert got["stats"]["rhs_norm_inf"] == pytest.approx(ref["stats"]["rhs_norm_inf"], rel=1e-12)
+    assert got["stats"]["rhs_mean_removed"] == pytest.approx(ref["stats"]["rhs_mean_removed"], abs=1e-12 * ref["stats"]["rhs_norm_inf"])
+    # the paper's constraint (Eq. 6) holds for the GPU result, checked with the oracle's operator
+    c = O.constraint(ref["g"], ref["b"], wl.beta0, got["u"], got["v"], got["w"], wl.S) - ref["stats"]["rhs_mean_removed"]
+    assert np.abs(c).max() <= wl.rel_tol * ref["stats"]["rhs_norm_inf"] * 1.01
+
+
+def test_edge_cases(oracle, mac):
+    import torch
+    O = oracle
+    # rhs == 0: OK, cycles 0, phi 0, velocities untouched
+    z = W.config1(N=8); z.u[:] = 0; z.v[:] = 0; z.w[:] = 0
+    got = gpu_project(mac, z)
+    assert got["status"] == 0 and got["stats"]["cycles"] == 0 and np.all(got["phi"] == 0) and np.all(got["u"] == 0)
+    # non-finite inputs
+    bad = W.config1(N=8); bad.u[1, 2, 3] = np.nan
+    assert gpu_project(mac, bad)["status"] == mac.ERR_NONFINITE
+    bad = W.config1(N=8); bad.rho[0, 0, 0] = -1.0
+    assert gpu_project(mac, bad)["status"] == mac.ERR_NONFINITE
+    # max_cycles reached: NOT_CONVERGED with the last iterate written, same as the oracle's
+    wl = W.config2(N=16)
+    got = gpu_project(mac, wl, max_cycles=2)
+    ref = oracle_project(O, wl, max_cycles=2)
+    assert got["status"] == mac.NOT_CONVERGED and ref["status"] == 1
+    assert rel_l2(got["phi"], ref["phi"]) <= E2E_TOL and rel_l2(got["w"], ref["w"]) <= E2E_TOL
+    # rel_tol = 0: exactly max_cycles cycles
+    got = gpu_project(mac, wl, rel_tol=0.0, max_cycles=3)
+    ref = oracle_project(O, wl, rel_tol=0.0, max_cycles=3)
+    assert got["status"] == 0 and got["stats"]["cycles"] == 3
+    assert rel_l2(got["phi"], ref["phi"]) <= E2E_TOL
+    assert got["stats"]["res_norm_inf"] == pytest.approx(ref["stats"]["res_norm_inf"], rel=1e-6)
+    # rho == NULL (base-state-only projection), S == NULL, phi == NULL
+    P = mac.MacProjector(mac.desc_from_workload(wl))
+    dv = mac.to_device(wl)
+    rc, st = P.project(dv["beta0"], dv["rho0"], None, dv["u"], dv["v"], dv["w"], None, None)
+    g, b, mg = oracle_structs(O, wl)
+    u, v, w = wl.u.copy(), wl.v.copy(), wl.w.copy()
+    ost, _, ostats = O.project(g, b, mg, wl.beta0, wl.rho0, None, u, v, w, None)
+    assert rc == ost == 0 and st["cycles"] == ostats["cycles"]
+    assert rel_l2(dv["u"].cpu().numpy(), u) <= E2E_TOL and rel_l2(dv["w"].cpu().numpy(), w) <= E2E_TOL
+    # argument errors
+    rc, _ = P.project(None, dv["rho0"], dv["rho"], dv["u"], dv["v"], dv["w"])
+    assert rc == mac.ERR_ARG
+    rc, _ = P.project(dv["beta0"], dv["rho0"], dv["rho"], dv["u"], dv["u"], dv["w"])
+    assert rc == mac.ERR_ARG
+    rc, _ = P.project_host(dv["beta0"], dv["rho0"], dv["rho"], dv["u"], dv["v"], dv["w"])
+    assert rc == mac.ERR_ARG                      # no staging reserved
+    P.close()
+    # a single-level problem (level 0 is the bottom): BiCGStab alone must solve it
+    tiny = W.mixed_bc_case(n=(6, 5, 7), bc_lo=(OUT, WALL, WALL), bc_hi=(WALL, OUT, WALL))
+    got = gpu_project(mac, tiny, bottom_rel_tol=1e-13, bottom_max_iter=500)
+    ref = oracle_project(O, tiny)
+    assert ref["stats"]["levels"] == 1 and got["stats"]["levels"] == 1
+    assert rel_l2(got["phi"], ref["phi"]) <= 1e-8
+    torch.cuda.synchronize()
+
+
+def test_project_host_matches_device_path(oracle, mac):
+    import torch
+    wl = W.config3(N=32, variant="D")
+    ref = gpu_project(mac, wl)
+    P = mac.MacProjector(mac.desc_from_workload(wl, host_staging=1))
+    pin = lambda a: torch.from_numpy(a.copy()).pin_memory()
+    u, v, w, phi = pin(wl.u), pin(wl.v), pin(wl.w), torch.empty(wl.rho.shape, dtype=torch.float64).pin_memory()
+    rc, st = P.project_host(pin(wl.beta0), pin(wl.rho0), pin(wl.rho), u, v, w, pin(wl.S), phi)
+    assert rc == 0 and st["cycles"] == ref["stats"]["cycles"]
+    assert np.array_equal(phi.numpy(), ref["phi"]) and np.array_equal(u.numpy(), ref["u"])
+    assert np.array_equal(w.numpy(), ref["w"])
+    P.close()
+
+
+def test_deterministic_across_runs(mac):
+    wl = W.config2(N=32)
+    a, b = gpu_project(mac, wl), gpu_project(mac, wl)
+    for key in ("phi", "u", "v", "w"):
+        assert np.array_equal(a[key], b[key])
