@@ -92,6 +92,10 @@ typedef struct {
     float ms_vcycles;         /* all cycles including the stop tests */
     float ms_correct;         /* mean shift, velocity correction, phi copy-out */
     int gpu_launches;         /* kernels launched by this call */
+    float ms_smooth0;         /* summed device time of the level-0 smoother launches that were timed
+                                 (one CUDA event pair per launch, on the call's stream) */
+    int smooth0_launches;     /* level-0 smoother sweeps launched by this call */
+    int smooth0_timed;        /* how many of them ms_smooth0 covers (at most 512) */
 } maestro_mac_stats;
 
 /* Fill *desc with defaults for an nx*ny*nz unit-spacing periodic planar problem. */

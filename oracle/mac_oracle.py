@@ -64,6 +64,9 @@ def lib():
     global _lib
     if _lib is None:
         build()
+        # harness setting, not arithmetic: idle OpenMP threads sleep instead of spinning (the tiny
+        # coarse-level loops otherwise stall for seconds when the host has fewer free cores than threads)
+        os.environ.setdefault("OMP_WAIT_POLICY", "passive")
         L = C.CDLL(_LIB_PATH)
         GP, BP, MP = C.POINTER(Grid), C.POINTER(Base), C.POINTER(MG)
         L.orc_num_threads.restype = C.c_int

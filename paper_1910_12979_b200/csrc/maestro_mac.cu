@@ -19,6 +19,7 @@ namespace {
 constexpr int kMaxLevels = 32;
 constexpr int kRedBlocks = 148 * 8;       // blocks of the row-walking reduction kernels
 constexpr int kBottomMax = 4096;          // largest coarsest level (unknowns)
+constexpr int kSmoothEvents = 512;        // level-0 smoother launches timed per call
 
 struct Level {
     int n[3];
@@ -51,6 +52,10 @@ struct maestro_mac_handle {
     int *host_flags;               // pinned, 4 ints
     cudaEvent_t ev[4];
     int launches;
+    // level-0 smoother timing: one event pair per launch, summed after the final synchronise
+    cudaEvent_t* sm_ev;            // 2 * kSmoothEvents events, or NULL
+    int sm_used;                   // pairs recorded by the current call
+    int sm_launches;               // level-0 smoother launches of the current call (recorded or not)
 };
 
 namespace {
@@ -238,6 +243,9 @@ int do_smooth(maestro_mac_handle* H, int l, int nsweeps, cudaStream_t s)
 {
     LevelDev L = dev_level(H, l);
     for (int sw = 0; sw < nsweeps; ++sw) {
+        const bool timed = l == 0 && H->sm_ev && H->sm_used < kSmoothEvents;
+        if (l == 0) ++H->sm_launches;
+        if (timed) CUDA_OK(cudaEventRecord(H->sm_ev[2 * H->sm_used], s));
         if (H->d.smoother == 0 && fused_sweep_supported(L)) {
             int rc = launch_fused_sweep(H->lev[l].phi, H->lev[l].phi2, L, s);
             if (rc != 0) return MAESTRO_MAC_ERR_CUDA;
@@ -253,6 +261,7 @@ int do_smooth(maestro_mac_handle* H, int l, int nsweeps, cudaStream_t s)
             k_rbgs_color<<<g, b, 0, s>>>(L, 1);
             LAUNCHED(H);
         }
+        if (timed) { CUDA_OK(cudaEventRecord(H->sm_ev[2 * H->sm_used + 1], s)); ++H->sm_used; }
     }
     return MAESTRO_MAC_OK;
 }
@@ -381,6 +390,13 @@ extern "C" int maestro_mac_setup(const maestro_mac_desc* desc, void* workspace, 
     bool ok = cudaMallocHost((void**)&H->host_scal, 8 * sizeof(double)) == cudaSuccess &&
               cudaMallocHost((void**)&H->host_flags, 4 * sizeof(int)) == cudaSuccess;
     for (int e = 0; ok && e < 4; ++e) ok = cudaEventCreate(&H->ev[e]) == cudaSuccess;
+    H->sm_ev = nullptr;
+    H->sm_used = H->sm_launches = 0;
+    if (ok) {
+        H->sm_ev = (cudaEvent_t*)std::calloc(2 * kSmoothEvents, sizeof(cudaEvent_t));
+        ok = H->sm_ev != nullptr;
+        for (int e = 0; ok && e < 2 * kSmoothEvents; ++e) ok = cudaEventCreate(&H->sm_ev[e]) == cudaSuccess;
+    }
     if (ok) ok = smoother_configure() == 0;
     if (!ok) {
         maestro_mac_free(H);
@@ -397,6 +413,11 @@ extern "C" int maestro_mac_free(maestro_mac_handle* H)
     if (H->host_flags) cudaFreeHost(H->host_flags);
     for (int e = 0; e < 4; ++e)
         if (H->ev[e]) cudaEventDestroy(H->ev[e]);
+    if (H->sm_ev) {
+        for (int e = 0; e < 2 * kSmoothEvents; ++e)
+            if (H->sm_ev[e]) cudaEventDestroy(H->sm_ev[e]);
+        std::free(H->sm_ev);
+    }
     delete H;
     return MAESTRO_MAC_OK;
 }
@@ -416,6 +437,7 @@ extern "C" int maestro_mac_project(maestro_mac_handle* H, const double* beta0, c
     st.singular = H->singular;
     st.levels = H->nlev;
     H->launches = 0;
+    H->sm_used = H->sm_launches = 0;
     int rc;
     int result = MAESTRO_MAC_OK;
     Level& L0 = H->lev[0];
@@ -477,6 +499,15 @@ extern "C" int maestro_mac_project(maestro_mac_handle* H, const double* beta0, c
         cudaEventElapsedTime(&st.ms_setup_kernels, H->ev[0], H->ev[1]);
         cudaEventElapsedTime(&st.ms_vcycles, H->ev[1], H->ev[2]);
         cudaEventElapsedTime(&st.ms_correct, H->ev[2], H->ev[3]);
+        st.smooth0_launches = H->sm_launches;
+        st.smooth0_timed = H->sm_used;
+        double acc = 0.0;
+        for (int q = 0; q < H->sm_used; ++q) {
+            float ms = 0.0f;
+            cudaEventElapsedTime(&ms, H->sm_ev[2 * q], H->sm_ev[2 * q + 1]);
+            acc += ms;
+        }
+        st.ms_smooth0 = (float)acc;
         if (d.rel_tol == 0.0 && !trivial) {   // fixed-cycle run: report the final residual too
             if ((rc = do_residual_norm(H, 0, s)) != 0) return rc;
             CUDA_OK(cudaMemcpyAsync(H->host_scal + 4, H->scal + 4, sizeof(double), cudaMemcpyDeviceToHost, s));
