@@ -78,8 +78,12 @@ typedef struct {
     int prolongation;         /* 0 = cell-centred trilinear (default), 1 = piecewise constant */
     int host_staging;         /* 1 = reserve device staging in the workspace so that
                                  maestro_mac_project_host() can be used */
-    int smoother;             /* 0 = default (fused red+black single pass), 1 = reference two-pass
-                                 (one kernel per colour).  Same arithmetic, same results. */
+    int smoother;             /* 0 = default: fused red+black single pass, planes staged by TMA where the
+                                 level allows it (x, y not periodic, nx >= 60), else by cp.async;
+                                 1 = reference two-pass (one kernel per colour);
+                                 2 = fused single pass, cp.async staging on every level;
+                                 3 = fused single pass, TMA staging with the 32x16 tile.
+                                 Same arithmetic, same results. */
 } maestro_mac_desc;
 
 typedef struct {

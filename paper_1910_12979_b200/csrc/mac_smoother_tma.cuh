@@ -1,0 +1,296 @@
+// mac_smoother_tma.cuh -- the fused red+black Gauss-Seidel sweep of mac_smoother.cuh with the z-plane
+// staging done by the Tensor Memory Accelerator (cp.async.bulk.tensor, SASS UTMALDG) instead of
+// per-thread cp.async (north_star bullet 3 "shared-memory or TMA z-plane
+// staging").
+//
+// Why: the cp.async version spends 5 LDGSTS + their address arithmetic per thread per plane and is
+// bound by the MIO instruction queue (profiles/r1a_smoother_512_ncu.txt).  Here ONE thread per CTA
+// issues five 3-D box loads per plane (phi, rhs, ax, ay, az) that land in the same shared-memory
+// stage layout and signal an mbarrier with their byte count; out-of-range box elements (the halo
+// outside the domain, planes below 0 / above nz) are zero-filled by the hardware, which is exactly
+// the "phi = 0 and a_f = 0 outside the domain" convention of the folded coefficients
+// (mac_common.cuh).  Arithmetic, marching order and results are those of fused::step.
+//
+// Used for levels whose x and y sides are not periodic (TMA cannot wrap); periodic levels keep the
+// cp.async kernel.  z may be periodic (the plane coordinate is wrapped by the issuing thread).
+#pragma once
+#include <cuda.h>
+
+#include "mac_smoother.cuh"
+
+namespace tma {
+
+using fused::A_AX; using fused::A_AY; using fused::A_AZ; using fused::A_COUNT; using fused::A_PHI; using fused::A_RHS;
+using fused::Coef; using fused::Ctx;
+
+__device__ __forceinline__ unsigned smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void mbar_init(unsigned bar, int count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;\n" ::"r"(bar), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(unsigned bar, unsigned bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;\n" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned bar, unsigned parity)
+{
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "WAIT_LOOP:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra DONE;\n"
+        "bra WAIT_LOOP;\n"
+        "DONE:\n"
+        "}\n" ::"r"(bar), "r"(parity) : "memory");
+}
+__device__ __forceinline__ void tma_load_3d(unsigned dst, const CUtensorMap* map, unsigned bar, int c0, int c1, int c2)
+{
+    asm volatile(
+        "cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5}], [%2];\n"
+        ::"r"(dst), "l"(map), "r"(bar), "r"(c0), "r"(c1), "r"(c2) : "memory");
+}
+
+template <int LN, int TYE, int NS>
+struct Cfg {
+    static constexpr int kRow = LN * 16;                       // bytes of one staged row (2*LN doubles)
+    static constexpr int kArr = TYE * kRow;                    // one array of a stage
+    static constexpr int kStage = A_COUNT * kArr;
+    static constexpr unsigned kTx = (unsigned)kRow * (TYE + (TYE - 1) + 3 * (TYE - 2));   // bytes landing per plane
+    static constexpr size_t kSmem = (size_t)kStage * NS + 8 * NS + 128;
+    static_assert(Ctx<LN, TYE>::kStage == kStage, "stage layout must match fused::step");
+};
+
+// issue the five box loads of plane p (unwrapped) into stage `stg`
+template <int LN, int TYE, int NS>
+__device__ __forceinline__ void issue_plane(const CUtensorMap* tm_phi, const CUtensorMap* tm_rhs, const CUtensorMap* tm_ax,
+                                            const CUtensorMap* tm_ay, const CUtensorMap* tm_az, unsigned stage0, unsigned bar0,
+                                            int stg, int p, int nz, bool perz, int cx, int cy)
+{
+    using C = Cfg<LN, TYE, NS>;
+    if (perz) { if (p < 0) p += nz; else if (p >= nz) p -= nz; }
+    const unsigned d = stage0 + stg * C::kStage;
+    const unsigned bar = bar0 + 8 * stg;
+    mbar_expect_tx(bar, C::kTx);
+    tma_load_3d(d + A_PHI * C::kArr, tm_phi, bar, cx, cy, p);                    // rows 0 .. TYE-1
+    tma_load_3d(d + A_RHS * C::kArr + C::kRow, tm_rhs, bar, cx, cy + 1, p);      // rows 1 .. TYE-2
+    tma_load_3d(d + A_AX * C::kArr + C::kRow, tm_ax, bar, cx, cy + 1, p);
+    tma_load_3d(d + A_AZ * C::kArr + C::kRow, tm_az, bar, cx, cy + 1, p);
+    tma_load_3d(d + A_AY * C::kArr + C::kRow, tm_ay, bar, cx, cy + 1, p);        // rows 1 .. TYE-1 (faces)
+}
+
+template <int LN, int TYE, int NS, bool REDX0>
+__device__ __forceinline__ void march(const Ctx<LN, TYE>& C, const CUtensorMap* tm_phi, const CUtensorMap* tm_rhs,
+                                      const CUtensorMap* tm_ax, const CUtensorMap* tm_ay, const CUtensorMap* tm_az,
+                                      unsigned stage0, unsigned bar0, bool producer, int cx, int cy, int ks, int k0, int k1,
+                                      bool red_x_ok, bool red_y_ok, bool own, double* __restrict__ out,
+                                      unsigned long long out_stride)
+{
+    using G = Cfg<LN, TYE, NS>;
+    double2 qm2 = make_double2(0.0, 0.0), qm1;
+    Coef cA, cB;
+    cB.ax = cB.ays = cB.ayn = cB.az = cB.rhs = qm2; cB.ax2 = 0.0;
+    // planes ks-1 .. ks+NS-3 were issued by the prologue into stages 0 .. NS-2 (plane ks-1+q -> stage q);
+    // the first NS-1 waits are on phase 0 of their barriers
+    mbar_wait(bar0 + 0, 0);
+    mbar_wait(bar0 + 8, 0);
+    int sI = 1;                                                // stage of plane k
+    unsigned phase_bits = 0;                                   // bit s: parity to wait for on stage s next
+    phase_bits |= 3u;                                          // stages 0 and 1 have completed phase 0
+    qm1 = fused::ld2<LN, TYE>(C.smem_gen + 0 * G::kStage, A_PHI, 0, 0);
+    double2 qn = fused::ld2<LN, TYE>(C.smem_gen + 1 * G::kStage, A_PHI, 0, 0);
+    double2 azn = fused::ld2<LN, TYE>(C.smem_gen + 1 * G::kStage, A_AZ, 0, 0);
+#pragma unroll 1
+    for (int k = ks; k <= k1; k += 2) {
+#pragma unroll
+        for (int h = 0; h < 2; ++h) {
+            const int kk = k + h;
+            if (kk > k1) break;
+            int sM = sI - 1; if (sM < 0) sM += NS;
+            int sP = sI + 1; if (sP >= NS) sP -= NS;
+            int sN = sI + (NS - 2); if (sN >= NS) sN -= NS;       // stage that plane kk-2 vacated at the end of step kk-1
+            // plane kk+1 must have landed; every thread must have finished step kk-1
+            mbar_wait(bar0 + 8 * sP, (phase_bits >> sP) & 1u);
+            phase_bits ^= 1u << sP;
+            __syncthreads();
+            if (producer && kk + NS - 2 <= k1 + 1) {           // never leave a load in flight at exit
+                asm volatile("fence.proxy.async.shared::cta;\n" ::: "memory");
+                issue_plane<LN, TYE, NS>(tm_phi, tm_rhs, tm_ax, tm_ay, tm_az, stage0, bar0, sN, kk + NS - 2, C.nz, C.perz, cx, cy);
+            }
+            unsigned char* s0 = C.smem_gen + sI * G::kStage;
+            const unsigned char* sm = C.smem_gen + sM * G::kStage;
+            const unsigned char* sp = C.smem_gen + sP * G::kStage;
+            const bool k_real = C.perz || (kk >= 0 && kk < C.nz);
+            const bool do_black = own && kk - 1 >= k0 && kk - 1 < k1;
+            if (h == 0)
+                fused::step<LN, TYE, REDX0>(C, s0, sm, sp, k_real && (REDX0 ? red_x_ok : red_y_ok), do_black, out, qm2, qm1, qn, azn, cA, cB);
+            else
+                fused::step<LN, TYE, !REDX0>(C, s0, sm, sp, k_real && (REDX0 ? red_y_ok : red_x_ok), do_black, out, qm2, qm1, qn, azn, cB, cA);
+            out += out_stride;
+            sI = sP;
+        }
+    }
+}
+
+template <int LN, int TYE, int NS, int MINB>
+__global__ void __launch_bounds__(LN * TYE, MINB)
+k_rbgs_tma(const __grid_constant__ CUtensorMap tm_phi, const __grid_constant__ CUtensorMap tm_rhs,
+           const __grid_constant__ CUtensorMap tm_ax, const __grid_constant__ CUtensorMap tm_ay,
+           const __grid_constant__ CUtensorMap tm_az, LevelDev L, double* __restrict__ pout, int zchunk)
+{
+    using G = Cfg<LN, TYE, NS>;
+    constexpr int TY = TYE - 4, kTX = 2 * LN - 4;
+    extern __shared__ __align__(128) unsigned char smem_dyn[];
+    // stages need 128-byte alignment for TMA; the dynamic segment is at least 16-byte aligned
+    unsigned char* smem_raw = reinterpret_cast<unsigned char*>((reinterpret_cast<uintptr_t>(smem_dyn) + 127) & ~(uintptr_t)127);
+    const unsigned stage0 = smem_u32(smem_raw);
+    const unsigned bar0 = stage0 + NS * G::kStage;
+
+    const int lane = threadIdx.x;
+    // a warp holds 32/LN rows; they must share their parity (the colour role is warp-uniform)
+    const int ty = (LN == 32) ? (int)threadIdx.y
+                              : 4 * ((int)threadIdx.y >> 2) + (((int)threadIdx.y >> 1) & 1) + 2 * ((int)threadIdx.y & 1);
+    static_assert(LN == 32 || (LN == 16 && TYE % 4 == 0), "row mapping");
+    const int x0 = blockIdx.x * kTX, y0 = blockIdx.y * TY;
+    const int k0 = blockIdx.z * zchunk, k1 = min(k0 + zchunk, L.nz);
+    const int gi = x0 - 2 + 2 * lane, gj = y0 - 2 + ty;
+    const bool x_ok = gi >= 0 && gi < L.nx, y_ok = gj >= 0 && gj < L.ny;
+    const bool col_ok = x_ok && y_ok;
+    const bool row_red = ty >= 1 && ty <= TYE - 2;
+    const bool own = col_ok && lane >= 1 && lane <= LN - 2 && ty >= 2 && ty <= TYE - 3 && gi < x0 + kTX && gj < y0 + TY;
+    const bool producer = threadIdx.x == 0 && threadIdx.y == 0;
+
+    Ctx<LN, TYE> C;
+    C.nz = L.nz;
+    C.perz = L.bclo[2] == MAC_PERIODIC;
+    const unsigned slot = (ty * LN + lane) * 16;
+    C.smem_gen = smem_raw + slot;
+    C.smem_u32 = stage0 + slot;
+
+    const int ks = k0 - 1;
+    if (producer) {
+        for (int s = 0; s < NS; ++s) mbar_init(bar0 + 8 * s, 1);
+        asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
+        asm volatile("fence.proxy.async.shared::cta;\n" ::: "memory");
+        for (int q = 0; q < NS - 1 && ks - 1 + q <= k1 + 1; ++q)
+            issue_plane<LN, TYE, NS>(&tm_phi, &tm_rhs, &tm_ax, &tm_ay, &tm_az, stage0, bar0, q, ks - 1 + q, L.nz, C.perz, x0 - 2, y0 - 2);
+    }
+    __syncthreads();                                             // barrier inits visible before anyone waits
+
+    const bool red_x_ok = col_ok && row_red && lane >= 1;
+    const bool red_y_ok = col_ok && row_red && lane <= LN - 2;
+    double* out = pout + ((size_t)(x_ok ? gi : 0) + (size_t)L.nx * (own ? gj : 0)) + (long long)(ks - 1) * (long long)((size_t)L.nx * L.ny);
+    const unsigned long long ostride = (unsigned long long)L.nx * L.ny;
+    if (((gj + ks) & 1) == 0)
+        march<LN, TYE, NS, true>(C, &tm_phi, &tm_rhs, &tm_ax, &tm_ay, &tm_az, stage0, bar0, producer, x0 - 2, y0 - 2, ks, k0, k1, red_x_ok, red_y_ok, own, out, ostride);
+    else
+        march<LN, TYE, NS, false>(C, &tm_phi, &tm_rhs, &tm_ax, &tm_ay, &tm_az, stage0, bar0, producer, x0 - 2, y0 - 2, ks, k0, k1, red_x_ok, red_y_ok, own, out, ostride);
+    // every plane that was issued (<= k1 + 1) has been waited for by the last step: nothing is in flight
+}
+
+template <int LN, int TYE, int NS> constexpr size_t smem_bytes() { return Cfg<LN, TYE, NS>::kSmem; }
+
+}  // namespace tma
+
+// ---- host side ---------------------------------------------------------------------------------
+
+struct TmaLevelMaps {                 // tensor maps of one level for one tile configuration
+    CUtensorMap phi, phi2, rhs, ax, ay, az;
+    int ok;                           // 0: level not eligible (periodic x/y, odd nx, encode failed)
+};
+
+#define MAC_TMA_BIG   32, 16, 5, 1    // 64 x 16 staged tile (60 x 12 interior), 512 threads, 1 CTA/SM
+#define MAC_TMA_MID   16, 16, 5, 2    // 32 x 16 staged tile (28 x 12 interior), 256 threads, 2 CTAs/SM
+
+typedef CUresult (*mac_encode_tiled_fn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                        const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                        CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+static inline mac_encode_tiled_fn tma_encode_fn()
+{
+    static mac_encode_tiled_fn fn = nullptr;
+    static bool tried = false;
+    if (!tried) {
+        tried = true;
+        void* p = nullptr;
+        cudaDriverEntryPointQueryResult q;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) == cudaSuccess &&
+            q == cudaDriverEntryPointSuccess)
+            fn = (mac_encode_tiled_fn)p;
+    }
+    return fn;
+}
+
+static inline bool tma_encode3(CUtensorMap* m, const double* base, uint64_t d0, uint64_t d1, uint64_t d2,
+                               uint64_t pitch0_elems, uint64_t rows_per_plane, uint32_t b0, uint32_t b1)
+{
+    mac_encode_tiled_fn fn = tma_encode_fn();
+    if (!fn) return false;
+    cuuint64_t dims[3] = {d0, d1, d2};
+    cuuint64_t strides[2] = {pitch0_elems * 8ull, pitch0_elems * rows_per_plane * 8ull};
+    cuuint32_t box[3] = {b0, b1, 1};
+    cuuint32_t estr[3] = {1, 1, 1};
+    return fn(m, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 3, (void*)base, dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+              CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
+// Build the maps of a level for a staged tile of 2*LN x TYE cells.  Returns ok.
+static inline int tma_build_maps(TmaLevelMaps* T, const LevelDev& L, int LN, int TYE)
+{
+    T->ok = 0;
+    if (L.bclo[0] == MAC_PERIODIC || L.bclo[1] == MAC_PERIODIC) return 0;
+    if ((L.nx & 1) || L.nx < 2 || (L.px & 1)) return 0;
+    const uint32_t bx = 2u * LN;
+    bool ok = tma_encode3(&T->phi, L.phi, L.nx, L.ny, L.nz, L.nx, L.ny, bx, TYE) &&
+              tma_encode3(&T->phi2, L.phi2, L.nx, L.ny, L.nz, L.nx, L.ny, bx, TYE) &&
+              tma_encode3(&T->rhs, L.rhs, L.nx, L.ny, L.nz, L.nx, L.ny, bx, TYE - 2) &&
+              tma_encode3(&T->ax, L.ax, (uint64_t)L.nx + 1, L.ny, L.nz, L.px, L.ny, bx, TYE - 2) &&
+              tma_encode3(&T->az, L.az, L.nx, L.ny, (uint64_t)L.nz + 1, L.nx, L.ny, bx, TYE - 2) &&
+              tma_encode3(&T->ay, L.ay, L.nx, (uint64_t)L.ny + 1, L.nz, L.nx, (uint64_t)L.ny + 1, bx, TYE - 1);
+    T->ok = ok ? 1 : 0;
+    return T->ok;
+}
+
+static inline int tma_smoother_configure()
+{
+    using namespace tma;
+    if (cudaFuncSetAttribute(k_rbgs_tma<MAC_TMA_BIG>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes<32, 16, 5>()) != cudaSuccess) return -1;
+    if (cudaFuncSetAttribute(k_rbgs_tma<MAC_TMA_MID>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes<16, 16, 5>()) != cudaSuccess) return -1;
+    return 0;
+}
+
+// z-chunking: pick the chunk count that minimises waves x (planes per chunk + restaged planes)
+static inline void tma_pick_chunks(int tiles, int nz, int slots, int* nchunk_out, int* zchunk_out)
+{
+    long best = -1; int bn = 1;
+    const int maxchunk = nz >= 32 ? nz / 16 : 1;
+    for (int n = 1; n <= maxchunk; ++n) {
+        const int zc = (nz + n - 1) / n;
+        const int nn = (nz + zc - 1) / zc;
+        const long waves = ((long)tiles * nn + slots - 1) / slots;
+        const long cost = waves * (zc + 4);
+        if (best < 0 || cost < best) { best = cost; bn = nn; }
+    }
+    *nchunk_out = bn;
+    *zchunk_out = (nz + bn - 1) / bn;
+}
+
+// One fused sweep through the TMA kernel: reads `in_is_phi2 ? phi2 : phi`, writes the other buffer.
+static inline int launch_tma_sweep(const TmaLevelMaps& T, bool in_is_phi2, double* phi_out, const LevelDev& L, int variant,
+                                   cudaStream_t s)
+{
+    using namespace tma;
+    const int LN = variant == 0 ? 32 : 16;
+    const int kTX = 2 * LN - 4, TY = 12;
+    const int tiles_x = (L.nx + kTX - 1) / kTX, tiles_y = (L.ny + TY - 1) / TY;
+    int nchunk, zchunk;
+    tma_pick_chunks(tiles_x * tiles_y, L.nz, variant == 0 ? 148 : 296, &nchunk, &zchunk);
+    dim3 grid(tiles_x, tiles_y, nchunk);
+    const CUtensorMap& tin = in_is_phi2 ? T.phi2 : T.phi;
+    if (variant == 0)
+        k_rbgs_tma<MAC_TMA_BIG><<<grid, dim3(32, 16), smem_bytes<32, 16, 5>(), s>>>(tin, T.rhs, T.ax, T.ay, T.az, L, phi_out, zchunk);
+    else
+        k_rbgs_tma<MAC_TMA_MID><<<grid, dim3(16, 16), smem_bytes<16, 16, 5>(), s>>>(tin, T.rhs, T.ax, T.ay, T.az, L, phi_out, zchunk);
+    return cudaPeekAtLastError() == cudaSuccess ? 0 : -1;
+}

@@ -13,6 +13,7 @@
 
 #include "mac_kernels.cuh"
 #include "mac_smoother.cuh"
+#include "mac_smoother_tma.cuh"
 
 namespace {
 
@@ -27,6 +28,8 @@ struct Level {
     int px;
     size_t ncell, nax, nay, naz;
     double *phi, *phi2, *rhs, *ax, *ay, *az;
+    double *phi_a;                 // the buffer `phi` pointed to at carve time (tensor map `phi`)
+    TmaLevelMaps tma[2];           // [0] MAC_TMA_BIG tile, [1] MAC_TMA_MID tile
 };
 
 struct Staging {
@@ -88,7 +91,7 @@ int validate_and_default(const maestro_mac_desc* in, maestro_mac_desc* d)
     if (!(d->bottom_rel_tol > 0.0)) d->bottom_rel_tol = 1e-8;
     if (d->prolongation != 0 && d->prolongation != 1) return MAESTRO_MAC_ERR_ARG;
     if (d->host_staging != 0 && d->host_staging != 1) return MAESTRO_MAC_ERR_ARG;
-    if (d->smoother != 0 && d->smoother != 1) return MAESTRO_MAC_ERR_ARG;
+    if (d->smoother < 0 || d->smoother > 3) return MAESTRO_MAC_ERR_ARG;
     return MAESTRO_MAC_OK;
 }
 
@@ -131,6 +134,7 @@ size_t carve(maestro_mac_handle* H, char* base)
     for (int l = 0; l < H->nlev; ++l) {
         Level& L = H->lev[l];
         L.phi = (double*)take(L.ncell, 8);
+        L.phi_a = L.phi;
         L.phi2 = (double*)take(L.ncell, 8);
         L.rhs = (double*)take(L.ncell, 8);
         L.ax = (double*)take(L.nax, 8);
@@ -246,7 +250,15 @@ int do_smooth(maestro_mac_handle* H, int l, int nsweeps, cudaStream_t s)
         const bool timed = l == 0 && H->sm_ev && H->sm_used < kSmoothEvents;
         if (l == 0) ++H->sm_launches;
         if (timed) CUDA_OK(cudaEventRecord(H->sm_ev[2 * H->sm_used], s));
-        if (H->d.smoother == 0 && fused_sweep_supported(L)) {
+        const int sm = H->d.smoother;
+        const int tv = (sm == 0 && L.nx >= 60) ? 0 : (sm == 3 ? 1 : -1);          // TMA tile variant, or -1
+        if (tv >= 0 && H->lev[l].tma[tv].ok) {
+            int rc = launch_tma_sweep(H->lev[l].tma[tv], H->lev[l].phi != H->lev[l].phi_a, H->lev[l].phi2, L, tv, s);
+            if (rc != 0) return MAESTRO_MAC_ERR_CUDA;
+            ++H->launches;
+            double* t = H->lev[l].phi; H->lev[l].phi = H->lev[l].phi2; H->lev[l].phi2 = t;
+            L = dev_level(H, l);
+        } else if (sm != 1 && fused_sweep_supported(L)) {
             int rc = launch_fused_sweep(H->lev[l].phi, H->lev[l].phi2, L, s);
             if (rc != 0) return MAESTRO_MAC_ERR_CUDA;
             ++H->launches;
@@ -397,7 +409,13 @@ extern "C" int maestro_mac_setup(const maestro_mac_desc* desc, void* workspace, 
         ok = H->sm_ev != nullptr;
         for (int e = 0; ok && e < 2 * kSmoothEvents; ++e) ok = cudaEventCreate(&H->sm_ev[e]) == cudaSuccess;
     }
-    if (ok) ok = smoother_configure() == 0;
+    if (ok) ok = smoother_configure() == 0 && tma_smoother_configure() == 0;
+    if (ok)
+        for (int l = 0; l < H->nlev; ++l) {          // tensor maps; a level that cannot use TMA keeps cp.async
+            LevelDev D = dev_level(H, l);
+            tma_build_maps(&H->lev[l].tma[0], D, 32, 16);
+            tma_build_maps(&H->lev[l].tma[1], D, 16, 16);
+        }
     if (!ok) {
         maestro_mac_free(H);
         return MAESTRO_MAC_ERR_CUDA;

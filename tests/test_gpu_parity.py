@@ -38,6 +38,9 @@ def small_cases():
         W.mixed_bc_case(n=(24, 20, 8), bc_lo=(PER, WALL, OUT), bc_hi=(PER, WALL, WALL), seed=12),
         W.mixed_bc_case(n=(8, 8, 40), bc_lo=(WALL, PER, PER), bc_hi=(OUT, PER, PER), seed=13),
         W.config1(N=16), W.config2(N=16), W.config3(N=16, variant="N"), W.config3(N=16, variant="D"),
+        # wide enough for the 64-column TMA tile (x, y not periodic), ragged in x and y, z periodic / not
+        W.mixed_bc_case(n=(72, 20, 16), bc_lo=(OUT, WALL, PER), bc_hi=(WALL, OUT, PER), seed=14),
+        W.mixed_bc_case(n=(136, 28, 16), bc_lo=(WALL, OUT, OUT), bc_hi=(OUT, WALL, WALL), geometry=W.SPHERICAL, seed=15),
     ]
 
 
@@ -62,8 +65,8 @@ def close(a, b, tol=KERNEL_TOL):
     return np.abs(a - b).max() <= tol * scale
 
 
-@pytest.mark.parametrize("case", range(8))
-@pytest.mark.parametrize("smoother", [0, 1])
+@pytest.mark.parametrize("case", range(10))
+@pytest.mark.parametrize("smoother", [0, 1, 2, 3])
 def test_per_kernel_parity(oracle, mac, case, smoother):
     import torch
     O = oracle
@@ -173,7 +176,7 @@ def gpu_project(mac, wl, **over):
 
 
 @pytest.mark.parametrize("name,N", E2E_CASES)
-@pytest.mark.parametrize("smoother", [0, 1])
+@pytest.mark.parametrize("smoother", [0, 1, 2, 3])
 def test_end_to_end_parity(oracle, mac, name, N, smoother):
     O = oracle
     wl = get_case(name, N)
