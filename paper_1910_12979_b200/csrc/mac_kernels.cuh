@@ -355,6 +355,73 @@ k_prolong_add(LevelDev F, LevelDev C, int prolongation)
     F.phi[cidx(F, i, j, k)] += val;
 }
 
+// a7, bandwidth form: one thread per COARSE cell adds the interpolant to its 8 children.  The 27
+// coarse values come from L1/L2 (the coarse array is 1/8 of the fine one); the children are read and
+// written as four 16-byte x pairs, so a warp moves 512 contiguous bytes per row.  Interpolation is
+// done axis by axis in the order x, y, z, i.e. the expression tree of k_prolong_add.
+__global__ void __launch_bounds__(256)
+k_prolong_add2(LevelDev F, LevelDev C, int prolongation)
+{
+    const int I = blockIdx.x * blockDim.x + threadIdx.x;
+    const int J = blockIdx.y * blockDim.y + threadIdx.y;
+    const int K = blockIdx.z;
+    if (I >= C.nx || J >= C.ny) return;
+    double out[2][2][2];                      // [dk][dj][di]
+    const double* __restrict__ e = C.phi;
+    if (prolongation == 1) {
+        const double v = e[cidx(C, I, J, K)];
+#pragma unroll
+        for (int q = 0; q < 8; ++q) out[q >> 2][(q >> 1) & 1][q & 1] = v;
+    } else {
+        int ix[3], jy[3], kz[3];
+        double wx[3], wy[3], wz[3];           // weight of the neighbour on side 0 (low) / 2 (high)
+        ix[1] = I; jy[1] = J; kz[1] = K;
+#pragma unroll
+        for (int sd = 0; sd < 3; sd += 2) {
+            double sg = 1.0;
+            ix[sd] = ghost_index(I + sd - 1, C.nx, C.bclo[0], C.bchi[0], sg); wx[sd] = 0.25 * sg;
+            sg = 1.0;
+            jy[sd] = ghost_index(J + sd - 1, C.ny, C.bclo[1], C.bchi[1], sg); wy[sd] = 0.25 * sg;
+            sg = 1.0;
+            kz[sd] = ghost_index(K + sd - 1, C.nz, C.bclo[2], C.bchi[2], sg); wz[sd] = 0.25 * sg;
+        }
+        double xi[3][3][2];                   // [dz][dy][child di] after x interpolation
+#pragma unroll
+        for (int dz = 0; dz < 3; ++dz)
+#pragma unroll
+            for (int dy = 0; dy < 3; ++dy) {
+                const size_t row = (size_t)C.nx * ((size_t)jy[dy] + (size_t)C.ny * (size_t)kz[dz]);
+                const double c0 = e[row + ix[1]], cm = e[row + ix[0]], cp = e[row + ix[2]];
+                xi[dz][dy][0] = 0.75 * c0 + wx[0] * cm;
+                xi[dz][dy][1] = 0.75 * c0 + wx[2] * cp;
+            }
+#pragma unroll
+        for (int di = 0; di < 2; ++di) {
+            double yi[3][2];                  // [dz][child dj]
+#pragma unroll
+            for (int dz = 0; dz < 3; ++dz) {
+                yi[dz][0] = 0.75 * xi[dz][1][di] + wy[0] * xi[dz][0][di];
+                yi[dz][1] = 0.75 * xi[dz][1][di] + wy[2] * xi[dz][2][di];
+            }
+#pragma unroll
+            for (int dj = 0; dj < 2; ++dj) {
+                out[0][dj][di] = 0.75 * yi[1][dj] + wz[0] * yi[0][dj];
+                out[1][dj][di] = 0.75 * yi[1][dj] + wz[2] * yi[2][dj];
+            }
+        }
+    }
+#pragma unroll
+    for (int dk = 0; dk < 2; ++dk)
+#pragma unroll
+        for (int dj = 0; dj < 2; ++dj) {
+            double2* p = reinterpret_cast<double2*>(F.phi + cidx(F, 2 * I, 2 * J + dj, 2 * K + dk));
+            double2 v = *p;
+            v.x += out[dk][dj][0];
+            v.y += out[dk][dj][1];
+            *p = v;
+        }
+}
+
 // ------------------------------------------------------------------------------------------------
 // a9  ||rhs - L phi||inf  (block partial maxima; folded by k_reduce_final)
 // ------------------------------------------------------------------------------------------------

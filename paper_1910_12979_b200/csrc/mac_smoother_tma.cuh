@@ -294,3 +294,172 @@ static inline int launch_tma_sweep(const TmaLevelMaps& T, bool in_is_phi2, doubl
         k_rbgs_tma<MAC_TMA_MID><<<grid, dim3(16, 16), smem_bytes<16, 16, 5>(), s>>>(tin, T.rhs, T.ax, T.ay, T.az, L, phi_out, zchunk);
     return cudaPeekAtLastError() == cudaSuccess ? 0 : -1;
 }
+
+// ================================================================================================
+// a6 / a9 on the same TMA plane ring:  r = rhs - L phi,  then (RESTRICT) coarse rhs = mean of the 8
+// children and coarse phi = 0, and/or (NORM) per-CTA partial of ||r||inf.
+//
+// Same staged tile as the smoother (64 x 16 cells: x halo 2, kept for 16-byte pair alignment; y halo
+// 1), same tensor maps.  A thread owns a 2 x 2 block of columns (an x pair in two adjacent rows), i.e.
+// the lateral footprint of ONE coarse cell; the two planes of the coarse cell are accumulated over
+// two consecutive marching steps, so the restriction needs no cross-thread reduction.  z-neighbours
+// of phi are carried in registers, lateral neighbours come from the staged plane.  Nothing is
+// written to shared memory, so a plane's stage is recycled as soon as every thread has passed it.
+// Algorithmic traffic: 40 B/cell read + 2 B/cell written (41 B/cell).
+// ================================================================================================
+namespace tma {
+
+enum { RES_RESTRICT = 1, RES_NORM = 2 };
+
+template <int NS, int MODE>
+__global__ void __launch_bounds__(32 * 7, 1)
+k_resid_tma(const __grid_constant__ CUtensorMap tm_phi, const __grid_constant__ CUtensorMap tm_rhs,
+            const __grid_constant__ CUtensorMap tm_ax, const __grid_constant__ CUtensorMap tm_ay,
+            const __grid_constant__ CUtensorMap tm_az, LevelDev L, double* __restrict__ crhs, double* __restrict__ cphi,
+            double* __restrict__ part_max, int zchunk)
+{
+    constexpr int LN = 32, TYE = 16;
+    using G = Cfg<LN, TYE, NS>;
+    constexpr int kTX = 60, kTY = 14;
+    extern __shared__ __align__(128) unsigned char smem_dyn[];
+    unsigned char* smem_raw = reinterpret_cast<unsigned char*>((reinterpret_cast<uintptr_t>(smem_dyn) + 127) & ~(uintptr_t)127);
+    const unsigned stage0 = smem_u32(smem_raw);
+    const unsigned bar0 = stage0 + NS * G::kStage;
+    __shared__ double sh_max[8];
+
+    const int lane = threadIdx.x, tr = threadIdx.y;
+    const int x0 = blockIdx.x * kTX, y0 = blockIdx.y * kTY;
+    const int k0 = blockIdx.z * zchunk, k1 = min(k0 + zchunk, L.nz);
+    const int gi = x0 - 2 + 2 * lane;                       // even
+    const int gja = y0 + 2 * tr;                            // even; rows gja, gja+1 = stage rows 2tr+1, 2tr+2
+    const bool own = lane >= 1 && lane <= LN - 2 && gi < L.nx && gja < L.ny;   // nx, ny even: the 2x2 block is all in or all out
+    const bool producer = threadIdx.x == 0 && threadIdx.y == 0;
+    const bool perz = L.bclo[2] == MAC_PERIODIC;
+    const unsigned char* base = smem_raw + ((2 * tr + 1) * LN + lane) * 16;   // row a of stage 0
+
+    if (producer) {
+        for (int s = 0; s < NS; ++s) mbar_init(bar0 + 8 * s, 1);
+        asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
+        asm volatile("fence.proxy.async.shared::cta;\n" ::: "memory");
+        for (int q = 0; q < NS && k0 - 1 + q <= k1; ++q)         // planes k0-1 .. ; plane p -> stage (p - (k0-1)) % NS
+            issue_plane<LN, TYE, NS>(&tm_phi, &tm_rhs, &tm_ax, &tm_ay, &tm_az, stage0, bar0, q, k0 - 1 + q, L.nz, perz, x0 - 2, y0 - 1);
+    }
+    __syncthreads();
+
+    unsigned phase_bits = 0;
+    mbar_wait(bar0 + 0, 0);
+    mbar_wait(bar0 + 8, 0);
+    phase_bits = 3u;
+    // own-column phi of planes k-1 (m), k (c); rows a, b
+    double2 pma = fused::ld2<LN, TYE>(base, A_PHI, 0, 0), pmb = fused::ld2<LN, TYE>(base, A_PHI, 1, 0);
+    double2 pca = fused::ld2<LN, TYE>(base + G::kStage, A_PHI, 0, 0), pcb = fused::ld2<LN, TYE>(base + G::kStage, A_PHI, 1, 0);
+    double2 aza = fused::ld2<LN, TYE>(base + G::kStage, A_AZ, 0, 0), azb = fused::ld2<LN, TYE>(base + G::kStage, A_AZ, 1, 0);
+    int sI = 1;
+    double acc = 0.0, vmax = 0.0;
+    const size_t cnx = (size_t)(L.nx >> 1), cny = (size_t)(L.ny >> 1);
+    double* co = crhs ? crhs + ((size_t)(gi >> 1) + cnx * ((size_t)(gja >> 1) + cny * (size_t)(k0 >> 1))) : nullptr;
+    double* cz = cphi ? cphi + ((size_t)(gi >> 1) + cnx * ((size_t)(gja >> 1) + cny * (size_t)(k0 >> 1))) : nullptr;
+
+#pragma unroll 1
+    for (int kk = k0; kk < k1; ++kk) {
+        int sP = sI + 1; if (sP >= NS) sP -= NS;
+        int sN = sI - 1; if (sN < 0) sN += NS;                    // stage of plane kk-1: last read during step kk-1
+        mbar_wait(bar0 + 8 * sP, (phase_bits >> sP) & 1u);
+        phase_bits ^= 1u << sP;
+        __syncthreads();
+        if (producer && kk + NS - 1 <= k1) {                      // (plane k0-1 was consumed into registers by the prologue)
+            asm volatile("fence.proxy.async.shared::cta;\n" ::: "memory");
+            issue_plane<LN, TYE, NS>(&tm_phi, &tm_rhs, &tm_ax, &tm_ay, &tm_az, stage0, bar0, sN, kk + NS - 1, L.nz, perz, x0 - 2, y0 - 1);
+        }
+        const unsigned char* s0 = base + sI * G::kStage;
+        const unsigned char* sp = base + sP * G::kStage;
+        const double2 pna = fused::ld2<LN, TYE>(sp, A_PHI, 0, 0), pnb = fused::ld2<LN, TYE>(sp, A_PHI, 1, 0);
+        const double2 azna = fused::ld2<LN, TYE>(sp, A_AZ, 0, 0), aznb = fused::ld2<LN, TYE>(sp, A_AZ, 1, 0);
+        if (own) {
+            const double2 axa = fused::ld2<LN, TYE>(s0, A_AX, 0, 0), axb = fused::ld2<LN, TYE>(s0, A_AX, 1, 0);
+            const double axa2 = fused::ld1<LN, TYE, true>(s0, A_AX, 0, 1), axb2 = fused::ld1<LN, TYE, true>(s0, A_AX, 1, 1);
+            const double2 ay0 = fused::ld2<LN, TYE>(s0, A_AY, 0, 0), ay1 = fused::ld2<LN, TYE>(s0, A_AY, 1, 0), ay2 = fused::ld2<LN, TYE>(s0, A_AY, 2, 0);
+            const double2 ra = fused::ld2<LN, TYE>(s0, A_RHS, 0, 0), rb = fused::ld2<LN, TYE>(s0, A_RHS, 1, 0);
+            const double2 ps = fused::ld2<LN, TYE>(s0, A_PHI, -1, 0), pn = fused::ld2<LN, TYE>(s0, A_PHI, 2, 0);
+            const double wa = fused::ld1<LN, TYE, false>(s0, A_PHI, 0, -1), ea = fused::ld1<LN, TYE, true>(s0, A_PHI, 0, 1);
+            const double wb = fused::ld1<LN, TYE, false>(s0, A_PHI, 1, -1), eb = fused::ld1<LN, TYE, true>(s0, A_PHI, 1, 1);
+            // residual r = rhs - (sum_f a_f phi_nb - phi_0 sum_f a_f) of the four cells
+            auto res = [](double rhs, double p0, double axw, double axe, double ays, double ayn, double azd, double azu,
+                          double w, double e, double s, double n, double d, double u) {
+                const double off = axw * w + axe * e + ays * s + ayn * n + azd * d + azu * u;
+                const double dg = ((axw + axe) + (ays + ayn)) + (azd + azu);
+                return rhs - (off - p0 * dg);
+            };
+            const double r00 = res(ra.x, pca.x, axa.x, axa.y, ay0.x, ay1.x, aza.x, azna.x, wa, pca.y, ps.x, pcb.x, pma.x, pna.x);
+            const double r10 = res(ra.y, pca.y, axa.y, axa2, ay0.y, ay1.y, aza.y, azna.y, pca.x, ea, ps.y, pcb.y, pma.y, pna.y);
+            const double r01 = res(rb.x, pcb.x, axb.x, axb.y, ay1.x, ay2.x, azb.x, aznb.x, wb, pcb.y, pca.x, pn.x, pmb.x, pnb.x);
+            const double r11 = res(rb.y, pcb.y, axb.y, axb2, ay1.y, ay2.y, azb.y, aznb.y, pcb.x, eb, pca.y, pn.y, pmb.y, pnb.y);
+            if (MODE & RES_NORM) {
+                vmax = nanmax(vmax, fabs(r00)); vmax = nanmax(vmax, fabs(r10));
+                vmax = nanmax(vmax, fabs(r01)); vmax = nanmax(vmax, fabs(r11));
+            }
+            if (MODE & RES_RESTRICT) {
+                const double s4 = (r00 + r10) + (r01 + r11);
+                if ((kk & 1) == 0) {
+                    acc = s4;
+                } else {
+                    *co = 0.125 * (acc + s4);
+                    *cz = 0.0;
+                    co += cnx * cny;
+                    cz += cnx * cny;
+                }
+            }
+        }
+        pma = pca; pmb = pcb; pca = pna; pcb = pnb; aza = azna; azb = aznb;
+        sI = sP;
+    }
+    if (MODE & RES_NORM) {
+        vmax = warp_nanmax(vmax);
+        if (lane == 0) sh_max[tr] = vmax;
+        __syncthreads();
+        if (tr == 0 && lane == 0) {
+            double m = sh_max[0];
+            for (int q = 1; q < 7; ++q) m = nanmax(m, sh_max[q]);
+            part_max[blockIdx.x + gridDim.x * (blockIdx.y + gridDim.y * blockIdx.z)] = m;
+        }
+    }
+}
+
+}  // namespace tma
+
+static inline int tma_resid_configure()
+{
+    using namespace tma;
+    const int sm = (int)smem_bytes<32, 16, 5>();
+    if (cudaFuncSetAttribute(k_resid_tma<5, RES_RESTRICT>, cudaFuncAttributeMaxDynamicSharedMemorySize, sm) != cudaSuccess) return -1;
+    if (cudaFuncSetAttribute(k_resid_tma<5, RES_NORM>, cudaFuncAttributeMaxDynamicSharedMemorySize, sm) != cudaSuccess) return -1;
+    if (cudaFuncSetAttribute(k_resid_tma<5, RES_RESTRICT | RES_NORM>, cudaFuncAttributeMaxDynamicSharedMemorySize, sm) != cudaSuccess) return -1;
+    return 0;
+}
+
+// mode: tma::RES_RESTRICT and/or tma::RES_NORM.  Returns the number of CTAs (= partial maxima written), or -1.
+static inline int launch_tma_resid(const TmaLevelMaps& T, bool in_is_phi2, const LevelDev& L, double* crhs, double* cphi,
+                                   double* part_max, int max_parts, int mode, cudaStream_t s)
+{
+    using namespace tma;
+    const int tiles_x = (L.nx + 59) / 60, tiles_y = (L.ny + 13) / 14;
+    int nchunk, zchunk;
+    tma_pick_chunks(tiles_x * tiles_y, L.nz, 148, &nchunk, &zchunk);
+    zchunk = (zchunk + 1) & ~1;                               // chunks start on even planes (coarse cells are not split)
+    nchunk = (L.nz + zchunk - 1) / zchunk;
+    while ((long)tiles_x * tiles_y * nchunk > max_parts && nchunk > 1) {
+        zchunk *= 2;
+        nchunk = (L.nz + zchunk - 1) / zchunk;
+    }
+    if ((long)tiles_x * tiles_y * nchunk > max_parts) return -1;
+    dim3 grid(tiles_x, tiles_y, nchunk), block(32, 7);
+    const CUtensorMap& tin = in_is_phi2 ? T.phi2 : T.phi;
+    const size_t sm = smem_bytes<32, 16, 5>();
+    if (mode == RES_RESTRICT)
+        k_resid_tma<5, RES_RESTRICT><<<grid, block, sm, s>>>(tin, T.rhs, T.ax, T.ay, T.az, L, crhs, cphi, part_max, zchunk);
+    else if (mode == RES_NORM)
+        k_resid_tma<5, RES_NORM><<<grid, block, sm, s>>>(tin, T.rhs, T.ax, T.ay, T.az, L, crhs, cphi, part_max, zchunk);
+    else
+        k_resid_tma<5, RES_RESTRICT | RES_NORM><<<grid, block, sm, s>>>(tin, T.rhs, T.ax, T.ay, T.az, L, crhs, cphi, part_max, zchunk);
+    return cudaPeekAtLastError() == cudaSuccess ? tiles_x * tiles_y * nchunk : -1;
+}

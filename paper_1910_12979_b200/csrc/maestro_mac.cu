@@ -19,6 +19,7 @@ namespace {
 
 constexpr int kMaxLevels = 32;
 constexpr int kRedBlocks = 148 * 8;       // blocks of the row-walking reduction kernels
+constexpr int kMaxParts = 16384;          // capacity of the partial-reduction arrays
 constexpr int kBottomMax = 4096;          // largest coarsest level (unknowns)
 constexpr int kSmoothEvents = 512;        // level-0 smoother launches timed per call
 
@@ -141,8 +142,8 @@ size_t carve(maestro_mac_handle* H, char* base)
         L.ay = (double*)take(L.nay, 8);
         L.az = (double*)take(L.naz, 8);
     }
-    H->part_sum = (double*)take(kRedBlocks, 8);
-    H->part_max = (double*)take(kRedBlocks, 8);
+    H->part_sum = (double*)take(kMaxParts, 8);
+    H->part_max = (double*)take(kMaxParts, 8);
     H->scal = (double*)take(16, 8);
     H->bottom_vecs = (double*)take(6 * H->lev[H->nlev - 1].ncell, 8);
     H->flags = (int*)take(16, 4);
@@ -278,8 +279,22 @@ int do_smooth(maestro_mac_handle* H, int l, int nsweeps, cudaStream_t s)
     return MAESTRO_MAC_OK;
 }
 
+// TMA transfer kernels are used with the default smoother on levels the tensor maps cover
+bool tma_aux(const maestro_mac_handle* H, int l)
+{
+    return H->d.smoother == 0 && H->lev[l].tma[0].ok && H->lev[l].n[0] >= 60 && H->lev[l].n[2] >= 2;
+}
+
 int do_residual_restrict(maestro_mac_handle* H, int l, cudaStream_t s)
 {
+    if (tma_aux(H, l)) {
+        Level& F = H->lev[l];
+        int n = launch_tma_resid(F.tma[0], F.phi != F.phi_a, dev_level(H, l), H->lev[l + 1].rhs, H->lev[l + 1].phi,
+                                 H->part_max, kMaxParts, tma::RES_RESTRICT, s);
+        if (n < 0) return MAESTRO_MAC_ERR_CUDA;
+        ++H->launches;
+        return MAESTRO_MAC_OK;
+    }
     LevelDev C = dev_level(H, l + 1);
     dim3 g, b;
     dims3(C.nx, C.ny, C.nz, &g, &b);
@@ -292,6 +307,13 @@ int do_prolong(maestro_mac_handle* H, int l, cudaStream_t s)
 {
     LevelDev F = dev_level(H, l);
     dim3 g, b;
+    if (H->d.smoother != 1 && (F.nx & 1) == 0) {             // bandwidth form: one thread per coarse cell
+        LevelDev C = dev_level(H, l + 1);
+        dims3(C.nx, C.ny, C.nz, &g, &b);
+        k_prolong_add2<<<g, b, 0, s>>>(F, C, H->d.prolongation);
+        LAUNCHED(H);
+        return MAESTRO_MAC_OK;
+    }
     dims3(F.nx, F.ny, F.nz, &g, &b);
     k_prolong_add<<<g, b, 0, s>>>(F, dev_level(H, l + 1), H->d.prolongation);
     LAUNCHED(H);
@@ -328,6 +350,15 @@ int do_vcycle(maestro_mac_handle* H, cudaStream_t s)
 int do_residual_norm(maestro_mac_handle* H, int l, cudaStream_t s)
 {
     LevelDev L = dev_level(H, l);
+    if (tma_aux(H, l)) {
+        Level& F = H->lev[l];
+        int n = launch_tma_resid(F.tma[0], F.phi != F.phi_a, L, nullptr, nullptr, H->part_max, kMaxParts, tma::RES_NORM, s);
+        if (n < 0) return MAESTRO_MAC_ERR_CUDA;
+        ++H->launches;
+        k_reduce_final<<<1, 1024, 0, s>>>(H->part_sum, H->part_max, n, H->scal + 3);
+        LAUNCHED(H);
+        return MAESTRO_MAC_OK;
+    }
     int rows = L.ny * L.nz;
     int nb = red_blocks(rows);
     int bt = L.nx >= 256 ? 256 : (L.nx >= 128 ? 128 : 64);
@@ -409,7 +440,7 @@ extern "C" int maestro_mac_setup(const maestro_mac_desc* desc, void* workspace, 
         ok = H->sm_ev != nullptr;
         for (int e = 0; ok && e < 2 * kSmoothEvents; ++e) ok = cudaEventCreate(&H->sm_ev[e]) == cudaSuccess;
     }
-    if (ok) ok = smoother_configure() == 0 && tma_smoother_configure() == 0;
+    if (ok) ok = smoother_configure() == 0 && tma_smoother_configure() == 0 && tma_resid_configure() == 0;
     if (ok)
         for (int l = 0; l < H->nlev; ++l) {          // tensor maps; a level that cannot use TMA keeps cp.async
             LevelDev D = dev_level(H, l);
