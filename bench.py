@@ -8,7 +8,7 @@ face coefficients -> coarsening -> rhs -> V-cycles to 1e-10 -> velocity correcti
 Prints ONE JSON line (rank 0).  `value` is level-0 cell-updates/s over the whole projection,
 N^3 (nu_pre + nu_post) cycles / t(project), inputs resident in HBM (SURVEY.md Sec. 8(d));
 `e2e` is the same metric through maestro_mac_project_host() with pinned HOST buffers, host<->device
-copies inside the timed region.  `roofline` is the level-0 fused red-black smoother: 48 B/cell/sweep
+copies inside the timed region.  `roofline` is the level-0 fused red-black smoother (k_rbgs_tma): 48 B/cell/sweep
  over the mean device time of its launches, timed by CUDA event pairs inside
 the library on the call's stream during the timed steps.  Multi-GPU: replicas only:
 every rank projects its own copy; value = all ranks' units / max-over-ranks time.
@@ -42,7 +42,7 @@ def parse_args():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", default="4N", help="workload: 1, 2, 3N, 3D, 4N, 4D, 5 (BASELINE.json configs)")
     ap.add_argument("--n", type=int, default=512, help="cells per side")
-    ap.add_argument("--smoother", type=int, default=0, help="0 fused single-pass (default), 1 two-pass")
+    ap.add_argument("--smoother", type=int, default=0, help="0 fused single pass, TMA staging (default); 1 two-pass; 2 fused, cp.async staging; 3 fused, TMA 32x16 tile")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--cpu-sample-n", type=int, default=0, help="cells per side of the oracle sample (0 = auto)")
@@ -271,7 +271,7 @@ def run_ours(a):
     sm_ms = sum(s["ms_smooth0"] for s in stats)
     sm_n = sum(s["smooth0_timed"] for s in stats)
     peak, peak_src = hbm_peak()
-    kname = "k_rbgs_fused" if a.smoother == 0 else "k_rbgs_color(x2)"
+    kname = {0: "k_rbgs_tma", 1: "k_rbgs_color(x2)", 2: "k_rbgs_fused", 3: "k_rbgs_tma"}[a.smoother]
     roof = None
     if sm_n > 0 and sm_ms > 0:
         per_launch_ms = sm_ms / sm_n
@@ -330,7 +330,7 @@ def run_ours(a):
             "ms_per_step": 1e3 * t_dev_max / max(a.steps, 1), "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": {"workload": workload_label(a.config, a.n), "cells": wl.ncells, "cycles_per_solve": cycles,
-                       "levels": stats[-1]["levels"], "smoother": "fused red+black single pass" if a.smoother == 0 else "two-pass",
+                       "levels": stats[-1]["levels"], "smoother": {0: "fused red+black single pass, TMA-staged", 1: "two-pass reference", 2: "fused single pass, cp.async-staged", 3: "fused single pass, TMA 32x16 tile"}[a.smoother],
                        "parallelism": "replicas only" if world > 1 else "single GPU",
                        "l2": "inputs larger than L2 (every level-0 array is %.2f GB)" % (wl.ncells * 8 / 1e9)
                              if wl.ncells * 8 > 126e6 else "level arrays fit in L2; no flush (the solve re-reads them by design)",

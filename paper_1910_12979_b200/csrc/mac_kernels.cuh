@@ -606,7 +606,7 @@ __device__ __forceinline__ void correct_face(const GeoDev& G, const double* __re
     auto cell = [&](int q) -> size_t {
         return (size_t)(D == 0 ? q : i) + (size_t)G.nx * ((size_t)(D == 1 ? q : j) + (size_t)G.ny * (size_t)(D == 2 ? q : k));
     };
-    const double grad = (ghi * phi[cell(hi)] - glo * phi[cell(lo)]) / h;
+    const double grad = (ghi * phi[cell(hi)] - glo * phi[cell(lo)]) * (1.0 / h);
     const double rf = 0.5 * (rho_cell(G, rho, rho0, D == 0 ? lo : i, D == 1 ? lo : j, D == 2 ? lo : k) +
                              rho_cell(G, rho, rho0, D == 0 ? hi : i, D == 1 ? hi : j, D == 2 ? hi : k));
     const double nv = vel[fi] - grad / rf;
@@ -645,4 +645,110 @@ __global__ void k_copy_ax(LevelDev L, double* pub, int to_public)
     size_t a = axidx(L, i, j, k), b = (size_t)i + (size_t)(L.nx + 1) * ((size_t)j + (size_t)L.ny * k);
     if (to_public) pub[b] = L.ax[a];
     else L.ax[a] = pub[b];
+}
+
+// ================================================================================================
+// Bandwidth forms of the once-per-projection kernels (a2, a4, a10).  One thread per (i, j) column
+// marches a chunk of z-planes; x-neighbours come from the adjacent lane (warp shuffle), the plane
+// below from registers.  Divisions by the grid spacing are multiplications by precomputed
+// reciprocals; the base-state profile is evaluated once per face instead of once per cell side.
+// ================================================================================================
+
+struct GeoInv { double idx, idy, idz, idx2, idy2, idz2, idr; };
+
+__device__ __forceinline__ double profile_eval_inv(const double* __restrict__ f, int nr, double idr, double r)
+{
+    double s = r * idr - 0.5;
+    if (s <= 0.0) return __ldg(f);
+    if (s >= (double)(nr - 1)) return __ldg(f + nr - 1);
+    int m = (int)s;
+    double t = s - (double)m;
+    return (1.0 - t) * __ldg(f + m) + t * __ldg(f + m + 1);
+}
+__device__ __forceinline__ double beta_inv(const GeoDev& G, const GeoInv& I, const double* __restrict__ f, double x, double y, double z)
+{
+    return profile_eval_inv(f, G.nr, I.idr, radius(G, x, y, z));
+}
+
+// a4: rhs = D(beta0 U_edge) - beta0 S with partial sum / max.  grid (ceil(nx/64), ceil(ny/4), chunks), block (64, 4)
+__global__ void __launch_bounds__(256)
+k_rhs2(GeoDev G, GeoInv I, const double* __restrict__ beta0, const double* __restrict__ u, const double* __restrict__ v,
+       const double* __restrict__ w, const double* __restrict__ S, double* __restrict__ rhs, int zchunk,
+       double* __restrict__ part_sum, double* __restrict__ part_max)
+{
+    const int i = blockIdx.x * 64 + threadIdx.x, j = blockIdx.y * 4 + threadIdx.y;
+    const int k0 = blockIdx.z * zchunk, k1 = min(k0 + zchunk, G.nz);
+    const bool in = i < G.nx && j < G.ny;
+    const bool px = G.bclo[0] == MAC_PERIODIC, py = G.bclo[1] == MAC_PERIODIC, pz = G.bclo[2] == MAC_PERIODIC;
+    double s = 0.0, m = 0.0;
+    const int ic = in ? i : 0, jc = in ? j : 0;                  // clamped: out-of-range threads still shuffle
+    const double xc = (ic + 0.5) * G.dx, yc = (jc + 0.5) * G.dy;
+    const int ih = (px && ic + 1 == G.nx) ? 0 : ic + 1;
+    const int jh = (py && jc + 1 == G.ny) ? 0 : jc + 1;
+    const bool last_x = (threadIdx.x & 31) == 31 || ic + 1 == G.nx;
+    const size_t sc = (size_t)G.nx * G.ny, su = (size_t)(G.nx + 1) * G.ny, sv = (size_t)G.nx * (G.ny + 1);
+    const double* up = u + (size_t)(G.nx + 1) * jc + su * k0;
+    const double* vp = v + ic + sv * k0;
+    const double* wp = w + ic + (size_t)G.nx * jc;
+    const size_t c0 = (size_t)ic + (size_t)G.nx * jc;
+    double fzl = beta_inv(G, I, beta0, xc, yc, k0 * G.dz) * __ldg(wp + sc * k0);
+#pragma unroll 4
+    for (int k = k0; k < k1; ++k) {
+        const double zc = (k + 0.5) * G.dz;
+        const int kh = (pz && k + 1 == G.nz) ? 0 : k + 1;
+        const double fxl = beta_inv(G, I, beta0, ic * G.dx, yc, zc) * __ldg(up + ic);
+        double fxh = __shfl_down_sync(0xffffffffu, fxl, 1);
+        if (last_x) fxh = beta_inv(G, I, beta0, ih * G.dx, yc, zc) * __ldg(up + ih);
+        const double fyl = beta_inv(G, I, beta0, xc, jc * G.dy, zc) * __ldg(vp + (size_t)G.nx * jc);
+        const double fyh = beta_inv(G, I, beta0, xc, jh * G.dy, zc) * __ldg(vp + (size_t)G.nx * jh);
+        const double fzh = beta_inv(G, I, beta0, xc, yc, kh * G.dz) * __ldg(wp + sc * kh);
+        double r = (fxh - fxl) * I.idx + (fyh - fyl) * I.idy + (fzh - fzl) * I.idz;
+        if (S) r -= beta_inv(G, I, beta0, xc, yc, zc) * __ldg(S + c0 + sc * k);
+        if (in) {
+            rhs[c0 + sc * k] = r;
+            s += r;
+            m = nanmax(m, fabs(r));
+        }
+        fzl = fzh;
+        up += su;
+        vp += sv;
+    }
+    block_reduce_store(s, m, part_sum, part_max, blockIdx.x + gridDim.x * (blockIdx.y + gridDim.y * blockIdx.z));
+}
+
+// a2: face coefficients.  Threads cover the extended index space i in [0,nx], j in [0,ny]; planes k in [k0,k1]
+// (the plane k == nz writes only the top z faces).  grid (ceil((nx+1)/64), ceil((ny+1)/4), chunks), block (64, 4)
+__global__ void __launch_bounds__(256)
+k_face_coeff2(GeoDev G, GeoInv I, LevelDev L, const double* __restrict__ beta0, const double* __restrict__ rho,
+              const double* __restrict__ rho0, int zchunk, int* __restrict__ flags)
+{
+    const int i = blockIdx.x * 64 + threadIdx.x, j = blockIdx.y * 4 + threadIdx.y;
+    const int k0 = blockIdx.z * zchunk, k1 = min(k0 + zchunk, G.nz + 1);
+    if (i > G.nx || j > G.ny) return;
+    const bool ci = i < G.nx, cj = j < G.ny;
+#pragma unroll 4
+    for (int k = k0; k < k1; ++k) {
+        const bool ck = k < G.nz;
+        double rf, cf;
+        int fp;
+        if (ci && cj && ck) {
+            const double r = rho_cell(G, rho, rho0, i, j, k);
+            if (!(r > 0.0) || !(r <= 1.79769313486231570e308)) atomicOr(flags, 1);
+        }
+        if (cj && ck) {
+            face_rho_weight<0>(G, rho, rho0, i, j, k, rf, cf, fp);
+            const double b = beta_inv(G, I, beta0, fp * G.dx, (j + 0.5) * G.dy, (k + 0.5) * G.dz);
+            L.ax[axidx(L, i, j, k)] = cf * (b / rf) * I.idx2;
+        }
+        if (ci && ck) {
+            face_rho_weight<1>(G, rho, rho0, i, j, k, rf, cf, fp);
+            const double b = beta_inv(G, I, beta0, (i + 0.5) * G.dx, fp * G.dy, (k + 0.5) * G.dz);
+            L.ay[ayidx(L, i, j, k)] = cf * (b / rf) * I.idy2;
+        }
+        if (ci && cj) {
+            face_rho_weight<2>(G, rho, rho0, i, j, k, rf, cf, fp);
+            const double b = beta_inv(G, I, beta0, (i + 0.5) * G.dx, (j + 0.5) * G.dy, fp * G.dz);
+            L.az[azidx(L, i, j, k)] = cf * (b / rf) * I.idz2;
+        }
+    }
 }

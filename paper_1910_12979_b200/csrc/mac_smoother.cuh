@@ -99,11 +99,13 @@ template <int LN, int TYE, bool X> __device__ __forceinline__ double ld1(const u
 
 // One marching step at plane k.  REDX: the x-column of the pair is red in plane k.
 // CUR receives the coefficients of plane k, PRV holds those of plane k-1.
-template <int LN, int TYE, bool REDX>
+// NORM: also fold |rhs - L phi_in| of the red cells it updates into *vmax (the residual of the sweep's
+// INPUT at red cells costs two extra operations because `off` and `dg` are at hand).
+template <int LN, int TYE, bool REDX, bool NORM = false>
 __device__ __forceinline__ void step(const Ctx<LN, TYE>& C, unsigned char* s0, const unsigned char* sm,
                                      const unsigned char* sp, bool do_red, bool do_black,
                                      double* __restrict__ out_km1, double2& qm2, double2& qm1,
-                                     double2& qn, double2& azn, Coef& CUR, const Coef& PRV)
+                                     double2& qn, double2& azn, Coef& CUR, const Coef& PRV, double* vmax = nullptr)
 {
     double2 q0 = qn;                                   // old phi of plane k (staged read of the last step)
     CUR.az = azn;
@@ -128,6 +130,7 @@ __device__ __forceinline__ void step(const Ctx<LN, TYE>& C, unsigned char* s0, c
         const double off = axw * w_ + axe * e_ + ays * s_ + ayn * n_ + azd * d_ + azu * u_;
         const double dg = ((axw + axe) + (ays + ayn)) + (azd + azu);
         const double nv = (off - pick<REDX>(CUR.rhs)) / dg;
+        if (NORM) *vmax = nanmax(*vmax, fabs(pick<REDX>(CUR.rhs) - (off - pick<REDX>(q0) * dg)));
         put<REDX>(q0, nv);
         *reinterpret_cast<double*>(s0 + A_PHI * Ctx<LN, TYE>::kArr + (REDX ? 0 : 8)) = nv;
     }

@@ -80,12 +80,12 @@ __device__ __forceinline__ void issue_plane(const CUtensorMap* tm_phi, const CUt
     tma_load_3d(d + A_AY * C::kArr + C::kRow, tm_ay, bar, cx, cy + 1, p);        // rows 1 .. TYE-1 (faces)
 }
 
-template <int LN, int TYE, int NS, bool REDX0>
+template <int LN, int TYE, int NS, bool REDX0, bool NORM>
 __device__ __forceinline__ void march(const Ctx<LN, TYE>& C, const CUtensorMap* tm_phi, const CUtensorMap* tm_rhs,
                                       const CUtensorMap* tm_ax, const CUtensorMap* tm_ay, const CUtensorMap* tm_az,
                                       unsigned stage0, unsigned bar0, bool producer, int cx, int cy, int ks, int k0, int k1,
                                       bool red_x_ok, bool red_y_ok, bool own, double* __restrict__ out,
-                                      unsigned long long out_stride)
+                                      unsigned long long out_stride, double* vmax)
 {
     using G = Cfg<LN, TYE, NS>;
     double2 qm2 = make_double2(0.0, 0.0), qm1;
@@ -124,20 +124,23 @@ __device__ __forceinline__ void march(const Ctx<LN, TYE>& C, const CUtensorMap* 
             const bool k_real = C.perz || (kk >= 0 && kk < C.nz);
             const bool do_black = own && kk - 1 >= k0 && kk - 1 < k1;
             if (h == 0)
-                fused::step<LN, TYE, REDX0>(C, s0, sm, sp, k_real && (REDX0 ? red_x_ok : red_y_ok), do_black, out, qm2, qm1, qn, azn, cA, cB);
+                fused::step<LN, TYE, REDX0, NORM>(C, s0, sm, sp, k_real && (REDX0 ? red_x_ok : red_y_ok), do_black, out, qm2, qm1, qn, azn, cA, cB, vmax);
             else
-                fused::step<LN, TYE, !REDX0>(C, s0, sm, sp, k_real && (REDX0 ? red_y_ok : red_x_ok), do_black, out, qm2, qm1, qn, azn, cB, cA);
+                fused::step<LN, TYE, !REDX0, NORM>(C, s0, sm, sp, k_real && (REDX0 ? red_y_ok : red_x_ok), do_black, out, qm2, qm1, qn, azn, cB, cA, vmax);
             out += out_stride;
             sI = sP;
         }
     }
 }
 
-template <int LN, int TYE, int NS, int MINB>
+// NORM: additionally writes, per CTA, max |rhs - L phi_in| over the red cells to part_max[linear CTA index]
+// (the stop test of the previous cycle rides on the first sweep of the next one; see maestro_mac.cu).
+template <int LN, int TYE, int NS, int MINB, bool NORM>
 __global__ void __launch_bounds__(LN * TYE, MINB)
 k_rbgs_tma(const __grid_constant__ CUtensorMap tm_phi, const __grid_constant__ CUtensorMap tm_rhs,
            const __grid_constant__ CUtensorMap tm_ax, const __grid_constant__ CUtensorMap tm_ay,
-           const __grid_constant__ CUtensorMap tm_az, LevelDev L, double* __restrict__ pout, int zchunk)
+           const __grid_constant__ CUtensorMap tm_az, LevelDev L, double* __restrict__ pout, int zchunk,
+           double* __restrict__ part_max)
 {
     using G = Cfg<LN, TYE, NS>;
     constexpr int TY = TYE - 4, kTX = 2 * LN - 4;
@@ -182,11 +185,24 @@ k_rbgs_tma(const __grid_constant__ CUtensorMap tm_phi, const __grid_constant__ C
     const bool red_y_ok = col_ok && row_red && lane <= LN - 2;
     double* out = pout + ((size_t)(x_ok ? gi : 0) + (size_t)L.nx * (own ? gj : 0)) + (long long)(ks - 1) * (long long)((size_t)L.nx * L.ny);
     const unsigned long long ostride = (unsigned long long)L.nx * L.ny;
+    double vmax = 0.0;
     if (((gj + ks) & 1) == 0)
-        march<LN, TYE, NS, true>(C, &tm_phi, &tm_rhs, &tm_ax, &tm_ay, &tm_az, stage0, bar0, producer, x0 - 2, y0 - 2, ks, k0, k1, red_x_ok, red_y_ok, own, out, ostride);
+        march<LN, TYE, NS, true, NORM>(C, &tm_phi, &tm_rhs, &tm_ax, &tm_ay, &tm_az, stage0, bar0, producer, x0 - 2, y0 - 2, ks, k0, k1, red_x_ok, red_y_ok, own, out, ostride, &vmax);
     else
-        march<LN, TYE, NS, false>(C, &tm_phi, &tm_rhs, &tm_ax, &tm_ay, &tm_az, stage0, bar0, producer, x0 - 2, y0 - 2, ks, k0, k1, red_x_ok, red_y_ok, own, out, ostride);
+        march<LN, TYE, NS, false, NORM>(C, &tm_phi, &tm_rhs, &tm_ax, &tm_ay, &tm_az, stage0, bar0, producer, x0 - 2, y0 - 2, ks, k0, k1, red_x_ok, red_y_ok, own, out, ostride, &vmax);
     // every plane that was issued (<= k1 + 1) has been waited for by the last step: nothing is in flight
+    if (NORM) {
+        __shared__ double sh_max[32];
+        const int tid = threadIdx.x + LN * threadIdx.y;
+        vmax = warp_nanmax(vmax);
+        if ((tid & 31) == 0) sh_max[tid >> 5] = vmax;
+        __syncthreads();
+        if (tid == 0) {
+            double m = sh_max[0];
+            for (int q = 1; q < (LN * TYE) / 32; ++q) m = nanmax(m, sh_max[q]);
+            part_max[blockIdx.x + gridDim.x * (blockIdx.y + gridDim.y * blockIdx.z)] = m;
+        }
+    }
 }
 
 template <int LN, int TYE, int NS> constexpr size_t smem_bytes() { return Cfg<LN, TYE, NS>::kSmem; }
@@ -200,8 +216,9 @@ struct TmaLevelMaps {                 // tensor maps of one level for one tile c
     int ok;                           // 0: level not eligible (periodic x/y, odd nx, encode failed)
 };
 
-#define MAC_TMA_BIG   32, 16, 5, 1    // 64 x 16 staged tile (60 x 12 interior), 512 threads, 1 CTA/SM
-#define MAC_TMA_MID   16, 16, 5, 2    // 32 x 16 staged tile (28 x 12 interior), 256 threads, 2 CTAs/SM
+#define MAC_TMA_BIG   32, 16, 5, 1, false    // 64 x 16 staged tile (60 x 12 interior), 512 threads, 1 CTA/SM
+#define MAC_TMA_BIGN  32, 16, 5, 1, true     // same, with the red-cell residual norm of the input
+#define MAC_TMA_MID   16, 16, 5, 2, false    // 32 x 16 staged tile (28 x 12 interior), 256 threads, 2 CTAs/SM
 
 typedef CUresult (*mac_encode_tiled_fn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
                                         const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
@@ -256,6 +273,7 @@ static inline int tma_smoother_configure()
 {
     using namespace tma;
     if (cudaFuncSetAttribute(k_rbgs_tma<MAC_TMA_BIG>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes<32, 16, 5>()) != cudaSuccess) return -1;
+    if (cudaFuncSetAttribute(k_rbgs_tma<MAC_TMA_BIGN>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes<32, 16, 5>()) != cudaSuccess) return -1;
     if (cudaFuncSetAttribute(k_rbgs_tma<MAC_TMA_MID>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes<16, 16, 5>()) != cudaSuccess) return -1;
     return 0;
 }
@@ -277,8 +295,10 @@ static inline void tma_pick_chunks(int tiles, int nz, int slots, int* nchunk_out
 }
 
 // One fused sweep through the TMA kernel: reads `in_is_phi2 ? phi2 : phi`, writes the other buffer.
+// part_max != NULL (variant 0 only): also write per-CTA maxima of the input's red-cell residual; *nparts
+// receives their count.
 static inline int launch_tma_sweep(const TmaLevelMaps& T, bool in_is_phi2, double* phi_out, const LevelDev& L, int variant,
-                                   cudaStream_t s)
+                                   cudaStream_t s, double* part_max = nullptr, int max_parts = 0, int* nparts = nullptr)
 {
     using namespace tma;
     const int LN = variant == 0 ? 32 : 16;
@@ -288,10 +308,14 @@ static inline int launch_tma_sweep(const TmaLevelMaps& T, bool in_is_phi2, doubl
     tma_pick_chunks(tiles_x * tiles_y, L.nz, variant == 0 ? 148 : 296, &nchunk, &zchunk);
     dim3 grid(tiles_x, tiles_y, nchunk);
     const CUtensorMap& tin = in_is_phi2 ? T.phi2 : T.phi;
-    if (variant == 0)
-        k_rbgs_tma<MAC_TMA_BIG><<<grid, dim3(32, 16), smem_bytes<32, 16, 5>(), s>>>(tin, T.rhs, T.ax, T.ay, T.az, L, phi_out, zchunk);
+    if (part_max) {
+        if (variant != 0 || (long)tiles_x * tiles_y * nchunk > max_parts) return -1;
+        *nparts = tiles_x * tiles_y * nchunk;
+        k_rbgs_tma<MAC_TMA_BIGN><<<grid, dim3(32, 16), smem_bytes<32, 16, 5>(), s>>>(tin, T.rhs, T.ax, T.ay, T.az, L, phi_out, zchunk, part_max);
+    } else if (variant == 0)
+        k_rbgs_tma<MAC_TMA_BIG><<<grid, dim3(32, 16), smem_bytes<32, 16, 5>(), s>>>(tin, T.rhs, T.ax, T.ay, T.az, L, phi_out, zchunk, nullptr);
     else
-        k_rbgs_tma<MAC_TMA_MID><<<grid, dim3(16, 16), smem_bytes<16, 16, 5>(), s>>>(tin, T.rhs, T.ax, T.ay, T.az, L, phi_out, zchunk);
+        k_rbgs_tma<MAC_TMA_MID><<<grid, dim3(16, 16), smem_bytes<16, 16, 5>(), s>>>(tin, T.rhs, T.ax, T.ay, T.az, L, phi_out, zchunk, nullptr);
     return cudaPeekAtLastError() == cudaSuccess ? 0 : -1;
 }
 

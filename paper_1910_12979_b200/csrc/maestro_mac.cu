@@ -185,6 +185,16 @@ GeoDev dev_geo(const maestro_mac_handle* H)
     return G;
 }
 
+GeoInv dev_geo_inv(const maestro_mac_handle* H)
+{
+    const maestro_mac_desc& d = H->d;
+    GeoInv I;
+    I.idx = 1.0 / d.dx[0]; I.idy = 1.0 / d.dx[1]; I.idz = 1.0 / d.dx[2];
+    I.idx2 = 1.0 / (d.dx[0] * d.dx[0]); I.idy2 = 1.0 / (d.dx[1] * d.dx[1]); I.idz2 = 1.0 / (d.dx[2] * d.dx[2]);
+    I.idr = 1.0 / d.dr;
+    return I;
+}
+
 // block (bx, by) with bx*by = 256 and grid covering (ex, ey, ez)
 void dims3(int ex, int ey, int ez, dim3* grid, dim3* block)
 {
@@ -206,9 +216,15 @@ int do_coefficients(maestro_mac_handle* H, const double* beta0, const double* rh
 {
     GeoDev G = dev_geo(H);
     dim3 g, b;
-    dims3(G.nx + 1, G.ny + 1, G.nz + 1, &g, &b);
     CUDA_OK(cudaMemsetAsync(H->flags, 0, 16 * sizeof(int), s));
-    k_face_coeff<<<g, b, 0, s>>>(G, dev_level(H, 0), beta0, rho, rho0, H->flags);
+    if (H->d.smoother != 1) {
+        const int zc = 16;
+        dim3 gg((G.nx + 64) / 64, (G.ny + 4) / 4, (G.nz + zc) / zc);
+        k_face_coeff2<<<gg, dim3(64, 4), 0, s>>>(G, dev_geo_inv(H), dev_level(H, 0), beta0, rho, rho0, zc, H->flags);
+    } else {
+        dims3(G.nx + 1, G.ny + 1, G.nz + 1, &g, &b);
+        k_face_coeff<<<g, b, 0, s>>>(G, dev_level(H, 0), beta0, rho, rho0, H->flags);
+    }
     LAUNCHED(H);
     for (int l = 0; l + 1 < H->nlev; ++l) {
         LevelDev C = dev_level(H, l + 1);
@@ -225,10 +241,19 @@ int do_rhs(maestro_mac_handle* H, const double* beta0, const double* u, const do
 {
     GeoDev G = dev_geo(H);
     Level& L0 = H->lev[0];
-    int rows = G.ny * G.nz;
-    int nb = red_blocks(rows);
-    int bt = G.nx >= 256 ? 256 : (G.nx >= 128 ? 128 : 64);
-    k_rhs<<<nb, bt, 0, s>>>(G, beta0, u, v, w, S, L0.rhs, H->part_sum, H->part_max);
+    int nb;
+    if (H->d.smoother != 1) {
+        int zc = 16;
+        dim3 gg((G.nx + 63) / 64, (G.ny + 3) / 4, (G.nz + zc - 1) / zc);
+        while ((long)gg.x * gg.y * gg.z > kMaxParts) { zc *= 2; gg.z = (G.nz + zc - 1) / zc; }
+        nb = (int)(gg.x * gg.y * gg.z);
+        k_rhs2<<<gg, dim3(64, 4), 0, s>>>(G, dev_geo_inv(H), beta0, u, v, w, S, L0.rhs, zc, H->part_sum, H->part_max);
+    } else {
+        int rows = G.ny * G.nz;
+        nb = red_blocks(rows);
+        int bt = G.nx >= 256 ? 256 : (G.nx >= 128 ? 128 : 64);
+        k_rhs<<<nb, bt, 0, s>>>(G, beta0, u, v, w, S, L0.rhs, H->part_sum, H->part_max);
+    }
     LAUNCHED(H);
     k_reduce_final<<<1, 1024, 0, s>>>(H->part_sum, H->part_max, nb, H->scal);
     LAUNCHED(H);
