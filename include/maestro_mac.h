@@ -84,6 +84,14 @@ typedef struct {
                                  2 = fused single pass, cp.async staging on every level;
                                  3 = fused single pass, TMA staging with the 32x16 tile.
                                  Same arithmetic, same results. */
+    int stop_test;            /* how ||rhs - L phi||inf is obtained after each cycle:
+                                 0 = default: where the level-0 TMA smoother runs (smoother 0, nu_pre >= 1,
+                                     nu_post >= 1) the test rides on the first pre-sweep of the NEXT cycle,
+                                     which evaluates the residual of its input at the red cells (after a
+                                     post-sweep the black residuals vanish up to rounding); the sweep writes
+                                     to a second buffer and is dropped when the test passes.  Elsewhere,
+                                     and after the last allowed cycle, as 1;
+                                 1 = a separate residual-norm kernel over all cells after every cycle. */
 } maestro_mac_desc;
 
 typedef struct {

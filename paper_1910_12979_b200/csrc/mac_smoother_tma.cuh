@@ -294,6 +294,18 @@ static inline void tma_pick_chunks(int tiles, int nz, int slots, int* nchunk_out
     *zchunk_out = (nz + bn - 1) / bn;
 }
 
+// grid of one TMA sweep of level L (variant 0: 64x16 tile, 1: 32x16 tile)
+static inline dim3 tma_sweep_grid(const LevelDev& L, int variant, int* zchunk_out)
+{
+    const int LN = variant == 0 ? 32 : 16;
+    const int kTX = 2 * LN - 4, TY = 12;
+    const int tiles_x = (L.nx + kTX - 1) / kTX, tiles_y = (L.ny + TY - 1) / TY;
+    int nchunk, zchunk;
+    tma_pick_chunks(tiles_x * tiles_y, L.nz, variant == 0 ? 148 : 296, &nchunk, &zchunk);
+    if (zchunk_out) *zchunk_out = zchunk;
+    return dim3(tiles_x, tiles_y, nchunk);
+}
+
 // One fused sweep through the TMA kernel: reads `in_is_phi2 ? phi2 : phi`, writes the other buffer.
 // part_max != NULL (variant 0 only): also write per-CTA maxima of the input's red-cell residual; *nparts
 // receives their count.
@@ -301,16 +313,12 @@ static inline int launch_tma_sweep(const TmaLevelMaps& T, bool in_is_phi2, doubl
                                    cudaStream_t s, double* part_max = nullptr, int max_parts = 0, int* nparts = nullptr)
 {
     using namespace tma;
-    const int LN = variant == 0 ? 32 : 16;
-    const int kTX = 2 * LN - 4, TY = 12;
-    const int tiles_x = (L.nx + kTX - 1) / kTX, tiles_y = (L.ny + TY - 1) / TY;
-    int nchunk, zchunk;
-    tma_pick_chunks(tiles_x * tiles_y, L.nz, variant == 0 ? 148 : 296, &nchunk, &zchunk);
-    dim3 grid(tiles_x, tiles_y, nchunk);
+    int zchunk;
+    const dim3 grid = tma_sweep_grid(L, variant, &zchunk);
     const CUtensorMap& tin = in_is_phi2 ? T.phi2 : T.phi;
     if (part_max) {
-        if (variant != 0 || (long)tiles_x * tiles_y * nchunk > max_parts) return -1;
-        *nparts = tiles_x * tiles_y * nchunk;
+        if (variant != 0 || (long)grid.x * grid.y * grid.z > max_parts) return -1;
+        *nparts = (int)(grid.x * grid.y * grid.z);
         k_rbgs_tma<MAC_TMA_BIGN><<<grid, dim3(32, 16), smem_bytes<32, 16, 5>(), s>>>(tin, T.rhs, T.ax, T.ay, T.az, L, phi_out, zchunk, part_max);
     } else if (variant == 0)
         k_rbgs_tma<MAC_TMA_BIG><<<grid, dim3(32, 16), smem_bytes<32, 16, 5>(), s>>>(tin, T.rhs, T.ax, T.ay, T.az, L, phi_out, zchunk, nullptr);

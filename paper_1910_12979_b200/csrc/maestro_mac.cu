@@ -19,7 +19,7 @@ namespace {
 
 constexpr int kMaxLevels = 32;
 constexpr int kRedBlocks = 148 * 8;       // blocks of the row-walking reduction kernels
-constexpr int kMaxParts = 16384;          // capacity of the partial-reduction arrays
+constexpr int kMaxParts = 131072;         // capacity of the partial-reduction arrays
 constexpr int kBottomMax = 4096;          // largest coarsest level (unknowns)
 constexpr int kSmoothEvents = 512;        // level-0 smoother launches timed per call
 
@@ -93,6 +93,7 @@ int validate_and_default(const maestro_mac_desc* in, maestro_mac_desc* d)
     if (d->prolongation != 0 && d->prolongation != 1) return MAESTRO_MAC_ERR_ARG;
     if (d->host_staging != 0 && d->host_staging != 1) return MAESTRO_MAC_ERR_ARG;
     if (d->smoother < 0 || d->smoother > 3) return MAESTRO_MAC_ERR_ARG;
+    if (d->stop_test != 0 && d->stop_test != 1) return MAESTRO_MAC_ERR_ARG;
     return MAESTRO_MAC_OK;
 }
 
@@ -269,37 +270,48 @@ int do_rhs(maestro_mac_handle* H, const double* beta0, const double* u, const do
     return MAESTRO_MAC_OK;
 }
 
-int do_smooth(maestro_mac_handle* H, int l, int nsweeps, cudaStream_t s)
+// One sweep on level l.  norm_parts != NULL (level-0 TMA path only, see fused_norm_ok): the sweep also
+// writes per-CTA maxima of the red-cell residual of its INPUT to part_max and their count to *norm_parts.
+// swap == false leaves the level's phi/phi2 roles untouched (the caller decides later; the result is in phi2).
+int do_sweep(maestro_mac_handle* H, int l, cudaStream_t s, int* norm_parts = nullptr, bool swap = true)
 {
     LevelDev L = dev_level(H, l);
+    const bool timed = l == 0 && H->sm_ev && H->sm_used < kSmoothEvents;
+    if (l == 0) ++H->sm_launches;
+    if (timed) CUDA_OK(cudaEventRecord(H->sm_ev[2 * H->sm_used], s));
+    const int sm = H->d.smoother;
+    const int tv = (sm == 0 && L.nx >= 60) ? 0 : (sm == 3 ? 1 : -1);          // TMA tile variant, or -1
+    if (tv >= 0 && H->lev[l].tma[tv].ok) {
+        int rc = launch_tma_sweep(H->lev[l].tma[tv], H->lev[l].phi != H->lev[l].phi_a, H->lev[l].phi2, L, tv, s,
+                                  norm_parts ? H->part_max : nullptr, kMaxParts, norm_parts);
+        if (rc != 0) return MAESTRO_MAC_ERR_CUDA;
+        ++H->launches;
+        if (swap) { double* t = H->lev[l].phi; H->lev[l].phi = H->lev[l].phi2; H->lev[l].phi2 = t; }
+    } else if (norm_parts) {
+        return MAESTRO_MAC_ERR_ARG;                                           // callers check fused_norm_ok first
+    } else if (sm != 1 && fused_sweep_supported(L)) {
+        int rc = launch_fused_sweep(H->lev[l].phi, H->lev[l].phi2, L, s);
+        if (rc != 0) return MAESTRO_MAC_ERR_CUDA;
+        ++H->launches;
+        // the fused sweep ping-pongs: result is in phi2; swap the level's buffers
+        if (swap) { double* t = H->lev[l].phi; H->lev[l].phi = H->lev[l].phi2; H->lev[l].phi2 = t; }
+    } else {
+        dim3 g, b;
+        dims3((L.nx + 1) / 2, L.ny, L.nz, &g, &b);
+        k_rbgs_color<<<g, b, 0, s>>>(L, 0);
+        LAUNCHED(H);
+        k_rbgs_color<<<g, b, 0, s>>>(L, 1);
+        LAUNCHED(H);
+    }
+    if (timed) { CUDA_OK(cudaEventRecord(H->sm_ev[2 * H->sm_used + 1], s)); ++H->sm_used; }
+    return MAESTRO_MAC_OK;
+}
+
+int do_smooth(maestro_mac_handle* H, int l, int nsweeps, cudaStream_t s)
+{
     for (int sw = 0; sw < nsweeps; ++sw) {
-        const bool timed = l == 0 && H->sm_ev && H->sm_used < kSmoothEvents;
-        if (l == 0) ++H->sm_launches;
-        if (timed) CUDA_OK(cudaEventRecord(H->sm_ev[2 * H->sm_used], s));
-        const int sm = H->d.smoother;
-        const int tv = (sm == 0 && L.nx >= 60) ? 0 : (sm == 3 ? 1 : -1);          // TMA tile variant, or -1
-        if (tv >= 0 && H->lev[l].tma[tv].ok) {
-            int rc = launch_tma_sweep(H->lev[l].tma[tv], H->lev[l].phi != H->lev[l].phi_a, H->lev[l].phi2, L, tv, s);
-            if (rc != 0) return MAESTRO_MAC_ERR_CUDA;
-            ++H->launches;
-            double* t = H->lev[l].phi; H->lev[l].phi = H->lev[l].phi2; H->lev[l].phi2 = t;
-            L = dev_level(H, l);
-        } else if (sm != 1 && fused_sweep_supported(L)) {
-            int rc = launch_fused_sweep(H->lev[l].phi, H->lev[l].phi2, L, s);
-            if (rc != 0) return MAESTRO_MAC_ERR_CUDA;
-            ++H->launches;
-            // the fused sweep ping-pongs: result is in phi2; swap the level's buffers
-            double* t = H->lev[l].phi; H->lev[l].phi = H->lev[l].phi2; H->lev[l].phi2 = t;
-            L = dev_level(H, l);
-        } else {
-            dim3 g, b;
-            dims3((L.nx + 1) / 2, L.ny, L.nz, &g, &b);
-            k_rbgs_color<<<g, b, 0, s>>>(L, 0);
-            LAUNCHED(H);
-            k_rbgs_color<<<g, b, 0, s>>>(L, 1);
-            LAUNCHED(H);
-        }
-        if (timed) { CUDA_OK(cudaEventRecord(H->sm_ev[2 * H->sm_used + 1], s)); ++H->sm_used; }
+        int rc = do_sweep(H, l, s);
+        if (rc != 0) return rc;
     }
     return MAESTRO_MAC_OK;
 }
@@ -356,11 +368,26 @@ int do_bottom(maestro_mac_handle* H, cudaStream_t s)
     return MAESTRO_MAC_OK;
 }
 
-int do_vcycle(maestro_mac_handle* H, cudaStream_t s)
+// The stop test can ride on the first level-0 pre-sweep of the NEXT cycle (k_rbgs_tma NORM variant): after
+// a post-sweep the black residuals are zero up to rounding (the black pass has just solved those
+// equations), so ||rhs - L phi||inf is the maximum over the red cells, which the red update has at hand.
+// The sweep writes to the ping-pong partner, so a converged phi is still intact when the test passes.
+bool fused_norm_ok(const maestro_mac_handle* H)
+{
+    const Level& L0 = H->lev[0];
+    if (H->d.stop_test != 0 || H->d.smoother != 0 || H->nlev < 2 || H->d.nu_pre < 1 || H->d.nu_post < 1) return false;
+    if (!L0.tma[0].ok || L0.n[0] < 60) return false;
+    const dim3 g = tma_sweep_grid(dev_level(H, 0), 0, nullptr);
+    return (long)g.x * g.y * g.z <= kMaxParts;
+}
+
+// first_pre_done: the first level-0 pre-sweep of this cycle has already been applied (it carried the
+// stop test of the previous cycle, see maestro_mac_project)
+int do_vcycle(maestro_mac_handle* H, cudaStream_t s, bool first_pre_done = false)
 {
     int rc;
     for (int l = 0; l + 1 < H->nlev; ++l) {
-        if ((rc = do_smooth(H, l, H->d.nu_pre, s)) != 0) return rc;
+        if ((rc = do_smooth(H, l, H->d.nu_pre - ((l == 0 && first_pre_done) ? 1 : 0), s)) != 0) return rc;
         if ((rc = do_residual_restrict(H, l, s)) != 0) return rc;
     }
     if ((rc = do_bottom(H, s)) != 0) return rc;
@@ -535,9 +562,18 @@ extern "C" int maestro_mac_project(maestro_mac_handle* H, const double* beta0, c
     if (!trivial) {
         result = d.rel_tol > 0.0 ? MAESTRO_MAC_NOT_CONVERGED : MAESTRO_MAC_OK;
         if (d.rel_tol > 0.0) {
+            const bool ride = fused_norm_ok(H);
+            bool first_pre_done = false;
             while (st.cycles < d.max_cycles) {
-                if ((rc = do_vcycle(H, s)) != 0) return rc;
-                if ((rc = do_residual_norm(H, 0, s)) != 0) return rc;
+                if ((rc = do_vcycle(H, s, first_pre_done)) != 0) return rc;
+                first_pre_done = false;
+                const bool spec = ride && st.cycles + 1 < d.max_cycles;   // speculative first sweep of the next cycle
+                if (spec) {
+                    int nparts = 0;
+                    if ((rc = do_sweep(H, 0, s, &nparts, false)) != 0) return rc;
+                    k_reduce_final<<<1, 1024, 0, s>>>(H->part_sum, H->part_max, nparts, H->scal + 3);
+                    LAUNCHED(H);
+                } else if ((rc = do_residual_norm(H, 0, s)) != 0) return rc;
                 CUDA_OK(cudaMemcpyAsync(H->host_scal + 4, H->scal + 4, sizeof(double), cudaMemcpyDeviceToHost, s));
                 CUDA_OK(cudaStreamSynchronize(s));
                 st.res_norm_inf = H->host_scal[4];
@@ -545,7 +581,11 @@ extern "C" int maestro_mac_project(maestro_mac_handle* H, const double* beta0, c
                 if (st.cycles < 128) st.res_history[st.cycles] = rel;
                 ++st.cycles;
                 if (rel != rel) { result = MAESTRO_MAC_ERR_NONFINITE; break; }
-                if (rel <= d.rel_tol) { result = MAESTRO_MAC_OK; break; }
+                if (rel <= d.rel_tol) { result = MAESTRO_MAC_OK; break; }   // (a speculative sweep's output is dropped)
+                if (spec) {                                                  // keep it: it is the next cycle's first pre-sweep
+                    double* t = L0.phi; L0.phi = L0.phi2; L0.phi2 = t;
+                    first_pre_done = true;
+                }
             }
         } else {
             for (; st.cycles < d.max_cycles; ++st.cycles)

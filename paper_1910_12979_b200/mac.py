@@ -35,7 +35,8 @@ class Desc(C.Structure):
                 ("center", C.c_double * 3), ("nu_pre", C.c_int), ("nu_post", C.c_int),
                 ("max_cycles", C.c_int), ("rel_tol", C.c_double), ("coarsest_n", C.c_int),
                 ("bottom_max_iter", C.c_int), ("bottom_rel_tol", C.c_double),
-                ("prolongation", C.c_int), ("host_staging", C.c_int), ("smoother", C.c_int)]
+                ("prolongation", C.c_int), ("host_staging", C.c_int), ("smoother", C.c_int),
+                ("stop_test", C.c_int)]
 
 
 class Stats(C.Structure):
@@ -105,7 +106,7 @@ class MacError(RuntimeError):
 def make_desc(n, dx, bc_lo, bc_hi, geometry=PLANAR, nr=None, dr=None, center=(0.0, 0.0, 0.0),
               nu_pre=2, nu_post=2, max_cycles=100, rel_tol=1e-10, coarsest_n=4,
               bottom_max_iter=100, bottom_rel_tol=1e-8, prolongation=0, host_staging=0,
-              smoother=0) -> Desc:
+              smoother=0, stop_test=0) -> Desc:
     d = Desc()
     lib().maestro_mac_default_desc(C.byref(d))
     d.nx, d.ny, d.nz = (int(x) for x in n)
@@ -117,6 +118,7 @@ def make_desc(n, dx, bc_lo, bc_hi, geometry=PLANAR, nr=None, dr=None, center=(0.
     d.nu_pre, d.nu_post, d.max_cycles, d.rel_tol = int(nu_pre), int(nu_post), int(max_cycles), float(rel_tol)
     d.coarsest_n, d.bottom_max_iter, d.bottom_rel_tol = int(coarsest_n), int(bottom_max_iter), float(bottom_rel_tol)
     d.prolongation, d.host_staging, d.smoother = int(prolongation), int(host_staging), int(smoother)
+    d.stop_test = int(stop_test)
     return d
 
 

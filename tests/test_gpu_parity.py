@@ -275,3 +275,23 @@ def test_deterministic_across_runs(mac):
     a, b = gpu_project(mac, wl), gpu_project(mac, wl)
     for key in ("phi", "u", "v", "w"):
         assert np.array_equal(a[key], b[key])
+
+
+@pytest.mark.parametrize("name,N", [("4D", 64), ("3N", 64), ("mixed_wide", 0)])
+def test_stop_test_riding_on_the_next_sweep(oracle, mac, name, N):
+    """stop_test 0 (red-cell residual from the next cycle's first pre-sweep) and 1 (separate kernel over all
+    cells) take the same decisions and leave bit-identical results: the speculative sweep is either the next
+    cycle's first pre-sweep or dropped."""
+    wl = (W.mixed_bc_case(n=(128, 80, 96), bc_lo=(WALL, OUT, OUT), bc_hi=(OUT, WALL, WALL), geometry=W.SPHERICAL, seed=15)
+          if name == "mixed_wide" else W.by_name(name, N))
+    a, b = gpu_project(mac, wl, stop_test=0), gpu_project(mac, wl, stop_test=1)
+    assert a["status"] == b["status"] == 0
+    assert a["stats"]["cycles"] == b["stats"]["cycles"]
+    assert a["stats"]["gpu_launches"] < b["stats"]["gpu_launches"]        # the riding test is actually in use
+    for key in ("phi", "u", "v", "w"):
+        assert np.array_equal(a[key], b[key]), key
+    # black residuals are at rounding level after a post-sweep: the two norms agree far above it
+    assert np.allclose(a["stats"]["res_history"], b["stats"]["res_history"], rtol=1e-4)
+    ref = oracle_project(oracle, wl)
+    assert ref["stats"]["cycles"] == a["stats"]["cycles"]
+    assert np.allclose(a["stats"]["res_history"], ref["stats"]["res_history"], rtol=1e-3)
