@@ -145,8 +145,9 @@ k_rbgs_tma(const __grid_constant__ CUtensorMap tm_phi, const __grid_constant__ C
     using G = Cfg<LN, TYE, NS>;
     constexpr int TY = TYE - 4, kTX = 2 * LN - 4;
     extern __shared__ __align__(128) unsigned char smem_dyn[];
-    // stages need 128-byte alignment for TMA; the dynamic segment is at least 16-byte aligned
-    unsigned char* smem_raw = reinterpret_cast<unsigned char*>((reinterpret_cast<uintptr_t>(smem_dyn) + 127) & ~(uintptr_t)127);
+    // stages need 128-byte alignment for TMA; the dynamic segment is at least 16-byte aligned.  (Pointer
+    // arithmetic on the __shared__ array, not an integer round trip: the accesses must stay LDS/STS.)
+    unsigned char* smem_raw = smem_dyn + ((128u - (smem_u32(smem_dyn) & 127u)) & 127u);
     const unsigned stage0 = smem_u32(smem_raw);
     const unsigned bar0 = stage0 + NS * G::kStage;
 
@@ -354,7 +355,7 @@ k_resid_tma(const __grid_constant__ CUtensorMap tm_phi, const __grid_constant__ 
     using G = Cfg<LN, TYE, NS>;
     constexpr int kTX = 60, kTY = 14;
     extern __shared__ __align__(128) unsigned char smem_dyn[];
-    unsigned char* smem_raw = reinterpret_cast<unsigned char*>((reinterpret_cast<uintptr_t>(smem_dyn) + 127) & ~(uintptr_t)127);
+    unsigned char* smem_raw = smem_dyn + ((128u - (smem_u32(smem_dyn) & 127u)) & 127u);
     const unsigned stage0 = smem_u32(smem_raw);
     const unsigned bar0 = stage0 + NS * G::kStage;
     __shared__ double sh_max[8];
