@@ -164,9 +164,9 @@ __device__ __forceinline__ double beta_at(const GeoDev& G, const double* __restr
 }
 
 __global__ void __launch_bounds__(256)
-k_rhs(GeoDev G, const double* __restrict__ beta0, const double* __restrict__ u,
+k_rhs(GeoDev G, LevelDev L, const double* __restrict__ beta0, const double* __restrict__ u,
       const double* __restrict__ v, const double* __restrict__ w, const double* __restrict__ S,
-      double* __restrict__ rhs, double* __restrict__ part_sum, double* __restrict__ part_max)
+      double* __restrict__ part_sum, double* __restrict__ part_max)
 {
     const int nrows = G.ny * G.nz;
     const bool px = G.bclo[0] == MAC_PERIODIC, py = G.bclo[1] == MAC_PERIODIC, pz = G.bclo[2] == MAC_PERIODIC;
@@ -189,7 +189,7 @@ k_rhs(GeoDev G, const double* __restrict__ beta0, const double* __restrict__ u,
             double r = (fxh - fxl) / G.dx + (fyh - fyl) / G.dy + (fzh - fzl) / G.dz;
             const size_t c = (size_t)i + (size_t)G.nx * ((size_t)j + (size_t)G.ny * k);
             if (S) r -= beta_at(G, beta0, xc, yc, zc) * S[c];
-            rhs[c] = r;
+            L.rhs[cidx(L, i, j, k)] = r;
             s += r;
             m = nanmax(m, fabs(r));
         }
@@ -197,32 +197,82 @@ k_rhs(GeoDev G, const double* __restrict__ beta0, const double* __restrict__ u,
     block_reduce_store(s, m, part_sum, part_max, blockIdx.x);
 }
 
-// a -= scal[0]/count  (mean removal), with partial sum / max of the shifted values
+// a -= scal[0]/count  (mean removal) over the interior of a cell array of level L, with partial sum / max of
+// the shifted values.  Blocks walk rows (j,k) grid-stride; threads walk i.
 __global__ void __launch_bounds__(256)
-k_shift_mean(double* __restrict__ a, size_t n, const double* __restrict__ scal, double inv_count,
+k_shift_mean(LevelDev L, double* __restrict__ a, const double* __restrict__ scal, double inv_count,
              double* __restrict__ part_sum, double* __restrict__ part_max)
 {
     const double c = scal[0] * inv_count;
+    const int nrows = L.ny * L.nz;
     double s = 0.0, m = 0.0;
-    for (size_t q = (size_t)blockIdx.x * blockDim.x + threadIdx.x; q < n; q += (size_t)gridDim.x * blockDim.x) {
-        double v = a[q] - c;
-        a[q] = v;
-        s += v;
-        m = nanmax(m, fabs(v));
+    for (int row = blockIdx.x; row < nrows; row += gridDim.x) {
+        double* __restrict__ p = a + cidx(L, 0, row % L.ny, row / L.ny);
+        for (int i = threadIdx.x; i < L.nx; i += blockDim.x) {
+            double v = p[i] - c;
+            p[i] = v;
+            s += v;
+            m = nanmax(m, fabs(v));
+        }
     }
     block_reduce_store(s, m, part_sum, part_max, blockIdx.x);
 }
 
 __global__ void __launch_bounds__(256)
-k_sum(const double* __restrict__ a, size_t n, double* __restrict__ part_sum, double* __restrict__ part_max)
+k_sum(LevelDev L, const double* __restrict__ a, double* __restrict__ part_sum, double* __restrict__ part_max)
 {
+    const int nrows = L.ny * L.nz;
     double s = 0.0, m = 0.0;
-    for (size_t q = (size_t)blockIdx.x * blockDim.x + threadIdx.x; q < n; q += (size_t)gridDim.x * blockDim.x) {
-        double v = a[q];
-        s += v;
-        m = nanmax(m, fabs(v));
+    for (int row = blockIdx.x; row < nrows; row += gridDim.x) {
+        const double* __restrict__ p = a + cidx(L, 0, row % L.ny, row / L.ny);
+        for (int i = threadIdx.x; i < L.nx; i += blockDim.x) {
+            double v = p[i];
+            s += v;
+            m = nanmax(m, fabs(v));
+        }
     }
     block_reduce_store(s, m, part_sum, part_max, blockIdx.x);
+}
+
+// Periodic images of a ghosted level (mac_common.cuh "Ghosts"): every ghost element of the selected arrays
+// := its interior image.  One thread per ghost element of a plane; blockIdx.y = plane.
+//   which bit 0: phi, 1: rhs, 2: ax, 3: ay, 4: az
+__device__ __forceinline__ void fill_one(double* __restrict__ a, int pitch, int rows, int nxe, int nye, int nx, int ny,
+                                         int gx, int gy, int k, int t)
+{
+    // the array holds nxe x nye own entries per plane (cells: nx x ny; ax: nx+1; ay: ny+1) plus ghosts
+    const int ncol = 2 * gx, wrows = nye + 2 * gy;
+    int i, j;
+    if (t < ncol * wrows) {                       // ghost columns, all rows (corners included)
+        const int c = t % ncol;
+        j = t / ncol - gy;
+        i = c < gx ? c - gx : nxe + (c - gx);
+    } else {                                      // ghost rows, own columns
+        t -= ncol * wrows;
+        if (t >= 2 * gy * nxe) return;
+        const int r = t / nxe;
+        i = t % nxe;
+        j = r < gy ? r - gy : nye + (r - gy);
+    }
+    int si = i, sj = j;
+    if (si < 0) si += nx; else if (si >= nxe) si -= nx;
+    if (sj < 0) sj += ny; else if (sj >= nye) sj -= ny;
+    const long long plane = (long long)pitch * rows * k;
+    a[plane + (long long)j * pitch + i] = a[plane + (long long)sj * pitch + si];
+}
+
+__global__ void __launch_bounds__(256)
+k_fill_ghosts(LevelDev L, int which)
+{
+    const int t = blockIdx.x * blockDim.x + threadIdx.x;
+    const int k = blockIdx.y;
+    if (k < L.nz) {
+        if (which & 1) fill_one(L.phi, L.cx, L.ry, L.nx, L.ny, L.nx, L.ny, L.gx, L.gy, k, t);
+        if (which & 2) fill_one(L.rhs, L.cx, L.ry, L.nx, L.ny, L.nx, L.ny, L.gx, L.gy, k, t);
+        if (which & 4) fill_one(L.ax, L.px, L.ry, L.nx + 1, L.ny, L.nx, L.ny, L.gx, L.gy, k, t);
+        if (which & 8) fill_one(L.ay, L.cx, L.ry + 1, L.nx, L.ny + 1, L.nx, L.ny, L.gx, L.gy, k, t);
+    }
+    if (which & 16) fill_one(L.az, L.cx, L.ry, L.nx, L.ny, L.nx, L.ny, L.gx, L.gy, k, t);   // nz + 1 planes
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -304,8 +354,9 @@ k_residual_restrict(LevelDev F, LevelDev C)
                 s += F.rhs[c] - (off - F.phi[c] * dg);
             }
     const size_t cc = cidx(C, I, J, K);
-    C.rhs[cc] = 0.125 * s;
-    C.phi[cc] = 0.0;
+    const long long ix = image_dx(C, I), iy = image_dy(C, J);
+    store_images(C.rhs + cc, 0.125 * s, ix, iy);
+    store_images(C.phi + cc, 0.0, ix, iy);
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -352,7 +403,8 @@ k_prolong_add(LevelDev F, LevelDev C, int prolongation)
               wz1 * (wy0 * (wx0 * e[cidx(C, I, J, K2)] + wx1 * e[cidx(C, I2, J, K2)]) +
                      wy1 * (wx0 * e[cidx(C, I, J2, K2)] + wx1 * e[cidx(C, I2, J2, K2)]));
     }
-    F.phi[cidx(F, i, j, k)] += val;
+    double* p = F.phi + cidx(F, i, j, k);
+    store_images(p, *p + val, image_dx(F, i), image_dy(F, j));
 }
 
 // a7, bandwidth form: one thread per COARSE cell adds the interpolant to its 8 children.  The 27
@@ -390,7 +442,7 @@ k_prolong_add2(LevelDev F, LevelDev C, int prolongation)
         for (int dz = 0; dz < 3; ++dz)
 #pragma unroll
             for (int dy = 0; dy < 3; ++dy) {
-                const size_t row = (size_t)C.nx * ((size_t)jy[dy] + (size_t)C.ny * (size_t)kz[dz]);
+                const size_t row = cidx(C, 0, jy[dy], kz[dz]);
                 const double c0 = e[row + ix[1]], cm = e[row + ix[0]], cp = e[row + ix[2]];
                 xi[dz][dy][0] = 0.75 * c0 + wx[0] * cm;
                 xi[dz][dy][1] = 0.75 * c0 + wx[2] * cp;
@@ -418,7 +470,7 @@ k_prolong_add2(LevelDev F, LevelDev C, int prolongation)
             double2 v = *p;
             v.x += out[dk][dj][0];
             v.y += out[dk][dj][1];
-            *p = v;
+            store_images(p, v, image_dx(F, 2 * I), image_dy(F, 2 * J + dj));
         }
 }
 
@@ -583,7 +635,7 @@ k_bottom_bicgstab(LevelDev L, double* __restrict__ vecs, int maxit, double tol, 
 // ------------------------------------------------------------------------------------------------
 
 template <int D>
-__device__ __forceinline__ void correct_face(const GeoDev& G, const double* __restrict__ phi,
+__device__ __forceinline__ void correct_face(const GeoDev& G, const LevelDev& L, const double* __restrict__ phi,
                                              const double* __restrict__ rho, const double* __restrict__ rho0,
                                              double* __restrict__ vel, int i, int j, int k)
 {
@@ -603,9 +655,7 @@ __device__ __forceinline__ void correct_face(const GeoDev& G, const double* __re
         if (G.bchi[D] == MAC_WALL) return;
         hi = n - 1; ghi = -1.0;
     }
-    auto cell = [&](int q) -> size_t {
-        return (size_t)(D == 0 ? q : i) + (size_t)G.nx * ((size_t)(D == 1 ? q : j) + (size_t)G.ny * (size_t)(D == 2 ? q : k));
-    };
+    auto cell = [&](int q) -> size_t { return cidx(L, D == 0 ? q : i, D == 1 ? q : j, D == 2 ? q : k); };
     const double grad = (ghi * phi[cell(hi)] - glo * phi[cell(lo)]) * (1.0 / h);
     const double rf = 0.5 * (rho_cell(G, rho, rho0, D == 0 ? lo : i, D == 1 ? lo : j, D == 2 ? lo : k) +
                              rho_cell(G, rho, rho0, D == 0 ? hi : i, D == 1 ? hi : j, D == 2 ? hi : k));
@@ -618,7 +668,7 @@ __device__ __forceinline__ void correct_face(const GeoDev& G, const double* __re
 }
 
 __global__ void __launch_bounds__(256)
-k_correct(GeoDev G, const double* __restrict__ phi, const double* __restrict__ rho,
+k_correct(GeoDev G, LevelDev L, const double* __restrict__ phi, const double* __restrict__ rho,
           const double* __restrict__ rho0, double* __restrict__ u, double* __restrict__ v,
           double* __restrict__ w)
 {
@@ -627,24 +677,26 @@ k_correct(GeoDev G, const double* __restrict__ phi, const double* __restrict__ r
     int k = blockIdx.z;
     if (i > G.nx || j > G.ny) return;
     const bool ci = i < G.nx, cj = j < G.ny, ck = k < G.nz;
-    if (cj && ck) correct_face<0>(G, phi, rho, rho0, u, i, j, k);
-    if (ci && ck) correct_face<1>(G, phi, rho, rho0, v, i, j, k);
-    if (ci && cj) correct_face<2>(G, phi, rho, rho0, w, i, j, k);
+    if (cj && ck) correct_face<0>(G, L, phi, rho, rho0, u, i, j, k);
+    if (ci && ck) correct_face<1>(G, L, phi, rho, rho0, v, i, j, k);
+    if (ci && cj) correct_face<2>(G, L, phi, rho, rho0, w, i, j, k);
 }
 
 // ------------------------------------------------------------------------------------------------
 // layout conversion for the step API: public face layout <-> internal (pitched) ax
 // ------------------------------------------------------------------------------------------------
 
-__global__ void k_copy_ax(LevelDev L, double* pub, int to_public)
+// which: 0 cell array `a` (phi or rhs), 2 ax, 3 ay, 4 az;  extents of the public array (ex, ey, ez)
+__global__ void k_copy_level(LevelDev L, double* a, double* pub, int which, int ex, int ey, int ez, int to_public)
 {
     int i = blockIdx.x * blockDim.x + threadIdx.x;
     int j = blockIdx.y * blockDim.y + threadIdx.y;
     int k = blockIdx.z;
-    if (i > L.nx || j >= L.ny) return;
-    size_t a = axidx(L, i, j, k), b = (size_t)i + (size_t)(L.nx + 1) * ((size_t)j + (size_t)L.ny * k);
-    if (to_public) pub[b] = L.ax[a];
-    else L.ax[a] = pub[b];
+    if (i >= ex || j >= ey || k >= ez) return;
+    const size_t q = which == 2 ? axidx(L, i, j, k) : (which == 3 ? ayidx(L, i, j, k) : cidx(L, i, j, k));
+    const size_t b = (size_t)i + (size_t)ex * ((size_t)j + (size_t)ey * k);
+    if (to_public) pub[b] = a[q];
+    else a[q] = pub[b];
 }
 
 // ================================================================================================
@@ -672,8 +724,8 @@ __device__ __forceinline__ double beta_inv(const GeoDev& G, const GeoInv& I, con
 
 // a4: rhs = D(beta0 U_edge) - beta0 S with partial sum / max.  grid (ceil(nx/64), ceil(ny/4), chunks), block (64, 4)
 __global__ void __launch_bounds__(256)
-k_rhs2(GeoDev G, GeoInv I, const double* __restrict__ beta0, const double* __restrict__ u, const double* __restrict__ v,
-       const double* __restrict__ w, const double* __restrict__ S, double* __restrict__ rhs, int zchunk,
+k_rhs2(GeoDev G, GeoInv I, LevelDev L, const double* __restrict__ beta0, const double* __restrict__ u, const double* __restrict__ v,
+       const double* __restrict__ w, const double* __restrict__ S, int zchunk,
        double* __restrict__ part_sum, double* __restrict__ part_max)
 {
     const int i = blockIdx.x * 64 + threadIdx.x, j = blockIdx.y * 4 + threadIdx.y;
@@ -705,7 +757,7 @@ k_rhs2(GeoDev G, GeoInv I, const double* __restrict__ beta0, const double* __res
         double r = (fxh - fxl) * I.idx + (fyh - fyl) * I.idy + (fzh - fzl) * I.idz;
         if (S) r -= beta_inv(G, I, beta0, xc, yc, zc) * __ldg(S + c0 + sc * k);
         if (in) {
-            rhs[c0 + sc * k] = r;
+            L.rhs[cidx(L, ic, jc, k)] = r;
             s += r;
             m = nanmax(m, fabs(r));
         }

@@ -84,6 +84,9 @@ struct Ctx {
     unsigned long long s_c, s_ax, s_ay;                    // plane strides in bytes
     int b_phi, b_co, b_ax, b_ay;                           // 16 if the lateral slot is loaded, else 0
     int nz, perz;
+    long long img_x, img_y;                                // offsets (doubles) of the periodic images of the own pair, 0 = none
+    bool own;                                              // the pair is one this CTA stores (NORM counts only those: ring
+                                                           // cells are duplicates, and outermost ghost reds are not valid)
     unsigned smem_u32;                                     // shared address of stage 0 + own slot
     unsigned char* smem_gen;                               // generic address of stage 0 + own slot
 };
@@ -148,7 +151,7 @@ __device__ __forceinline__ void step(const Ctx<LN, TYE>& C, unsigned char* s0, c
         const double off = axw * w_ + axe * e_ + ays * s_ + ayn * n_ + azd * d_ + azu * u_;
         const double dg = ((axw + axe) + (ays + ayn)) + (azd + azu);
         const double nv = gs_div(off - pick<REDX>(CUR.rhs), dg);
-        if (NORM) *vmax = nanmax(*vmax, fabs(pick<REDX>(CUR.rhs) - (off - pick<REDX>(q0) * dg)));
+        if (NORM && C.own) *vmax = nanmax(*vmax, fabs(pick<REDX>(CUR.rhs) - (off - pick<REDX>(q0) * dg)));
         put<REDX>(q0, nv);
         *reinterpret_cast<double*>(s0 + A_PHI * Ctx<LN, TYE>::kArr + (REDX ? 0 : 8)) = nv;
     }
@@ -164,7 +167,7 @@ __device__ __forceinline__ void step(const Ctx<LN, TYE>& C, unsigned char* s0, c
         const double off = axw * w_ + axe * e_ + ays * s_ + ayn * n_ + azd * d_ + azu * u_;
         const double dg = ((axw + axe) + (ays + ayn)) + (azd + azu);
         put<REDX>(qm1, gs_div(off - pick<REDX>(PRV.rhs), dg));
-        *reinterpret_cast<double2*>(out_km1) = qm1;
+        store_images(reinterpret_cast<double2*>(out_km1), qm1, C.img_x, C.img_y);
     }
     qm2 = qm1;
     qm1 = q0;
@@ -240,6 +243,7 @@ k_rbgs_fused(LevelDev L, const double* __restrict__ pin, double* __restrict__ po
                      gi >= 0 && gi < L.nx && gi < x0 + kTX && gj >= 0 && gj < L.ny && gj < y0 + TY;
 
     Ctx<LN, TYE> C;
+    // (this kernel wraps by index and runs on levels without ghost columns / rows: cx == nx, ry == ny)
     const size_t lat = col_ok ? (size_t)wi + (size_t)L.nx * wj : 0;
     C.g_phi = reinterpret_cast<const unsigned char*>(pin + lat);
     C.g_rhs = reinterpret_cast<const unsigned char*>(L.rhs + lat);
@@ -259,6 +263,8 @@ k_rbgs_fused(LevelDev L, const double* __restrict__ pin, double* __restrict__ po
     C.b_ax = ax_ok ? 16 : 0;
     C.nz = L.nz;
     C.perz = L.bclo[2] == MAC_PERIODIC;
+    C.img_x = C.img_y = 0;
+    C.own = own;
     const unsigned slot = (ty * kLanes + lane) * 16;
     C.smem_gen = smem_raw + slot;
     C.smem_u32 = (unsigned)__cvta_generic_to_shared(smem_raw) + slot;
@@ -285,7 +291,7 @@ template <int LN, int TYE> constexpr size_t smem_bytes() { return (size_t)Ctx<LN
 
 static inline bool fused_sweep_supported(const LevelDev& L)
 {
-    return (L.nx % 2) == 0 && L.nx >= 2;
+    return (L.nx % 2) == 0 && L.nx >= 2 && L.gx == 0 && L.gy == 0;
 }
 
 // Tile configurations: <pairs per row, rows incl. halo, min CTAs per SM>.

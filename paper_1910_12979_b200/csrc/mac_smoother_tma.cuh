@@ -159,18 +159,24 @@ k_rbgs_tma(const __grid_constant__ CUtensorMap tm_phi, const __grid_constant__ C
     const int x0 = blockIdx.x * kTX, y0 = blockIdx.y * TY;
     const int k0 = blockIdx.z * zchunk, k1 = min(k0 + zchunk, L.nz);
     const int gi = x0 - 2 + 2 * lane, gj = y0 - 2 + ty;
-    const bool x_ok = gi >= 0 && gi < L.nx, y_ok = gj >= 0 && gj < L.ny;
+    // ghost columns / rows of a periodic level hold valid images: their reds are recomputed like any halo
+    const bool x_ok = gi >= -L.gx && gi < L.nx + L.gx, y_ok = gj >= -L.gy && gj < L.ny + L.gy;
     const bool col_ok = x_ok && y_ok;
     const bool row_red = ty >= 1 && ty <= TYE - 2;
-    const bool own = col_ok && lane >= 1 && lane <= LN - 2 && ty >= 2 && ty <= TYE - 3 && gi < x0 + kTX && gj < y0 + TY;
+    const bool own = lane >= 1 && lane <= LN - 2 && ty >= 2 && ty <= TYE - 3 && gi < x0 + kTX && gj < y0 + TY &&
+                     gi < L.nx && gj < L.ny;                           // (gi >= x0 >= 0, gj >= y0 >= 0 for these threads)
     const bool producer = threadIdx.x == 0 && threadIdx.y == 0;
 
     Ctx<LN, TYE> C;
     C.nz = L.nz;
     C.perz = L.bclo[2] == MAC_PERIODIC;
+    C.own = own;
+    C.img_x = own ? image_dx(L, gi) : 0;
+    C.img_y = own ? image_dy(L, gj) : 0;
     const unsigned slot = (ty * LN + lane) * 16;
     C.smem_gen = smem_raw + slot;
     C.smem_u32 = stage0 + slot;
+    const int cx0 = x0 - 2 + L.gx, cy0 = y0 - 2 + L.gy;          // tensor-map coordinates of the tile origin
 
     const int ks = k0 - 1;
     if (producer) {
@@ -178,19 +184,19 @@ k_rbgs_tma(const __grid_constant__ CUtensorMap tm_phi, const __grid_constant__ C
         asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
         asm volatile("fence.proxy.async.shared::cta;\n" ::: "memory");
         for (int q = 0; q < NS - 1 && ks - 1 + q <= k1 + 1; ++q)
-            issue_plane<LN, TYE, NS>(&tm_phi, &tm_rhs, &tm_ax, &tm_ay, &tm_az, stage0, bar0, q, ks - 1 + q, L.nz, C.perz, x0 - 2, y0 - 2);
+            issue_plane<LN, TYE, NS>(&tm_phi, &tm_rhs, &tm_ax, &tm_ay, &tm_az, stage0, bar0, q, ks - 1 + q, L.nz, C.perz, cx0, cy0);
     }
     __syncthreads();                                             // barrier inits visible before anyone waits
 
     const bool red_x_ok = col_ok && row_red && lane >= 1;
     const bool red_y_ok = col_ok && row_red && lane <= LN - 2;
-    double* out = pout + ((size_t)(x_ok ? gi : 0) + (size_t)L.nx * (own ? gj : 0)) + (long long)(ks - 1) * (long long)((size_t)L.nx * L.ny);
-    const unsigned long long ostride = (unsigned long long)L.nx * L.ny;
+    const unsigned long long ostride = (unsigned long long)L.cx * L.ry;
+    double* out = pout + (own ? (long long)gi + (long long)L.cx * gj : 0) + (long long)(ks - 1) * (long long)ostride;
     double vmax = 0.0;
     if (((gj + ks) & 1) == 0)
-        march<LN, TYE, NS, true, NORM>(C, &tm_phi, &tm_rhs, &tm_ax, &tm_ay, &tm_az, stage0, bar0, producer, x0 - 2, y0 - 2, ks, k0, k1, red_x_ok, red_y_ok, own, out, ostride, &vmax);
+        march<LN, TYE, NS, true, NORM>(C, &tm_phi, &tm_rhs, &tm_ax, &tm_ay, &tm_az, stage0, bar0, producer, cx0, cy0, ks, k0, k1, red_x_ok, red_y_ok, own, out, ostride, &vmax);
     else
-        march<LN, TYE, NS, false, NORM>(C, &tm_phi, &tm_rhs, &tm_ax, &tm_ay, &tm_az, stage0, bar0, producer, x0 - 2, y0 - 2, ks, k0, k1, red_x_ok, red_y_ok, own, out, ostride, &vmax);
+        march<LN, TYE, NS, false, NORM>(C, &tm_phi, &tm_rhs, &tm_ax, &tm_ay, &tm_az, stage0, bar0, producer, cx0, cy0, ks, k0, k1, red_x_ok, red_y_ok, own, out, ostride, &vmax);
     // every plane that was issued (<= k1 + 1) has been waited for by the last step: nothing is in flight
     if (NORM) {
         __shared__ double sh_max[32];
@@ -240,6 +246,8 @@ static inline mac_encode_tiled_fn tma_encode_fn()
     return fn;
 }
 
+// 3-D map over an array whose allocation starts at `base` (ghost origin): d0 x d1 x d2 entries, row pitch
+// pitch0 (elements), rows_per_plane rows between planes
 static inline bool tma_encode3(CUtensorMap* m, const double* base, uint64_t d0, uint64_t d1, uint64_t d2,
                                uint64_t pitch0_elems, uint64_t rows_per_plane, uint32_t b0, uint32_t b1)
 {
@@ -253,19 +261,23 @@ static inline bool tma_encode3(CUtensorMap* m, const double* base, uint64_t d0, 
               CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
-// Build the maps of a level for a staged tile of 2*LN x TYE cells.  Returns ok.
+// Build the maps of a level for a staged tile of 2*LN x TYE cells.  Returns ok.  Coordinate (0, 0) of every
+// map is the ghost origin (-gx, -gy); kernels add (gx, gy) to their tile origins.  Out-of-range box elements
+// are zero-filled, which is the "phi = 0, a_f = 0 outside the domain" convention on non-periodic sides.
 static inline int tma_build_maps(TmaLevelMaps* T, const LevelDev& L, int LN, int TYE)
 {
     T->ok = 0;
-    if (L.bclo[0] == MAC_PERIODIC || L.bclo[1] == MAC_PERIODIC) return 0;
+    if ((L.bclo[0] == MAC_PERIODIC && L.gx == 0) || (L.bclo[1] == MAC_PERIODIC && L.gy == 0)) return 0;   // cannot wrap
     if ((L.nx & 1) || L.nx < 2 || (L.px & 1)) return 0;
     const uint32_t bx = 2u * LN;
-    bool ok = tma_encode3(&T->phi, L.phi, L.nx, L.ny, L.nz, L.nx, L.ny, bx, TYE) &&
-              tma_encode3(&T->phi2, L.phi2, L.nx, L.ny, L.nz, L.nx, L.ny, bx, TYE) &&
-              tma_encode3(&T->rhs, L.rhs, L.nx, L.ny, L.nz, L.nx, L.ny, bx, TYE - 2) &&
-              tma_encode3(&T->ax, L.ax, (uint64_t)L.nx + 1, L.ny, L.nz, L.px, L.ny, bx, TYE - 2) &&
-              tma_encode3(&T->az, L.az, L.nx, L.ny, (uint64_t)L.nz + 1, L.nx, L.ny, bx, TYE - 2) &&
-              tma_encode3(&T->ay, L.ay, L.nx, (uint64_t)L.ny + 1, L.nz, L.nx, (uint64_t)L.ny + 1, bx, TYE - 1);
+    const uint64_t ex = (uint64_t)L.nx + 2 * L.gx, ey = (uint64_t)L.ny + 2 * L.gy;
+    const long long oc = (long long)L.gx + (long long)L.cx * L.gy, oa = (long long)L.gx + (long long)L.px * L.gy;
+    bool ok = tma_encode3(&T->phi, L.phi - oc, ex, ey, L.nz, L.cx, L.ry, bx, TYE) &&
+              tma_encode3(&T->phi2, L.phi2 - oc, ex, ey, L.nz, L.cx, L.ry, bx, TYE) &&
+              tma_encode3(&T->rhs, L.rhs - oc, ex, ey, L.nz, L.cx, L.ry, bx, TYE - 2) &&
+              tma_encode3(&T->ax, L.ax - oa, ex + 1, ey, L.nz, L.px, L.ry, bx, TYE - 2) &&
+              tma_encode3(&T->az, L.az - oc, ex, ey, (uint64_t)L.nz + 1, L.cx, L.ry, bx, TYE - 2) &&
+              tma_encode3(&T->ay, L.ay - oc, ex, ey + 1, L.nz, L.cx, (uint64_t)L.ry + 1, bx, TYE - 1);
     T->ok = ok ? 1 : 0;
     return T->ok;
 }
@@ -348,8 +360,7 @@ template <int NS, int MODE>
 __global__ void __launch_bounds__(32 * 7, 1)
 k_resid_tma(const __grid_constant__ CUtensorMap tm_phi, const __grid_constant__ CUtensorMap tm_rhs,
             const __grid_constant__ CUtensorMap tm_ax, const __grid_constant__ CUtensorMap tm_ay,
-            const __grid_constant__ CUtensorMap tm_az, LevelDev L, double* __restrict__ crhs, double* __restrict__ cphi,
-            double* __restrict__ part_max, int zchunk)
+            const __grid_constant__ CUtensorMap tm_az, LevelDev L, LevelDev Cc, double* __restrict__ part_max, int zchunk)
 {
     constexpr int LN = 32, TYE = 16;
     using G = Cfg<LN, TYE, NS>;
@@ -375,7 +386,7 @@ k_resid_tma(const __grid_constant__ CUtensorMap tm_phi, const __grid_constant__ 
         asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
         asm volatile("fence.proxy.async.shared::cta;\n" ::: "memory");
         for (int q = 0; q < NS && k0 - 1 + q <= k1; ++q)         // planes k0-1 .. ; plane p -> stage (p - (k0-1)) % NS
-            issue_plane<LN, TYE, NS>(&tm_phi, &tm_rhs, &tm_ax, &tm_ay, &tm_az, stage0, bar0, q, k0 - 1 + q, L.nz, perz, x0 - 2, y0 - 1);
+            issue_plane<LN, TYE, NS>(&tm_phi, &tm_rhs, &tm_ax, &tm_ay, &tm_az, stage0, bar0, q, k0 - 1 + q, L.nz, perz, x0 - 2 + L.gx, y0 - 1 + L.gy);
     }
     __syncthreads();
 
@@ -389,9 +400,13 @@ k_resid_tma(const __grid_constant__ CUtensorMap tm_phi, const __grid_constant__ 
     double2 aza = fused::ld2<LN, TYE>(base + G::kStage, A_AZ, 0, 0), azb = fused::ld2<LN, TYE>(base + G::kStage, A_AZ, 1, 0);
     int sI = 1;
     double acc = 0.0, vmax = 0.0;
-    const size_t cnx = (size_t)(L.nx >> 1), cny = (size_t)(L.ny >> 1);
-    double* co = crhs ? crhs + ((size_t)(gi >> 1) + cnx * ((size_t)(gja >> 1) + cny * (size_t)(k0 >> 1))) : nullptr;
-    double* cz = cphi ? cphi + ((size_t)(gi >> 1) + cnx * ((size_t)(gja >> 1) + cny * (size_t)(k0 >> 1))) : nullptr;
+    // coarse outputs (RES_RESTRICT): cell (gi/2, gja/2) of the coarse level, with its periodic images
+    const long long cplane = (long long)Cc.cx * Cc.ry;
+    const size_t c0 = (MODE & RES_RESTRICT) && own ? cidx(Cc, gi >> 1, gja >> 1, k0 >> 1) : 0;
+    double* co = (MODE & RES_RESTRICT) ? Cc.rhs + c0 : nullptr;
+    double* cz = (MODE & RES_RESTRICT) ? Cc.phi + c0 : nullptr;
+    const long long cix = (MODE & RES_RESTRICT) && own ? image_dx(Cc, gi >> 1) : 0;
+    const long long ciy = (MODE & RES_RESTRICT) && own ? image_dy(Cc, gja >> 1) : 0;
 
 #pragma unroll 1
     for (int kk = k0; kk < k1; ++kk) {
@@ -402,7 +417,7 @@ k_resid_tma(const __grid_constant__ CUtensorMap tm_phi, const __grid_constant__ 
         __syncthreads();
         if (producer && kk + NS - 1 <= k1) {                      // (plane k0-1 was consumed into registers by the prologue)
             asm volatile("fence.proxy.async.shared::cta;\n" ::: "memory");
-            issue_plane<LN, TYE, NS>(&tm_phi, &tm_rhs, &tm_ax, &tm_ay, &tm_az, stage0, bar0, sN, kk + NS - 1, L.nz, perz, x0 - 2, y0 - 1);
+            issue_plane<LN, TYE, NS>(&tm_phi, &tm_rhs, &tm_ax, &tm_ay, &tm_az, stage0, bar0, sN, kk + NS - 1, L.nz, perz, x0 - 2 + L.gx, y0 - 1 + L.gy);
         }
         const unsigned char* s0 = base + sI * G::kStage;
         const unsigned char* sp = base + sP * G::kStage;
@@ -436,10 +451,10 @@ k_resid_tma(const __grid_constant__ CUtensorMap tm_phi, const __grid_constant__ 
                 if ((kk & 1) == 0) {
                     acc = s4;
                 } else {
-                    *co = 0.125 * (acc + s4);
-                    *cz = 0.0;
-                    co += cnx * cny;
-                    cz += cnx * cny;
+                    store_images(co, 0.125 * (acc + s4), cix, ciy);
+                    store_images(cz, 0.0, cix, ciy);
+                    co += cplane;
+                    cz += cplane;
                 }
             }
         }
@@ -471,7 +486,7 @@ static inline int tma_resid_configure()
 }
 
 // mode: tma::RES_RESTRICT and/or tma::RES_NORM.  Returns the number of CTAs (= partial maxima written), or -1.
-static inline int launch_tma_resid(const TmaLevelMaps& T, bool in_is_phi2, const LevelDev& L, double* crhs, double* cphi,
+static inline int launch_tma_resid(const TmaLevelMaps& T, bool in_is_phi2, const LevelDev& L, const LevelDev& Cc,
                                    double* part_max, int max_parts, int mode, cudaStream_t s)
 {
     using namespace tma;
@@ -489,10 +504,10 @@ static inline int launch_tma_resid(const TmaLevelMaps& T, bool in_is_phi2, const
     const CUtensorMap& tin = in_is_phi2 ? T.phi2 : T.phi;
     const size_t sm = smem_bytes<32, 16, 5>();
     if (mode == RES_RESTRICT)
-        k_resid_tma<5, RES_RESTRICT><<<grid, block, sm, s>>>(tin, T.rhs, T.ax, T.ay, T.az, L, crhs, cphi, part_max, zchunk);
+        k_resid_tma<5, RES_RESTRICT><<<grid, block, sm, s>>>(tin, T.rhs, T.ax, T.ay, T.az, L, Cc, part_max, zchunk);
     else if (mode == RES_NORM)
-        k_resid_tma<5, RES_NORM><<<grid, block, sm, s>>>(tin, T.rhs, T.ax, T.ay, T.az, L, crhs, cphi, part_max, zchunk);
+        k_resid_tma<5, RES_NORM><<<grid, block, sm, s>>>(tin, T.rhs, T.ax, T.ay, T.az, L, Cc, part_max, zchunk);
     else
-        k_resid_tma<5, RES_RESTRICT | RES_NORM><<<grid, block, sm, s>>>(tin, T.rhs, T.ax, T.ay, T.az, L, crhs, cphi, part_max, zchunk);
+        k_resid_tma<5, RES_RESTRICT | RES_NORM><<<grid, block, sm, s>>>(tin, T.rhs, T.ax, T.ay, T.az, L, Cc, part_max, zchunk);
     return cudaPeekAtLastError() == cudaSuccess ? tiles_x * tiles_y * nchunk : -1;
 }

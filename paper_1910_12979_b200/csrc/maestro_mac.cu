@@ -26,10 +26,14 @@ constexpr int kSmoothEvents = 512;        // level-0 smoother launches timed per
 struct Level {
     int n[3];
     double h[3];
-    int px;
-    size_t ncell, nax, nay, naz;
-    double *phi, *phi2, *rhs, *ax, *ay, *az;
-    double *phi_a;                 // the buffer `phi` pointed to at carve time (tensor map `phi`)
+    int px;                        // x pitch of ax
+    int gx, gy;                    // ghost columns / rows per side (mac_common.cuh "Ghosts")
+    int cx, ry;                    // x pitch of the cell-shaped arrays, rows per plane
+    size_t ncell;                  // interior cells
+    size_t acell, nax, nay, naz;   // allocated entries (ghosts included)
+    size_t off_c, off_ax;          // entries from an allocation's base to the interior origin
+    double *phi, *phi2, *rhs, *ax, *ay, *az;   // interior origins
+    double* phi_a;                 // the buffer `phi` pointed to at carve time (tensor map `phi`)
     TmaLevelMaps tma[2];           // [0] MAC_TMA_BIG tile, [1] MAC_TMA_MID tile
 };
 
@@ -106,11 +110,20 @@ int build_levels(const maestro_mac_desc& d, Level* lev, int* nlev)
     for (;;) {
         Level& L = lev[l];
         for (int a = 0; a < 3; ++a) { L.n[a] = n[a]; L.h[a] = h[a]; }
-        L.px = (int)align_up((size_t)n[0] + 1, 4);
+        // levels that run the TMA-staged kernels carry periodic image columns / rows (TMA cannot wrap)
+        const bool tma_level = (d.smoother == 0 || d.smoother == 3) && n[0] >= 60 && (n[0] & 1) == 0 && n[1] >= 4;
+        L.gx = (tma_level && d.bc_lo[0] == MAESTRO_MAC_PERIODIC) ? 2 : 0;
+        L.gy = (tma_level && d.bc_lo[1] == MAESTRO_MAC_PERIODIC) ? 2 : 0;
+        L.cx = n[0] + 2 * L.gx;
+        L.ry = n[1] + 2 * L.gy;
+        L.px = (int)align_up((size_t)n[0] + 1 + 2 * L.gx, 4);
         L.ncell = (size_t)n[0] * n[1] * n[2];
-        L.nax = (size_t)L.px * n[1] * n[2];
-        L.nay = (size_t)n[0] * (n[1] + 1) * n[2];
-        L.naz = (size_t)n[0] * n[1] * (n[2] + 1);
+        L.acell = (size_t)L.cx * L.ry * n[2];
+        L.nax = (size_t)L.px * L.ry * n[2];
+        L.nay = (size_t)L.cx * (L.ry + 1) * n[2];
+        L.naz = (size_t)L.cx * L.ry * (n[2] + 1);
+        L.off_c = (size_t)L.gx + (size_t)L.cx * L.gy;
+        L.off_ax = (size_t)L.gx + (size_t)L.px * L.gy;
         ++l;
         bool can = l < kMaxLevels;
         for (int a = 0; a < 3; ++a)
@@ -135,13 +148,14 @@ size_t carve(maestro_mac_handle* H, char* base)
     };
     for (int l = 0; l < H->nlev; ++l) {
         Level& L = H->lev[l];
-        L.phi = (double*)take(L.ncell, 8);
+        auto at = [&](void* b, size_t o) -> double* { return b ? (double*)b + o : nullptr; };
+        L.phi = at(take(L.acell, 8), L.off_c);
         L.phi_a = L.phi;
-        L.phi2 = (double*)take(L.ncell, 8);
-        L.rhs = (double*)take(L.ncell, 8);
-        L.ax = (double*)take(L.nax, 8);
-        L.ay = (double*)take(L.nay, 8);
-        L.az = (double*)take(L.naz, 8);
+        L.phi2 = at(take(L.acell, 8), L.off_c);
+        L.rhs = at(take(L.acell, 8), L.off_c);
+        L.ax = at(take(L.nax, 8), L.off_ax);
+        L.ay = at(take(L.nay, 8), L.off_c);
+        L.az = at(take(L.naz, 8), L.off_c);
     }
     H->part_sum = (double*)take(kMaxParts, 8);
     H->part_max = (double*)take(kMaxParts, 8);
@@ -169,6 +183,7 @@ LevelDev dev_level(const maestro_mac_handle* H, int l)
     const Level& L = H->lev[l];
     LevelDev D;
     D.nx = L.n[0]; D.ny = L.n[1]; D.nz = L.n[2]; D.px = L.px;
+    D.cx = L.cx; D.ry = L.ry; D.gx = L.gx; D.gy = L.gy;
     for (int a = 0; a < 3; ++a) { D.bclo[a] = H->d.bc_lo[a]; D.bchi[a] = H->d.bc_hi[a]; }
     D.phi = L.phi; D.phi2 = L.phi2; D.rhs = L.rhs; D.ax = L.ax; D.ay = L.ay; D.az = L.az;
     return D;
@@ -211,6 +226,19 @@ void dims3(int ex, int ey, int ez, dim3* grid, dim3* block)
 
 int red_blocks(int rows) { return rows < kRedBlocks ? rows : kRedBlocks; }
 
+enum { GH_PHI = 1, GH_RHS = 2, GH_AX = 4, GH_AY = 8, GH_AZ = 16 };
+
+// periodic images of the selected arrays of a ghosted level (no-op on other levels)
+int do_fill_ghosts(maestro_mac_handle* H, int l, int which, cudaStream_t s)
+{
+    const Level& L = H->lev[l];
+    if (L.gx == 0 && L.gy == 0) return MAESTRO_MAC_OK;
+    const int per_plane = 2 * L.gx * (L.n[1] + 1 + 2 * L.gy) + 2 * L.gy * (L.n[0] + 1);
+    k_fill_ghosts<<<dim3((per_plane + 255) / 256, L.n[2] + 1), 256, 0, s>>>(dev_level(H, l), which);
+    LAUNCHED(H);
+    return MAESTRO_MAC_OK;
+}
+
 // ---- individual steps ------------------------------------------------------------------------
 
 int do_coefficients(maestro_mac_handle* H, const double* beta0, const double* rho0, const double* rho, cudaStream_t s)
@@ -227,11 +255,14 @@ int do_coefficients(maestro_mac_handle* H, const double* beta0, const double* rh
         k_face_coeff<<<g, b, 0, s>>>(G, dev_level(H, 0), beta0, rho, rho0, H->flags);
     }
     LAUNCHED(H);
+    int rc;
+    if ((rc = do_fill_ghosts(H, 0, GH_AX | GH_AY | GH_AZ, s)) != 0) return rc;
     for (int l = 0; l + 1 < H->nlev; ++l) {
         LevelDev C = dev_level(H, l + 1);
         dims3(C.nx + 1, C.ny + 1, C.nz + 1, &g, &b);
         k_coarsen_coeff<<<g, b, 0, s>>>(dev_level(H, l), C);
         LAUNCHED(H);
+        if ((rc = do_fill_ghosts(H, l + 1, GH_AX | GH_AY | GH_AZ, s)) != 0) return rc;
     }
     return MAESTRO_MAC_OK;
 }
@@ -248,26 +279,26 @@ int do_rhs(maestro_mac_handle* H, const double* beta0, const double* u, const do
         dim3 gg((G.nx + 63) / 64, (G.ny + 3) / 4, (G.nz + zc - 1) / zc);
         while ((long)gg.x * gg.y * gg.z > kMaxParts) { zc *= 2; gg.z = (G.nz + zc - 1) / zc; }
         nb = (int)(gg.x * gg.y * gg.z);
-        k_rhs2<<<gg, dim3(64, 4), 0, s>>>(G, dev_geo_inv(H), beta0, u, v, w, S, L0.rhs, zc, H->part_sum, H->part_max);
+        k_rhs2<<<gg, dim3(64, 4), 0, s>>>(G, dev_geo_inv(H), dev_level(H, 0), beta0, u, v, w, S, zc, H->part_sum, H->part_max);
     } else {
         int rows = G.ny * G.nz;
         nb = red_blocks(rows);
         int bt = G.nx >= 256 ? 256 : (G.nx >= 128 ? 128 : 64);
-        k_rhs<<<nb, bt, 0, s>>>(G, beta0, u, v, w, S, L0.rhs, H->part_sum, H->part_max);
+        k_rhs<<<nb, bt, 0, s>>>(G, dev_level(H, 0), beta0, u, v, w, S, H->part_sum, H->part_max);
     }
     LAUNCHED(H);
     k_reduce_final<<<1, 1024, 0, s>>>(H->part_sum, H->part_max, nb, H->scal);
     LAUNCHED(H);
     if (H->singular) {
         CUDA_OK(cudaMemcpyAsync(H->scal + 2, H->scal, sizeof(double), cudaMemcpyDeviceToDevice, s));
-        k_shift_mean<<<kRedBlocks, 256, 0, s>>>(L0.rhs, L0.ncell, H->scal + 2, 1.0 / (double)L0.ncell, H->part_sum, H->part_max);
+        k_shift_mean<<<kRedBlocks, 256, 0, s>>>(dev_level(H, 0), L0.rhs, H->scal + 2, 1.0 / (double)L0.ncell, H->part_sum, H->part_max);
         LAUNCHED(H);
         k_reduce_final<<<1, 1024, 0, s>>>(H->part_sum, H->part_max, kRedBlocks, H->scal);
         LAUNCHED(H);
     } else {
         CUDA_OK(cudaMemsetAsync(H->scal + 2, 0, sizeof(double), s));
     }
-    return MAESTRO_MAC_OK;
+    return do_fill_ghosts(H, 0, GH_RHS, s);
 }
 
 // One sweep on level l.  norm_parts != NULL (level-0 TMA path only, see fused_norm_ok): the sweep also
@@ -326,7 +357,7 @@ int do_residual_restrict(maestro_mac_handle* H, int l, cudaStream_t s)
 {
     if (tma_aux(H, l)) {
         Level& F = H->lev[l];
-        int n = launch_tma_resid(F.tma[0], F.phi != F.phi_a, dev_level(H, l), H->lev[l + 1].rhs, H->lev[l + 1].phi,
+        int n = launch_tma_resid(F.tma[0], F.phi != F.phi_a, dev_level(H, l), dev_level(H, l + 1),
                                  H->part_max, kMaxParts, tma::RES_RESTRICT, s);
         if (n < 0) return MAESTRO_MAC_ERR_CUDA;
         ++H->launches;
@@ -404,7 +435,7 @@ int do_residual_norm(maestro_mac_handle* H, int l, cudaStream_t s)
     LevelDev L = dev_level(H, l);
     if (tma_aux(H, l)) {
         Level& F = H->lev[l];
-        int n = launch_tma_resid(F.tma[0], F.phi != F.phi_a, L, nullptr, nullptr, H->part_max, kMaxParts, tma::RES_NORM, s);
+        int n = launch_tma_resid(F.tma[0], F.phi != F.phi_a, L, L, H->part_max, kMaxParts, tma::RES_NORM, s);
         if (n < 0) return MAESTRO_MAC_ERR_CUDA;
         ++H->launches;
         k_reduce_final<<<1, 1024, 0, s>>>(H->part_sum, H->part_max, n, H->scal + 3);
@@ -427,7 +458,7 @@ int do_correct(maestro_mac_handle* H, const double* phi, const double* rho0, con
     GeoDev G = dev_geo(H);
     dim3 g, b;
     dims3(G.nx + 1, G.ny + 1, G.nz + 1, &g, &b);
-    k_correct<<<g, b, 0, s>>>(G, phi, rho, rho0, u, v, w);
+    k_correct<<<g, b, 0, s>>>(G, dev_level(H, 0), phi, rho, rho0, u, v, w);
     LAUNCHED(H);
     return MAESTRO_MAC_OK;
 }
@@ -498,6 +529,8 @@ extern "C" int maestro_mac_setup(const maestro_mac_desc* desc, void* workspace, 
             LevelDev D = dev_level(H, l);
             tma_build_maps(&H->lev[l].tma[0], D, 32, 16);
             tma_build_maps(&H->lev[l].tma[1], D, 16, 16);
+            // a level laid out with periodic images has no other smoother: its tensor maps must exist
+            if ((D.gx || D.gy) && !H->lev[l].tma[H->d.smoother == 3 ? 1 : 0].ok) ok = false;
         }
     if (!ok) {
         maestro_mac_free(H);
@@ -548,7 +581,7 @@ extern "C" int maestro_mac_project(maestro_mac_handle* H, const double* beta0, c
     if ((rc = do_rhs(H, beta0, u, v, w, S, s)) != 0) return rc;
     CUDA_OK(cudaMemcpyAsync(H->host_scal, H->scal, 3 * sizeof(double), cudaMemcpyDeviceToHost, s));
     CUDA_OK(cudaMemcpyAsync(H->host_flags, H->flags, sizeof(int), cudaMemcpyDeviceToHost, s));
-    CUDA_OK(cudaMemsetAsync(L0.phi, 0, L0.ncell * sizeof(double), s));   // A16: phi = 0
+    CUDA_OK(cudaMemsetAsync(L0.phi - L0.off_c, 0, L0.acell * sizeof(double), s));   // A16: phi = 0 (ghosts too)
     CUDA_OK(cudaEventRecord(H->ev[1], s));
     CUDA_OK(cudaStreamSynchronize(s));
     st.rhs_norm_inf = H->host_scal[1];
@@ -595,16 +628,25 @@ extern "C" int maestro_mac_project(maestro_mac_handle* H, const double* beta0, c
     CUDA_OK(cudaEventRecord(H->ev[2], s));
     if (!trivial && result != MAESTRO_MAC_ERR_NONFINITE) {
         if (H->singular) {   // A10: zero-mean phi
-            k_sum<<<kRedBlocks, 256, 0, s>>>(H->lev[0].phi, L0.ncell, H->part_sum, H->part_max);
+            k_sum<<<kRedBlocks, 256, 0, s>>>(dev_level(H, 0), H->lev[0].phi, H->part_sum, H->part_max);
             LAUNCHED(H);
             k_reduce_final<<<1, 1024, 0, s>>>(H->part_sum, H->part_max, kRedBlocks, H->scal + 6);
             LAUNCHED(H);
-            k_shift_mean<<<kRedBlocks, 256, 0, s>>>(H->lev[0].phi, L0.ncell, H->scal + 6, 1.0 / (double)L0.ncell, H->part_sum, H->part_max);
+            k_shift_mean<<<kRedBlocks, 256, 0, s>>>(dev_level(H, 0), H->lev[0].phi, H->scal + 6, 1.0 / (double)L0.ncell, H->part_sum, H->part_max);
             LAUNCHED(H);
         }
         if ((rc = do_correct(H, H->lev[0].phi, rho0, rho, u, v, w, s)) != 0) return rc;
     }
-    if (phi) CUDA_OK(cudaMemcpyAsync(phi, H->lev[0].phi, L0.ncell * sizeof(double), cudaMemcpyDeviceToDevice, s));
+    if (phi) {
+        if (L0.gx == 0 && L0.gy == 0) {
+            CUDA_OK(cudaMemcpyAsync(phi, L0.phi, L0.ncell * sizeof(double), cudaMemcpyDeviceToDevice, s));
+        } else {
+            dim3 g, b;
+            dims3(L0.n[0], L0.n[1], L0.n[2], &g, &b);
+            k_copy_level<<<g, b, 0, s>>>(dev_level(H, 0), L0.phi, phi, 0, L0.n[0], L0.n[1], L0.n[2], 1);
+            LAUNCHED(H);
+        }
+    }
     CUDA_OK(cudaEventRecord(H->ev[3], s));
     if (stats || d.rel_tol > 0.0) {
         CUDA_OK(cudaMemcpyAsync(H->host_flags + 1, H->flags + 1, sizeof(int), cudaMemcpyDeviceToHost, s));
@@ -681,25 +723,20 @@ static int level_copy(maestro_mac_handle* H, int level, int which, double* pub, 
     if (!H || !pub || level < 0 || level >= H->nlev) return MAESTRO_MAC_ERR_ARG;
     Level& L = H->lev[level];
     double* internal = nullptr;
-    size_t count = 0;
+    int e[3] = {L.n[0], L.n[1], L.n[2]}, kind = 0, ghosts = 0;
     switch (which) {
-        case MAESTRO_MAC_ARR_PHI: internal = L.phi; count = L.ncell; break;
-        case MAESTRO_MAC_ARR_RHS: internal = L.rhs; count = L.ncell; break;
-        case MAESTRO_MAC_ARR_BY: internal = L.ay; count = L.nay; break;
-        case MAESTRO_MAC_ARR_BZ: internal = L.az; count = L.naz; break;
-        case MAESTRO_MAC_ARR_BX: {
-            LevelDev D = dev_level(H, level);
-            dim3 g, b;
-            dims3(D.nx + 1, D.ny, D.nz, &g, &b);
-            k_copy_ax<<<g, b, 0, s>>>(D, pub, to_public);
-            LAUNCHED(H);
-            return MAESTRO_MAC_OK;
-        }
+        case MAESTRO_MAC_ARR_PHI: internal = L.phi; ghosts = GH_PHI; break;
+        case MAESTRO_MAC_ARR_RHS: internal = L.rhs; ghosts = GH_RHS; break;
+        case MAESTRO_MAC_ARR_BX: internal = L.ax; kind = 2; ++e[0]; ghosts = GH_AX; break;
+        case MAESTRO_MAC_ARR_BY: internal = L.ay; kind = 3; ++e[1]; ghosts = GH_AY; break;
+        case MAESTRO_MAC_ARR_BZ: internal = L.az; kind = 4; ++e[2]; ghosts = GH_AZ; break;
         default: return MAESTRO_MAC_ERR_ARG;
     }
-    if (to_public) CUDA_OK(cudaMemcpyAsync(pub, internal, count * sizeof(double), cudaMemcpyDeviceToDevice, s));
-    else CUDA_OK(cudaMemcpyAsync(internal, pub, count * sizeof(double), cudaMemcpyDeviceToDevice, s));
-    return MAESTRO_MAC_OK;
+    dim3 g, b;
+    dims3(e[0], e[1], e[2], &g, &b);
+    k_copy_level<<<g, b, 0, s>>>(dev_level(H, level), internal, pub, kind, e[0], e[1], e[2], to_public);
+    LAUNCHED(H);
+    return to_public ? MAESTRO_MAC_OK : do_fill_ghosts(H, level, ghosts, s);
 }
 
 extern "C" int maestro_mac_level_get(maestro_mac_handle* H, int level, int which, double* dst, void* cuda_stream)

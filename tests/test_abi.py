@@ -34,12 +34,13 @@ def test_struct_sizes_match(mac):
 
 
 def test_workspace_query_and_validation(mac):
-    d = mac.make_desc((64, 64, 64), (1 / 64,) * 3, (0, 0, 1), (0, 0, 1))
+    d = mac.make_desc((128, 128, 128), (1 / 128,) * 3, (0, 0, 1), (0, 0, 1))
     need = mac.workspace_bytes(d)
-    # level 0: phi, phi2, rhs + three face arrays; all levels ~ 8/7 of that
-    cells = 64 ** 3
+    # level 0: phi, phi2, rhs + three face arrays; all levels ~ 8/7 of that (+ periodic image columns / rows
+    # on the TMA levels, + 2 MB of reduction scratch)
+    cells = 128 ** 3
     assert 6 * cells * 8 < need < 8 * cells * 8
-    d2 = mac.make_desc((64, 64, 64), (1 / 64,) * 3, (0, 0, 1), (0, 0, 1), host_staging=1)
+    d2 = mac.make_desc((128, 128, 128), (1 / 128,) * 3, (0, 0, 1), (0, 0, 1), host_staging=1)
     assert mac.workspace_bytes(d2) > need + 6 * cells * 8
 
     def rc_of(desc):

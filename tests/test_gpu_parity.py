@@ -41,6 +41,11 @@ def small_cases():
         # wide enough for the 64-column TMA tile (x, y not periodic), ragged in x and y, z periodic / not
         W.mixed_bc_case(n=(72, 20, 16), bc_lo=(OUT, WALL, PER), bc_hi=(WALL, OUT, PER), seed=14),
         W.mixed_bc_case(n=(136, 28, 16), bc_lo=(WALL, OUT, OUT), bc_hi=(OUT, WALL, WALL), geometry=W.SPHERICAL, seed=15),
+        # wide AND periodic in x and/or y: TMA levels with periodic image columns / rows (ghost layout)
+        W.mixed_bc_case(n=(64, 24, 16), bc_lo=(PER, PER, WALL), bc_hi=(PER, PER, OUT), seed=16),
+        W.mixed_bc_case(n=(72, 20, 16), bc_lo=(PER, WALL, PER), bc_hi=(PER, OUT, PER), geometry=W.SPHERICAL, seed=17),
+        W.mixed_bc_case(n=(120, 16, 16), bc_lo=(OUT, PER, WALL), bc_hi=(OUT, PER, WALL), seed=18),
+        W.config1(N=64),
     ]
 
 
@@ -65,7 +70,7 @@ def close(a, b, tol=KERNEL_TOL):
     return np.abs(a - b).max() <= tol * scale
 
 
-@pytest.mark.parametrize("case", range(10))
+@pytest.mark.parametrize("case", range(14))
 @pytest.mark.parametrize("smoother", [0, 1, 2, 3])
 def test_per_kernel_parity(oracle, mac, case, smoother):
     import torch
@@ -152,7 +157,7 @@ def test_per_kernel_parity(oracle, mac, case, smoother):
 
 
 E2E_CASES = [("1", 32), ("2", 32), ("3N", 32), ("3D", 32), ("4N", 32), ("4D", 64), ("5", 32),
-             ("2", 64), ("3N", 64), ("mixed", 0), ("mixed_sph", 0)]
+             ("2", 64), ("3N", 64), ("mixed", 0), ("mixed_sph", 0), ("1", 64), ("5", 128)]
 
 
 def get_case(name, N):
