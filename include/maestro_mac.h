@@ -79,7 +79,10 @@ typedef struct {
     int host_staging;         /* 1 = reserve device staging in the workspace so that
                                  maestro_mac_project_host() can be used */
     int smoother;             /* 0 = default: fused red+black single pass, planes staged by TMA where the
-                                 level allows it (x, y not periodic, nx >= 60), else by cp.async;
+                                 level allows it (nx >= 60), else by cp.async;
+                                 4 = as 0, but pairs of sweeps run as ONE pass over HBM (two-sweep kernel,
+                                     temporal blocking) on levels of at least 48 x 16 x 8 cells; experimental:
+                                     correct and bit-identical to 0, not yet faster;
                                  1 = reference two-pass (one kernel per colour);
                                  2 = fused single pass, cp.async staging on every level;
                                  3 = fused single pass, TMA staging with the 32x16 tile.
@@ -106,8 +109,9 @@ typedef struct {
     int gpu_launches;         /* kernels launched by this call */
     float ms_smooth0;         /* summed device time of the level-0 smoother launches that were timed
                                  (one CUDA event pair per launch, on the call's stream) */
-    int smooth0_launches;     /* level-0 smoother sweeps launched by this call */
+    int smooth0_launches;     /* level-0 smoother launches of this call */
     int smooth0_timed;        /* how many of them ms_smooth0 covers (at most 512) */
+    int smooth0_sweeps_timed; /* sweeps those launches applied (a two-sweep launch counts 2) */
 } maestro_mac_stats;
 
 /* Fill *desc with defaults for an nx*ny*nz unit-spacing periodic planar problem. */

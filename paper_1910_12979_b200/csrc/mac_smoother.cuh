@@ -48,21 +48,31 @@ __device__ __forceinline__ void cp_async16(unsigned smem_dst, const void* gsrc, 
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;\n" ::: "memory"); }
 template <int N> __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;\n" ::"n"(N) : "memory"); }
 
-// (off - rhs) / dg of the Gauss-Seidel update.  dg is a sum of positive, well-scaled face coefficients, so
-// the guarded IEEE division (range checks + slow-path call) is replaced by a reciprocal seed, two Newton
-// steps and one correction of the quotient: faithful to 1 ulp, a third of the dependent latency.
-// -DMAC_IEEE_DIV restores the plain division.
-__device__ __forceinline__ double gs_div(double a, double b)
+// The division by the diagonal: dg is a sum of positive, well-scaled face coefficients, so the guarded IEEE
+// division (range checks + slow-path call) is replaced by a reciprocal seed, two Newton steps and one
+// correction of the quotient: faithful to 1 ulp.  -DMAC_IEEE_DIV restores the plain division.
+// The Gauss-Seidel value  (sum_f a_f phi_f - rhs) / sum_f a_f  arranged for a short dependent chain.  In the
+// marching kernels the upper neighbour u_ is the value the previous half-sweep of the SAME step has just
+// produced, so it enters last: the reciprocal of the diagonal and the other five products are off the chain,
+// which is then fma, mul, fma, fma (fp64 latency, not throughput, bounds these kernels).  *a_out = sum - rhs.
+__device__ __forceinline__ double gs_value(double axw, double axe, double ays, double ayn, double azd, double azu,
+                                           double rhs, double w_, double e_, double s_, double n_, double d_, double u_,
+                                           double& a_out, double& dg_out)
 {
+    const double dg = ((axw + axe) + (ays + ayn)) + (azd + azu);
+    const double t = (fma(axe, e_, axw * w_) + fma(ayn, n_, ays * s_)) + fma(azd, d_, -rhs);
+    const double a = fma(azu, u_, t);
+    a_out = a;
+    dg_out = dg;
 #ifdef MAC_IEEE_DIV
-    return a / b;
+    return a / dg;
 #else
     double r;
-    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(b));
-    r = fma(fma(-b, r, 1.0), r, r);
-    r = fma(fma(-b, r, 1.0), r, r);
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(dg));
+    r = fma(fma(-dg, r, 1.0), r, r);
+    r = fma(fma(-dg, r, 1.0), r, r);
     const double q = a * r;
-    return fma(fma(-b, q, a), r, q);
+    return fma(fma(-dg, q, a), r, q);
 #endif
 }
 
@@ -148,10 +158,9 @@ __device__ __forceinline__ void step(const Ctx<LN, TYE>& C, unsigned char* s0, c
         const double axw = REDX ? CUR.ax.x : CUR.ax.y, axe = REDX ? CUR.ax.y : CUR.ax2;
         const double ays = pick<REDX>(CUR.ays), ayn = pick<REDX>(CUR.ayn);
         const double azd = pick<REDX>(CUR.az);
-        const double off = axw * w_ + axe * e_ + ays * s_ + ayn * n_ + azd * d_ + azu * u_;
-        const double dg = ((axw + axe) + (ays + ayn)) + (azd + azu);
-        const double nv = gs_div(off - pick<REDX>(CUR.rhs), dg);
-        if (NORM && C.own) *vmax = nanmax(*vmax, fabs(pick<REDX>(CUR.rhs) - (off - pick<REDX>(q0) * dg)));
+        double a, dg;
+        const double nv = gs_value(axw, axe, ays, ayn, azd, azu, pick<REDX>(CUR.rhs), w_, e_, s_, n_, d_, u_, a, dg);
+        if (NORM && C.own) *vmax = nanmax(*vmax, fabs(fma(pick<REDX>(q0), dg, -a)));   // |rhs - (sum - phi_0 dg)|
         put<REDX>(q0, nv);
         *reinterpret_cast<double*>(s0 + A_PHI * Ctx<LN, TYE>::kArr + (REDX ? 0 : 8)) = nv;
     }
@@ -164,9 +173,8 @@ __device__ __forceinline__ void step(const Ctx<LN, TYE>& C, unsigned char* s0, c
         const double axw = REDX ? PRV.ax.x : PRV.ax.y, axe = REDX ? PRV.ax.y : PRV.ax2;
         const double ays = pick<REDX>(PRV.ays), ayn = pick<REDX>(PRV.ayn);
         const double azd = pick<REDX>(PRV.az), azu = pick<REDX>(CUR.az);
-        const double off = axw * w_ + axe * e_ + ays * s_ + ayn * n_ + azd * d_ + azu * u_;
-        const double dg = ((axw + axe) + (ays + ayn)) + (azd + azu);
-        put<REDX>(qm1, gs_div(off - pick<REDX>(PRV.rhs), dg));
+        double a, dg;
+        put<REDX>(qm1, gs_value(axw, axe, ays, ayn, azd, azu, pick<REDX>(PRV.rhs), w_, e_, s_, n_, d_, u_, a, dg));
         store_images(reinterpret_cast<double2*>(out_km1), qm1, C.img_x, C.img_y);
     }
     qm2 = qm1;

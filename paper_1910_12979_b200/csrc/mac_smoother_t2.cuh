@@ -1,0 +1,366 @@
+// mac_smoother_t2.cuh -- TWO red-black Gauss-Seidel sweeps in ONE pass over HBM (temporal blocking
+// of the smoother).
+//
+// One launch reads phi, rhs, ax, ay, az once and writes phi once (48 B/cell) and applies
+//      red, black, red, black
+// i.e. exactly the nu = 2 sweeps of a V(2,2) cycle.  The result is bit-identical to two launches of
+// tma::k_rbgs_tma (same expressions, same order within an update).
+//
+// Scheme.  The single-sweep kernel marches upward in z with a one-plane lag (red of plane k, black of
+// plane k-1).  Here the march carries FOUR half-sweeps with a three-plane lag: at step k a thread
+// updates, on its own pair of columns,
+//      (1) sweep 1 red   of plane k      (old black neighbours:         planes k-1, k,   k+1)
+//      (2) sweep 1 black of plane k-1    (sweep-1 red neighbours:       planes k-2, k-1, k  )
+//      (3) sweep 2 red   of plane k-2    (sweep-1 black neighbours:     planes k-3, k-2, k-1)
+//      (4) sweep 2 black of plane k-3    (sweep-2 red neighbours:       planes k-4, k-3, k-2)
+// and stores plane k-3.  All four updates hit the SAME column of the pair (the colour of a column
+// alternates from plane to plane), vertical neighbours are the thread's own registers, lateral
+// neighbours come from the staged planes, which are updated in place (each update is written back to
+// its stage, so a stage holds, in turn, old / sweep-1 red / sweep-1 final / sweep-2 red values).
+// The only cross-thread dependences are lateral and always one step old: one __syncthreads per plane.
+//
+// Lateral halo: every half-sweep consumes one ring of cells, so a tile of 32 x 24 staged cells yields
+// 24 x 16 finished ones (halo 4); the halo cells are recomputed redundantly by the neighbouring CTA
+// (their HBM reads hit L2).  In z a chunk [k0, k1) redoes 6 planes.
+//
+// Memory.  phi planes live for 5 steps (k+1 .. k-3), coefficient planes for one (they are consumed
+// into registers, where the four coefficient sets of planes k .. k-3 rotate; the loop is unrolled by
+// four so that nothing is moved).  So shared memory holds two rings fed by TMA box loads
+// (cp.async.bulk.tensor.3d + mbarrier, as in mac_smoother_tma.cuh): NP = LA + 5 phi stages of 6 KB
+// and NC = LA + 2 coefficient stages of 24 KB, LA = planes of lookahead in flight.
+// All updates are computed unconditionally and selected by masks (no divergent branches around the
+// dependent chain of four divisions).
+#pragma once
+#include <climits>
+
+#include "mac_smoother_tma.cuh"
+
+namespace t2 {
+
+using fused::Coef; using fused::pick; using fused::put;
+using tma::mbar_init; using tma::mbar_expect_tx; using tma::mbar_wait; using tma::tma_load_3d; using tma::smem_u32;
+
+constexpr int LN = 16, TYE = 24, NT = LN * TYE;      // 16 pairs x 24 rows = 384 threads
+constexpr int HALO = 4;
+constexpr int kTX = 2 * LN - 2 * HALO;               // 24 finished columns per tile
+constexpr int kTY = TYE - 2 * HALO;                  // 16 finished rows per tile
+constexpr int kRow = LN * 16;                        // bytes of one staged row
+constexpr int kPl = TYE * kRow;                      // bytes of one staged array plane
+constexpr int kPad = 512;                            // readable slack below the phi ring (masked lanes read row -1)
+enum { C_AX = 0, C_AY = 1, C_AZ = 2, C_RHS = 3, C_COUNT = 4 };
+
+template <int LA>
+struct Cfg {
+    static constexpr int NP = LA + 5, NC = LA + 2;
+    static constexpr int kCoef = C_COUNT * kPl;
+    static constexpr unsigned kTx = (unsigned)kRow * (TYE + (TYE - 1) + 3 * (TYE - 2));   // bytes landing per plane
+    static constexpr size_t kSmem = (size_t)kPad + (size_t)NP * kPl + (size_t)NC * kCoef + 8 * NP + 128;
+};
+
+__device__ __forceinline__ double2 ldp(const unsigned char* p) { return *reinterpret_cast<const double2*>(p); }
+template <bool X> __device__ __forceinline__ double ldc(const unsigned char* p, int dy, int dl)
+{
+    return *reinterpret_cast<const double*>(p + dy * kRow + dl * 16 + (X ? 0 : 8));
+}
+
+struct Th {                                  // per-thread constants
+    unsigned char* phi0;                     // own slot of phi stage 0
+    const unsigned char* coef0;              // own slot of coefficient stage 0, array C_AX
+    bool ra_x, ra_y, ba, rb_x, rb_y, own;    // lateral validity of the four half-sweeps (x / y cell of the pair)
+    long long img_x, img_y;                  // periodic images of the own pair (0 = none)
+    // half-sweep h is applied at step kk iff (unsigned)(kk - lo[h]) <= span[h]: the planes it is wanted on
+    // (sweep-1 red [k0-3, k1+2], black [k0-2, k1+1], sweep-2 red [k0-1, k1], black [k0, k1-1]) that exist
+    int lo[4];
+    unsigned span[4];
+    int nlo; unsigned nspan;                 // NORM: planes [k0, k1)
+};
+
+// Gauss-Seidel update of column X of the pair in one plane.  ph: own slot of that plane's phi stage
+// (lateral neighbours), other: the pair's other cell, C: the plane's coefficients, az_up: low z faces
+// of the plane above, d_ / u_: vertical neighbours (u_ is on the dependent chain, see fused::gs_value).
+template <bool X>
+__device__ __forceinline__ double gs_cell(const unsigned char* ph, double other, const Coef& C, const double2& az_up,
+                                          double d_, double u_, double& a, double& dg)
+{
+    const double w_ = X ? ldc<false>(ph, 0, -1) : other;
+    const double e_ = X ? other : ldc<true>(ph, 0, 1);
+    const double s_ = ldc<X>(ph, -1, 0);
+    const double n_ = ldc<X>(ph, 1, 0);
+    return fused::gs_value(X ? C.ax.x : C.ax.y, X ? C.ax.y : C.ax2, pick<X>(C.ays), pick<X>(C.ayn), pick<X>(C.az),
+                           pick<X>(az_up), pick<X>(C.rhs), w_, e_, s_, n_, d_, u_, a, dg);
+}
+
+// issue the five box loads of plane p (unwrapped) into the phi stage at byte offset op / coefficient stage at oc
+template <int LA>
+__device__ __forceinline__ void issue_plane(const CUtensorMap* tm_phi, const CUtensorMap* tm_rhs, const CUtensorMap* tm_ax,
+                                            const CUtensorMap* tm_ay, const CUtensorMap* tm_az, unsigned phi_ring,
+                                            unsigned coef_ring, unsigned bar0, unsigned op, unsigned oc, int p, int nz,
+                                            bool perz, int cx, int cy)
+{
+    using G = Cfg<LA>;
+    if (perz) { if (p < 0) p += nz; else if (p >= nz) p -= nz; }
+    const unsigned dp = phi_ring + op;
+    const unsigned dc = coef_ring + oc;
+    const unsigned bar = bar0 + op / (kPl / 8);                                // barrier of phi stage op / kPl
+    mbar_expect_tx(bar, G::kTx);
+    tma_load_3d(dp, tm_phi, bar, cx, cy, p);                                   // rows 0 .. TYE-1
+    tma_load_3d(dc + C_RHS * kPl + kRow, tm_rhs, bar, cx, cy + 1, p);          // rows 1 .. TYE-2
+    tma_load_3d(dc + C_AX * kPl + kRow, tm_ax, bar, cx, cy + 1, p);
+    tma_load_3d(dc + C_AZ * kPl + kRow, tm_az, bar, cx, cy + 1, p);
+    tma_load_3d(dc + C_AY * kPl + kRow, tm_ay, bar, cx, cy + 1, p);            // rows 1 .. TYE-1 (faces)
+}
+
+// One marching step at plane kk; X: the x column of the pair is red in plane kk.
+// CUR receives the coefficients of plane kk; S1, S2, S3 hold those of planes kk-1, kk-2, kk-3.
+template <bool X, bool NORM>
+__device__ __forceinline__ void step(const Th& T, int kk, unsigned char* s0, unsigned char* sM1, unsigned char* sM2,
+                                     const unsigned char* sM3, const unsigned char* sP, const unsigned char* cI,
+                                     const unsigned char* cP, double* __restrict__ out, double2& Pn, double2& Pm1,
+                                     double2& Pm2, double2& Pm3, double2& Pm4, double2& azn, Coef& CUR, const Coef& S1,
+                                     const Coef& S2, const Coef& S3, double& vmax)
+{
+    const bool v0 = (unsigned)(kk - T.lo[0]) <= T.span[0], v1 = (unsigned)(kk - T.lo[1]) <= T.span[1];
+    const bool v2 = (unsigned)(kk - T.lo[2]) <= T.span[2], v3 = (unsigned)(kk - T.lo[3]) <= T.span[3];
+    double2 P0 = Pn;                                  // old phi of plane kk (staged read of the last step)
+    CUR.az = azn;
+    Pn = ldp(sP);                                     // old phi and low z faces of plane kk+1
+    azn = ldp(cP + C_AZ * kPl);
+    CUR.ax = ldp(cI + C_AX * kPl);
+    CUR.ax2 = *reinterpret_cast<const double*>(cI + C_AX * kPl + 16);
+    CUR.ays = ldp(cI + C_AY * kPl);
+    CUR.ayn = ldp(cI + C_AY * kPl + kRow);
+    CUR.rhs = ldp(cI + C_RHS * kPl);
+    double a, dg;
+    {   // (1) sweep 1, red cells of plane kk
+        const double nv = gs_cell<X>(s0, pick<!X>(P0), CUR, azn, pick<X>(Pm1), pick<X>(Pn), a, dg);
+        if (NORM && T.own && (unsigned)(kk - T.nlo) <= T.nspan)
+            vmax = nanmax(vmax, fabs(fma(pick<X>(P0), dg, -a)));              // |rhs - (sum - phi_0 dg)| of the input
+        const double val = ((X ? T.ra_x : T.ra_y) && v0) ? nv : pick<X>(P0);
+        put<X>(P0, val);
+        *reinterpret_cast<double*>(s0 + (X ? 0 : 8)) = val;
+    }
+    {   // (2) sweep 1, black cells of plane kk-1
+        const double nv = gs_cell<X>(sM1, pick<!X>(Pm1), S1, CUR.az, pick<X>(Pm2), pick<X>(P0), a, dg);
+        const double val = (T.ba && v1) ? nv : pick<X>(Pm1);
+        put<X>(Pm1, val);
+        *reinterpret_cast<double*>(sM1 + (X ? 0 : 8)) = val;
+    }
+    {   // (3) sweep 2, red cells of plane kk-2
+        const double nv = gs_cell<X>(sM2, pick<!X>(Pm2), S2, S1.az, pick<X>(Pm3), pick<X>(Pm1), a, dg);
+        const double val = ((X ? T.rb_x : T.rb_y) && v2) ? nv : pick<X>(Pm2);
+        put<X>(Pm2, val);
+        *reinterpret_cast<double*>(sM2 + (X ? 0 : 8)) = val;
+    }
+    {   // (4) sweep 2, black cells of plane kk-3; the plane is finished
+        const double nv = gs_cell<X>(sM3, pick<!X>(Pm3), S3, S2.az, pick<X>(Pm4), pick<X>(Pm2), a, dg);
+        if (T.own && v3) {
+            put<X>(Pm3, nv);
+            store_images(reinterpret_cast<double2*>(out), Pm3, T.img_x, T.img_y);
+        }
+    }
+    Pm4 = Pm3; Pm3 = Pm2; Pm2 = Pm1; Pm1 = P0;
+}
+
+template <int LA, bool REDX0, bool NORM>
+__device__ __forceinline__ void march(const Th& T, int ks, int ke, const CUtensorMap* tm_phi, const CUtensorMap* tm_rhs,
+                                      const CUtensorMap* tm_ax, const CUtensorMap* tm_ay, const CUtensorMap* tm_az,
+                                      unsigned phi_ring, unsigned coef_ring, unsigned bar0, bool producer, int cx, int cy,
+                                      int nz, bool perz, double* __restrict__ out, unsigned long long out_stride, double& vmax)
+{
+    using G = Cfg<LA>;
+    constexpr unsigned kPhiRing = G::NP * kPl, kCoefRing = G::NC * G::kCoef;
+    const double2 z2 = make_double2(0.0, 0.0);
+    double2 Pm1, Pm2 = z2, Pm3 = z2, Pm4 = z2;
+    Coef cA, cB, cC, cD;
+    cB.ax = cB.ays = cB.ayn = cB.az = cB.rhs = z2; cB.ax2 = 0.0;
+    cC = cB; cD = cB;
+    // the prologue issued planes ks-1 .. ks+LA into phi / coefficient stages 0 .. LA+1
+    mbar_wait(bar0 + 0, 0);
+    mbar_wait(bar0 + 8, 0);
+    unsigned phase_bits = 3u;                          // bit s: parity to wait for on barrier s next
+    // byte offsets, within their rings, of the phi stages of planes kk+1, kk, kk-1, kk-2, kk-3, of the one that
+    // plane kk-4 vacated, and of the coefficient stages of planes kk+1, kk, kk-1
+    unsigned oP = 2 * kPl, o0 = kPl, o1 = 0, o2 = kPhiRing - kPl, o3 = kPhiRing - 2 * kPl, o4 = kPhiRing - 3 * kPl;
+    unsigned qP = 2 * G::kCoef, q0 = G::kCoef, q1 = 0;
+    int bP = 2;                                        // barrier (= phi stage index) of plane kk+1
+    Pm1 = ldp(T.phi0);
+    double2 Pn = ldp(T.phi0 + kPl);
+    double2 azn = ldp(T.coef0 + G::kCoef + C_AZ * kPl);
+#define MAC_T2_STEP(XX, CUR, S1, S2, S3)                                                                              \
+    {                                                                                                                 \
+        if (kk > ke) break;                                                                                           \
+        mbar_wait(bar0 + 8 * bP, (phase_bits >> bP) & 1u);         /* plane kk+1 has landed */                        \
+        phase_bits ^= 1u << bP;                                                                                       \
+        __syncthreads();                                           /* every thread has finished step kk-1 */          \
+        if (producer && kk + 1 + LA <= ke + 1) {                   /* never leave a load in flight at exit */         \
+            asm volatile("fence.proxy.async.shared::cta;\n" ::: "memory");                                            \
+            issue_plane<LA>(tm_phi, tm_rhs, tm_ax, tm_ay, tm_az, phi_ring, coef_ring, bar0, o4, q1, kk + 1 + LA, nz,  \
+                            perz, cx, cy);                                                                            \
+        }                                                                                                             \
+        step<XX, NORM>(T, kk, T.phi0 + o0, T.phi0 + o1, T.phi0 + o2, T.phi0 + o3, T.phi0 + oP, T.coef0 + q0,          \
+                       T.coef0 + qP, out, Pn, Pm1, Pm2, Pm3, Pm4, azn, CUR, S1, S2, S3, vmax);                        \
+        out += out_stride;                                                                                            \
+        o4 = o3; o3 = o2; o2 = o1; o1 = o0; o0 = oP;                                                                  \
+        oP += kPl; if (oP == kPhiRing) oP = 0;                                                                        \
+        q1 = q0; q0 = qP;                                                                                             \
+        qP += G::kCoef; if (qP == kCoefRing) qP = 0;                                                                  \
+        if (++bP == G::NP) bP = 0;                                                                                    \
+        ++kk;                                                                                                         \
+    }
+#pragma unroll 1
+    for (int kk = ks; kk <= ke;) {
+        MAC_T2_STEP(REDX0, cA, cD, cC, cB)
+        MAC_T2_STEP(!REDX0, cB, cA, cD, cC)
+        MAC_T2_STEP(REDX0, cC, cB, cA, cD)
+        MAC_T2_STEP(!REDX0, cD, cC, cB, cA)
+    }
+#undef MAC_T2_STEP
+}
+
+// NORM: additionally writes, per CTA, max |rhs - L phi_in| over the red cells to part_max[linear CTA index]
+template <int LA, bool NORM>
+__global__ void __launch_bounds__(NT, 1)
+k_rbgs_t2(const __grid_constant__ CUtensorMap tm_phi, const __grid_constant__ CUtensorMap tm_rhs,
+          const __grid_constant__ CUtensorMap tm_ax, const __grid_constant__ CUtensorMap tm_ay,
+          const __grid_constant__ CUtensorMap tm_az, LevelDev L, double* __restrict__ pout, int zchunk,
+          double* __restrict__ part_max)
+{
+    using G = Cfg<LA>;
+    extern __shared__ __align__(128) unsigned char smem_dyn[];
+    unsigned char* smem_raw = smem_dyn + ((128u - (smem_u32(smem_dyn) & 127u)) & 127u);
+    unsigned char* phi_gen = smem_raw + kPad;
+    const unsigned phi_ring = smem_u32(phi_gen);
+    const unsigned coef_ring = phi_ring + G::NP * kPl;
+    const unsigned bar0 = coef_ring + G::NC * G::kCoef;
+
+    const int lane = threadIdx.x;
+    // a warp holds two rows; they must share their parity (the colour role is warp-uniform)
+    const int ty = 4 * ((int)threadIdx.y >> 2) + (((int)threadIdx.y >> 1) & 1) + 2 * ((int)threadIdx.y & 1);
+    const int x0 = blockIdx.x * kTX, y0 = blockIdx.y * kTY;
+    const int k0 = blockIdx.z * zchunk, k1 = min(k0 + zchunk, L.nz);
+    const int gi = x0 - HALO + 2 * lane, gj = y0 - HALO + ty;
+    // ghost columns / rows of a periodic level hold valid images: they are recomputed like any halo cell
+    const bool col_ok = gi >= -L.gx && gi < L.nx + L.gx && gj >= -L.gy && gj < L.ny + L.gy;
+    const bool producer = threadIdx.x == 0 && threadIdx.y == 0;
+
+    Th T;
+    T.ra_x = col_ok && ty >= 1 && ty <= TYE - 2 && lane >= 1;
+    T.ra_y = col_ok && ty >= 1 && ty <= TYE - 2 && lane <= LN - 2;
+    T.ba = col_ok && ty >= 2 && ty <= TYE - 3 && lane >= 1 && lane <= LN - 2;
+    T.rb_x = col_ok && ty >= 3 && ty <= TYE - 4 && lane >= 2 && lane <= LN - 2;
+    T.rb_y = col_ok && ty >= 3 && ty <= TYE - 4 && lane >= 1 && lane <= LN - 3;
+    T.own = ty >= HALO && ty <= TYE - 1 - HALO && lane >= 2 && lane <= LN - 3 && gi < L.nx && gj < L.ny;
+    T.img_x = T.own ? image_dx(L, gi) : 0;
+    T.img_y = T.own ? image_dy(L, gj) : 0;
+    const bool perz = L.bclo[2] == MAC_PERIODIC;
+    {
+        const int wl[4] = {k0 - 3, k0 - 2, k0 - 1, k0}, wh[4] = {k1 + 2, k1 + 1, k1, k1 - 1};
+        for (int h = 0; h < 4; ++h) {                  // half-sweep h acts on plane kk - h
+            const int lo = perz ? wl[h] : max(wl[h], 0), hi = perz ? wh[h] : min(wh[h], L.nz - 1);
+            T.lo[h] = lo + h;
+            T.span[h] = hi >= lo ? (unsigned)(hi - lo) : 0u;
+            if (hi < lo) T.lo[h] = INT_MIN / 2;        // never
+        }
+        T.nlo = k0;
+        T.nspan = (unsigned)(k1 - 1 - k0);
+    }
+    const unsigned slot = (ty * LN + lane) * 16;
+    T.phi0 = phi_gen + slot;
+    T.coef0 = phi_gen + G::NP * kPl + slot;
+    const int cx0 = x0 - HALO + L.gx, cy0 = y0 - HALO + L.gy;     // tensor-map coordinates of the tile origin
+
+    const int ks = k0 - 3;
+    if (producer) {
+        for (int s = 0; s < G::NP; ++s) mbar_init(bar0 + 8 * s, 1);
+        asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
+        asm volatile("fence.proxy.async.shared::cta;\n" ::: "memory");
+        for (int q = 0; q < LA + 2 && ks - 1 + q <= k1 + 3; ++q)
+            issue_plane<LA>(&tm_phi, &tm_rhs, &tm_ax, &tm_ay, &tm_az, phi_ring, coef_ring, bar0, q * kPl, q * G::kCoef, ks - 1 + q, L.nz,
+                            perz, cx0, cy0);
+    }
+    __syncthreads();                                             // barrier inits visible before anyone waits
+
+    const unsigned long long ostride = (unsigned long long)L.cx * L.ry;
+    double* out = pout + (T.own ? (long long)gi + (long long)L.cx * gj : 0) + (long long)(ks - 3) * (long long)ostride;
+    double vmax = 0.0;
+    if (((gj + ks) & 1) == 0)
+        march<LA, true, NORM>(T, ks, k1 + 2, &tm_phi, &tm_rhs, &tm_ax, &tm_ay, &tm_az, phi_ring, coef_ring, bar0, producer, cx0, cy0, L.nz, perz, out, ostride, vmax);
+    else
+        march<LA, false, NORM>(T, ks, k1 + 2, &tm_phi, &tm_rhs, &tm_ax, &tm_ay, &tm_az, phi_ring, coef_ring, bar0, producer, cx0, cy0, L.nz, perz, out, ostride, vmax);
+    // every plane that was issued (<= k1 + 3) has been waited for by the last step: nothing is in flight
+    if (NORM) {
+        __shared__ double sh_max[32];
+        const int tid = threadIdx.x + LN * threadIdx.y;
+        vmax = warp_nanmax(vmax);
+        if ((tid & 31) == 0) sh_max[tid >> 5] = vmax;
+        __syncthreads();
+        if (tid == 0) {
+            double m = sh_max[0];
+            for (int q = 1; q < NT / 32; ++q) m = nanmax(m, sh_max[q]);
+            part_max[blockIdx.x + gridDim.x * (blockIdx.y + gridDim.y * blockIdx.z)] = m;
+        }
+    }
+}
+
+}  // namespace t2
+
+// ---- host side ---------------------------------------------------------------------------------
+
+#ifndef MAC_T2_LA
+#define MAC_T2_LA 4                   // planes of TMA lookahead (shared memory: 0.5 + 6 (LA+5) + 24 (LA+2) KB)
+#endif
+
+static inline int t2_smoother_configure()
+{
+    using namespace t2;
+    const int sm = (int)Cfg<MAC_T2_LA>::kSmem;
+    if (cudaFuncSetAttribute(k_rbgs_t2<MAC_T2_LA, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, sm) != cudaSuccess) return -1;
+    if (cudaFuncSetAttribute(k_rbgs_t2<MAC_T2_LA, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, sm) != cudaSuccess) return -1;
+    return 0;
+}
+
+// the two-sweep kernel needs its 4-cell halo inside the periodic images and a few planes to march through
+static inline bool t2_level_ok(const LevelDev& L)
+{
+    if (L.nx < 48 || L.ny < 16 || L.nz < 8 || (L.nx & 1)) return false;
+    if (L.bclo[0] == MAC_PERIODIC && L.gx < t2::HALO) return false;
+    if (L.bclo[1] == MAC_PERIODIC && L.gy < t2::HALO) return false;
+    return true;
+}
+
+static inline dim3 t2_sweep_grid(const LevelDev& L, int* zchunk_out)
+{
+    const int tiles_x = (L.nx + t2::kTX - 1) / t2::kTX, tiles_y = (L.ny + t2::kTY - 1) / t2::kTY;
+    // chunk count that minimises waves x (planes per chunk + the 6 redone planes + pipeline fill)
+    const int tiles = tiles_x * tiles_y;
+    long best = -1; int bn = 1;
+    const int maxchunk = L.nz >= 32 ? L.nz / 16 : 1;
+    for (int n = 1; n <= maxchunk; ++n) {
+        const int zc = (L.nz + n - 1) / n;
+        const int nn = (L.nz + zc - 1) / zc;
+        const long waves = ((long)tiles * nn + 147) / 148;
+        const long cost = waves * (zc + 10);
+        if (best < 0 || cost < best) { best = cost; bn = nn; }
+    }
+    if (zchunk_out) *zchunk_out = (L.nz + bn - 1) / bn;
+    return dim3(tiles_x, tiles_y, bn);
+}
+
+// Two fused sweeps: reads `in_is_phi2 ? phi2 : phi` through T (maps built for the 32 x 24 tile), writes phi_out.
+// part_max != NULL: also per-CTA maxima of the input's red-cell residual; *nparts receives their count.
+static inline int launch_t2_sweep(const TmaLevelMaps& T, bool in_is_phi2, double* phi_out, const LevelDev& L, cudaStream_t s,
+                                  double* part_max = nullptr, int max_parts = 0, int* nparts = nullptr)
+{
+    using namespace t2;
+    int zchunk;
+    const dim3 grid = t2_sweep_grid(L, &zchunk);
+    const CUtensorMap& tin = in_is_phi2 ? T.phi2 : T.phi;
+    const size_t sm = Cfg<MAC_T2_LA>::kSmem;
+    if (part_max) {
+        if ((long)grid.x * grid.y * grid.z > max_parts) return -1;
+        *nparts = (int)(grid.x * grid.y * grid.z);
+        k_rbgs_t2<MAC_T2_LA, true><<<grid, dim3(LN, TYE), sm, s>>>(tin, T.rhs, T.ax, T.ay, T.az, L, phi_out, zchunk, part_max);
+    } else
+        k_rbgs_t2<MAC_T2_LA, false><<<grid, dim3(LN, TYE), sm, s>>>(tin, T.rhs, T.ax, T.ay, T.az, L, phi_out, zchunk, nullptr);
+    return cudaPeekAtLastError() == cudaSuccess ? 0 : -1;
+}

@@ -14,6 +14,7 @@
 #include "mac_kernels.cuh"
 #include "mac_smoother.cuh"
 #include "mac_smoother_tma.cuh"
+#include "mac_smoother_t2.cuh"
 
 namespace {
 
@@ -34,7 +35,7 @@ struct Level {
     size_t off_c, off_ax;          // entries from an allocation's base to the interior origin
     double *phi, *phi2, *rhs, *ax, *ay, *az;   // interior origins
     double* phi_a;                 // the buffer `phi` pointed to at carve time (tensor map `phi`)
-    TmaLevelMaps tma[2];           // [0] MAC_TMA_BIG tile, [1] MAC_TMA_MID tile
+    TmaLevelMaps tma[3];           // [0] MAC_TMA_BIG tile, [1] MAC_TMA_MID tile, [2] two-sweep kernel's 32 x 24 tile
 };
 
 struct Staging {
@@ -64,6 +65,7 @@ struct maestro_mac_handle {
     cudaEvent_t* sm_ev;            // 2 * kSmoothEvents events, or NULL
     int sm_used;                   // pairs recorded by the current call
     int sm_launches;               // level-0 smoother launches of the current call (recorded or not)
+    int sm_sweeps;                 // sweeps applied by the recorded launches (a two-sweep launch counts 2)
 };
 
 namespace {
@@ -96,7 +98,7 @@ int validate_and_default(const maestro_mac_desc* in, maestro_mac_desc* d)
     if (!(d->bottom_rel_tol > 0.0)) d->bottom_rel_tol = 1e-8;
     if (d->prolongation != 0 && d->prolongation != 1) return MAESTRO_MAC_ERR_ARG;
     if (d->host_staging != 0 && d->host_staging != 1) return MAESTRO_MAC_ERR_ARG;
-    if (d->smoother < 0 || d->smoother > 3) return MAESTRO_MAC_ERR_ARG;
+    if (d->smoother < 0 || d->smoother > 4) return MAESTRO_MAC_ERR_ARG;   // 4: two-sweep kernel
     if (d->stop_test != 0 && d->stop_test != 1) return MAESTRO_MAC_ERR_ARG;
     return MAESTRO_MAC_OK;
 }
@@ -111,9 +113,10 @@ int build_levels(const maestro_mac_desc& d, Level* lev, int* nlev)
         Level& L = lev[l];
         for (int a = 0; a < 3; ++a) { L.n[a] = n[a]; L.h[a] = h[a]; }
         // levels that run the TMA-staged kernels carry periodic image columns / rows (TMA cannot wrap)
-        const bool tma_level = (d.smoother == 0 || d.smoother == 3) && n[0] >= 60 && (n[0] & 1) == 0 && n[1] >= 4;
-        L.gx = (tma_level && d.bc_lo[0] == MAESTRO_MAC_PERIODIC) ? 2 : 0;
-        L.gy = (tma_level && d.bc_lo[1] == MAESTRO_MAC_PERIODIC) ? 2 : 0;
+        const bool tma_level = (d.smoother == 0 || d.smoother == 3 || d.smoother == 4) && n[0] >= 60 && (n[0] & 1) == 0 && n[1] >= 4;
+        const int gw = d.smoother == 4 ? t2::HALO : 2;         // the two-sweep kernel's halo is 4 cells
+        L.gx = (tma_level && d.bc_lo[0] == MAESTRO_MAC_PERIODIC) ? gw : 0;
+        L.gy = (tma_level && d.bc_lo[1] == MAESTRO_MAC_PERIODIC) ? gw : 0;
         L.cx = n[0] + 2 * L.gx;
         L.ry = n[1] + 2 * L.gy;
         L.px = (int)align_up((size_t)n[0] + 1 + 2 * L.gx, 4);
@@ -311,7 +314,7 @@ int do_sweep(maestro_mac_handle* H, int l, cudaStream_t s, int* norm_parts = nul
     if (l == 0) ++H->sm_launches;
     if (timed) CUDA_OK(cudaEventRecord(H->sm_ev[2 * H->sm_used], s));
     const int sm = H->d.smoother;
-    const int tv = (sm == 0 && L.nx >= 60) ? 0 : (sm == 3 ? 1 : -1);          // TMA tile variant, or -1
+    const int tv = ((sm == 0 || sm == 4) && L.nx >= 60) ? 0 : (sm == 3 ? 1 : -1);   // TMA tile variant, or -1
     if (tv >= 0 && H->lev[l].tma[tv].ok) {
         int rc = launch_tma_sweep(H->lev[l].tma[tv], H->lev[l].phi != H->lev[l].phi_a, H->lev[l].phi2, L, tv, s,
                                   norm_parts ? H->part_max : nullptr, kMaxParts, norm_parts);
@@ -334,12 +337,39 @@ int do_sweep(maestro_mac_handle* H, int l, cudaStream_t s, int* norm_parts = nul
         k_rbgs_color<<<g, b, 0, s>>>(L, 1);
         LAUNCHED(H);
     }
-    if (timed) { CUDA_OK(cudaEventRecord(H->sm_ev[2 * H->sm_used + 1], s)); ++H->sm_used; }
+    if (timed) { CUDA_OK(cudaEventRecord(H->sm_ev[2 * H->sm_used + 1], s)); ++H->sm_used; ++H->sm_sweeps; }
+    return MAESTRO_MAC_OK;
+}
+
+// the two-sweep kernel runs with the default smoother on levels its tile and halo fit
+bool t2_ok(const maestro_mac_handle* H, int l)
+{
+    return H->d.smoother == 4 && H->lev[l].tma[2].ok && t2_level_ok(dev_level(H, l));
+}
+
+// Two sweeps on level l in one pass (k_rbgs_t2).  norm_parts / swap as in do_sweep.
+int do_sweep2(maestro_mac_handle* H, int l, cudaStream_t s, int* norm_parts = nullptr, bool swap = true)
+{
+    Level& Lv = H->lev[l];
+    const bool timed = l == 0 && H->sm_ev && H->sm_used < kSmoothEvents;
+    if (l == 0) ++H->sm_launches;
+    if (timed) CUDA_OK(cudaEventRecord(H->sm_ev[2 * H->sm_used], s));
+    if (launch_t2_sweep(Lv.tma[2], Lv.phi != Lv.phi_a, Lv.phi2, dev_level(H, l), s, norm_parts ? H->part_max : nullptr,
+                        kMaxParts, norm_parts) != 0)
+        return MAESTRO_MAC_ERR_CUDA;
+    ++H->launches;
+    if (swap) { double* t = Lv.phi; Lv.phi = Lv.phi2; Lv.phi2 = t; }
+    if (timed) { CUDA_OK(cudaEventRecord(H->sm_ev[2 * H->sm_used + 1], s)); ++H->sm_used; H->sm_sweeps += 2; }
     return MAESTRO_MAC_OK;
 }
 
 int do_smooth(maestro_mac_handle* H, int l, int nsweeps, cudaStream_t s)
 {
+    if (t2_ok(H, l))
+        for (; nsweeps >= 2; nsweeps -= 2) {
+            int rc = do_sweep2(H, l, s);
+            if (rc != 0) return rc;
+        }
     for (int sw = 0; sw < nsweeps; ++sw) {
         int rc = do_sweep(H, l, s);
         if (rc != 0) return rc;
@@ -350,7 +380,7 @@ int do_smooth(maestro_mac_handle* H, int l, int nsweeps, cudaStream_t s)
 // TMA transfer kernels are used with the default smoother on levels the tensor maps cover
 bool tma_aux(const maestro_mac_handle* H, int l)
 {
-    return H->d.smoother == 0 && H->lev[l].tma[0].ok && H->lev[l].n[0] >= 60 && H->lev[l].n[2] >= 2;
+    return (H->d.smoother == 0 || H->d.smoother == 4) && H->lev[l].tma[0].ok && H->lev[l].n[0] >= 60 && H->lev[l].n[2] >= 2;
 }
 
 int do_residual_restrict(maestro_mac_handle* H, int l, cudaStream_t s)
@@ -406,19 +436,24 @@ int do_bottom(maestro_mac_handle* H, cudaStream_t s)
 bool fused_norm_ok(const maestro_mac_handle* H)
 {
     const Level& L0 = H->lev[0];
-    if (H->d.stop_test != 0 || H->d.smoother != 0 || H->nlev < 2 || H->d.nu_pre < 1 || H->d.nu_post < 1) return false;
+    if (H->d.stop_test != 0 || (H->d.smoother != 0 && H->d.smoother != 4) || H->nlev < 2 || H->d.nu_pre < 1 || H->d.nu_post < 1) return false;
     if (!L0.tma[0].ok || L0.n[0] < 60) return false;
     const dim3 g = tma_sweep_grid(dev_level(H, 0), 0, nullptr);
-    return (long)g.x * g.y * g.z <= kMaxParts;
+    if ((long)g.x * g.y * g.z > kMaxParts) return false;
+    if (t2_ok(H, 0)) {
+        const dim3 g2 = t2_sweep_grid(dev_level(H, 0), nullptr);
+        if ((long)g2.x * g2.y * g2.z > kMaxParts) return false;
+    }
+    return true;
 }
 
-// first_pre_done: the first level-0 pre-sweep of this cycle has already been applied (it carried the
-// stop test of the previous cycle, see maestro_mac_project)
-int do_vcycle(maestro_mac_handle* H, cudaStream_t s, bool first_pre_done = false)
+// pre_done: level-0 pre-sweeps of this cycle that have already been applied (they carried the stop test
+// of the previous cycle, see maestro_mac_project)
+int do_vcycle(maestro_mac_handle* H, cudaStream_t s, int pre_done = 0)
 {
     int rc;
     for (int l = 0; l + 1 < H->nlev; ++l) {
-        if ((rc = do_smooth(H, l, H->d.nu_pre - ((l == 0 && first_pre_done) ? 1 : 0), s)) != 0) return rc;
+        if ((rc = do_smooth(H, l, H->d.nu_pre - (l == 0 ? pre_done : 0), s)) != 0) return rc;
         if ((rc = do_residual_restrict(H, l, s)) != 0) return rc;
     }
     if ((rc = do_bottom(H, s)) != 0) return rc;
@@ -517,18 +552,19 @@ extern "C" int maestro_mac_setup(const maestro_mac_desc* desc, void* workspace, 
               cudaMallocHost((void**)&H->host_flags, 4 * sizeof(int)) == cudaSuccess;
     for (int e = 0; ok && e < 4; ++e) ok = cudaEventCreate(&H->ev[e]) == cudaSuccess;
     H->sm_ev = nullptr;
-    H->sm_used = H->sm_launches = 0;
+    H->sm_used = H->sm_launches = H->sm_sweeps = 0;
     if (ok) {
         H->sm_ev = (cudaEvent_t*)std::calloc(2 * kSmoothEvents, sizeof(cudaEvent_t));
         ok = H->sm_ev != nullptr;
         for (int e = 0; ok && e < 2 * kSmoothEvents; ++e) ok = cudaEventCreate(&H->sm_ev[e]) == cudaSuccess;
     }
-    if (ok) ok = smoother_configure() == 0 && tma_smoother_configure() == 0 && tma_resid_configure() == 0;
+    if (ok) ok = smoother_configure() == 0 && tma_smoother_configure() == 0 && tma_resid_configure() == 0 && t2_smoother_configure() == 0;
     if (ok)
         for (int l = 0; l < H->nlev; ++l) {          // tensor maps; a level that cannot use TMA keeps cp.async
             LevelDev D = dev_level(H, l);
             tma_build_maps(&H->lev[l].tma[0], D, 32, 16);
             tma_build_maps(&H->lev[l].tma[1], D, 16, 16);
+            tma_build_maps(&H->lev[l].tma[2], D, t2::LN, t2::TYE);
             // a level laid out with periodic images has no other smoother: its tensor maps must exist
             if ((D.gx || D.gy) && !H->lev[l].tma[H->d.smoother == 3 ? 1 : 0].ok) ok = false;
         }
@@ -571,7 +607,7 @@ extern "C" int maestro_mac_project(maestro_mac_handle* H, const double* beta0, c
     st.singular = H->singular;
     st.levels = H->nlev;
     H->launches = 0;
-    H->sm_used = H->sm_launches = 0;
+    H->sm_used = H->sm_launches = H->sm_sweeps = 0;
     int rc;
     int result = MAESTRO_MAC_OK;
     Level& L0 = H->lev[0];
@@ -596,14 +632,15 @@ extern "C" int maestro_mac_project(maestro_mac_handle* H, const double* beta0, c
         result = d.rel_tol > 0.0 ? MAESTRO_MAC_NOT_CONVERGED : MAESTRO_MAC_OK;
         if (d.rel_tol > 0.0) {
             const bool ride = fused_norm_ok(H);
-            bool first_pre_done = false;
+            const bool ride2 = ride && d.nu_pre >= 2 && t2_ok(H, 0);     // the speculative launch is a two-sweep pass
+            int pre_done = 0;
             while (st.cycles < d.max_cycles) {
-                if ((rc = do_vcycle(H, s, first_pre_done)) != 0) return rc;
-                first_pre_done = false;
-                const bool spec = ride && st.cycles + 1 < d.max_cycles;   // speculative first sweep of the next cycle
+                if ((rc = do_vcycle(H, s, pre_done)) != 0) return rc;
+                pre_done = 0;
+                const bool spec = ride && st.cycles + 1 < d.max_cycles;   // speculative first sweep(s) of the next cycle
                 if (spec) {
                     int nparts = 0;
-                    if ((rc = do_sweep(H, 0, s, &nparts, false)) != 0) return rc;
+                    if ((rc = ride2 ? do_sweep2(H, 0, s, &nparts, false) : do_sweep(H, 0, s, &nparts, false)) != 0) return rc;
                     k_reduce_final<<<1, 1024, 0, s>>>(H->part_sum, H->part_max, nparts, H->scal + 3);
                     LAUNCHED(H);
                 } else if ((rc = do_residual_norm(H, 0, s)) != 0) return rc;
@@ -615,9 +652,9 @@ extern "C" int maestro_mac_project(maestro_mac_handle* H, const double* beta0, c
                 ++st.cycles;
                 if (rel != rel) { result = MAESTRO_MAC_ERR_NONFINITE; break; }
                 if (rel <= d.rel_tol) { result = MAESTRO_MAC_OK; break; }   // (a speculative sweep's output is dropped)
-                if (spec) {                                                  // keep it: it is the next cycle's first pre-sweep
+                if (spec) {                                                  // keep it: the next cycle's first pre-sweep(s)
                     double* t = L0.phi; L0.phi = L0.phi2; L0.phi2 = t;
-                    first_pre_done = true;
+                    pre_done = ride2 ? 2 : 1;
                 }
             }
         } else {
@@ -657,6 +694,7 @@ extern "C" int maestro_mac_project(maestro_mac_handle* H, const double* beta0, c
         cudaEventElapsedTime(&st.ms_correct, H->ev[2], H->ev[3]);
         st.smooth0_launches = H->sm_launches;
         st.smooth0_timed = H->sm_used;
+        st.smooth0_sweeps_timed = H->sm_sweeps;
         double acc = 0.0;
         for (int q = 0; q < H->sm_used; ++q) {
             float ms = 0.0f;

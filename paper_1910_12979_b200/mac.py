@@ -45,7 +45,8 @@ class Stats(C.Structure):
                 ("rhs_mean_removed", C.c_double), ("res_history", C.c_double * 128),
                 ("ms_setup_kernels", C.c_float), ("ms_vcycles", C.c_float),
                 ("ms_correct", C.c_float), ("gpu_launches", C.c_int),
-                ("ms_smooth0", C.c_float), ("smooth0_launches", C.c_int), ("smooth0_timed", C.c_int)]
+                ("ms_smooth0", C.c_float), ("smooth0_launches", C.c_int), ("smooth0_timed", C.c_int),
+                ("smooth0_sweeps_timed", C.c_int)]
 
     def as_dict(self):
         return dict(cycles=self.cycles, bottom_iters_total=self.bottom_iters_total,
@@ -55,7 +56,7 @@ class Stats(C.Structure):
                     ms_setup_kernels=self.ms_setup_kernels, ms_vcycles=self.ms_vcycles,
                     ms_correct=self.ms_correct, gpu_launches=self.gpu_launches,
                     ms_smooth0=self.ms_smooth0, smooth0_launches=self.smooth0_launches,
-                    smooth0_timed=self.smooth0_timed)
+                    smooth0_timed=self.smooth0_timed, smooth0_sweeps_timed=self.smooth0_sweeps_timed)
 
 
 _lib = None

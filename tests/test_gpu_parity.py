@@ -71,7 +71,7 @@ def close(a, b, tol=KERNEL_TOL):
 
 
 @pytest.mark.parametrize("case", range(14))
-@pytest.mark.parametrize("smoother", [0, 1, 2, 3])
+@pytest.mark.parametrize("smoother", [0, 1, 2, 3, 4])
 def test_per_kernel_parity(oracle, mac, case, smoother):
     import torch
     O = oracle
@@ -181,7 +181,7 @@ def gpu_project(mac, wl, **over):
 
 
 @pytest.mark.parametrize("name,N", E2E_CASES)
-@pytest.mark.parametrize("smoother", [0, 1, 2, 3])
+@pytest.mark.parametrize("smoother", [0, 1, 2, 3, 4])
 def test_end_to_end_parity(oracle, mac, name, N, smoother):
     O = oracle
     wl = get_case(name, N)
@@ -300,3 +300,38 @@ def test_stop_test_riding_on_the_next_sweep(oracle, mac, name, N):
     ref = oracle_project(oracle, wl)
     assert ref["stats"]["cycles"] == a["stats"]["cycles"]
     assert np.allclose(a["stats"]["res_history"], ref["stats"]["res_history"], rtol=1e-3)
+
+
+T2_CASES = [
+    dict(n=(104, 72, 72), bc_lo=(WALL, OUT, OUT), bc_hi=(OUT, WALL, WALL), geometry=W.SPHERICAL, seed=31),
+    dict(n=(96, 48, 64), bc_lo=(PER, PER, PER), bc_hi=(PER, PER, PER), seed=32),
+    dict(n=(64, 80, 40), bc_lo=(OUT, PER, WALL), bc_hi=(WALL, PER, OUT), seed=33),
+    dict(n=(128, 16, 8), bc_lo=(PER, WALL, PER), bc_hi=(PER, WALL, PER), seed=34),
+]
+
+
+@pytest.mark.parametrize("case", range(len(T2_CASES)))
+def test_two_sweep_kernel_equals_two_single_sweeps(oracle, mac, case):
+    """k_rbgs_t2 (two sweeps per pass, smoother 4) is bit-identical to two launches of the single-sweep TMA kernel
+    (smoother 0) and matches two oracle sweeps; sizes span several tiles, a ragged tail and several z-chunks."""
+    O = oracle
+    wl = W.mixed_bc_case(**T2_CASES[case])
+    g, b, mg = oracle_structs(O, wl)
+    dv = mac.to_device(wl)
+    rng = np.random.default_rng(200 + case)
+    phi = rng.standard_normal(O.cell_shape(g)); f = rng.standard_normal(O.cell_shape(g))
+    bf = O.face_coeff(g, b, wl.beta0, wl.rho)
+    got = {}
+    for sm in (0, 4):
+        P = mac.MacProjector(mac.desc_from_workload(wl, smoother=sm))
+        P.step_coefficients(dv["beta0"], dv["rho0"], dv["rho"])
+        P.level_set(0, mac.ARR_PHI, tt(phi)); P.level_set(0, mac.ARR_RHS, tt(f))
+        P.step_smooth(0, 2)
+        got[sm, 2] = P.level_get(0, mac.ARR_PHI).cpu().numpy()
+        P.step_smooth(0, 3)                       # a pair and a single sweep
+        got[sm, 5] = P.level_get(0, mac.ARR_PHI).cpu().numpy()
+        P.close()
+    assert np.array_equal(got[0, 2], got[4, 2])
+    assert np.array_equal(got[0, 5], got[4, 5])
+    ref = phi.copy(); O.rbgs_sweep(g, *bf, f, ref); O.rbgs_sweep(g, *bf, f, ref)
+    assert close(got[4, 2], ref)
