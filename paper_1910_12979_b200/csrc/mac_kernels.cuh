@@ -659,7 +659,12 @@ __device__ __forceinline__ void correct_face(const GeoDev& G, const LevelDev& L,
     const double grad = (ghi * phi[cell(hi)] - glo * phi[cell(lo)]) * (1.0 / h);
     const double rf = 0.5 * (rho_cell(G, rho, rho0, D == 0 ? lo : i, D == 1 ? lo : j, D == 2 ? lo : k) +
                              rho_cell(G, rho, rho0, D == 0 ? hi : i, D == 1 ? hi : j, D == 2 ? hi : k));
-    const double nv = vel[fi] - grad / rf;
+    double rr;                                       // grad / rf, rf > 0 (validated by the coefficient pass)
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(rr) : "d"(rf));
+    rr = fma(fma(-rf, rr, 1.0), rr, rr);
+    rr = fma(fma(-rf, rr, 1.0), rr, rr);
+    const double qq = grad * rr;
+    const double nv = vel[fi] - fma(fma(-rf, qq, grad), rr, qq);
     vel[fi] = nv;
     if (f == 0 && per) {
         const size_t fn = (size_t)(D == 0 ? n : i) + sx * ((size_t)(D == 1 ? n : j) + sy * (size_t)(D == 2 ? n : k));

@@ -12,6 +12,7 @@
 #include <vector>
 
 #include "mac_kernels.cuh"
+#include "mac_setup.cuh"
 #include "mac_smoother.cuh"
 #include "mac_smoother_tma.cuh"
 #include "mac_smoother_t2.cuh"
@@ -244,12 +245,30 @@ int do_fill_ghosts(maestro_mac_handle* H, int l, int which, cudaStream_t s)
 
 // ---- individual steps ------------------------------------------------------------------------
 
+int do_coarsen(maestro_mac_handle* H, cudaStream_t s);
+int do_rhs_finish(maestro_mac_handle* H, int nb, cudaStream_t s);
+
+// grid of k_setup over the extended index space; the z-chunk grows until the block partials fit
+dim3 setup_grid(const GeoDev& G, int* zchunk)
+{
+    int zc = 16;
+    dim3 gg((G.nx + 64) / 64, (G.ny + 4) / 4, (G.nz + zc - 1) / zc);
+    while ((long)gg.x * gg.y * gg.z > kMaxParts) { zc *= 2; gg.z = (G.nz + zc - 1) / zc; }
+    *zchunk = zc;
+    return gg;
+}
+
 int do_coefficients(maestro_mac_handle* H, const double* beta0, const double* rho0, const double* rho, cudaStream_t s)
 {
     GeoDev G = dev_geo(H);
     dim3 g, b;
     CUDA_OK(cudaMemsetAsync(H->flags, 0, 16 * sizeof(int), s));
-    if (H->d.smoother != 1) {
+    if (H->d.smoother != 1 && rho) {
+        const int zc = 16;
+        dim3 gg((G.nx + 64) / 64, (G.ny + 4) / 4, (G.nz + zc - 1) / zc);
+        k_setup<true, false><<<gg, dim3(64, 4), 0, s>>>(G, dev_geo_inv(H), dev_level(H, 0), beta0, rho, nullptr, nullptr, nullptr,
+                                                        nullptr, zc, H->flags, nullptr, nullptr);
+    } else if (H->d.smoother != 1) {
         const int zc = 16;
         dim3 gg((G.nx + 64) / 64, (G.ny + 4) / 4, (G.nz + zc) / zc);
         k_face_coeff2<<<gg, dim3(64, 4), 0, s>>>(G, dev_geo_inv(H), dev_level(H, 0), beta0, rho, rho0, zc, H->flags);
@@ -258,6 +277,13 @@ int do_coefficients(maestro_mac_handle* H, const double* beta0, const double* rh
         k_face_coeff<<<g, b, 0, s>>>(G, dev_level(H, 0), beta0, rho, rho0, H->flags);
     }
     LAUNCHED(H);
+    return do_coarsen(H, s);
+}
+
+// a3: periodic images of the level-0 coefficients, then every coarser level
+int do_coarsen(maestro_mac_handle* H, cudaStream_t s)
+{
+    dim3 g, b;
     int rc;
     if ((rc = do_fill_ghosts(H, 0, GH_AX | GH_AY | GH_AZ, s)) != 0) return rc;
     for (int l = 0; l + 1 < H->nlev; ++l) {
@@ -275,14 +301,13 @@ int do_rhs(maestro_mac_handle* H, const double* beta0, const double* u, const do
            const double* S, cudaStream_t s)
 {
     GeoDev G = dev_geo(H);
-    Level& L0 = H->lev[0];
     int nb;
     if (H->d.smoother != 1) {
-        int zc = 16;
-        dim3 gg((G.nx + 63) / 64, (G.ny + 3) / 4, (G.nz + zc - 1) / zc);
-        while ((long)gg.x * gg.y * gg.z > kMaxParts) { zc *= 2; gg.z = (G.nz + zc - 1) / zc; }
+        int zc;
+        const dim3 gg = setup_grid(G, &zc);
         nb = (int)(gg.x * gg.y * gg.z);
-        k_rhs2<<<gg, dim3(64, 4), 0, s>>>(G, dev_geo_inv(H), dev_level(H, 0), beta0, u, v, w, S, zc, H->part_sum, H->part_max);
+        k_setup<false, true><<<gg, dim3(64, 4), 0, s>>>(G, dev_geo_inv(H), dev_level(H, 0), beta0, nullptr, u, v, w, S, zc,
+                                                        H->flags, H->part_sum, H->part_max);
     } else {
         int rows = G.ny * G.nz;
         nb = red_blocks(rows);
@@ -290,6 +315,29 @@ int do_rhs(maestro_mac_handle* H, const double* beta0, const double* u, const do
         k_rhs<<<nb, bt, 0, s>>>(G, dev_level(H, 0), beta0, u, v, w, S, H->part_sum, H->part_max);
     }
     LAUNCHED(H);
+    return do_rhs_finish(H, nb, s);
+}
+
+// a2 + a4 in one pass (k_setup<true, true>), then coarsening and the rhs reductions
+int do_setup_fused(maestro_mac_handle* H, const double* beta0, const double* rho, const double* u, const double* v,
+                   const double* w, const double* S, cudaStream_t s)
+{
+    GeoDev G = dev_geo(H);
+    CUDA_OK(cudaMemsetAsync(H->flags, 0, 16 * sizeof(int), s));
+    int zc;
+    const dim3 gg = setup_grid(G, &zc);
+    k_setup<true, true><<<gg, dim3(64, 4), 0, s>>>(G, dev_geo_inv(H), dev_level(H, 0), beta0, rho, u, v, w, S, zc, H->flags,
+                                                   H->part_sum, H->part_max);
+    LAUNCHED(H);
+    int rc;
+    if ((rc = do_coarsen(H, s)) != 0) return rc;
+    return do_rhs_finish(H, (int)(gg.x * gg.y * gg.z), s);
+}
+
+// folds the nb block partials of the rhs pass: sum/max of the final rhs in scal[0..1], removed sum in scal[2]
+int do_rhs_finish(maestro_mac_handle* H, int nb, cudaStream_t s)
+{
+    Level& L0 = H->lev[0];
     k_reduce_final<<<1, 1024, 0, s>>>(H->part_sum, H->part_max, nb, H->scal);
     LAUNCHED(H);
     if (H->singular) {
@@ -492,6 +540,13 @@ int do_correct(maestro_mac_handle* H, const double* phi, const double* rho0, con
 {
     GeoDev G = dev_geo(H);
     dim3 g, b;
+    if (rho && H->d.smoother == 2) {      // column-marching form: measured slower than one thread per face index
+        const int zc = 16;
+        dim3 gg((G.nx + 64) / 64, (G.ny + 4) / 4, (G.nz + zc - 1) / zc);
+        k_correct2<<<gg, dim3(64, 4), 0, s>>>(G, dev_geo_inv(H), dev_level(H, 0), phi, rho, u, v, w, zc);
+        LAUNCHED(H);
+        return MAESTRO_MAC_OK;
+    }
     dims3(G.nx + 1, G.ny + 1, G.nz + 1, &g, &b);
     k_correct<<<g, b, 0, s>>>(G, dev_level(H, 0), phi, rho, rho0, u, v, w);
     LAUNCHED(H);
@@ -613,8 +668,12 @@ extern "C" int maestro_mac_project(maestro_mac_handle* H, const double* beta0, c
     Level& L0 = H->lev[0];
 
     CUDA_OK(cudaEventRecord(H->ev[0], s));
-    if ((rc = do_coefficients(H, beta0, rho0, rho, s)) != 0) return rc;
-    if ((rc = do_rhs(H, beta0, u, v, w, S, s)) != 0) return rc;
+    if (rho && d.smoother != 1) {
+        if ((rc = do_setup_fused(H, beta0, rho, u, v, w, S, s)) != 0) return rc;
+    } else {
+        if ((rc = do_coefficients(H, beta0, rho0, rho, s)) != 0) return rc;
+        if ((rc = do_rhs(H, beta0, u, v, w, S, s)) != 0) return rc;
+    }
     CUDA_OK(cudaMemcpyAsync(H->host_scal, H->scal, 3 * sizeof(double), cudaMemcpyDeviceToHost, s));
     CUDA_OK(cudaMemcpyAsync(H->host_flags, H->flags, sizeof(int), cudaMemcpyDeviceToHost, s));
     CUDA_OK(cudaMemsetAsync(L0.phi - L0.off_c, 0, L0.acell * sizeof(double), s));   // A16: phi = 0 (ghosts too)
