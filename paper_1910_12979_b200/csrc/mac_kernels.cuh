@@ -514,7 +514,9 @@ k_residual(LevelDev L, double* __restrict__ out)
 // by warp shuffles + one shared-memory stage (deterministic).  Stops at ||r||2 <= tol ||f||2,
 // maxit iterations, or breakdown (the current iterate is kept) -- reading A15.
 // Singular problems: f is projected to zero mean first and x to zero mean last.
-// Vectors r, rhat, p, v, s, t live in `vecs` (6 * nb doubles, cache resident).
+// Vectors r, rhat, p, v, s, t and the iterate x live in shared memory when 7 * nb doubles fit
+// (use_smem; every vector operation is then an on-chip round trip instead of an L2 one: a value
+// written by one thread and read by another does not stay in L1), else in `vecs` / L.phi.
 // ------------------------------------------------------------------------------------------------
 
 struct Dot2 { double a, b; };
@@ -544,19 +546,21 @@ __device__ __forceinline__ double bottom_matvec_at(const LevelDev& L, const doub
 }
 
 __global__ void __launch_bounds__(1024)
-k_bottom_bicgstab(LevelDev L, double* __restrict__ vecs, int maxit, double tol, int singular,
-                  int* __restrict__ iters_accum)
+k_bottom_bicgstab(LevelDev L, double* vecs, int maxit, double tol, int singular,
+                  int* __restrict__ iters_accum, int use_smem)
 {
     __shared__ double sh[64];
+    extern __shared__ double bottom_sm[];
     const int nb = L.nx * L.ny * L.nz;
-    double* __restrict__ x = L.phi;
     const double* __restrict__ f = L.rhs;
-    double* r = vecs;
-    double* rhat = vecs + nb;
-    double* p = vecs + 2 * (size_t)nb;
-    double* v = vecs + 3 * (size_t)nb;
-    double* s = vecs + 4 * (size_t)nb;
-    double* t = vecs + 5 * (size_t)nb;
+    double* base = use_smem ? bottom_sm : vecs;
+    double* r = base;
+    double* rhat = base + nb;
+    double* p = base + 2 * (size_t)nb;
+    double* v = base + 3 * (size_t)nb;
+    double* s = base + 4 * (size_t)nb;
+    double* t = base + 5 * (size_t)nb;
+    double* x = use_smem ? base + 6 * (size_t)nb : L.phi;
     const int tid = threadIdx.x, nt = blockDim.x;
 
     double fm = 0.0;
@@ -619,13 +623,15 @@ k_bottom_bicgstab(LevelDev L, double* __restrict__ vecs, int maxit, double tol, 
             if (omega == 0.0) break;
         }
     }
+    double xm = 0.0;
     if (singular) {
         __syncthreads();
         double a = 0.0;
         for (int c = tid; c < nb; c += nt) a += x[c];
-        const double xm = block_dot2(a, 0.0, sh).a / (double)nb;
-        for (int c = tid; c < nb; c += nt) x[c] -= xm;
+        xm = block_dot2(a, 0.0, sh).a / (double)nb;
     }
+    if (singular || use_smem)
+        for (int c = tid; c < nb; c += nt) L.phi[c] = x[c] - xm;
     if (tid == 0 && iters_accum) *iters_accum += it;
 }
 

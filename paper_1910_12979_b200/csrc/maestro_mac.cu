@@ -23,6 +23,7 @@ constexpr int kMaxLevels = 32;
 constexpr int kRedBlocks = 148 * 8;       // blocks of the row-walking reduction kernels
 constexpr int kMaxParts = 131072;         // capacity of the partial-reduction arrays
 constexpr int kBottomMax = 4096;          // largest coarsest level (unknowns)
+constexpr size_t kBottomSmem = 200 * 1024; // bottom-solver vectors live in shared memory up to this size
 constexpr int kSmoothEvents = 512;        // level-0 smoother launches timed per call
 
 struct Level {
@@ -104,6 +105,25 @@ int validate_and_default(const maestro_mac_desc* in, maestro_mac_desc* d)
     return MAESTRO_MAC_OK;
 }
 
+// geometry of one level; ghosts: the level runs TMA-staged kernels and carries periodic images
+void set_level(const maestro_mac_desc& d, Level& L, const int n[3], const double h[3], bool ghosts)
+{
+    for (int a = 0; a < 3; ++a) { L.n[a] = n[a]; L.h[a] = h[a]; }
+    const int gw = d.smoother == 4 ? t2::HALO : 2;         // the two-sweep kernel's halo is 4 cells
+    L.gx = (ghosts && d.bc_lo[0] == MAESTRO_MAC_PERIODIC) ? gw : 0;
+    L.gy = (ghosts && d.bc_lo[1] == MAESTRO_MAC_PERIODIC) ? gw : 0;
+    L.cx = n[0] + 2 * L.gx;
+    L.ry = n[1] + 2 * L.gy;
+    L.px = (int)align_up((size_t)n[0] + 1 + 2 * L.gx, 4);
+    L.ncell = (size_t)n[0] * n[1] * n[2];
+    L.acell = (size_t)L.cx * L.ry * n[2];
+    L.nax = (size_t)L.px * L.ry * n[2];
+    L.nay = (size_t)L.cx * (L.ry + 1) * n[2];
+    L.naz = (size_t)L.cx * L.ry * (n[2] + 1);
+    L.off_c = (size_t)L.gx + (size_t)L.cx * L.gy;
+    L.off_ax = (size_t)L.gx + (size_t)L.px * L.gy;
+}
+
 // Build level geometry; returns OK or UNSUPPORTED.
 int build_levels(const maestro_mac_desc& d, Level* lev, int* nlev)
 {
@@ -111,27 +131,13 @@ int build_levels(const maestro_mac_desc& d, Level* lev, int* nlev)
     double h[3] = {d.dx[0], d.dx[1], d.dx[2]};
     int l = 0;
     for (;;) {
-        Level& L = lev[l];
-        for (int a = 0; a < 3; ++a) { L.n[a] = n[a]; L.h[a] = h[a]; }
         // levels that run the TMA-staged kernels carry periodic image columns / rows (TMA cannot wrap)
         const bool tma_level = (d.smoother == 0 || d.smoother == 3 || d.smoother == 4) && n[0] >= 60 && (n[0] & 1) == 0 && n[1] >= 4;
-        const int gw = d.smoother == 4 ? t2::HALO : 2;         // the two-sweep kernel's halo is 4 cells
-        L.gx = (tma_level && d.bc_lo[0] == MAESTRO_MAC_PERIODIC) ? gw : 0;
-        L.gy = (tma_level && d.bc_lo[1] == MAESTRO_MAC_PERIODIC) ? gw : 0;
-        L.cx = n[0] + 2 * L.gx;
-        L.ry = n[1] + 2 * L.gy;
-        L.px = (int)align_up((size_t)n[0] + 1 + 2 * L.gx, 4);
-        L.ncell = (size_t)n[0] * n[1] * n[2];
-        L.acell = (size_t)L.cx * L.ry * n[2];
-        L.nax = (size_t)L.px * L.ry * n[2];
-        L.nay = (size_t)L.cx * (L.ry + 1) * n[2];
-        L.naz = (size_t)L.cx * L.ry * (n[2] + 1);
-        L.off_c = (size_t)L.gx + (size_t)L.cx * L.gy;
-        L.off_ax = (size_t)L.gx + (size_t)L.px * L.gy;
-        ++l;
-        bool can = l < kMaxLevels;
+        bool can = l + 1 < kMaxLevels;
         for (int a = 0; a < 3; ++a)
             if ((n[a] & 1) || n[a] / 2 < d.coarsest_n) can = false;
+        set_level(d, lev[l], n, h, tma_level && can);      // the coarsest level is only solved, never smoothed: plain layout
+        ++l;
         if (!can) break;
         for (int a = 0; a < 3; ++a) { n[a] /= 2; h[a] *= 2.0; }
     }
@@ -471,8 +477,10 @@ int do_bottom(maestro_mac_handle* H, cudaStream_t s)
     int l = H->nlev - 1;
     int nb = (int)H->lev[l].ncell;
     int threads = nb >= 1024 ? 1024 : ((nb + 31) / 32) * 32;
-    k_bottom_bicgstab<<<1, threads, 0, s>>>(dev_level(H, l), H->bottom_vecs, H->d.bottom_max_iter,
-                                            H->d.bottom_rel_tol, H->singular, H->flags + 1);
+    const size_t sm = 7 * (size_t)nb * sizeof(double);
+    const int use_smem = sm <= kBottomSmem ? 1 : 0;
+    k_bottom_bicgstab<<<1, threads, use_smem ? sm : 0, s>>>(dev_level(H, l), H->bottom_vecs, H->d.bottom_max_iter,
+                                                            H->d.bottom_rel_tol, H->singular, H->flags + 1, use_smem);
     LAUNCHED(H);
     return MAESTRO_MAC_OK;
 }
@@ -613,6 +621,7 @@ extern "C" int maestro_mac_setup(const maestro_mac_desc* desc, void* workspace, 
         ok = H->sm_ev != nullptr;
         for (int e = 0; ok && e < 2 * kSmoothEvents; ++e) ok = cudaEventCreate(&H->sm_ev[e]) == cudaSuccess;
     }
+    if (ok) ok = cudaFuncSetAttribute(k_bottom_bicgstab, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kBottomSmem) == cudaSuccess;
     if (ok) ok = smoother_configure() == 0 && tma_smoother_configure() == 0 && tma_resid_configure() == 0 && t2_smoother_configure() == 0;
     if (ok)
         for (int l = 0; l < H->nlev; ++l) {          // tensor maps; a level that cannot use TMA keeps cp.async

@@ -157,12 +157,17 @@ def test_per_kernel_parity(oracle, mac, case, smoother):
 
 
 E2E_CASES = [("1", 32), ("2", 32), ("3N", 32), ("3D", 32), ("4N", 32), ("4D", 64), ("5", 32),
-             ("2", 64), ("3N", 64), ("mixed", 0), ("mixed_sph", 0), ("1", 64), ("5", 128)]
+             ("2", 64), ("3N", 64), ("mixed", 0), ("mixed_sph", 0), ("1", 64), ("5", 128), ("wide_bottom", 0)]
 
 
 def get_case(name, N):
     if name == "mixed":
         return W.mixed_bc_case(n=(32, 16, 24))
+    if name == "wide_bottom":    # the coarsest level (64 x 8 x 4, periodic in x) is as wide as a TMA level: it keeps the plain layout
+        wl = W.mixed_bc_case(n=(128, 16, 8), bc_lo=(PER, WALL, OUT), bc_hi=(PER, WALL, WALL), seed=22)
+        wl.dx = (1.0 / 128,) * 3          # cubic cells (point Gauss-Seidel does not like the 20:1 boxes of the recipe)
+        wl.dr = wl.dx[2]
+        return wl
     if name == "mixed_sph":
         return W.mixed_bc_case(n=(16, 48, 32), geometry=W.SPHERICAL, seed=21)
     return W.by_name(name, N)
