@@ -545,24 +545,14 @@ __device__ __forceinline__ double bottom_matvec_at(const LevelDev& L, const doub
     return off - x[c] * dg;
 }
 
-__global__ void __launch_bounds__(1024)
-k_bottom_bicgstab(LevelDev L, double* vecs, int maxit, double tol, int singular,
-                  int* __restrict__ iters_accum, int use_smem)
+// The solver proper, run by one thread block: solves L x = f (x, f and the six work vectors may live in shared or
+// global memory; x and f in the level's plain layout).  Returns the iteration count (same in every thread).
+__device__ __forceinline__ int bicgstab_block(const LevelDev& L, double* x, const double* f, double* r, double* rhat,
+                                              double* p, double* v, double* s, double* t, int maxit, double tol,
+                                              int singular, double* sh)
 {
-    __shared__ double sh[64];
-    extern __shared__ double bottom_sm[];
     const int nb = L.nx * L.ny * L.nz;
-    const double* __restrict__ f = L.rhs;
-    double* base = use_smem ? bottom_sm : vecs;
-    double* r = base;
-    double* rhat = base + nb;
-    double* p = base + 2 * (size_t)nb;
-    double* v = base + 3 * (size_t)nb;
-    double* s = base + 4 * (size_t)nb;
-    double* t = base + 5 * (size_t)nb;
-    double* x = use_smem ? base + 6 * (size_t)nb : L.phi;
     const int tid = threadIdx.x, nt = blockDim.x;
-
     double fm = 0.0;
     if (singular) {
         double a = 0.0;
@@ -623,16 +613,31 @@ k_bottom_bicgstab(LevelDev L, double* vecs, int maxit, double tol, int singular,
             if (omega == 0.0) break;
         }
     }
-    double xm = 0.0;
-    if (singular) {
+    if (singular) {                            // zero-mean x
         __syncthreads();
         double a = 0.0;
         for (int c = tid; c < nb; c += nt) a += x[c];
-        xm = block_dot2(a, 0.0, sh).a / (double)nb;
+        const double xm = block_dot2(a, 0.0, sh).a / (double)nb;
+        for (int c = tid; c < nb; c += nt) x[c] -= xm;
     }
-    if (singular || use_smem)
-        for (int c = tid; c < nb; c += nt) L.phi[c] = x[c] - xm;
-    if (tid == 0 && iters_accum) *iters_accum += it;
+    __syncthreads();
+    return it;
+}
+
+__global__ void __launch_bounds__(1024)
+k_bottom_bicgstab(LevelDev L, double* vecs, int maxit, double tol, int singular,
+                  int* __restrict__ iters_accum, int use_smem)
+{
+    __shared__ double sh[64];
+    extern __shared__ double bottom_sm[];
+    const int nb = L.nx * L.ny * L.nz;
+    double* base = use_smem ? bottom_sm : vecs;
+    double* x = use_smem ? base + 6 * (size_t)nb : L.phi;
+    const int it = bicgstab_block(L, x, L.rhs, base, base + nb, base + 2 * (size_t)nb, base + 3 * (size_t)nb,
+                                  base + 4 * (size_t)nb, base + 5 * (size_t)nb, maxit, tol, singular, sh);
+    if (use_smem)
+        for (int c = threadIdx.x; c < nb; c += blockDim.x) L.phi[c] = x[c];
+    if (threadIdx.x == 0 && iters_accum) *iters_accum += it;
 }
 
 // ------------------------------------------------------------------------------------------------

@@ -16,6 +16,7 @@
 #include "mac_smoother.cuh"
 #include "mac_smoother_tma.cuh"
 #include "mac_smoother_t2.cuh"
+#include "mac_tail.cuh"
 
 namespace {
 
@@ -51,6 +52,8 @@ struct maestro_mac_handle {
     int nlev;
     Level lev[kMaxLevels];
     int singular;
+    int tail_start;                // first level of the one-launch coarse tail (k_coarse_tail), or -1
+    size_t tail_smem;
     // scratch carved from the workspace
     double *part_sum, *part_max;   // kRedBlocks each
     double *scal;                  // device scalars: [0] sum, [1] max (k_reduce_final output) ...
@@ -472,6 +475,44 @@ int do_prolong(maestro_mac_handle* H, int l, cudaStream_t s)
     return MAESTRO_MAC_OK;
 }
 
+// The coarse tail: the first level of at most kTailMaxCells cells from which everything down to the coarsest
+// level fits one thread block's shared memory.  Not with the reference (1) and cp.async-only (2) smoothers,
+// which keep one launch per step on every level.
+void plan_tail(maestro_mac_handle* H)
+{
+    H->tail_start = -1;
+    H->tail_smem = 0;
+    if (H->d.smoother == 1 || H->d.smoother == 2) return;
+    for (int t0 = 0; t0 + 1 < H->nlev; ++t0) {
+        if (H->lev[t0].ncell > (size_t)kTailMaxCells || H->nlev - t0 > kTailMaxLevels) continue;
+        if (H->lev[t0].gx || H->lev[t0].gy) continue;
+        size_t need = 0;
+        for (int l = t0; l < H->nlev; ++l) need += 2 * H->lev[l].ncell * sizeof(double);
+        need += 6 * H->lev[H->nlev - 1].ncell * sizeof(double);
+        if (need > kTailSmem) continue;
+        H->tail_start = t0;
+        H->tail_smem = need;
+        return;
+    }
+}
+
+// levels tail_start .. coarsest in one launch; load_phi: level tail_start is level 0 of the solve
+int do_tail(maestro_mac_handle* H, cudaStream_t s)
+{
+    TailArgs A;
+    A.nlev = H->nlev - H->tail_start;
+    for (int q = 0; q < A.nlev; ++q) A.L[q] = dev_level(H, H->tail_start + q);
+    A.nu_pre = H->d.nu_pre; A.nu_post = H->d.nu_post;
+    A.maxit = H->d.bottom_max_iter; A.tol = H->d.bottom_rel_tol;
+    A.singular = H->singular; A.prolongation = H->d.prolongation;
+    A.load_phi = H->tail_start == 0 ? 1 : 0;
+    const size_t nc = H->lev[H->tail_start].ncell;
+    const int threads = nc >= 2048 ? 1024 : (nc >= 512 ? 256 : 64);
+    k_coarse_tail<<<1, threads, H->tail_smem, s>>>(A, H->flags + 1);
+    LAUNCHED(H);
+    return MAESTRO_MAC_OK;
+}
+
 int do_bottom(maestro_mac_handle* H, cudaStream_t s)
 {
     int l = H->nlev - 1;
@@ -508,12 +549,15 @@ bool fused_norm_ok(const maestro_mac_handle* H)
 int do_vcycle(maestro_mac_handle* H, cudaStream_t s, int pre_done = 0)
 {
     int rc;
-    for (int l = 0; l + 1 < H->nlev; ++l) {
+    // with a coarse tail the levels from tail_start down are one launch (pre_done only ever concerns a level-0
+    // TMA sweep, i.e. a level far above the tail)
+    const int lend = H->tail_start >= 0 ? H->tail_start : H->nlev - 1;
+    for (int l = 0; l < lend; ++l) {
         if ((rc = do_smooth(H, l, H->d.nu_pre - (l == 0 ? pre_done : 0), s)) != 0) return rc;
         if ((rc = do_residual_restrict(H, l, s)) != 0) return rc;
     }
-    if ((rc = do_bottom(H, s)) != 0) return rc;
-    for (int l = H->nlev - 2; l >= 0; --l) {
+    if ((rc = H->tail_start >= 0 ? do_tail(H, s) : do_bottom(H, s)) != 0) return rc;
+    for (int l = lend - 1; l >= 0; --l) {
         if ((rc = do_prolong(H, l, s)) != 0) return rc;
         if ((rc = do_smooth(H, l, H->d.nu_post, s)) != 0) return rc;
     }
@@ -621,6 +665,8 @@ extern "C" int maestro_mac_setup(const maestro_mac_desc* desc, void* workspace, 
         ok = H->sm_ev != nullptr;
         for (int e = 0; ok && e < 2 * kSmoothEvents; ++e) ok = cudaEventCreate(&H->sm_ev[e]) == cudaSuccess;
     }
+    plan_tail(H);
+    if (ok) ok = cudaFuncSetAttribute(k_coarse_tail, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kTailSmem) == cudaSuccess;
     if (ok) ok = cudaFuncSetAttribute(k_bottom_bicgstab, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kBottomSmem) == cudaSuccess;
     if (ok) ok = smoother_configure() == 0 && tma_smoother_configure() == 0 && tma_resid_configure() == 0 && t2_smoother_configure() == 0;
     if (ok)
