@@ -521,14 +521,18 @@ k_residual(LevelDev L, double* __restrict__ out)
 
 struct Dot2 { double a, b; };
 
-__device__ __forceinline__ Dot2 block_dot2(double a, double b, double* sh)
+// barrier among the first nt threads of the block (nt a multiple of 32): the solver runs on as many warps as
+// the coarsest level has work for, also inside a larger block (k_coarse_tail)
+__device__ __forceinline__ void group_sync(int nt) { asm volatile("bar.sync 1, %0;" ::"r"(nt) : "memory"); }
+
+__device__ __forceinline__ Dot2 block_dot2(double a, double b, double* sh, int nt)
 {
     a = warp_sum(a);
     b = warp_sum(b);
-    const int w = threadIdx.x >> 5, l = threadIdx.x & 31, nw = (blockDim.x + 31) >> 5;
-    __syncthreads();                      // protect sh from the previous use
+    const int w = threadIdx.x >> 5, l = threadIdx.x & 31, nw = (nt + 31) >> 5;
+    group_sync(nt);                      // protect sh from the previous use
     if (l == 0) { sh[2 * w] = a; sh[2 * w + 1] = b; }
-    __syncthreads();
+    group_sync(nt);
     a = l < nw ? sh[2 * l] : 0.0;
     b = l < nw ? sh[2 * l + 1] : 0.0;
     Dot2 r;
@@ -545,19 +549,19 @@ __device__ __forceinline__ double bottom_matvec_at(const LevelDev& L, const doub
     return off - x[c] * dg;
 }
 
-// The solver proper, run by one thread block: solves L x = f (x, f and the six work vectors may live in shared or
+// The solver proper, run by the first nt threads of one thread block: solves L x = f (x, f and the six work vectors may live in shared or
 // global memory; x and f in the level's plain layout).  Returns the iteration count (same in every thread).
 __device__ __forceinline__ int bicgstab_block(const LevelDev& L, double* x, const double* f, double* r, double* rhat,
                                               double* p, double* v, double* s, double* t, int maxit, double tol,
-                                              int singular, double* sh)
+                                              int singular, double* sh, int nt)
 {
     const int nb = L.nx * L.ny * L.nz;
-    const int tid = threadIdx.x, nt = blockDim.x;
+    const int tid = threadIdx.x;                   // < nt: only the first nt threads of the block call this
     double fm = 0.0;
     if (singular) {
         double a = 0.0;
         for (int c = tid; c < nb; c += nt) a += f[c];
-        fm = block_dot2(a, 0.0, sh).a / (double)nb;
+        fm = block_dot2(a, 0.0, sh, nt).a / (double)nb;
     }
     double rr = 0.0;
     for (int c = tid; c < nb; c += nt) {
@@ -565,7 +569,7 @@ __device__ __forceinline__ int bicgstab_block(const LevelDev& L, double* x, cons
         r[c] = fv; rhat[c] = fv; p[c] = 0.0; v[c] = 0.0; x[c] = 0.0;
         rr += fv * fv;
     }
-    rr = block_dot2(rr, 0.0, sh).a;            // (r,r) = (rhat,r)
+    rr = block_dot2(rr, 0.0, sh, nt).a;            // (r,r) = (rhat,r)
     const double bnorm2 = rr;
     int it = 0;
     if (bnorm2 > 0.0 && bnorm2 == bnorm2) {
@@ -575,15 +579,15 @@ __device__ __forceinline__ int bicgstab_block(const LevelDev& L, double* x, cons
             if (rho == 0.0) break;                                   // breakdown
             const double beta = it == 0 ? 0.0 : (rho / rho_old) * (alpha / omega);
             for (int c = tid; c < nb; c += nt) p[c] = r[c] + beta * (p[c] - omega * v[c]);
-            __syncthreads();
+            group_sync(nt);
             double d = 0.0;
             for (int c = tid; c < nb; c += nt) { double y = bottom_matvec_at(L, p, c); v[c] = y; d += rhat[c] * y; }
-            d = block_dot2(d, 0.0, sh).a;
+            d = block_dot2(d, 0.0, sh, nt).a;
             if (d == 0.0) break;
             alpha = rho / d;
             double ss = 0.0;
             for (int c = tid; c < nb; c += nt) { double y = r[c] - alpha * v[c]; s[c] = y; ss += y * y; }
-            ss = block_dot2(ss, 0.0, sh).a;                          // also makes s visible
+            ss = block_dot2(ss, 0.0, sh, nt).a;                          // also makes s visible
             ++it;
             if (ss <= stop2) {
                 for (int c = tid; c < nb; c += nt) x[c] += alpha * p[c];
@@ -592,7 +596,7 @@ __device__ __forceinline__ int bicgstab_block(const LevelDev& L, double* x, cons
             }
             double ts = 0.0, tt = 0.0;
             for (int c = tid; c < nb; c += nt) { double y = bottom_matvec_at(L, s, c); t[c] = y; ts += y * s[c]; tt += y * y; }
-            Dot2 q = block_dot2(ts, tt, sh);
+            Dot2 q = block_dot2(ts, tt, sh, nt);
             if (q.b == 0.0) {
                 for (int c = tid; c < nb; c += nt) x[c] += alpha * p[c];
                 break;
@@ -606,7 +610,7 @@ __device__ __forceinline__ int bicgstab_block(const LevelDev& L, double* x, cons
                 r2 += y * y;
                 hr += rhat[c] * y;
             }
-            q = block_dot2(r2, hr, sh);
+            q = block_dot2(r2, hr, sh, nt);
             rr = q.a;
             rho_old = rho;
             rho = q.b;
@@ -614,13 +618,13 @@ __device__ __forceinline__ int bicgstab_block(const LevelDev& L, double* x, cons
         }
     }
     if (singular) {                            // zero-mean x
-        __syncthreads();
+        group_sync(nt);
         double a = 0.0;
         for (int c = tid; c < nb; c += nt) a += x[c];
-        const double xm = block_dot2(a, 0.0, sh).a / (double)nb;
+        const double xm = block_dot2(a, 0.0, sh, nt).a / (double)nb;
         for (int c = tid; c < nb; c += nt) x[c] -= xm;
     }
-    __syncthreads();
+    group_sync(nt);
     return it;
 }
 
@@ -634,7 +638,7 @@ k_bottom_bicgstab(LevelDev L, double* vecs, int maxit, double tol, int singular,
     double* base = use_smem ? bottom_sm : vecs;
     double* x = use_smem ? base + 6 * (size_t)nb : L.phi;
     const int it = bicgstab_block(L, x, L.rhs, base, base + nb, base + 2 * (size_t)nb, base + 3 * (size_t)nb,
-                                  base + 4 * (size_t)nb, base + 5 * (size_t)nb, maxit, tol, singular, sh);
+                                  base + 4 * (size_t)nb, base + 5 * (size_t)nb, maxit, tol, singular, sh, blockDim.x);
     if (use_smem)
         for (int c = threadIdx.x; c < nb; c += blockDim.x) L.phi[c] = x[c];
     if (threadIdx.x == 0 && iters_accum) *iters_accum += it;

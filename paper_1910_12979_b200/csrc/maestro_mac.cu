@@ -54,6 +54,7 @@ struct maestro_mac_handle {
     int singular;
     int tail_start;                // first level of the one-launch coarse tail (k_coarse_tail), or -1
     size_t tail_smem;
+    TailArgs tail;                 // prepared by plan_tail; level pointers are filled in at launch
     // scratch carved from the workspace
     double *part_sum, *part_max;   // kRedBlocks each
     double *scal;                  // device scalars: [0] sum, [1] max (k_reduce_final output) ...
@@ -478,6 +479,8 @@ int do_prolong(maestro_mac_handle* H, int l, cudaStream_t s)
 // The coarse tail: the first level of at most kTailMaxCells cells from which everything down to the coarsest
 // level fits one thread block's shared memory.  Not with the reference (1) and cp.async-only (2) smoothers,
 // which keep one launch per step on every level.
+unsigned tail_magic(int d) { return d <= 1 ? 0u : (unsigned)((1ull << 32) / (unsigned)d + 1ull); }
+
 void plan_tail(maestro_mac_handle* H)
 {
     H->tail_start = -1;
@@ -486,21 +489,38 @@ void plan_tail(maestro_mac_handle* H)
     for (int t0 = 0; t0 + 1 < H->nlev; ++t0) {
         if (H->lev[t0].ncell > (size_t)kTailMaxCells || H->nlev - t0 > kTailMaxLevels) continue;
         if (H->lev[t0].gx || H->lev[t0].gy) continue;
-        size_t need = 0;
-        for (int l = t0; l < H->nlev; ++l) need += 2 * H->lev[l].ncell * sizeof(double);
-        need += 6 * H->lev[H->nlev - 1].ncell * sizeof(double);
-        if (need > kTailSmem) continue;
+        TailArgs& A = H->tail;
+        size_t off = 0;
+        A.nlev = H->nlev - t0;
+        for (int q = 0; q < A.nlev; ++q) {
+            const Level& L = H->lev[t0 + q];
+            TailLevel& T = A.T[q];
+            T.nx = L.n[0]; T.ny = L.n[1]; T.nz = L.n[2]; T.nc = (int)L.ncell;
+            const int hx = (T.nx + 1) / 2;
+            T.mx = tail_magic(T.nx); T.mxy = tail_magic(T.nx * T.ny); T.mhx = tail_magic(hx); T.mhxy = tail_magic(hx * T.ny);
+            for (int a = 0; a < 3; ++a) T.per[a] = H->d.bc_lo[a] == MAESTRO_MAC_PERIODIC;
+            T.o_phi = (int)off; off += (size_t)T.nc + 1;
+            T.o_rhs = (int)off; off += (size_t)T.nc;
+            T.o_ax = T.o_ay = T.o_az = 0;
+            if (q + 1 < A.nlev) {                      // the coarsest level is solved by BiCGStab from the global coefficients
+                T.o_ax = (int)off; off += (size_t)(T.nx + 1) * T.ny * T.nz;
+                T.o_ay = (int)off; off += (size_t)T.nx * (T.ny + 1) * T.nz;
+                T.o_az = (int)off; off += (size_t)T.nx * T.ny * (T.nz + 1);
+            }
+        }
+        A.o_vecs = (int)off;
+        off += 6 * H->lev[H->nlev - 1].ncell;
+        if (off * sizeof(double) > kTailSmem) continue;
         H->tail_start = t0;
-        H->tail_smem = need;
+        H->tail_smem = off * sizeof(double);
         return;
     }
 }
 
-// levels tail_start .. coarsest in one launch; load_phi: level tail_start is level 0 of the solve
+// levels tail_start .. coarsest in one launch
 int do_tail(maestro_mac_handle* H, cudaStream_t s)
 {
-    TailArgs A;
-    A.nlev = H->nlev - H->tail_start;
+    TailArgs& A = H->tail;
     for (int q = 0; q < A.nlev; ++q) A.L[q] = dev_level(H, H->tail_start + q);
     A.nu_pre = H->d.nu_pre; A.nu_post = H->d.nu_post;
     A.maxit = H->d.bottom_max_iter; A.tol = H->d.bottom_rel_tol;
