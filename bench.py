@@ -193,6 +193,21 @@ def run_reference(a):
 
 # ---- our arm ------------------------------------------------------------------------------------
 
+def aggregate_replicas(units_this_rank: float, t_dev_this_rank: float, world: int, device):
+    """Replicas only: every rank projects its own copy.  Whole-job value = the units ALL ranks
+    processed / the MAX over ranks of the device time.  Returns (value, t_max).  No data-path collective: one
+    all_reduce(MAX) of the time and one all_reduce(SUM) of the unit count, after the timed region."""
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([t_dev_this_rank], dtype=torch.float64, device=device)
+    n = torch.tensor([units_this_rank], dtype=torch.float64, device=device)
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        dist.all_reduce(n, op=dist.ReduceOp.SUM)
+    t_max = float(t.item())
+    return float(n.item()) / t_max, t_max
+
+
 def run_ours(a):
     import numpy as np
     import torch
@@ -258,13 +273,9 @@ def run_ours(a):
     clocks = sampler.stop() if rank == 0 else None
     ms = [e0.elapsed_time(e1) for e0, e1 in ev]
     t_dev = sum(ms) / 1e3
-    tmax = torch.tensor([t_dev], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
-    t_dev_max = float(tmax.item())
     cycles = stats[-1]["cycles"]
     units_per_rank = sum(wl.ncells * nu * s["cycles"] for s in stats)
-    value = world * units_per_rank / t_dev_max
+    value, t_dev_max = aggregate_replicas(units_per_rank, t_dev, world, dev)
     launches = sum(s["gpu_launches"] for s in stats)
 
     # roofline of the dominant kernel (level-0 smoother), live from the timed steps
