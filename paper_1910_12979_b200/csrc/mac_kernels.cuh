@@ -411,13 +411,21 @@ k_prolong_add(LevelDev F, LevelDev C, int prolongation)
 // coarse values come from L1/L2 (the coarse array is 1/8 of the fine one); the children are read and
 // written as four 16-byte x pairs, so a warp moves 512 contiguous bytes per row.  Interpolation is
 // done axis by axis in the order x, y, z, i.e. the expression tree of k_prolong_add.
-__global__ void __launch_bounds__(256)
+__global__ void __launch_bounds__(256, 4)
 k_prolong_add2(LevelDev F, LevelDev C, int prolongation)
 {
     const int I = blockIdx.x * blockDim.x + threadIdx.x;
     const int J = blockIdx.y * blockDim.y + threadIdx.y;
     const int K = blockIdx.z;
     if (I >= C.nx || J >= C.ny) return;
+    // the eight children, requested first: their HBM latency overlaps the (cache-resident) coarse reads below
+    double2* const fp = reinterpret_cast<double2*>(F.phi + cidx(F, 2 * I, 2 * J, 2 * K));
+    const long long frow = F.cx / 2, fpl = (long long)F.cx * F.ry / 2;      // strides in double2 (cx is even here)
+    double2 fv[2][2];
+#pragma unroll
+    for (int dk = 0; dk < 2; ++dk)
+#pragma unroll
+        for (int dj = 0; dj < 2; ++dj) fv[dk][dj] = fp[dk * fpl + dj * frow];
     double out[2][2][2];                      // [dk][dj][di]
     const double* __restrict__ e = C.phi;
     if (prolongation == 1) {
@@ -437,12 +445,15 @@ k_prolong_add2(LevelDev F, LevelDev C, int prolongation)
             sg = 1.0;
             kz[sd] = ghost_index(K + sd - 1, C.nz, C.bclo[2], C.bchi[2], sg); wz[sd] = 0.25 * sg;
         }
+        long long jo[3], ko[3];
+#pragma unroll
+        for (int q = 0; q < 3; ++q) { jo[q] = (long long)C.cx * jy[q]; ko[q] = (long long)C.cx * C.ry * kz[q]; }
         double xi[3][3][2];                   // [dz][dy][child di] after x interpolation
 #pragma unroll
         for (int dz = 0; dz < 3; ++dz)
 #pragma unroll
             for (int dy = 0; dy < 3; ++dy) {
-                const size_t row = cidx(C, 0, jy[dy], kz[dz]);
+                const long long row = jo[dy] + ko[dz];
                 const double c0 = e[row + ix[1]], cm = e[row + ix[0]], cp = e[row + ix[2]];
                 xi[dz][dy][0] = 0.75 * c0 + wx[0] * cm;
                 xi[dz][dy][1] = 0.75 * c0 + wx[2] * cp;
@@ -466,8 +477,8 @@ k_prolong_add2(LevelDev F, LevelDev C, int prolongation)
     for (int dk = 0; dk < 2; ++dk)
 #pragma unroll
         for (int dj = 0; dj < 2; ++dj) {
-            double2* p = reinterpret_cast<double2*>(F.phi + cidx(F, 2 * I, 2 * J + dj, 2 * K + dk));
-            double2 v = *p;
+            double2* p = fp + dk * fpl + dj * frow;
+            double2 v = fv[dk][dj];
             v.x += out[dk][dj][0];
             v.y += out[dk][dj][1];
             store_images(p, v, image_dx(F, 2 * I), image_dy(F, 2 * J + dj));
@@ -557,6 +568,37 @@ __device__ __forceinline__ int bicgstab_block(const LevelDev& L, double* x, cons
 {
     const int nb = L.nx * L.ny * L.nz;
     const int tid = threadIdx.x;                   // < nt: only the first nt threads of the block call this
+    // one unknown per thread (the usual 4^3 bottom): the thread keeps its row of the matrix in registers
+    // (coefficient 0 and the own index where the neighbour is outside the domain), so a matrix-vector product is
+    // six shared-memory reads instead of index arithmetic, boundary branches and global coefficient loads
+    const bool row_regs = nb <= nt;
+    double ra[6] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0}, rdg = 0.0;
+    int ri[6] = {0, 0, 0, 0, 0, 0};
+    if (row_regs && tid < nb) {
+        const int i = tid % L.nx, j = (tid / L.nx) % L.ny, k = tid / (L.nx * L.ny);
+        ra[0] = L.ax[axidx(L, i, j, k)]; ra[1] = L.ax[axidx(L, i + 1, j, k)];
+        ra[2] = L.ay[ayidx(L, i, j, k)]; ra[3] = L.ay[ayidx(L, i, j + 1, k)];
+        ra[4] = L.az[azidx(L, i, j, k)]; ra[5] = L.az[azidx(L, i, j, k + 1)];
+        rdg = ((ra[0] + ra[1]) + (ra[2] + ra[3])) + (ra[4] + ra[5]);
+        const int n3[3] = {L.nx, L.ny, L.nz}, st[3] = {1, L.nx, L.nx * L.ny}, f3[3] = {i, j, k};
+#pragma unroll
+        for (int a = 0; a < 3; ++a)
+#pragma unroll
+            for (int sd = 0; sd < 2; ++sd) {
+                const int g = f3[a] + (sd ? 1 : -1);
+                int idx = tid + (sd ? st[a] : -st[a]);
+                if (g < 0 || g >= n3[a]) {
+                    if (L.bclo[a] == MAC_PERIODIC) idx = tid + (sd ? -(n3[a] - 1) * st[a] : (n3[a] - 1) * st[a]);
+                    else { idx = tid; ra[2 * a + sd] = 0.0; }          // (rdg keeps the folded boundary coefficient)
+                }
+                ri[2 * a + sd] = idx;
+            }
+    }
+    auto matvec = [&](const double* x, int c) -> double {
+        if (!row_regs) return bottom_matvec_at(L, x, c);
+        const double off = ra[0] * x[ri[0]] + ra[1] * x[ri[1]] + ra[2] * x[ri[2]] + ra[3] * x[ri[3]] + ra[4] * x[ri[4]] + ra[5] * x[ri[5]];
+        return off - x[c] * rdg;
+    };
     double fm = 0.0;
     if (singular) {
         double a = 0.0;
@@ -581,7 +623,7 @@ __device__ __forceinline__ int bicgstab_block(const LevelDev& L, double* x, cons
             for (int c = tid; c < nb; c += nt) p[c] = r[c] + beta * (p[c] - omega * v[c]);
             group_sync(nt);
             double d = 0.0;
-            for (int c = tid; c < nb; c += nt) { double y = bottom_matvec_at(L, p, c); v[c] = y; d += rhat[c] * y; }
+            for (int c = tid; c < nb; c += nt) { double y = matvec(p, c); v[c] = y; d += rhat[c] * y; }
             d = block_dot2(d, 0.0, sh, nt).a;
             if (d == 0.0) break;
             alpha = rho / d;
@@ -595,7 +637,7 @@ __device__ __forceinline__ int bicgstab_block(const LevelDev& L, double* x, cons
                 break;
             }
             double ts = 0.0, tt = 0.0;
-            for (int c = tid; c < nb; c += nt) { double y = bottom_matvec_at(L, s, c); t[c] = y; ts += y * s[c]; tt += y * y; }
+            for (int c = tid; c < nb; c += nt) { double y = matvec(s, c); t[c] = y; ts += y * s[c]; tt += y * y; }
             Dot2 q = block_dot2(ts, tt, sh, nt);
             if (q.b == 0.0) {
                 for (int c = tid; c < nb; c += nt) x[c] += alpha * p[c];
