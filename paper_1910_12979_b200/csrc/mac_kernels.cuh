@@ -738,6 +738,31 @@ k_correct(GeoDev G, LevelDev L, const double* __restrict__ phi, const double* __
     int j = blockIdx.y * blockDim.y + threadIdx.y;
     int k = blockIdx.z;
     if (i > G.nx || j > G.ny) return;
+    if (rho && i > 0 && i < G.nx && j > 0 && j < G.ny && k > 0 && k < G.nz) {
+        // all three low faces are interior (all but a surface layer of threads): no boundary logic, one index each
+        const size_t sx = (size_t)G.nx, sxy = sx * G.ny;
+        const size_t c = (size_t)i + sx * ((size_t)j + (size_t)G.ny * k);
+        const size_t cp = cidx(L, i, j, k), px = (size_t)L.cx, pxy = px * L.ry;
+        double* pu = u + c + (size_t)j + (size_t)G.ny * k;            // (nx+1)-pitched rows
+        double* pv = v + c + sx * k;                                   // (ny+1) rows per plane
+        double* pw = w + c;
+        const double p0 = phi[cp], r0 = __ldg(rho + c);
+        const double pxm = phi[cp - 1], pym = phi[cp - px], pzm = phi[cp - pxy];
+        const double rxm = __ldg(rho + c - 1), rym = __ldg(rho + c - sx), rzm = __ldg(rho + c - sxy);
+        const double u0 = *pu, v0 = *pv, w0 = *pw;
+        auto quot = [](double g, double rf) {                          // g / rf, rf > 0
+            double rr;
+            asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(rr) : "d"(rf));
+            rr = fma(fma(-rf, rr, 1.0), rr, rr);
+            rr = fma(fma(-rf, rr, 1.0), rr, rr);
+            const double qq = g * rr;
+            return fma(fma(-rf, qq, g), rr, qq);
+        };
+        *pu = u0 - quot((p0 - pxm) * (1.0 / G.dx), 0.5 * (rxm + r0));
+        *pv = v0 - quot((p0 - pym) * (1.0 / G.dy), 0.5 * (rym + r0));
+        *pw = w0 - quot((p0 - pzm) * (1.0 / G.dz), 0.5 * (rzm + r0));
+        return;
+    }
     const bool ci = i < G.nx, cj = j < G.ny, ck = k < G.nz;
     if (cj && ck) correct_face<0>(G, L, phi, rho, rho0, u, i, j, k);
     if (ci && ck) correct_face<1>(G, L, phi, rho, rho0, v, i, j, k);
