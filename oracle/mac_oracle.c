@@ -157,6 +157,34 @@ void orc_rho_from_profile(const orc_grid *g, const orc_base *b, const double *rh
                 rho[cidx(g, i, j, k)] = beta_cell(g, b, rho0, i, j, k);
 }
 
+/* ---------- O11, O12: the base state of Eq. 5 and the dp0/dt term of Eq. 6 -------------------- */
+
+void orc_make_beta0(int nr, const double *rho0, const double *p0, const double *gamma1bar, double *beta0)
+{
+    double lnb = log(rho0[0]);                       /* beta0(0) = rho0(0)  (Eq. 5) */
+    beta0[0] = rho0[0];
+    for (int m = 0; m + 1 < nr; ++m) {
+        const double gmid = 0.5 * (gamma1bar[m] + gamma1bar[m + 1]);
+        lnb += (log(p0[m + 1]) - log(p0[m])) / gmid; /* int (1/(Gamma1bar p0)) dp0/dr dr over [r_m, r_m+1] */
+        beta0[m + 1] = exp(lnb);
+    }
+}
+
+void orc_dpdt_term(int nr, const double *p0, const double *gamma1bar, const double *dp0dt, double *q)
+{
+    for (int m = 0; m < nr; ++m) q[m] = dp0dt[m] / (gamma1bar[m] * p0[m]);
+}
+
+void orc_effective_source(const orc_grid *g, const orc_base *b, const double *S, const double *q, double *S_eff)
+{
+    for (int k = 0; k < g->n[2]; ++k)
+        for (int j = 0; j < g->n[1]; ++j)
+            for (int i = 0; i < g->n[0]; ++i) {
+                const ll c = cidx(g, i, j, k);
+                S_eff[c] = (S ? S[c] : 0.0) - beta_cell(g, b, q, i, j, k);   /* beta_cell: any profile at the cell centre */
+            }
+}
+
 /* ---------- O4: right-hand side  D(beta0 U_edge) - beta0 S   (Eq. 6) ------------------- */
 
 /* velocity on face (i,j,k) of axis d; on a periodic axis face n reads entry 0 */

@@ -132,6 +132,19 @@ int orc_project(const orc_grid *g, const orc_base *b, const orc_mg *mg,
                 double *u, double *v, double *w, const double *S, double *phi,
                 orc_stats *stats);
 
+/* O11 (Eq. 5): beta0 on the profile samples r_m = (m + 1/2) dr from p0 and Gamma1bar.
+ *   beta0_0 = rho0_0 (the innermost sample stands for r = 0; a constant factor of beta0 does not change U, pin P8),
+ *   ln beta0_{m+1} = ln beta0_m + (ln p0_{m+1} - ln p0_m) / (0.5 (Gamma1bar_m + Gamma1bar_{m+1}))
+ * i.e. the integrand (1/(Gamma1bar p0)) dp0/dr integrated as d(ln p0)/Gamma1bar with Gamma1bar taken at the
+ * midpoint; exact where Gamma1bar is constant (readings A26, A27). */
+void orc_make_beta0(int nr, const double *rho0, const double *p0, const double *gamma1bar, double *beta0);
+/* O12 (Eq. 6): the base-state term of the constraint on the samples,
+ *   q_m = dp0dt_m / (Gamma1bar_m p0_m),
+ * and the effective source  S_eff = S - q(r_cell)  (q evaluated at cell centres by O1; S may be NULL = 0),
+ * so that  rhs = D(beta0 U_edge) - beta0 (S - (1/(Gamma1bar p0)) dp0/dt)  (reading A28). */
+void orc_dpdt_term(int nr, const double *p0, const double *gamma1bar, const double *dp0dt, double *q);
+void orc_effective_source(const orc_grid *g, const orc_base *b, const double *S, const double *q, double *S_eff);
+
 /* Constraint residual  D(beta0 U) - beta0 S  (same discrete operators as orc_rhs). */
 void orc_constraint(const orc_grid *g, const orc_base *b, const double *beta0,
                     const double *u, const double *v, const double *w, const double *S,

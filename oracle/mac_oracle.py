@@ -77,6 +77,9 @@ def lib():
         L.orc_radius.argtypes = [BP, C.c_double, C.c_double, C.c_double]
         L.orc_face_coeff.argtypes = [GP, BP, _DP, _DP, _DP, _DP, _DP]
         L.orc_rho_from_profile.argtypes = [GP, BP, _DP, _DP]
+        L.orc_make_beta0.argtypes = [C.c_int, _DP, _DP, _DP, _DP]
+        L.orc_dpdt_term.argtypes = [C.c_int, _DP, _DP, _DP, _DP]
+        L.orc_effective_source.argtypes = [GP, BP, _DP, _DP, _DP]
         L.orc_rhs.argtypes = [GP, BP, _DP, _DP, _DP, _DP, _DP, _DP]
         L.orc_constraint.argtypes = [GP, BP, _DP, _DP, _DP, _DP, _DP, _DP]
         L.orc_norm_inf.restype = C.c_double
@@ -166,6 +169,27 @@ def rho_from_profile(g, b, rho0):
     rho = np.empty(cell_shape(g))
     lib().orc_rho_from_profile(C.byref(g), C.byref(b), _p(rho0), _p(rho))
     return rho
+
+
+def make_beta0(rho0, p0, gamma1bar):
+    """O11 (Eq. 5)."""
+    out = np.empty(len(rho0))
+    lib().orc_make_beta0(len(rho0), _p(rho0), _p(p0), _p(gamma1bar), _p(out))
+    return out
+
+
+def dpdt_term(p0, gamma1bar, dp0dt):
+    """O12: q = dp0dt / (Gamma1bar p0) on the samples (Eq. 6)."""
+    out = np.empty(len(p0))
+    lib().orc_dpdt_term(len(p0), _p(p0), _p(gamma1bar), _p(dp0dt), _p(out))
+    return out
+
+
+def effective_source(g, b, S, q):
+    """O12: S - q(r_cell)."""
+    out = np.empty(cell_shape(g))
+    lib().orc_effective_source(C.byref(g), C.byref(b), _p(S), _p(q), _p(out))
+    return out
 
 
 def rhs(g, b, beta0, u, v, w, S=None):

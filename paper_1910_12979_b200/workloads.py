@@ -289,6 +289,20 @@ def by_name(name: str, N: int | None = None, seed: int | None = None) -> Workloa
     return fn(**kw)
 
 
+def with_base_state(wl: Workload, gamma: float = 5.0 / 3.0, seed: int = 77) -> Workload:
+    """Adds the 1-D thermodynamic base state that Eq. 5 / Eq. 6 of the paper consume to a
+    workload, in wl.meta: p0 = rho0^gamma (a polytrope consistent with the density profile), Gamma1bar = gamma
+    (1 + 2 % smooth variation) and a smooth dp0/dt of a few per cent of p0 per unit time.  Inputs only."""
+    rng = np.random.Generator(np.random.PCG64(seed))
+    r = _profile_r(wl.nr, wl.dr)
+    L = r[-1] + 0.5 * wl.dr
+    ph = rng.uniform(0.0, 2.0 * np.pi, size=2)
+    wl.meta["p0"] = wl.rho0 ** gamma
+    wl.meta["gamma1bar"] = gamma * (1.0 + 0.02 * np.sin(2.0 * np.pi * r / L + ph[0]))
+    wl.meta["dp0dt"] = 0.05 * wl.meta["p0"] * np.cos(3.0 * np.pi * r / L + ph[1])
+    return wl
+
+
 def mixed_bc_case(n=(16, 8, 12), seed: int = 7, bc_lo=(OUTFLOW, WALL, PERIODIC),
                   bc_hi=(WALL, OUTFLOW, PERIODIC), geometry: int = PLANAR) -> Workload:
     """Small non-cubic case with every boundary type and anisotropic spacing (edge-case tests)."""
