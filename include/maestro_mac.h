@@ -162,6 +162,26 @@ int maestro_mac_project_host(maestro_mac_handle *h, const double *beta0, const d
                              const double *rho, double *u, double *v, double *w, const double *S,
                              double *phi, maestro_mac_stats *stats, void *cuda_stream);
 
+/*
+ * maestro_mac_base_state: the 1-D base-state quantities the projection consumes, from the thermodynamic
+ * base state, on the nr profile samples r_m = (m + 1/2) dr (one small kernel on `cuda_stream`):
+ *   beta0[m]      PAPER.md:45 Eq. 5, beta0(r) = rho0(0) exp(int_0^r (1/(Gamma1bar p0)) dp0/dr' dr'):
+ *                 beta0[0] = rho0[0],  ln beta0[m+1] = ln beta0[m] + (ln p0[m+1] - ln p0[m]) / (0.5 (G[m] + G[m+1]))
+ *   dpdt_term[m]  PAPER.md:49 Eq. 6, (1/(Gamma1bar p0)) dp0/dt = dp0dt[m] / (gamma1bar[m] p0[m])
+ * All pointers are DEVICE arrays of nr doubles owned by the caller; dp0dt and dpdt_term may both be NULL.
+ * p0, gamma1bar, rho0[0] must be positive.  Returns OK, ERR_ARG or ERR_CUDA.
+ */
+int maestro_mac_base_state(int nr, const double *rho0, const double *p0, const double *gamma1bar,
+                           const double *dp0dt, double *beta0, double *dpdt_term, void *cuda_stream);
+
+/*
+ * maestro_mac_set_dpdt_term: register the profile q = (1/(Gamma1bar p0)) dp0/dt (device, [nr], caller-owned,
+ * alive and unchanged during every later project call) or NULL to clear it.  With it the right-hand side is the
+ * full constraint of PAPER.md:49 Eq. 6,  rhs = D(beta0 U_edge) - beta0 (S - q(r)),  q evaluated at cell centres
+ * like every profile; without it the caller folds that term into S.  Returns OK or ERR_ARG.
+ */
+int maestro_mac_set_dpdt_term(maestro_mac_handle *h, const double *dpdt_term);
+
 /* Release the handle (host memory, pinned words, events).  NULL is a no-op.  Returns OK. */
 int maestro_mac_free(maestro_mac_handle *h);
 

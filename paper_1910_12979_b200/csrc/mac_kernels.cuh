@@ -166,7 +166,7 @@ __device__ __forceinline__ double beta_at(const GeoDev& G, const double* __restr
 __global__ void __launch_bounds__(256)
 k_rhs(GeoDev G, LevelDev L, const double* __restrict__ beta0, const double* __restrict__ u,
       const double* __restrict__ v, const double* __restrict__ w, const double* __restrict__ S,
-      double* __restrict__ part_sum, double* __restrict__ part_max)
+      const double* __restrict__ qprof, double* __restrict__ part_sum, double* __restrict__ part_max)
 {
     const int nrows = G.ny * G.nz;
     const bool px = G.bclo[0] == MAC_PERIODIC, py = G.bclo[1] == MAC_PERIODIC, pz = G.bclo[2] == MAC_PERIODIC;
@@ -188,7 +188,11 @@ k_rhs(GeoDev G, LevelDev L, const double* __restrict__ beta0, const double* __re
             double fzh = beta_at(G, beta0, xc, yc, kh * G.dz) * w[(size_t)i + (size_t)G.nx * ((size_t)j + (size_t)G.ny * kh)];
             double r = (fxh - fxl) / G.dx + (fyh - fyl) / G.dy + (fzh - fzl) / G.dz;
             const size_t c = (size_t)i + (size_t)G.nx * ((size_t)j + (size_t)G.ny * k);
-            if (S) r -= beta_at(G, beta0, xc, yc, zc) * S[c];
+            if (S || qprof) {             // source S - q(r): the dp0/dt term of PAPER.md:49 Eq. 6 rides on the profile q
+                double se = S ? S[c] : 0.0;
+                if (qprof) se -= profile_eval(qprof, G.nr, G.dr, radius(G, xc, yc, zc));
+                r -= beta_at(G, beta0, xc, yc, zc) * se;
+            }
             L.rhs[cidx(L, i, j, k)] = r;
             s += r;
             m = nanmax(m, fabs(r));

@@ -17,6 +17,7 @@
 #include "mac_smoother_tma.cuh"
 #include "mac_smoother_t2.cuh"
 #include "mac_tail.cuh"
+#include "mac_base.cuh"
 
 namespace {
 
@@ -52,6 +53,7 @@ struct maestro_mac_handle {
     int nlev;
     Level lev[kMaxLevels];
     int singular;
+    const double* dpdt_term;       // device profile q[nr] of Eq. 6 registered by maestro_mac_set_dpdt_term, or NULL
     int tail_start;                // first level of the one-launch coarse tail (k_coarse_tail), or -1
     size_t tail_smem;
     TailArgs tail;                 // prepared by plan_tail; level pointers are filled in at launch
@@ -277,7 +279,7 @@ int do_coefficients(maestro_mac_handle* H, const double* beta0, const double* rh
         const int zc = 16;
         dim3 gg((G.nx + 64) / 64, (G.ny + 4) / 4, (G.nz + zc - 1) / zc);
         k_setup<true, false><<<gg, dim3(64, 4), 0, s>>>(G, dev_geo_inv(H), dev_level(H, 0), beta0, rho, nullptr, nullptr, nullptr,
-                                                        nullptr, zc, H->flags, nullptr, nullptr);
+                                                        nullptr, nullptr, zc, H->flags, nullptr, nullptr);
     } else if (H->d.smoother != 1) {
         const int zc = 16;
         dim3 gg((G.nx + 64) / 64, (G.ny + 4) / 4, (G.nz + zc) / zc);
@@ -316,13 +318,13 @@ int do_rhs(maestro_mac_handle* H, const double* beta0, const double* u, const do
         int zc;
         const dim3 gg = setup_grid(G, &zc);
         nb = (int)(gg.x * gg.y * gg.z);
-        k_setup<false, true><<<gg, dim3(64, 4), 0, s>>>(G, dev_geo_inv(H), dev_level(H, 0), beta0, nullptr, u, v, w, S, zc,
-                                                        H->flags, H->part_sum, H->part_max);
+        k_setup<false, true><<<gg, dim3(64, 4), 0, s>>>(G, dev_geo_inv(H), dev_level(H, 0), beta0, nullptr, u, v, w, S, H->dpdt_term,
+                                                        zc, H->flags, H->part_sum, H->part_max);
     } else {
         int rows = G.ny * G.nz;
         nb = red_blocks(rows);
         int bt = G.nx >= 256 ? 256 : (G.nx >= 128 ? 128 : 64);
-        k_rhs<<<nb, bt, 0, s>>>(G, dev_level(H, 0), beta0, u, v, w, S, H->part_sum, H->part_max);
+        k_rhs<<<nb, bt, 0, s>>>(G, dev_level(H, 0), beta0, u, v, w, S, H->dpdt_term, H->part_sum, H->part_max);
     }
     LAUNCHED(H);
     return do_rhs_finish(H, nb, s);
@@ -336,8 +338,8 @@ int do_setup_fused(maestro_mac_handle* H, const double* beta0, const double* rho
     CUDA_OK(cudaMemsetAsync(H->flags, 0, 16 * sizeof(int), s));
     int zc;
     const dim3 gg = setup_grid(G, &zc);
-    k_setup<true, true><<<gg, dim3(64, 4), 0, s>>>(G, dev_geo_inv(H), dev_level(H, 0), beta0, rho, u, v, w, S, zc, H->flags,
-                                                   H->part_sum, H->part_max);
+    k_setup<true, true><<<gg, dim3(64, 4), 0, s>>>(G, dev_geo_inv(H), dev_level(H, 0), beta0, rho, u, v, w, S, H->dpdt_term, zc,
+                                                   H->flags, H->part_sum, H->part_max);
     LAUNCHED(H);
     int rc;
     if ((rc = do_coarsen(H, s)) != 0) return rc;
@@ -874,6 +876,23 @@ extern "C" int maestro_mac_project_host(maestro_mac_handle* H, const double* bet
     if (phi) CUDA_OK(cudaMemcpyAsync(phi, T.phi, nc * sizeof(double), cudaMemcpyDeviceToHost, s));
     CUDA_OK(cudaStreamSynchronize(s));
     return rc;
+}
+
+// ---- base state ---------------------------------------------------
+
+extern "C" int maestro_mac_base_state(int nr, const double* rho0, const double* p0, const double* gamma1bar,
+                                      const double* dp0dt, double* beta0, double* dpdt_term, void* cuda_stream)
+{
+    if (nr <= 0 || !rho0 || !p0 || !gamma1bar || !beta0 || (dpdt_term && !dp0dt)) return MAESTRO_MAC_ERR_ARG;
+    k_base_state<<<1, 32, 0, (cudaStream_t)cuda_stream>>>(nr, rho0, p0, gamma1bar, dp0dt, beta0, dpdt_term);
+    return cudaPeekAtLastError() == cudaSuccess ? MAESTRO_MAC_OK : MAESTRO_MAC_ERR_CUDA;
+}
+
+extern "C" int maestro_mac_set_dpdt_term(maestro_mac_handle* H, const double* dpdt_term)
+{
+    if (!H) return MAESTRO_MAC_ERR_ARG;
+    H->dpdt_term = dpdt_term;
+    return MAESTRO_MAC_OK;
 }
 
 // ---- step API ----------------------------------------------------------------------------------

@@ -25,6 +25,7 @@ EXPORTS = [
     "maestro_mac_step_coefficients", "maestro_mac_step_rhs", "maestro_mac_step_smooth",
     "maestro_mac_step_residual_restrict", "maestro_mac_step_prolong", "maestro_mac_step_bottom",
     "maestro_mac_step_vcycle", "maestro_mac_step_residual_norm", "maestro_mac_step_correct",
+    "maestro_mac_base_state", "maestro_mac_set_dpdt_term",
 ]
 
 
@@ -91,6 +92,8 @@ def lib():
         L.maestro_mac_step_vcycle.argtypes = [_VP, _VP]
         L.maestro_mac_step_residual_norm.argtypes = [_VP, C.c_int, C.POINTER(C.c_double), _VP]
         L.maestro_mac_step_correct.argtypes = [_VP, _VP, _VP, _VP, _VP, _VP, _VP]
+        L.maestro_mac_base_state.argtypes = [C.c_int, _VP, _VP, _VP, _VP, _VP, _VP, _VP]
+        L.maestro_mac_set_dpdt_term.argtypes = [_VP, _VP]
         for name in EXPORTS:
             if name != "maestro_mac_default_desc":
                 getattr(L, name).restype = C.c_int
@@ -260,8 +263,26 @@ class MacProjector:
         self._ck(lib().maestro_mac_step_residual_norm(self._h, level, C.byref(nrm), _stream()), "step_residual_norm")
         return nrm.value
 
+    def set_dpdt_term(self, q):
+        """Register (or clear, q = None) the profile (1/(Gamma1bar p0)) dp0/dt of PAPER.md:49 Eq. 6."""
+        self._dpdt_keepalive = q
+        self._ck(lib().maestro_mac_set_dpdt_term(self._h, _ptr(q)), "set_dpdt_term")
+
     def step_correct(self, rho0, rho, u, v, w):
         self._ck(lib().maestro_mac_step_correct(self._h, _ptr(rho0), _ptr(rho), _ptr(u), _ptr(v), _ptr(w), _stream()), "step_correct")
+
+
+def base_state(rho0, p0, gamma1bar, dp0dt=None):
+    """maestro_mac_base_state: (beta0, dpdt_term or None) as device tensors from device profiles (Eq. 5,
+    PAPER.md:49 Eq. 6)."""
+    import torch
+    beta0 = torch.empty_like(rho0)
+    q = torch.empty_like(rho0) if dp0dt is not None else None
+    rc = lib().maestro_mac_base_state(int(rho0.numel()), _ptr(rho0), _ptr(p0), _ptr(gamma1bar), _ptr(dp0dt), _ptr(beta0),
+                                      _ptr(q), _stream())
+    if rc != 0:
+        raise MacError(rc, "maestro_mac_base_state")
+    return beta0, q
 
 
 def to_device(wl, device="cuda:0"):
