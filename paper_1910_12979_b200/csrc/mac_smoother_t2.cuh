@@ -51,7 +51,7 @@ enum { C_AX = 0, C_AY = 1, C_AZ = 2, C_RHS = 3, C_COUNT = 4 };
 
 template <int LA>
 struct Cfg {
-    static constexpr int NP = LA + 5, NC = LA + 2;
+    static constexpr int NP = 8, NC = LA + 2;        // phi: planes k-3 .. k+1 resident + LA in flight (+1 spare so that NP = 8)
     static constexpr int kCoef = C_COUNT * kPl;
     static constexpr unsigned kTx = (unsigned)kRow * (TYE + (TYE - 1) + 3 * (TYE - 2));   // bytes landing per plane
     static constexpr size_t kSmem = (size_t)kPad + (size_t)NP * kPl + (size_t)NC * kCoef + 8 * NP + 128;
@@ -75,19 +75,26 @@ struct Th {                                  // per-thread constants
     int nlo; unsigned nspan;                 // NORM: planes [k0, k1)
 };
 
-// Gauss-Seidel update of column X of the pair in one plane.  ph: own slot of that plane's phi stage
-// (lateral neighbours), other: the pair's other cell, C: the plane's coefficients, az_up: low z faces
-// of the plane above, d_ / u_: vertical neighbours (u_ is on the dependent chain, see fused::gs_value).
+// the three lateral neighbours of column X of the pair that other threads own, from a plane's phi stage
+struct Lat { double we, s, n; };
+template <bool X> __device__ __forceinline__ Lat lat_load(const unsigned char* ph)
+{
+    Lat l;
+    l.we = X ? ldc<false>(ph, 0, -1) : ldc<true>(ph, 0, 1);     // west of the x cell / east of the y cell
+    l.s = ldc<X>(ph, -1, 0);
+    l.n = ldc<X>(ph, 1, 0);
+    return l;
+}
+
+// Gauss-Seidel update of column X of the pair in one plane.  l: lateral neighbours, other: the pair's other cell,
+// C: the plane's coefficients, az_up: low z faces of the plane above, d_ / u_: vertical neighbours (u_ is on the
+// dependent chain, see fused::gs_value).
 template <bool X>
-__device__ __forceinline__ double gs_cell(const unsigned char* ph, double other, const Coef& C, const double2& az_up,
+__device__ __forceinline__ double gs_cell(const Lat& l, double other, const Coef& C, const double2& az_up,
                                           double d_, double u_, double& a, double& dg)
 {
-    const double w_ = X ? ldc<false>(ph, 0, -1) : other;
-    const double e_ = X ? other : ldc<true>(ph, 0, 1);
-    const double s_ = ldc<X>(ph, -1, 0);
-    const double n_ = ldc<X>(ph, 1, 0);
     return fused::gs_value(X ? C.ax.x : C.ax.y, X ? C.ax.y : C.ax2, pick<X>(C.ays), pick<X>(C.ayn), pick<X>(C.az),
-                           pick<X>(az_up), pick<X>(C.rhs), w_, e_, s_, n_, d_, u_, a, dg);
+                           pick<X>(az_up), pick<X>(C.rhs), X ? l.we : other, X ? other : l.we, l.s, l.n, d_, u_, a, dg);
 }
 
 // issue the five box loads of plane p (unwrapped) into the phi stage at byte offset op / coefficient stage at oc
@@ -112,6 +119,8 @@ __device__ __forceinline__ void issue_plane(const CUtensorMap* tm_phi, const CUt
 
 // One marching step at plane kk; X: the x column of the pair is red in plane kk.
 // CUR receives the coefficients of plane kk; S1, S2, S3 hold those of planes kk-1, kk-2, kk-3.
+// Every shared-memory read of the step (the lateral neighbours of all four half-sweeps were written in EARLIER
+// steps) is issued before the first write, so the loads overlap instead of queueing behind possibly-aliasing stores.
 template <bool X, bool NORM>
 __device__ __forceinline__ void step(const Th& T, int kk, unsigned char* s0, unsigned char* sM1, unsigned char* sM2,
                                      const unsigned char* sM3, const unsigned char* sP, const unsigned char* cI,
@@ -130,35 +139,55 @@ __device__ __forceinline__ void step(const Th& T, int kk, unsigned char* s0, uns
     CUR.ays = ldp(cI + C_AY * kPl);
     CUR.ayn = ldp(cI + C_AY * kPl + kRow);
     CUR.rhs = ldp(cI + C_RHS * kPl);
+    const Lat l0 = lat_load<X>(s0), l1 = lat_load<X>(sM1), l2 = lat_load<X>(sM2), l3 = lat_load<X>(sM3);
     double a, dg;
-    {   // (1) sweep 1, red cells of plane kk
-        const double nv = gs_cell<X>(s0, pick<!X>(P0), CUR, azn, pick<X>(Pm1), pick<X>(Pn), a, dg);
-        if (NORM && T.own && (unsigned)(kk - T.nlo) <= T.nspan)
-            vmax = nanmax(vmax, fabs(fma(pick<X>(P0), dg, -a)));              // |rhs - (sum - phi_0 dg)| of the input
-        const double val = ((X ? T.ra_x : T.ra_y) && v0) ? nv : pick<X>(P0);
-        put<X>(P0, val);
-        *reinterpret_cast<double*>(s0 + (X ? 0 : 8)) = val;
-    }
-    {   // (2) sweep 1, black cells of plane kk-1
-        const double nv = gs_cell<X>(sM1, pick<!X>(Pm1), S1, CUR.az, pick<X>(Pm2), pick<X>(P0), a, dg);
-        const double val = (T.ba && v1) ? nv : pick<X>(Pm1);
-        put<X>(Pm1, val);
-        *reinterpret_cast<double*>(sM1 + (X ? 0 : 8)) = val;
-    }
-    {   // (3) sweep 2, red cells of plane kk-2
-        const double nv = gs_cell<X>(sM2, pick<!X>(Pm2), S2, S1.az, pick<X>(Pm3), pick<X>(Pm1), a, dg);
-        const double val = ((X ? T.rb_x : T.rb_y) && v2) ? nv : pick<X>(Pm2);
-        put<X>(Pm2, val);
-        *reinterpret_cast<double*>(sM2 + (X ? 0 : 8)) = val;
-    }
-    {   // (4) sweep 2, black cells of plane kk-3; the plane is finished
-        const double nv = gs_cell<X>(sM3, pick<!X>(Pm3), S3, S2.az, pick<X>(Pm4), pick<X>(Pm2), a, dg);
-        if (T.own && v3) {
-            put<X>(Pm3, nv);
-            store_images(reinterpret_cast<double2*>(out), Pm3, T.img_x, T.img_y);
-        }
+    // (1) sweep 1, red cells of plane kk
+    const double n0 = gs_cell<X>(l0, pick<!X>(P0), CUR, azn, pick<X>(Pm1), pick<X>(Pn), a, dg);
+    if (NORM && T.own && (unsigned)(kk - T.nlo) <= T.nspan)
+        vmax = nanmax(vmax, fabs(fma(pick<X>(P0), dg, -a)));                  // |rhs - (sum - phi_0 dg)| of the input
+    put<X>(P0, ((X ? T.ra_x : T.ra_y) && v0) ? n0 : pick<X>(P0));
+    // (2) sweep 1, black cells of plane kk-1
+    const double n1 = gs_cell<X>(l1, pick<!X>(Pm1), S1, CUR.az, pick<X>(Pm2), pick<X>(P0), a, dg);
+    put<X>(Pm1, (T.ba && v1) ? n1 : pick<X>(Pm1));
+    // (3) sweep 2, red cells of plane kk-2
+    const double n2 = gs_cell<X>(l2, pick<!X>(Pm2), S2, S1.az, pick<X>(Pm3), pick<X>(Pm1), a, dg);
+    put<X>(Pm2, ((X ? T.rb_x : T.rb_y) && v2) ? n2 : pick<X>(Pm2));
+    // (4) sweep 2, black cells of plane kk-3; the plane is finished
+    const double n3 = gs_cell<X>(l3, pick<!X>(Pm3), S3, S2.az, pick<X>(Pm4), pick<X>(Pm2), a, dg);
+    *reinterpret_cast<double*>(s0 + (X ? 0 : 8)) = pick<X>(P0);
+    *reinterpret_cast<double*>(sM1 + (X ? 0 : 8)) = pick<X>(Pm1);
+    *reinterpret_cast<double*>(sM2 + (X ? 0 : 8)) = pick<X>(Pm2);
+    if (T.own && v3) {
+        put<X>(Pm3, n3);
+        store_images(reinterpret_cast<double2*>(out), Pm3, T.img_x, T.img_y);
     }
     Pm4 = Pm3; Pm3 = Pm2; Pm2 = Pm1; Pm1 = P0;
+}
+
+// Stage J (0 .. 7) of the eight-fold unrolled march: plane kk sits in phi stage (1 + J) % 8 and coefficient stage
+// (1 + J) % 4, so every shared-memory offset is a compile-time constant.
+template <int LA, int J, bool X, bool NORM>
+__device__ __forceinline__ void stage(const Th& T, int kk, int ke, unsigned par, const CUtensorMap* tm_phi,
+                                      const CUtensorMap* tm_rhs, const CUtensorMap* tm_ax, const CUtensorMap* tm_ay,
+                                      const CUtensorMap* tm_az, unsigned phi_ring, unsigned coef_ring, unsigned bar0,
+                                      bool producer, int cx, int cy, int nz, bool perz, double* __restrict__ out,
+                                      double2& Pn, double2& Pm1, double2& Pm2, double2& Pm3, double2& Pm4, double2& azn,
+                                      Coef& CUR, const Coef& S1, const Coef& S2, const Coef& S3, double& vmax)
+{
+    using G = Cfg<LA>;
+    static_assert(G::NP == 8 && G::NC == 4, "the unrolled march assumes 8 phi and 4 coefficient stages");
+    constexpr int i0 = (1 + J) % 8, iP = (2 + J) % 8, i1 = J % 8, i2 = (J + 7) % 8, i3 = (J + 6) % 8, iN = (J + 4) % 8;
+    constexpr int c0 = (1 + J) % 4, cP = (2 + J) % 4, cN = J % 4;
+    // plane kk+1 (barrier iP) has landed: a barrier is reused every 8 steps, its parity flips with every reuse
+    mbar_wait(bar0 + 8 * iP, (par + (J >= 6 ? 1u : 0u)) & 1u);
+    __syncthreads();                                           // every thread has finished step kk-1
+    if (producer && kk + 1 + LA <= ke + 1) {                   // never leave a load in flight at exit
+        asm volatile("fence.proxy.async.shared::cta;\n" ::: "memory");
+        issue_plane<LA>(tm_phi, tm_rhs, tm_ax, tm_ay, tm_az, phi_ring, coef_ring, bar0, iN * kPl, cN * G::kCoef,
+                        kk + 1 + LA, nz, perz, cx, cy);
+    }
+    step<X, NORM>(T, kk, T.phi0 + i0 * kPl, T.phi0 + i1 * kPl, T.phi0 + i2 * kPl, T.phi0 + i3 * kPl, T.phi0 + iP * kPl,
+                  T.coef0 + c0 * G::kCoef, T.coef0 + cP * G::kCoef, out, Pn, Pm1, Pm2, Pm3, Pm4, azn, CUR, S1, S2, S3, vmax);
 }
 
 template <int LA, bool REDX0, bool NORM>
@@ -168,53 +197,35 @@ __device__ __forceinline__ void march(const Th& T, int ks, int ke, const CUtenso
                                       int nz, bool perz, double* __restrict__ out, unsigned long long out_stride, double& vmax)
 {
     using G = Cfg<LA>;
-    constexpr unsigned kPhiRing = G::NP * kPl, kCoefRing = G::NC * G::kCoef;
     const double2 z2 = make_double2(0.0, 0.0);
     double2 Pm1, Pm2 = z2, Pm3 = z2, Pm4 = z2;
     Coef cA, cB, cC, cD;
     cB.ax = cB.ays = cB.ayn = cB.az = cB.rhs = z2; cB.ax2 = 0.0;
     cC = cB; cD = cB;
-    // the prologue issued planes ks-1 .. ks+LA into phi / coefficient stages 0 .. LA+1
+    // the prologue issued planes ks-1 .. ks+LA into phi / coefficient stages 0 .. LA+1 (phase 0 of their barriers)
     mbar_wait(bar0 + 0, 0);
     mbar_wait(bar0 + 8, 0);
-    unsigned phase_bits = 3u;                          // bit s: parity to wait for on barrier s next
-    // byte offsets, within their rings, of the phi stages of planes kk+1, kk, kk-1, kk-2, kk-3, of the one that
-    // plane kk-4 vacated, and of the coefficient stages of planes kk+1, kk, kk-1
-    unsigned oP = 2 * kPl, o0 = kPl, o1 = 0, o2 = kPhiRing - kPl, o3 = kPhiRing - 2 * kPl, o4 = kPhiRing - 3 * kPl;
-    unsigned qP = 2 * G::kCoef, q0 = G::kCoef, q1 = 0;
-    int bP = 2;                                        // barrier (= phi stage index) of plane kk+1
     Pm1 = ldp(T.phi0);
     double2 Pn = ldp(T.phi0 + kPl);
     double2 azn = ldp(T.coef0 + G::kCoef + C_AZ * kPl);
-#define MAC_T2_STEP(XX, CUR, S1, S2, S3)                                                                              \
-    {                                                                                                                 \
-        if (kk > ke) break;                                                                                           \
-        mbar_wait(bar0 + 8 * bP, (phase_bits >> bP) & 1u);         /* plane kk+1 has landed */                        \
-        phase_bits ^= 1u << bP;                                                                                       \
-        __syncthreads();                                           /* every thread has finished step kk-1 */          \
-        if (producer && kk + 1 + LA <= ke + 1) {                   /* never leave a load in flight at exit */         \
-            asm volatile("fence.proxy.async.shared::cta;\n" ::: "memory");                                            \
-            issue_plane<LA>(tm_phi, tm_rhs, tm_ax, tm_ay, tm_az, phi_ring, coef_ring, bar0, o4, q1, kk + 1 + LA, nz,  \
-                            perz, cx, cy);                                                                            \
-        }                                                                                                             \
-        step<XX, NORM>(T, kk, T.phi0 + o0, T.phi0 + o1, T.phi0 + o2, T.phi0 + o3, T.phi0 + oP, T.coef0 + q0,          \
-                       T.coef0 + qP, out, Pn, Pm1, Pm2, Pm3, Pm4, azn, CUR, S1, S2, S3, vmax);                        \
-        out += out_stride;                                                                                            \
-        o4 = o3; o3 = o2; o2 = o1; o1 = o0; o0 = oP;                                                                  \
-        oP += kPl; if (oP == kPhiRing) oP = 0;                                                                        \
-        q1 = q0; q0 = qP;                                                                                             \
-        qP += G::kCoef; if (qP == kCoefRing) qP = 0;                                                                  \
-        if (++bP == G::NP) bP = 0;                                                                                    \
-        ++kk;                                                                                                         \
-    }
+    unsigned par = 0;
+#define MAC_T2_STAGE(J, XX, CUR, S1, S2, S3)                                                                          \
+    if (kk > ke) break;                                                                                               \
+    stage<LA, J, XX, NORM>(T, kk, ke, par, tm_phi, tm_rhs, tm_ax, tm_ay, tm_az, phi_ring, coef_ring, bar0, producer,  \
+                           cx, cy, nz, perz, out, Pn, Pm1, Pm2, Pm3, Pm4, azn, CUR, S1, S2, S3, vmax);                \
+    out += out_stride; ++kk;
 #pragma unroll 1
-    for (int kk = ks; kk <= ke;) {
-        MAC_T2_STEP(REDX0, cA, cD, cC, cB)
-        MAC_T2_STEP(!REDX0, cB, cA, cD, cC)
-        MAC_T2_STEP(REDX0, cC, cB, cA, cD)
-        MAC_T2_STEP(!REDX0, cD, cC, cB, cA)
+    for (int kk = ks; kk <= ke; par ^= 1u) {
+        MAC_T2_STAGE(0, REDX0, cA, cD, cC, cB)
+        MAC_T2_STAGE(1, !REDX0, cB, cA, cD, cC)
+        MAC_T2_STAGE(2, REDX0, cC, cB, cA, cD)
+        MAC_T2_STAGE(3, !REDX0, cD, cC, cB, cA)
+        MAC_T2_STAGE(4, REDX0, cA, cD, cC, cB)
+        MAC_T2_STAGE(5, !REDX0, cB, cA, cD, cC)
+        MAC_T2_STAGE(6, REDX0, cC, cB, cA, cD)
+        MAC_T2_STAGE(7, !REDX0, cD, cC, cB, cA)
     }
-#undef MAC_T2_STEP
+#undef MAC_T2_STAGE
 }
 
 // NORM: additionally writes, per CTA, max |rhs - L phi_in| over the red cells to part_max[linear CTA index]
@@ -307,7 +318,7 @@ k_rbgs_t2(const __grid_constant__ CUtensorMap tm_phi, const __grid_constant__ CU
 // ---- host side ---------------------------------------------------------------------------------
 
 #ifndef MAC_T2_LA
-#define MAC_T2_LA 4                   // planes of TMA lookahead (shared memory: 0.5 + 6 (LA+5) + 24 (LA+2) KB)
+#define MAC_T2_LA 2                   // planes of TMA lookahead (shared memory: 0.5 + 6 (LA+5) + 24 (LA+2) KB)
 #endif
 
 static inline int t2_smoother_configure()
