@@ -108,7 +108,8 @@ static double beta_face(const orc_grid *g, const orc_base *b, const double *beta
 /* ---------- O2: density on a face ----------------------------------------------------------- */
 
 /* rho_face = (rho_L + rho_R)/2 ; periodic axis wraps; non-periodic boundary face takes the one
- * interior cell (readings A3, A17). */
+ * interior cell (readings A3, A17).  g->rho_mean == 1 (the harmonic variant of A3): the face takes the mean of
+ * 1/rho instead, rho_face = 2 / (1/rho_L + 1/rho_R); coefficient (O3) and correction (O10) both use it. */
 static double rho_face(const orc_grid *g, const double *rho, int d, int i, int j, int k)
 {
     int id[3] = {i, j, k};
@@ -128,7 +129,9 @@ static double rho_face(const orc_grid *g, const double *rho, int d, int i, int j
         lo[d] = f - 1;
         hi[d] = f;
     }
-    return 0.5 * (rho[cidx(g, lo[0], lo[1], lo[2])] + rho[cidx(g, hi[0], hi[1], hi[2])]);
+    const double rl = rho[cidx(g, lo[0], lo[1], lo[2])], rh = rho[cidx(g, hi[0], hi[1], hi[2])];
+    if (g->rho_mean == 1) return 2.0 / (1.0 / rl + 1.0 / rh);
+    return 0.5 * (rl + rh);
 }
 
 /* ---------- O3: face coefficient b = beta0 / rho  (Eq. 2: the factor beta0/rho) --------- */
@@ -424,6 +427,7 @@ void orc_coarsen_grid(const orc_grid *f, orc_grid *c)
         c->bc_lo[d] = f->bc_lo[d];
         c->bc_hi[d] = f->bc_hi[d];
     }
+    c->rho_mean = f->rho_mean;
 }
 
 /* coarse face coefficient = arithmetic mean of the 4 fine faces that tile it (reading A11) */

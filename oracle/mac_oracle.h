@@ -44,6 +44,7 @@ typedef struct {
     int n[3];
     double h[3];
     int bc_lo[3], bc_hi[3];
+    int rho_mean;             /* face density: 0 arithmetic mean of rho (default), 1 harmonic (mean of 1/rho); A3 */
 } orc_grid;
 
 /* 1-D base-state sampling: nr samples at r_m = (m + 1/2) dr.  Planar: r = z. */

@@ -36,7 +36,7 @@ def build(force: bool = False) -> str:
 
 class Grid(C.Structure):
     _fields_ = [("n", C.c_int * 3), ("h", C.c_double * 3),
-                ("bc_lo", C.c_int * 3), ("bc_hi", C.c_int * 3)]
+                ("bc_lo", C.c_int * 3), ("bc_hi", C.c_int * 3), ("rho_mean", C.c_int)]
 
 
 class Base(C.Structure):
@@ -119,8 +119,9 @@ def _p(a):
     return a.ctypes.data_as(_DP)
 
 
-def make_grid(n, h, bc_lo, bc_hi) -> Grid:
+def make_grid(n, h, bc_lo, bc_hi, rho_mean=0) -> Grid:
     g = Grid()
+    g.rho_mean = int(rho_mean)
     for d in range(3):
         g.n[d], g.h[d], g.bc_lo[d], g.bc_hi[d] = int(n[d]), float(h[d]), int(bc_lo[d]), int(bc_hi[d])
     return g

@@ -3,7 +3,7 @@ import numpy as np
 
 
 def oracle_structs(O, wl, **mg_kw):
-    g = O.make_grid(wl.n, wl.dx, wl.bc_lo, wl.bc_hi)
+    g = O.make_grid(wl.n, wl.dx, wl.bc_lo, wl.bc_hi, rho_mean=wl.meta.get("rho_mean", 0))
     b = O.make_base(wl.geometry, wl.nr, wl.dr, wl.center)
     kw = dict(nu_pre=wl.nu_pre, nu_post=wl.nu_post, max_cycles=wl.max_cycles, rel_tol=wl.rel_tol)
     kw.update(mg_kw)
