@@ -95,6 +95,9 @@ typedef struct {
                                      to a second buffer and is dropped when the test passes.  Elsewhere,
                                      and after the last allowed cycle, as 1;
                                  1 = a separate residual-norm kernel over all cells after every cycle. */
+    int rho_mean;             /* density on a face from the two cells it separates, in the coefficient
+                                 beta0/rho_face and in the correction (1/rho_face) G phi alike:
+                                 0 = arithmetic mean of rho (default), 1 = harmonic (mean of 1/rho). */
 } maestro_mac_desc;
 
 typedef struct {

@@ -41,7 +41,14 @@ struct GeoDev {                // level-0 geometry for base-state profile evalua
     int bclo[3], bchi[3];
     int geometry, nr;
     double dr, cx, cy, cz;
+    int rho_mean;              // face density: 0 arithmetic mean of rho, 1 harmonic (mean of 1/rho); reading A3
 };
+
+// density on a face from the two cells it separates (O2; `harmonic`: the variant of reading A3)
+__device__ __forceinline__ double face_rho(double rl, double rr, int harmonic)
+{
+    return harmonic ? 2.0 / (1.0 / rl + 1.0 / rr) : 0.5 * (rl + rr);
+}
 
 __device__ __forceinline__ size_t cidx(const LevelDev& L, int i, int j, int k)
 {

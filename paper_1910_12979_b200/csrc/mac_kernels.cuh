@@ -41,7 +41,7 @@ __device__ __forceinline__ void face_rho_weight(const GeoDev& G, const double* _
     }
     double rl = rho_cell(G, rho, rho0, D == 0 ? lo : i, D == 1 ? lo : j, D == 2 ? lo : k);
     double rr = rho_cell(G, rho, rho0, D == 0 ? hi : i, D == 1 ? hi : j, D == 2 ? hi : k);
-    rf = 0.5 * (rl + rr);
+    rf = face_rho(rl, rr, G.rho_mean);
 }
 
 __global__ void __launch_bounds__(256)
@@ -718,8 +718,8 @@ __device__ __forceinline__ void correct_face(const GeoDev& G, const LevelDev& L,
     }
     auto cell = [&](int q) -> size_t { return cidx(L, D == 0 ? q : i, D == 1 ? q : j, D == 2 ? q : k); };
     const double grad = (ghi * phi[cell(hi)] - glo * phi[cell(lo)]) * (1.0 / h);
-    const double rf = 0.5 * (rho_cell(G, rho, rho0, D == 0 ? lo : i, D == 1 ? lo : j, D == 2 ? lo : k) +
-                             rho_cell(G, rho, rho0, D == 0 ? hi : i, D == 1 ? hi : j, D == 2 ? hi : k));
+    const double rf = face_rho(rho_cell(G, rho, rho0, D == 0 ? lo : i, D == 1 ? lo : j, D == 2 ? lo : k),
+                               rho_cell(G, rho, rho0, D == 0 ? hi : i, D == 1 ? hi : j, D == 2 ? hi : k), G.rho_mean);
     double rr;                                       // grad / rf, rf > 0 (validated by the coefficient pass)
     asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(rr) : "d"(rf));
     rr = fma(fma(-rf, rr, 1.0), rr, rr);
@@ -762,9 +762,9 @@ k_correct(GeoDev G, LevelDev L, const double* __restrict__ phi, const double* __
             const double qq = g * rr;
             return fma(fma(-rf, qq, g), rr, qq);
         };
-        *pu = u0 - quot((p0 - pxm) * (1.0 / G.dx), 0.5 * (rxm + r0));
-        *pv = v0 - quot((p0 - pym) * (1.0 / G.dy), 0.5 * (rym + r0));
-        *pw = w0 - quot((p0 - pzm) * (1.0 / G.dz), 0.5 * (rzm + r0));
+        *pu = u0 - quot((p0 - pxm) * (1.0 / G.dx), face_rho(rxm, r0, G.rho_mean));
+        *pv = v0 - quot((p0 - pym) * (1.0 / G.dy), face_rho(rym, r0, G.rho_mean));
+        *pw = w0 - quot((p0 - pzm) * (1.0 / G.dz), face_rho(rzm, r0, G.rho_mean));
         return;
     }
     const bool ci = i < G.nx, cj = j < G.ny, ck = k < G.nz;

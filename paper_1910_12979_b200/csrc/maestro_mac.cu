@@ -108,6 +108,7 @@ int validate_and_default(const maestro_mac_desc* in, maestro_mac_desc* d)
     if (d->host_staging != 0 && d->host_staging != 1) return MAESTRO_MAC_ERR_ARG;
     if (d->smoother < 0 || d->smoother > 4) return MAESTRO_MAC_ERR_ARG;   // 4: two-sweep kernel
     if (d->stop_test != 0 && d->stop_test != 1) return MAESTRO_MAC_ERR_ARG;
+    if (d->rho_mean != 0 && d->rho_mean != 1) return MAESTRO_MAC_ERR_ARG;
     return MAESTRO_MAC_OK;
 }
 
@@ -214,6 +215,7 @@ GeoDev dev_geo(const maestro_mac_handle* H)
     for (int a = 0; a < 3; ++a) { G.bclo[a] = d.bc_lo[a]; G.bchi[a] = d.bc_hi[a]; }
     G.geometry = d.geometry; G.nr = d.nr; G.dr = d.dr;
     G.cx = d.center[0]; G.cy = d.center[1]; G.cz = d.center[2];
+    G.rho_mean = d.rho_mean;
     return G;
 }
 

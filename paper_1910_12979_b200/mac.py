@@ -37,7 +37,7 @@ class Desc(C.Structure):
                 ("max_cycles", C.c_int), ("rel_tol", C.c_double), ("coarsest_n", C.c_int),
                 ("bottom_max_iter", C.c_int), ("bottom_rel_tol", C.c_double),
                 ("prolongation", C.c_int), ("host_staging", C.c_int), ("smoother", C.c_int),
-                ("stop_test", C.c_int)]
+                ("stop_test", C.c_int), ("rho_mean", C.c_int)]
 
 
 class Stats(C.Structure):
@@ -110,7 +110,7 @@ class MacError(RuntimeError):
 def make_desc(n, dx, bc_lo, bc_hi, geometry=PLANAR, nr=None, dr=None, center=(0.0, 0.0, 0.0),
               nu_pre=2, nu_post=2, max_cycles=100, rel_tol=1e-10, coarsest_n=4,
               bottom_max_iter=100, bottom_rel_tol=1e-8, prolongation=0, host_staging=0,
-              smoother=0, stop_test=0) -> Desc:
+              smoother=0, stop_test=0, rho_mean=0) -> Desc:
     d = Desc()
     lib().maestro_mac_default_desc(C.byref(d))
     d.nx, d.ny, d.nz = (int(x) for x in n)
@@ -123,13 +123,14 @@ def make_desc(n, dx, bc_lo, bc_hi, geometry=PLANAR, nr=None, dr=None, center=(0.
     d.coarsest_n, d.bottom_max_iter, d.bottom_rel_tol = int(coarsest_n), int(bottom_max_iter), float(bottom_rel_tol)
     d.prolongation, d.host_staging, d.smoother = int(prolongation), int(host_staging), int(smoother)
     d.stop_test = int(stop_test)
+    d.rho_mean = int(rho_mean)
     return d
 
 
 def desc_from_workload(wl, **over) -> Desc:
     kw = dict(n=wl.n, dx=wl.dx, bc_lo=wl.bc_lo, bc_hi=wl.bc_hi, geometry=wl.geometry, nr=wl.nr,
               dr=wl.dr, center=wl.center, nu_pre=wl.nu_pre, nu_post=wl.nu_post,
-              max_cycles=wl.max_cycles, rel_tol=wl.rel_tol)
+              max_cycles=wl.max_cycles, rel_tol=wl.rel_tol, rho_mean=wl.meta.get("rho_mean", 0))
     kw.update(over)
     return make_desc(**kw)
 

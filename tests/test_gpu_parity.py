@@ -340,3 +340,35 @@ def test_two_sweep_kernel_equals_two_single_sweeps(oracle, mac, case):
     assert np.array_equal(got[0, 5], got[4, 5])
     ref = phi.copy(); O.rbgs_sweep(g, *bf, f, ref); O.rbgs_sweep(g, *bf, f, ref)
     assert close(got[4, 2], ref)
+
+
+@pytest.mark.parametrize("name,N,smoother", [("2", 32, 0), ("3D", 32, 0), ("4N", 32, 1), ("mixed_sph", 0, 2), ("wide_bottom", 0, 0)])
+def test_harmonic_face_density_variant(oracle, mac, name, N, smoother):
+    """desc.rho_mean = 1 (reading A3, harmonic variant): coefficients, correction and the whole projection match the
+    oracle run with the same flag."""
+    O = oracle
+    wl = get_case(name, N)
+    wl.meta["rho_mean"] = 1
+    g, b, mg = oracle_structs(O, wl)
+    P = mac.MacProjector(mac.desc_from_workload(wl, smoother=smoother))
+    dv = mac.to_device(wl)
+    P.step_coefficients(dv["beta0"], dv["rho0"], dv["rho"])
+    exp = folded(O, g, [c.copy() for c in O.face_coeff(g, b, wl.beta0, wl.rho)])
+    for which, e in zip((mac.ARR_BX, mac.ARR_BY, mac.ARR_BZ), exp):
+        assert close(P.level_get(0, which), e), which
+    rng = np.random.default_rng(3)
+    phi = rng.standard_normal(O.cell_shape(g))
+    P.level_set(0, mac.ARR_PHI, tt(phi))
+    u, v, w = tt(wl.u), tt(wl.v), tt(wl.w)
+    P.step_correct(dv["rho0"], dv["rho"], u, v, w)
+    ru, rv, rw = wl.u.copy(), wl.v.copy(), wl.w.copy()
+    O.correct(g, wl.rho, phi, ru, rv, rw)
+    assert close(u, ru) and close(v, rv) and close(w, rw)
+    P.close()
+    ref = oracle_project(O, wl)
+    got = gpu_project(mac, wl, smoother=smoother)
+    if got["stats"]["cycles"] != ref["stats"]["cycles"]:
+        got = gpu_project(mac, wl, smoother=smoother, rel_tol=0.0, max_cycles=ref["stats"]["cycles"])
+    assert got["status"] == ref["status"] == 0 and got["stats"]["cycles"] == ref["stats"]["cycles"]
+    for key in ("phi", "u", "v", "w"):
+        assert rel_l2(got[key], ref[key]) <= E2E_TOL, key
