@@ -188,6 +188,49 @@ void orc_effective_source(const orc_grid *g, const orc_base *b, const double *S,
             }
 }
 
+/* ---------- O13: lateral average  rho -> rho0(r) -------------------------------------- */
+
+void orc_lateral_average(const orc_grid *g, const orc_base *b, const double *rho, double *rho0, long long *count)
+{
+    const int nr = b->nr;
+    double *sum = (double *)calloc((size_t)nr, sizeof(double));
+    ll *cnt = (ll *)calloc((size_t)nr, sizeof(ll));
+    for (int k = 0; k < g->n[2]; ++k)
+        for (int j = 0; j < g->n[1]; ++j)
+            for (int i = 0; i < g->n[0]; ++i) {
+                double p[3];
+                cell_pos(g, i, j, k, p);
+                const double r = orc_radius(b, p[0], p[1], p[2]);
+                int m = (int)floor(r / b->dr);
+                if (m > nr - 1) m = nr - 1;
+                if (m < 0) m = 0;
+                sum[m] += rho[cidx(g, i, j, k)];
+                cnt[m] += 1;
+            }
+    /* means of the samples that have cells */
+    for (int m = 0; m < nr; ++m)
+        if (cnt[m] > 0) rho0[m] = sum[m] / (double)cnt[m];
+    /* samples without cells: linear in m between the nearest filled samples, constant beyond the ends */
+    int prev = -1;
+    for (int m = 0; m < nr; ++m) {
+        if (cnt[m] == 0) continue;
+        if (prev < 0)
+            for (int q = 0; q < m; ++q) rho0[q] = rho0[m];
+        else
+            for (int q = prev + 1; q < m; ++q) {
+                const double t = (double)(q - prev) / (double)(m - prev);
+                rho0[q] = (1.0 - t) * rho0[prev] + t * rho0[m];
+            }
+        prev = m;
+    }
+    if (prev >= 0)
+        for (int q = prev + 1; q < nr; ++q) rho0[q] = rho0[prev];
+    if (count)
+        for (int m = 0; m < nr; ++m) count[m] = cnt[m];
+    free(sum);
+    free(cnt);
+}
+
 /* ---------- O4: right-hand side  D(beta0 U_edge) - beta0 S   (Eq. 6) ------------------- */
 
 /* velocity on face (i,j,k) of axis d; on a periodic axis face n reads entry 0 */

@@ -146,6 +146,15 @@ void orc_make_beta0(int nr, const double *rho0, const double *p0, const double *
 void orc_dpdt_term(int nr, const double *p0, const double *gamma1bar, const double *dp0dt, double *q);
 void orc_effective_source(const orc_grid *g, const orc_base *b, const double *S, const double *q, double *S_eff);
 
+/* O13 ("rho0 ... represents the lateral average"): the base-state density from the cell density.
+ * Cell (i,j,k) with centre radius r (planar: r = z) belongs to sample m = min(nr - 1, floor(r / dr)), i.e. to the
+ * shell [m dr, (m+1) dr) around r_m = (m + 1/2) dr; rho0[m] = mean of rho over the cells of sample m.  Samples
+ * without a cell (spherical geometry with dr < dx has many near the centre) are filled by linear interpolation in
+ * m between the nearest samples that have cells, constant beyond the first / last such sample (readings A29, A30,
+ * DESIGN.md).  count[m] (may be NULL) receives the number of cells of sample m.  Planar with nr = nz, dr = dz:
+ * rho0[k] is the mean of plane k. */
+void orc_lateral_average(const orc_grid *g, const orc_base *b, const double *rho, double *rho0, long long *count);
+
 /* Constraint residual  D(beta0 U) - beta0 S  (same discrete operators as orc_rhs). */
 void orc_constraint(const orc_grid *g, const orc_base *b, const double *beta0,
                     const double *u, const double *v, const double *w, const double *S,

@@ -78,6 +78,7 @@ def lib():
         L.orc_face_coeff.argtypes = [GP, BP, _DP, _DP, _DP, _DP, _DP]
         L.orc_rho_from_profile.argtypes = [GP, BP, _DP, _DP]
         L.orc_make_beta0.argtypes = [C.c_int, _DP, _DP, _DP, _DP]
+        L.orc_lateral_average.argtypes = [GP, BP, _DP, _DP, C.c_void_p]
         L.orc_dpdt_term.argtypes = [C.c_int, _DP, _DP, _DP, _DP]
         L.orc_effective_source.argtypes = [GP, BP, _DP, _DP, _DP]
         L.orc_rhs.argtypes = [GP, BP, _DP, _DP, _DP, _DP, _DP, _DP]
@@ -170,6 +171,14 @@ def rho_from_profile(g, b, rho0):
     rho = np.empty(cell_shape(g))
     lib().orc_rho_from_profile(C.byref(g), C.byref(b), _p(rho0), _p(rho))
     return rho
+
+
+def lateral_average(g, b, rho):
+    """O13 (PAPER.md:39).  Returns (rho0[nr], count[nr])."""
+    rho0 = np.empty(b.nr)
+    cnt = np.zeros(b.nr, dtype=np.int64)
+    lib().orc_lateral_average(C.byref(g), C.byref(b), _p(rho), _p(rho0), cnt.ctypes.data_as(C.c_void_p))
+    return rho0, cnt
 
 
 def make_beta0(rho0, p0, gamma1bar):
