@@ -178,6 +178,16 @@ int maestro_mac_base_state(int nr, const double *rho0, const double *p0, const d
                            const double *dp0dt, double *beta0, double *dpdt_term, void *cuda_stream);
 
 /*
+ * maestro_mac_lateral_average: the base-state density from the cell density ("rho0 ... represents
+ * the lateral average"), with the handle's geometry and profile sampling: cell (i,j,k) with centre radius r
+ * (planar: z) belongs to sample m = min(nr-1, floor(r / dr)); rho0[m] = mean of rho over the cells of sample m;
+ * samples without a cell are filled by linear interpolation in m between the nearest samples that have cells
+ * (constant beyond the ends).  rho: device [nx*ny*nz]; rho0: device [nr], out.  Uses the handle's scratch
+ * (not during a project call).  Asynchronous on `cuda_stream`.  Returns OK, ERR_ARG, ERR_UNSUPPORTED, ERR_CUDA.
+ */
+int maestro_mac_lateral_average(maestro_mac_handle *h, const double *rho, double *rho0, void *cuda_stream);
+
+/*
  * maestro_mac_set_dpdt_term: register the profile q = (1/(Gamma1bar p0)) dp0/dt (device, [nr], caller-owned,
  * alive and unchanged during every later project call) or NULL to clear it.  With it the right-hand side is the
  * full constraint of PAPER.md:49 Eq. 6,  rhs = D(beta0 U_edge) - beta0 (S - q(r)),  q evaluated at cell centres

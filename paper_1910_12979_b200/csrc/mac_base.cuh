@@ -39,3 +39,69 @@ k_base_state(int nr, const double* __restrict__ rho0, const double* __restrict__
     if (q && dp0dt)
         for (int m = lane; m < nr; m += 32) q[m] = __ldg(dp0dt + m) / (__ldg(gamma1bar + m) * __ldg(p0 + m));
 }
+
+// ------------------------------------------------------------------------------------------------
+// Lateral average rho -> rho0(r)  ("rho0 ... represents the lateral average"; SURVEY.md
+// Sec. 8(f) rank 4).  Cell (i,j,k) belongs to sample m = min(nr-1, floor(r / dr)), r the radius of its
+// centre (planar: z).  The decision is an integer taken from floating point, so r and r / dr are formed
+// with exactly the oracle's operations (no FMA contraction, IEEE sqrt and division): both sides bin
+// every cell alike.  Sums and counts are accumulated with atomics (a warp whose cells share one sample
+// -- every warp in planar geometry -- reduces first and issues one), so the sums are exact up to the
+// order of additions; k_average_finish divides and fills samples without cells by linear interpolation
+// in m (constant beyond the ends).
+// ------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256)
+k_lateral_sum(GeoDev G, const double* __restrict__ rho, double* __restrict__ sum, unsigned long long* __restrict__ cnt)
+{
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarp = blockDim.x >> 5;
+    const int nrows = G.ny * G.nz;
+    for (int row = blockIdx.x; row < nrows; row += gridDim.x) {
+        const int j = row % G.ny, k = row / G.ny;
+        const double ay = __dsub_rn(__dmul_rn((double)j + 0.5, G.dy), G.cy), az = __dsub_rn(__dmul_rn((double)k + 0.5, G.dz), G.cz);
+        const double zc = __dmul_rn((double)k + 0.5, G.dz);
+        const double* __restrict__ p = rho + (size_t)G.nx * ((size_t)j + (size_t)G.ny * k);
+        for (int i0 = warp * 32; i0 < G.nx; i0 += nwarp * 32) {
+            const int i = i0 + lane;
+            const bool on = i < G.nx;
+            double r = zc;
+            if (G.geometry != 0) {
+                const double ax = __dsub_rn(__dmul_rn((double)i + 0.5, G.dx), G.cx);
+                r = __dsqrt_rn(__dadd_rn(__dadd_rn(__dmul_rn(ax, ax), __dmul_rn(ay, ay)), __dmul_rn(az, az)));
+            }
+            int m = (int)floor(__ddiv_rn(r, G.dr));
+            m = max(0, min(m, G.nr - 1));
+            const double v = on ? __ldg(p + i) : 0.0;
+            const unsigned act = __ballot_sync(0xffffffffu, on);
+            const int m0 = __shfl_sync(0xffffffffu, m, 0);
+            if (__all_sync(0xffffffffu, !on || m == m0)) {           // one sample for the whole warp
+                const double s = warp_sum(v);
+                if (lane == 0) { atomicAdd(sum + m0, s); atomicAdd(cnt + m0, (unsigned long long)__popc(act)); }
+            } else if (on) {
+                atomicAdd(sum + m, v);
+                atomicAdd(cnt + m, 1ull);
+            }
+        }
+    }
+}
+
+__global__ void __launch_bounds__(256)
+k_average_finish(int nr, const double* __restrict__ sum, const unsigned long long* __restrict__ cnt, double* __restrict__ rho0)
+{
+    for (int m = threadIdx.x; m < nr; m += blockDim.x)
+        if (cnt[m] > 0) rho0[m] = sum[m] / (double)cnt[m];
+    __syncthreads();
+    if (threadIdx.x == 0) {                                          // samples without cells
+        int prev = -1;
+        for (int m = 0; m < nr; ++m) {
+            if (cnt[m] == 0) continue;
+            if (prev < 0) for (int q = 0; q < m; ++q) rho0[q] = rho0[m];
+            else
+                for (int q = prev + 1; q < m; ++q) {
+                    const double t = (double)(q - prev) / (double)(m - prev);
+                    rho0[q] = (1.0 - t) * rho0[prev] + t * rho0[m];
+                }
+            prev = m;
+        }
+        if (prev >= 0) for (int q = prev + 1; q < nr; ++q) rho0[q] = rho0[prev];
+    }
+}

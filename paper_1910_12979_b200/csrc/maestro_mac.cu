@@ -890,6 +890,22 @@ extern "C" int maestro_mac_base_state(int nr, const double* rho0, const double* 
     return cudaPeekAtLastError() == cudaSuccess ? MAESTRO_MAC_OK : MAESTRO_MAC_ERR_CUDA;
 }
 
+extern "C" int maestro_mac_lateral_average(maestro_mac_handle* H, const double* rho, double* rho0, void* cuda_stream)
+{
+    if (!H || !rho || !rho0) return MAESTRO_MAC_ERR_ARG;
+    if (H->d.nr > kMaxParts) return MAESTRO_MAC_ERR_UNSUPPORTED;
+    cudaStream_t s = (cudaStream_t)cuda_stream;
+    unsigned long long* cnt = reinterpret_cast<unsigned long long*>(H->part_max);
+    CUDA_OK(cudaMemsetAsync(H->part_sum, 0, H->d.nr * sizeof(double), s));
+    CUDA_OK(cudaMemsetAsync(cnt, 0, H->d.nr * sizeof(unsigned long long), s));
+    const int rows = H->d.ny * H->d.nz;
+    k_lateral_sum<<<rows < 148 * 16 ? rows : 148 * 16, 256, 0, s>>>(dev_geo(H), rho, H->part_sum, cnt);
+    LAUNCHED(H);
+    k_average_finish<<<1, 256, 0, s>>>(H->d.nr, H->part_sum, cnt, rho0);
+    LAUNCHED(H);
+    return MAESTRO_MAC_OK;
+}
+
 extern "C" int maestro_mac_set_dpdt_term(maestro_mac_handle* H, const double* dpdt_term)
 {
     if (!H) return MAESTRO_MAC_ERR_ARG;

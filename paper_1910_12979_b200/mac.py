@@ -25,7 +25,7 @@ EXPORTS = [
     "maestro_mac_step_coefficients", "maestro_mac_step_rhs", "maestro_mac_step_smooth",
     "maestro_mac_step_residual_restrict", "maestro_mac_step_prolong", "maestro_mac_step_bottom",
     "maestro_mac_step_vcycle", "maestro_mac_step_residual_norm", "maestro_mac_step_correct",
-    "maestro_mac_base_state", "maestro_mac_set_dpdt_term",
+    "maestro_mac_base_state", "maestro_mac_set_dpdt_term", "maestro_mac_lateral_average",
 ]
 
 
@@ -94,6 +94,7 @@ def lib():
         L.maestro_mac_step_correct.argtypes = [_VP, _VP, _VP, _VP, _VP, _VP, _VP]
         L.maestro_mac_base_state.argtypes = [C.c_int, _VP, _VP, _VP, _VP, _VP, _VP, _VP]
         L.maestro_mac_set_dpdt_term.argtypes = [_VP, _VP]
+        L.maestro_mac_lateral_average.argtypes = [_VP, _VP, _VP, _VP]
         for name in EXPORTS:
             if name != "maestro_mac_default_desc":
                 getattr(L, name).restype = C.c_int
@@ -263,6 +264,13 @@ class MacProjector:
         nrm = C.c_double(0)
         self._ck(lib().maestro_mac_step_residual_norm(self._h, level, C.byref(nrm), _stream()), "step_residual_norm")
         return nrm.value
+
+    def lateral_average(self, rho):
+        """rho0[nr] = lateral average of rho as a device tensor."""
+        import torch
+        out = torch.empty(self.desc.nr, dtype=torch.float64, device=rho.device)
+        self._ck(lib().maestro_mac_lateral_average(self._h, _ptr(rho), _ptr(out), _stream()), "lateral_average")
+        return out
 
     def set_dpdt_term(self, q):
         """Register (or clear, q = None) the profile (1/(Gamma1bar p0)) dp0/dt of PAPER.md:49 Eq. 6."""

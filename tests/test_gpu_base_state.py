@@ -83,3 +83,19 @@ def test_rhs_and_projection_with_dpdt_term(oracle, mac, name, N, smoother):
     rhs0 = O.rhs(g, b, beta0, wl.u, wl.v, wl.w, wl.S)
     assert close(P.level_get(0, mac.ARR_RHS), rhs0 - (O.mean(rhs0) if O.is_singular(g) else 0.0))
     P.close()
+
+
+@pytest.mark.parametrize("name,N", [("2", 32), ("3D", 32), ("mixed_sph", 0), ("5", 64), ("4N", 64)])
+def test_lateral_average_matches_oracle(oracle, mac, name, N):
+    """maestro_mac_lateral_average vs oracle O13: every cell lands in the same sample on both sides
+    (the binning arithmetic is the oracle's, operation by operation), so the means agree to the order of additions
+    and the filled samples to rounding."""
+    wl = W.mixed_bc_case(n=(16, 48, 32), geometry=W.SPHERICAL, seed=21) if name == "mixed_sph" else W.by_name(name, N)
+    g, b, _ = oracle_structs(oracle, wl)
+    ref, cnt = oracle.lateral_average(g, b, wl.rho)
+    P = mac.MacProjector(mac.desc_from_workload(wl))
+    got = P.lateral_average(tt(wl.rho)).cpu().numpy()
+    assert np.abs(got - ref).max() <= 1e-13 * np.abs(ref).max()
+    again = P.lateral_average(tt(wl.rho)).cpu().numpy()           # scratch is re-zeroed on every call
+    assert np.abs(again - ref).max() <= 1e-13 * np.abs(ref).max()
+    P.close()
