@@ -23,13 +23,18 @@
 // 24 x 16 finished ones (halo 4); the halo cells are recomputed redundantly by the neighbouring CTA
 // (their HBM reads hit L2).  In z a chunk [k0, k1) redoes 6 planes.
 //
-// Memory.  phi planes live for 5 steps (k+1 .. k-3), coefficient planes for one (they are consumed
-// into registers, where the four coefficient sets of planes k .. k-3 rotate; the loop is unrolled by
-// four so that nothing is moved).  So shared memory holds two rings fed by TMA box loads
-// (cp.async.bulk.tensor.3d + mbarrier, as in mac_smoother_tma.cuh): NP = LA + 5 phi stages of 6 KB
-// and NC = LA + 2 coefficient stages of 24 KB, LA = planes of lookahead in flight.
+// Memory.  Shared memory holds two TMA-fed rings (cp.async.bulk.tensor.3d + mbarrier, as in
+// mac_smoother_tma.cuh) of 4 stages each -- phi (6 KB per plane: the OLD values, read by half-sweep (1)
+// and for the plane above) and coefficients (24 KB per plane, consumed into registers, where the four
+// coefficient sets of planes k .. k-3 rotate) -- and six small EXCHANGE buffers: the values a half-sweep
+// produces are what the next half-sweep of the neighbouring threads reads one step later, so each thread
+// writes its new value into a compact, colour-split plane (one double per pair: in a given row and plane
+// all updated cells are the same column of their pairs) that is double-buffered by step parity.  Those
+// reads and writes are 8-byte accesses at an 8-byte pitch (conflict-free), whereas the staged phi planes
+// interleave the two colours at a 16-byte pitch (two-way bank conflicts).  The march is unrolled four-fold
+// so that every shared-memory offset is a compile-time constant and nothing is moved between registers.
 // All updates are computed unconditionally and selected by masks (no divergent branches around the
-// dependent chain of four divisions).
+// dependent chain of four updates); every shared-memory read of a step precedes its writes.
 #pragma once
 #include <climits>
 
@@ -48,13 +53,16 @@ constexpr int kRow = LN * 16;                        // bytes of one staged row
 constexpr int kPl = TYE * kRow;                      // bytes of one staged array plane
 constexpr int kPad = 512;                            // readable slack below the phi ring (masked lanes read row -1)
 enum { C_AX = 0, C_AY = 1, C_AZ = 2, C_RHS = 3, C_COUNT = 4 };
+constexpr int kExRow = LN * 8;                       // exchange plane: one double per pair, TYE + 2 rows (a pad row each side)
+constexpr int kEx = (TYE + 2) * kExRow;
+enum { EX_RA = 0, EX_BA = 2, EX_RB = 4 };            // sweep-1 red, sweep-1 black, sweep-2 red; two buffers each
 
 template <int LA>
 struct Cfg {
-    static constexpr int NP = 8, NC = LA + 2;        // phi: planes k-3 .. k+1 resident + LA in flight (+1 spare so that NP = 8)
+    static constexpr int NP = LA + 2, NC = LA + 2;   // planes k, k+1 resident + LA in flight
     static constexpr int kCoef = C_COUNT * kPl;
     static constexpr unsigned kTx = (unsigned)kRow * (TYE + (TYE - 1) + 3 * (TYE - 2));   // bytes landing per plane
-    static constexpr size_t kSmem = (size_t)kPad + (size_t)NP * kPl + (size_t)NC * kCoef + 8 * NP + 128;
+    static constexpr size_t kSmem = (size_t)kPad + (size_t)NP * kPl + (size_t)NC * kCoef + 6 * kEx + 8 * NP + 128;
 };
 
 __device__ __forceinline__ double2 ldp(const unsigned char* p) { return *reinterpret_cast<const double2*>(p); }
@@ -66,6 +74,7 @@ template <bool X> __device__ __forceinline__ double ldc(const unsigned char* p, 
 struct Th {                                  // per-thread constants
     unsigned char* phi0;                     // own slot of phi stage 0
     const unsigned char* coef0;              // own slot of coefficient stage 0, array C_AX
+    unsigned char* ex0;                      // own element of exchange buffer 0
     bool ra_x, ra_y, ba, rb_x, rb_y, own;    // lateral validity of the four half-sweeps (x / y cell of the pair)
     long long img_x, img_y;                  // periodic images of the own pair (0 = none)
     // half-sweep h is applied at step kk iff (unsigned)(kk - lo[h]) <= span[h]: the planes it is wanted on
@@ -83,6 +92,16 @@ template <bool X> __device__ __forceinline__ Lat lat_load(const unsigned char* p
     l.we = X ? ldc<false>(ph, 0, -1) : ldc<true>(ph, 0, 1);     // west of the x cell / east of the y cell
     l.s = ldc<X>(ph, -1, 0);
     l.n = ldc<X>(ph, 1, 0);
+    return l;
+}
+
+// the same three neighbours from an exchange plane (own element pointer): one double per pair
+template <bool X> __device__ __forceinline__ Lat lat_ex(const unsigned char* pe)
+{
+    Lat l;
+    l.we = *reinterpret_cast<const double*>(pe + (X ? -8 : 8));
+    l.s = *reinterpret_cast<const double*>(pe - kExRow);
+    l.n = *reinterpret_cast<const double*>(pe + kExRow);
     return l;
 }
 
@@ -117,17 +136,16 @@ __device__ __forceinline__ void issue_plane(const CUtensorMap* tm_phi, const CUt
     tma_load_3d(dc + C_AY * kPl + kRow, tm_ay, bar, cx, cy + 1, p);            // rows 1 .. TYE-1 (faces)
 }
 
-// One marching step at plane kk; X: the x column of the pair is red in plane kk.
+// One marching step at plane kk; X: the x column of the pair is red in plane kk; W: exchange buffers written by this
+// step (the other ones, written by the previous step, are read).
 // CUR receives the coefficients of plane kk; S1, S2, S3 hold those of planes kk-1, kk-2, kk-3.
-// Every shared-memory read of the step (the lateral neighbours of all four half-sweeps were written in EARLIER
-// steps) is issued before the first write, so the loads overlap instead of queueing behind possibly-aliasing stores.
-template <bool X, bool NORM>
-__device__ __forceinline__ void step(const Th& T, int kk, unsigned char* s0, unsigned char* sM1, unsigned char* sM2,
-                                     const unsigned char* sM3, const unsigned char* sP, const unsigned char* cI,
-                                     const unsigned char* cP, double* __restrict__ out, double2& Pn, double2& Pm1,
-                                     double2& Pm2, double2& Pm3, double2& Pm4, double2& azn, Coef& CUR, const Coef& S1,
-                                     const Coef& S2, const Coef& S3, double& vmax)
+template <bool X, int W, bool NORM>
+__device__ __forceinline__ void step(const Th& T, int kk, const unsigned char* s0, const unsigned char* sP,
+                                     const unsigned char* cI, const unsigned char* cP, double* __restrict__ out,
+                                     double2& Pn, double2& Pm1, double2& Pm2, double2& Pm3, double2& Pm4, double2& azn,
+                                     Coef& CUR, const Coef& S1, const Coef& S2, const Coef& S3, double& vmax)
 {
+    constexpr int R = 1 - W;
     const bool v0 = (unsigned)(kk - T.lo[0]) <= T.span[0], v1 = (unsigned)(kk - T.lo[1]) <= T.span[1];
     const bool v2 = (unsigned)(kk - T.lo[2]) <= T.span[2], v3 = (unsigned)(kk - T.lo[3]) <= T.span[3];
     double2 P0 = Pn;                                  // old phi of plane kk (staged read of the last step)
@@ -139,7 +157,10 @@ __device__ __forceinline__ void step(const Th& T, int kk, unsigned char* s0, uns
     CUR.ays = ldp(cI + C_AY * kPl);
     CUR.ayn = ldp(cI + C_AY * kPl + kRow);
     CUR.rhs = ldp(cI + C_RHS * kPl);
-    const Lat l0 = lat_load<X>(s0), l1 = lat_load<X>(sM1), l2 = lat_load<X>(sM2), l3 = lat_load<X>(sM3);
+    const Lat l0 = lat_load<X>(s0);                                   // old black neighbours in plane kk
+    const Lat l1 = lat_ex<X>(T.ex0 + (EX_RA + R) * kEx);              // sweep-1 red neighbours in plane kk-1
+    const Lat l2 = lat_ex<X>(T.ex0 + (EX_BA + R) * kEx);              // sweep-1 black neighbours in plane kk-2
+    const Lat l3 = lat_ex<X>(T.ex0 + (EX_RB + R) * kEx);              // sweep-2 red neighbours in plane kk-3
     double a, dg;
     // (1) sweep 1, red cells of plane kk
     const double n0 = gs_cell<X>(l0, pick<!X>(P0), CUR, azn, pick<X>(Pm1), pick<X>(Pn), a, dg);
@@ -154,9 +175,9 @@ __device__ __forceinline__ void step(const Th& T, int kk, unsigned char* s0, uns
     put<X>(Pm2, ((X ? T.rb_x : T.rb_y) && v2) ? n2 : pick<X>(Pm2));
     // (4) sweep 2, black cells of plane kk-3; the plane is finished
     const double n3 = gs_cell<X>(l3, pick<!X>(Pm3), S3, S2.az, pick<X>(Pm4), pick<X>(Pm2), a, dg);
-    *reinterpret_cast<double*>(s0 + (X ? 0 : 8)) = pick<X>(P0);
-    *reinterpret_cast<double*>(sM1 + (X ? 0 : 8)) = pick<X>(Pm1);
-    *reinterpret_cast<double*>(sM2 + (X ? 0 : 8)) = pick<X>(Pm2);
+    *reinterpret_cast<double*>(T.ex0 + (EX_RA + W) * kEx) = pick<X>(P0);
+    *reinterpret_cast<double*>(T.ex0 + (EX_BA + W) * kEx) = pick<X>(Pm1);
+    *reinterpret_cast<double*>(T.ex0 + (EX_RB + W) * kEx) = pick<X>(Pm2);
     if (T.own && v3) {
         put<X>(Pm3, n3);
         store_images(reinterpret_cast<double2*>(out), Pm3, T.img_x, T.img_y);
@@ -164,8 +185,8 @@ __device__ __forceinline__ void step(const Th& T, int kk, unsigned char* s0, uns
     Pm4 = Pm3; Pm3 = Pm2; Pm2 = Pm1; Pm1 = P0;
 }
 
-// Stage J (0 .. 7) of the eight-fold unrolled march: plane kk sits in phi stage (1 + J) % 8 and coefficient stage
-// (1 + J) % 4, so every shared-memory offset is a compile-time constant.
+// Stage J (0 .. 3) of the four-fold unrolled march: plane kk sits in stage (1 + J) % 4 of both rings, so every
+// shared-memory offset is a compile-time constant.
 template <int LA, int J, bool X, bool NORM>
 __device__ __forceinline__ void stage(const Th& T, int kk, int ke, unsigned par, const CUtensorMap* tm_phi,
                                       const CUtensorMap* tm_rhs, const CUtensorMap* tm_ax, const CUtensorMap* tm_ay,
@@ -175,19 +196,18 @@ __device__ __forceinline__ void stage(const Th& T, int kk, int ke, unsigned par,
                                       Coef& CUR, const Coef& S1, const Coef& S2, const Coef& S3, double& vmax)
 {
     using G = Cfg<LA>;
-    static_assert(G::NP == 8 && G::NC == 4, "the unrolled march assumes 8 phi and 4 coefficient stages");
-    constexpr int i0 = (1 + J) % 8, iP = (2 + J) % 8, i1 = J % 8, i2 = (J + 7) % 8, i3 = (J + 6) % 8, iN = (J + 4) % 8;
-    constexpr int c0 = (1 + J) % 4, cP = (2 + J) % 4, cN = J % 4;
-    // plane kk+1 (barrier iP) has landed: a barrier is reused every 8 steps, its parity flips with every reuse
-    mbar_wait(bar0 + 8 * iP, (par + (J >= 6 ? 1u : 0u)) & 1u);
+    static_assert(G::NP == 4 && G::NC == 4 && LA == 2, "the unrolled march assumes 4 stages per ring");
+    constexpr int i0 = (1 + J) % 4, iP = (2 + J) % 4, iN = J % 4;
+    // plane kk+1 (barrier iP) has landed: a barrier is reused every 4 steps, its parity flips with every reuse
+    mbar_wait(bar0 + 8 * iP, (par + (J >= 2 ? 1u : 0u)) & 1u);
     __syncthreads();                                           // every thread has finished step kk-1
     if (producer && kk + 1 + LA <= ke + 1) {                   // never leave a load in flight at exit
         asm volatile("fence.proxy.async.shared::cta;\n" ::: "memory");
-        issue_plane<LA>(tm_phi, tm_rhs, tm_ax, tm_ay, tm_az, phi_ring, coef_ring, bar0, iN * kPl, cN * G::kCoef,
+        issue_plane<LA>(tm_phi, tm_rhs, tm_ax, tm_ay, tm_az, phi_ring, coef_ring, bar0, iN * kPl, iN * G::kCoef,
                         kk + 1 + LA, nz, perz, cx, cy);
     }
-    step<X, NORM>(T, kk, T.phi0 + i0 * kPl, T.phi0 + i1 * kPl, T.phi0 + i2 * kPl, T.phi0 + i3 * kPl, T.phi0 + iP * kPl,
-                  T.coef0 + c0 * G::kCoef, T.coef0 + cP * G::kCoef, out, Pn, Pm1, Pm2, Pm3, Pm4, azn, CUR, S1, S2, S3, vmax);
+    step<X, J & 1, NORM>(T, kk, T.phi0 + i0 * kPl, T.phi0 + iP * kPl, T.coef0 + i0 * G::kCoef, T.coef0 + iP * G::kCoef,
+                         out, Pn, Pm1, Pm2, Pm3, Pm4, azn, CUR, S1, S2, S3, vmax);
 }
 
 template <int LA, bool REDX0, bool NORM>
@@ -202,7 +222,7 @@ __device__ __forceinline__ void march(const Th& T, int ks, int ke, const CUtenso
     Coef cA, cB, cC, cD;
     cB.ax = cB.ays = cB.ayn = cB.az = cB.rhs = z2; cB.ax2 = 0.0;
     cC = cB; cD = cB;
-    // the prologue issued planes ks-1 .. ks+LA into phi / coefficient stages 0 .. LA+1 (phase 0 of their barriers)
+    // the prologue issued planes ks-1 .. ks+LA into stages 0 .. LA+1 of both rings (phase 0 of their barriers)
     mbar_wait(bar0 + 0, 0);
     mbar_wait(bar0 + 8, 0);
     Pm1 = ldp(T.phi0);
@@ -220,10 +240,6 @@ __device__ __forceinline__ void march(const Th& T, int ks, int ke, const CUtenso
         MAC_T2_STAGE(1, !REDX0, cB, cA, cD, cC)
         MAC_T2_STAGE(2, REDX0, cC, cB, cA, cD)
         MAC_T2_STAGE(3, !REDX0, cD, cC, cB, cA)
-        MAC_T2_STAGE(4, REDX0, cA, cD, cC, cB)
-        MAC_T2_STAGE(5, !REDX0, cB, cA, cD, cC)
-        MAC_T2_STAGE(6, REDX0, cC, cB, cA, cD)
-        MAC_T2_STAGE(7, !REDX0, cD, cC, cB, cA)
     }
 #undef MAC_T2_STAGE
 }
@@ -242,7 +258,7 @@ k_rbgs_t2(const __grid_constant__ CUtensorMap tm_phi, const __grid_constant__ CU
     unsigned char* phi_gen = smem_raw + kPad;
     const unsigned phi_ring = smem_u32(phi_gen);
     const unsigned coef_ring = phi_ring + G::NP * kPl;
-    const unsigned bar0 = coef_ring + G::NC * G::kCoef;
+    const unsigned bar0 = coef_ring + G::NC * G::kCoef + 6 * kEx;     // (the exchange buffers sit between the rings and the barriers)
 
     const int lane = threadIdx.x;
     // a warp holds two rows; they must share their parity (the colour role is warp-uniform)
@@ -278,6 +294,7 @@ k_rbgs_t2(const __grid_constant__ CUtensorMap tm_phi, const __grid_constant__ CU
     const unsigned slot = (ty * LN + lane) * 16;
     T.phi0 = phi_gen + slot;
     T.coef0 = phi_gen + G::NP * kPl + slot;
+    T.ex0 = phi_gen + G::NP * kPl + G::NC * G::kCoef + ((ty + 1) * LN + lane) * 8;
     const int cx0 = x0 - HALO + L.gx, cy0 = y0 - HALO + L.gy;     // tensor-map coordinates of the tile origin
 
     const int ks = k0 - 3;
@@ -318,7 +335,7 @@ k_rbgs_t2(const __grid_constant__ CUtensorMap tm_phi, const __grid_constant__ CU
 // ---- host side ---------------------------------------------------------------------------------
 
 #ifndef MAC_T2_LA
-#define MAC_T2_LA 2                   // planes of TMA lookahead (shared memory: 0.5 + 6 (LA+5) + 24 (LA+2) KB)
+#define MAC_T2_LA 2                   // planes of TMA lookahead (4 stages per ring)
 #endif
 
 static inline int t2_smoother_configure()
