@@ -8,8 +8,8 @@ face coefficients -> coarsening -> rhs -> V-cycles to 1e-10 -> velocity correcti
 Prints ONE JSON line (rank 0).  `value` is level-0 cell-updates/s over the whole projection,
 N^3 (nu_pre + nu_post) cycles / t(project), inputs resident in HBM (SURVEY.md Sec. 8(d));
 `e2e` is the same metric through maestro_mac_project_host() with pinned HOST buffers, host<->device
-copies inside the timed region.  `roofline` is the level-0 fused red-black smoother (k_rbgs_tma): 48 B/cell/sweep
- over the mean device time of its launches, timed by CUDA event pairs inside
+copies inside the timed region.  `roofline` is the level-0 fused red-black smoother (k_rbgs_t2, two sweeps per launch): 48 B/cell/sweep
+ x the cell-sweeps of a launch over the mean device time of its launches, timed by CUDA event pairs inside
 the library on the call's stream during the timed steps.  Multi-GPU: replicas only:
 every rank projects its own copy; value = all ranks' units / max-over-ranks time.
 """
@@ -42,7 +42,7 @@ def parse_args():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", default="4N", help="workload: 1, 2, 3N, 3D, 4N, 4D, 5 (BASELINE.json configs)")
     ap.add_argument("--n", type=int, default=512, help="cells per side")
-    ap.add_argument("--smoother", type=int, default=0, help="0 fused single pass, TMA staging (default); 1 two-pass; 2 fused, cp.async staging; 3 fused, TMA 32x16 tile; 4 two sweeps per pass (experimental)")
+    ap.add_argument("--smoother", type=int, default=0, help="0 two sweeps per HBM pass, TMA staging (default); 1 two-pass reference; 2 fused, cp.async staging; 3 fused, TMA 32x16 tile; 4 one sweep per pass, TMA staging")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--cpu-sample-n", type=int, default=0, help="cells per side of the oracle sample (0 = auto)")
@@ -282,17 +282,23 @@ def run_ours(a):
     sm_ms = sum(s["ms_smooth0"] for s in stats)
     sm_n = sum(s["smooth0_timed"] for s in stats)
     peak, peak_src = hbm_peak()
-    kname = {0: "k_rbgs_tma", 1: "k_rbgs_color(x2)", 2: "k_rbgs_fused", 3: "k_rbgs_tma", 4: "k_rbgs_t2"}[a.smoother]
+    kname = {0: "k_rbgs_t2", 1: "k_rbgs_color(x2)", 2: "k_rbgs_fused", 3: "k_rbgs_tma", 4: "k_rbgs_tma"}[a.smoother]
     roof = None
     if sm_n > 0 and sm_ms > 0:
         per_launch_ms = sm_ms / sm_n
-        ach = SMOOTHER_BYTES_PER_CELL * wl.ncells / (per_launch_ms * 1e-3) / 1e9
+        sweeps = sum(s["smooth0_sweeps_timed"] for s in stats) / sm_n      # 2 with the two-sweep kernel
+        # algorithmic bytes per launch = 48 B per cell per sweep x the cell-sweeps one launch
+        # processes; the two-sweep kernel moves half of that through HBM (temporal blocking), so its fraction of the
+        # per-sweep roofline can exceed 1 -- `one_pass_bytes` / `frac_one_pass` state what it must move at least
+        alg = SMOOTHER_BYTES_PER_CELL * wl.ncells * sweeps
+        ach = alg / (per_launch_ms * 1e-3) / 1e9
+        one_pass = SMOOTHER_BYTES_PER_CELL * wl.ncells
         roof = {"bound": "hbm", "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
                 "traffic": ncu_traffic(kname, a.n), "kernel": kname + " level 0",
-                "algorithmic_bytes_per_launch": SMOOTHER_BYTES_PER_CELL * wl.ncells,
+                "algorithmic_bytes_per_launch": alg, "sweeps_per_launch": sweeps,
                 "avg_launch_ms": per_launch_ms, "launches_timed": sm_n, "peak_source": peak_src,
                 "frac_of_8000_nominal": ach / 8000.0,
-                "sweeps_per_launch": sum(s["smooth0_sweeps_timed"] for s in stats) / sm_n,
+                "one_pass_bytes": one_pass, "frac_one_pass": one_pass / (per_launch_ms * 1e-3) / 1e9 / peak,
                 "share_of_step": sm_ms / (t_dev * 1e3) if t_dev > 0 else None}
 
     # end to end through the host-buffer entry point
@@ -342,7 +348,7 @@ def run_ours(a):
             "ms_per_step": 1e3 * t_dev_max / max(a.steps, 1), "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": {"workload": workload_label(a.config, a.n), "cells": wl.ncells, "cycles_per_solve": cycles,
-                       "levels": stats[-1]["levels"], "smoother": {0: "fused red+black single pass, TMA-staged", 1: "two-pass reference", 2: "fused single pass, cp.async-staged", 3: "fused single pass, TMA 32x16 tile", 4: "two sweeps per pass (temporal blocking), TMA-staged"}[a.smoother],
+                       "levels": stats[-1]["levels"], "smoother": {0: "fused red+black, two sweeps per HBM pass (temporal blocking), TMA-staged", 1: "two-pass reference", 2: "fused single pass, cp.async-staged", 3: "fused single pass, TMA 32x16 tile", 4: "fused red+black, one sweep per pass, TMA-staged"}[a.smoother],
                        "parallelism": "replicas only" if world > 1 else "single GPU",
                        "l2": "inputs larger than L2 (every level-0 array is %.2f GB)" % (wl.ncells * 8 / 1e9)
                              if wl.ncells * 8 > 126e6 else "level arrays fit in L2; no flush (the solve re-reads them by design)",

@@ -78,11 +78,11 @@ typedef struct {
     int prolongation;         /* 0 = cell-centred trilinear (default), 1 = piecewise constant */
     int host_staging;         /* 1 = reserve device staging in the workspace so that
                                  maestro_mac_project_host() can be used */
-    int smoother;             /* 0 = default: fused red+black single pass, planes staged by TMA where the
-                                 level allows it (nx >= 60), else by cp.async;
-                                 4 = as 0, but pairs of sweeps run as ONE pass over HBM (two-sweep kernel,
-                                     temporal blocking) on levels of at least 48 x 16 x 8 cells; experimental:
-                                     correct and bit-identical to 0, not yet faster;
+    int smoother;             /* 0 = default: fused red+black passes with planes staged by TMA where the level
+                                     allows it (nx >= 60), else by cp.async; pairs of sweeps run as ONE pass
+                                     over HBM (two-sweep kernel, temporal blocking) on levels of at least
+                                     48 x 16 x 8 cells;
+                                 4 = as 0 but always one sweep per pass (bit-identical results);
                                  1 = reference two-pass (one kernel per colour);
                                  2 = fused single pass, cp.async staging on every level;
                                  3 = fused single pass, TMA staging with the 32x16 tile.

@@ -106,7 +106,7 @@ int validate_and_default(const maestro_mac_desc* in, maestro_mac_desc* d)
     if (!(d->bottom_rel_tol > 0.0)) d->bottom_rel_tol = 1e-8;
     if (d->prolongation != 0 && d->prolongation != 1) return MAESTRO_MAC_ERR_ARG;
     if (d->host_staging != 0 && d->host_staging != 1) return MAESTRO_MAC_ERR_ARG;
-    if (d->smoother < 0 || d->smoother > 4) return MAESTRO_MAC_ERR_ARG;   // 4: two-sweep kernel
+    if (d->smoother < 0 || d->smoother > 4) return MAESTRO_MAC_ERR_ARG;   // 4: one sweep per pass everywhere
     if (d->stop_test != 0 && d->stop_test != 1) return MAESTRO_MAC_ERR_ARG;
     if (d->rho_mean != 0 && d->rho_mean != 1) return MAESTRO_MAC_ERR_ARG;
     return MAESTRO_MAC_OK;
@@ -116,7 +116,7 @@ int validate_and_default(const maestro_mac_desc* in, maestro_mac_desc* d)
 void set_level(const maestro_mac_desc& d, Level& L, const int n[3], const double h[3], bool ghosts)
 {
     for (int a = 0; a < 3; ++a) { L.n[a] = n[a]; L.h[a] = h[a]; }
-    const int gw = d.smoother == 4 ? t2::HALO : 2;         // the two-sweep kernel's halo is 4 cells
+    const int gw = d.smoother == 0 ? t2::HALO : 2;         // the two-sweep kernel's halo is 4 cells
     L.gx = (ghosts && d.bc_lo[0] == MAESTRO_MAC_PERIODIC) ? gw : 0;
     L.gy = (ghosts && d.bc_lo[1] == MAESTRO_MAC_PERIODIC) ? gw : 0;
     L.cx = n[0] + 2 * L.gx;
@@ -406,7 +406,7 @@ int do_sweep(maestro_mac_handle* H, int l, cudaStream_t s, int* norm_parts = nul
 // the two-sweep kernel runs with the default smoother on levels its tile and halo fit
 bool t2_ok(const maestro_mac_handle* H, int l)
 {
-    return H->d.smoother == 4 && H->lev[l].tma[2].ok && t2_level_ok(dev_level(H, l));
+    return H->d.smoother == 0 && H->lev[l].tma[2].ok && t2_level_ok(dev_level(H, l));
 }
 
 // Two sweeps on level l in one pass (k_rbgs_t2).  norm_parts / swap as in do_sweep.
