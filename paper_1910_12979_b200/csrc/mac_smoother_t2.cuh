@@ -164,8 +164,10 @@ __device__ __forceinline__ void step(const Th& T, int kk, const unsigned char* s
     double a, dg;
     // (1) sweep 1, red cells of plane kk
     const double n0 = gs_cell<X>(l0, pick<!X>(P0), CUR, azn, pick<X>(Pm1), pick<X>(Pn), a, dg);
-    if (NORM && T.own && (unsigned)(kk - T.nlo) <= T.nspan)
-        vmax = nanmax(vmax, fabs(fma(pick<X>(P0), dg, -a)));                  // |rhs - (sum - phi_0 dg)| of the input
+    if (NORM) {                                       // |rhs - (sum - phi_0 dg)| of the input, selected (no branch)
+        const double rr = fabs(fma(pick<X>(P0), dg, -a));
+        vmax = (T.own && (unsigned)(kk - T.nlo) <= T.nspan) ? nanmax(vmax, rr) : vmax;
+    }
     put<X>(P0, ((X ? T.ra_x : T.ra_y) && v0) ? n0 : pick<X>(P0));
     // (2) sweep 1, black cells of plane kk-1
     const double n1 = gs_cell<X>(l1, pick<!X>(Pm1), S1, CUR.az, pick<X>(Pm2), pick<X>(P0), a, dg);
