@@ -15,9 +15,8 @@
 //      (4) sweep 2 black of plane k-3    (sweep-2 red neighbours:       planes k-4, k-3, k-2)
 // and stores plane k-3.  All four updates hit the SAME column of the pair (the colour of a column
 // alternates from plane to plane), vertical neighbours are the thread's own registers, lateral
-// neighbours come from the staged planes, which are updated in place (each update is written back to
-// its stage, so a stage holds, in turn, old / sweep-1 red / sweep-1 final / sweep-2 red values).
-// The only cross-thread dependences are lateral and always one step old: one __syncthreads per plane.
+// neighbours are values other threads produced ONE STEP EARLIER (exchange buffers, see "Memory"):
+// the only cross-thread dependences are lateral and one step old, hence one __syncthreads per plane.
 //
 // Lateral halo: every half-sweep consumes one ring of cells, so a tile of 32 x 24 staged cells yields
 // 24 x 16 finished ones (halo 4); the halo cells are recomputed redundantly by the neighbouring CTA
