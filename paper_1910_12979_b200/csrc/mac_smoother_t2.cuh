@@ -142,7 +142,7 @@ template <bool X, int W, bool NORM>
 __device__ __forceinline__ void step(const Th& T, int kk, const unsigned char* s0, const unsigned char* sP,
                                      const unsigned char* cI, const unsigned char* cP, double* __restrict__ out,
                                      double2& Pn, double2& Pm1, double2& Pm2, double2& Pm3, double2& Pm4, double2& azn,
-                                     Coef& CUR, const Coef& S1, const Coef& S2, const Coef& S3, double& vmax)
+                                     Coef& CUR, const Coef& S1, const Coef& S2, const Coef& S3, double& vmax, bool& vnan)
 {
     constexpr int R = 1 - W;
     const bool v0 = (unsigned)(kk - T.lo[0]) <= T.span[0], v1 = (unsigned)(kk - T.lo[1]) <= T.span[1];
@@ -163,9 +163,11 @@ __device__ __forceinline__ void step(const Th& T, int kk, const unsigned char* s
     double a, dg;
     // (1) sweep 1, red cells of plane kk
     const double n0 = gs_cell<X>(l0, pick<!X>(P0), CUR, azn, pick<X>(Pm1), pick<X>(Pn), a, dg);
-    if (NORM) {                                       // |rhs - (sum - phi_0 dg)| of the input, selected (no branch)
+    if (NORM) {                                       // |rhs - (sum - phi_0 dg)| of the input; a NaN sets the sign of vmax
         const double rr = fabs(fma(pick<X>(P0), dg, -a));
-        vmax = (T.own && (unsigned)(kk - T.nlo) <= T.nspan) ? nanmax(vmax, rr) : vmax;
+        const bool on = T.own && (unsigned)(kk - T.nlo) <= T.nspan;
+        vmax = fmax(vmax, on ? rr : 0.0);             // (fmax drops NaNs: they are recorded separately)
+        vnan = vnan || (on && rr != rr);
     }
     put<X>(P0, ((X ? T.ra_x : T.ra_y) && v0) ? n0 : pick<X>(P0));
     // (2) sweep 1, black cells of plane kk-1
@@ -194,7 +196,7 @@ __device__ __forceinline__ void stage(const Th& T, int kk, int ke, unsigned par,
                                       const CUtensorMap* tm_az, unsigned phi_ring, unsigned coef_ring, unsigned bar0,
                                       bool producer, int cx, int cy, int nz, bool perz, double* __restrict__ out,
                                       double2& Pn, double2& Pm1, double2& Pm2, double2& Pm3, double2& Pm4, double2& azn,
-                                      Coef& CUR, const Coef& S1, const Coef& S2, const Coef& S3, double& vmax)
+                                      Coef& CUR, const Coef& S1, const Coef& S2, const Coef& S3, double& vmax, bool& vnan)
 {
     using G = Cfg<LA>;
     static_assert(G::NP == 4 && G::NC == 4 && LA == 2, "the unrolled march assumes 4 stages per ring");
@@ -208,14 +210,14 @@ __device__ __forceinline__ void stage(const Th& T, int kk, int ke, unsigned par,
                         kk + 1 + LA, nz, perz, cx, cy);
     }
     step<X, J & 1, NORM>(T, kk, T.phi0 + i0 * kPl, T.phi0 + iP * kPl, T.coef0 + i0 * G::kCoef, T.coef0 + iP * G::kCoef,
-                         out, Pn, Pm1, Pm2, Pm3, Pm4, azn, CUR, S1, S2, S3, vmax);
+                         out, Pn, Pm1, Pm2, Pm3, Pm4, azn, CUR, S1, S2, S3, vmax, vnan);
 }
 
 template <int LA, bool REDX0, bool NORM>
 __device__ __forceinline__ void march(const Th& T, int ks, int ke, const CUtensorMap* tm_phi, const CUtensorMap* tm_rhs,
                                       const CUtensorMap* tm_ax, const CUtensorMap* tm_ay, const CUtensorMap* tm_az,
                                       unsigned phi_ring, unsigned coef_ring, unsigned bar0, bool producer, int cx, int cy,
-                                      int nz, bool perz, double* __restrict__ out, unsigned long long out_stride, double& vmax)
+                                      int nz, bool perz, double* __restrict__ out, unsigned long long out_stride, double& vmax, bool& vnan)
 {
     using G = Cfg<LA>;
     const double2 z2 = make_double2(0.0, 0.0);
@@ -233,7 +235,7 @@ __device__ __forceinline__ void march(const Th& T, int ks, int ke, const CUtenso
 #define MAC_T2_STAGE(J, XX, CUR, S1, S2, S3)                                                                          \
     if (kk > ke) break;                                                                                               \
     stage<LA, J, XX, NORM>(T, kk, ke, par, tm_phi, tm_rhs, tm_ax, tm_ay, tm_az, phi_ring, coef_ring, bar0, producer,  \
-                           cx, cy, nz, perz, out, Pn, Pm1, Pm2, Pm3, Pm4, azn, CUR, S1, S2, S3, vmax);                \
+                           cx, cy, nz, perz, out, Pn, Pm1, Pm2, Pm3, Pm4, azn, CUR, S1, S2, S3, vmax, vnan);                \
     out += out_stride; ++kk;
 #pragma unroll 1
     for (int kk = ks; kk <= ke; par ^= 1u) {
@@ -312,14 +314,16 @@ k_rbgs_t2(const __grid_constant__ CUtensorMap tm_phi, const __grid_constant__ CU
     const unsigned long long ostride = (unsigned long long)L.cx * L.ry;
     double* out = pout + (T.own ? (long long)gi + (long long)L.cx * gj : 0) + (long long)(ks - 3) * (long long)ostride;
     double vmax = 0.0;
+    bool vnan = false;
     if (((gj + ks) & 1) == 0)
-        march<LA, true, NORM>(T, ks, k1 + 2, &tm_phi, &tm_rhs, &tm_ax, &tm_ay, &tm_az, phi_ring, coef_ring, bar0, producer, cx0, cy0, L.nz, perz, out, ostride, vmax);
+        march<LA, true, NORM>(T, ks, k1 + 2, &tm_phi, &tm_rhs, &tm_ax, &tm_ay, &tm_az, phi_ring, coef_ring, bar0, producer, cx0, cy0, L.nz, perz, out, ostride, vmax, vnan);
     else
-        march<LA, false, NORM>(T, ks, k1 + 2, &tm_phi, &tm_rhs, &tm_ax, &tm_ay, &tm_az, phi_ring, coef_ring, bar0, producer, cx0, cy0, L.nz, perz, out, ostride, vmax);
+        march<LA, false, NORM>(T, ks, k1 + 2, &tm_phi, &tm_rhs, &tm_ax, &tm_ay, &tm_az, phi_ring, coef_ring, bar0, producer, cx0, cy0, L.nz, perz, out, ostride, vmax, vnan);
     // every plane that was issued (<= k1 + 3) has been waited for by the last step: nothing is in flight
     if (NORM) {
         __shared__ double sh_max[32];
         const int tid = threadIdx.x + LN * threadIdx.y;
+        if (vnan) vmax = __longlong_as_double(0x7ff8000000000000ll);
         vmax = warp_nanmax(vmax);
         if ((tid & 31) == 0) sh_max[tid >> 5] = vmax;
         __syncthreads();
