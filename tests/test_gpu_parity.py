@@ -372,3 +372,20 @@ def test_harmonic_face_density_variant(oracle, mac, name, N, smoother):
     assert got["status"] == ref["status"] == 0 and got["stats"]["cycles"] == ref["stats"]["cycles"]
     for key in ("phi", "u", "v", "w"):
         assert rel_l2(got[key], ref[key]) <= E2E_TOL, key
+
+
+@pytest.mark.parametrize("nu_pre,nu_post", [(1, 1), (3, 1), (1, 2), (4, 3)])
+@pytest.mark.parametrize("name,N", [("1", 64), ("4D", 64)])
+def test_sweep_counts_other_than_two(oracle, mac, name, N, nu_pre, nu_post):
+    """Pairs of sweeps run through the two-sweep kernel, a remaining one through the single-sweep kernel, and the
+    riding stop test follows (one- or two-sweep speculative pass): parity for odd and larger sweep counts."""
+    wl = W.by_name(name, N)
+    wl.nu_pre, wl.nu_post = nu_pre, nu_post
+    ref = oracle_project(oracle, wl)
+    K = ref["stats"]["cycles"]
+    got = gpu_project(mac, wl)
+    if got["stats"]["cycles"] != K:
+        got = gpu_project(mac, wl, rel_tol=0.0, max_cycles=K)
+    assert got["status"] == ref["status"] == 0 and got["stats"]["cycles"] == K
+    for key in ("phi", "u", "v", "w"):
+        assert rel_l2(got[key], ref[key]) <= E2E_TOL, key
