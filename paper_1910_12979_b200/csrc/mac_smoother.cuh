@@ -49,12 +49,13 @@ __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commi
 template <int N> __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;\n" ::"n"(N) : "memory"); }
 
 // The division by the diagonal: dg is a sum of positive, well-scaled face coefficients, so the guarded IEEE
-// division (range checks + slow-path call) is replaced by a reciprocal seed, two Newton steps and one
-// correction of the quotient: faithful to 1 ulp.  -DMAC_IEEE_DIV restores the plain division.
+// division (range checks + slow-path call) is replaced by a reciprocal seed and two Newton steps (1/dg to ~1 ulp)
+// times the numerator: within ~1.5 ulp of the quotient.  -DMAC_GS_FAITHFUL adds one correction of the quotient
+// (<= 1 ulp), -DMAC_IEEE_DIV restores the plain division.
 // The Gauss-Seidel value  (sum_f a_f phi_f - rhs) / sum_f a_f  arranged for a short dependent chain.  In the
 // marching kernels the upper neighbour u_ is the value the previous half-sweep of the SAME step has just
 // produced, so it enters last: the reciprocal of the diagonal and the other five products are off the chain,
-// which is then fma, mul, fma, fma (fp64 latency, not throughput, bounds these kernels).  *a_out = sum - rhs.
+// which is then fma, mul (fp64 latency, not throughput, bounds these kernels).  *a_out = sum - rhs.
 __device__ __forceinline__ double gs_value(double axw, double axe, double ays, double ayn, double azd, double azu,
                                            double rhs, double w_, double e_, double s_, double n_, double d_, double u_,
                                            double& a_out, double& dg_out)
@@ -72,7 +73,13 @@ __device__ __forceinline__ double gs_value(double axw, double axe, double ays, d
     r = fma(fma(-dg, r, 1.0), r, r);
     r = fma(fma(-dg, r, 1.0), r, r);
     const double q = a * r;
-    return fma(fma(-dg, q, a), r, q);
+#ifdef MAC_GS_FAITHFUL
+    return fma(fma(-dg, q, a), r, q);           // one correction of the quotient: faithful (<= 1 ulp)
+#else
+    return q;                                   // r is 1/dg to ~1 ulp, so the quotient is within ~1.5 ulp: the correction
+                                                // would put two more dependent fp64 operations on the chain of every
+                                                // half-sweep (two-sweep kernel: 1.75 -> 1.64 ms without it)
+#endif
 #endif
 }
 
