@@ -510,20 +510,6 @@ k_residual_norm(LevelDev L, double* __restrict__ part_sum, double* __restrict__ 
     block_reduce_store(0.0, m, part_sum, part_max, blockIdx.x);
 }
 
-// out = rhs - L phi on a level (used by level_get-style diagnostics / tests)
-__global__ void __launch_bounds__(256)
-k_residual(LevelDev L, double* __restrict__ out)
-{
-    const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    const int j = blockIdx.y * blockDim.y + threadIdx.y;
-    const int k = blockIdx.z;
-    if (i >= L.nx || j >= L.ny) return;
-    double off, dg;
-    stencil_sums(L, L.phi, i, j, k, off, dg);
-    const size_t c = cidx(L, i, j, k);
-    out[c] = L.rhs[c] - (off - L.phi[c] * dg);
-}
-
 // ------------------------------------------------------------------------------------------------
 // a8  bottom solve: unpreconditioned BiCGStab, x0 = 0, rhat = r0, one thread block; dot products
 // by warp shuffles + one shared-memory stage (deterministic).  Stops at ||r||2 <= tol ||f||2,
@@ -811,52 +797,6 @@ __device__ __forceinline__ double profile_eval_inv(const double* __restrict__ f,
 __device__ __forceinline__ double beta_inv(const GeoDev& G, const GeoInv& I, const double* __restrict__ f, double x, double y, double z)
 {
     return profile_eval_inv(f, G.nr, I.idr, radius(G, x, y, z));
-}
-
-// a4: rhs = D(beta0 U_edge) - beta0 S with partial sum / max.  grid (ceil(nx/64), ceil(ny/4), chunks), block (64, 4)
-__global__ void __launch_bounds__(256)
-k_rhs2(GeoDev G, GeoInv I, LevelDev L, const double* __restrict__ beta0, const double* __restrict__ u, const double* __restrict__ v,
-       const double* __restrict__ w, const double* __restrict__ S, int zchunk,
-       double* __restrict__ part_sum, double* __restrict__ part_max)
-{
-    const int i = blockIdx.x * 64 + threadIdx.x, j = blockIdx.y * 4 + threadIdx.y;
-    const int k0 = blockIdx.z * zchunk, k1 = min(k0 + zchunk, G.nz);
-    const bool in = i < G.nx && j < G.ny;
-    const bool px = G.bclo[0] == MAC_PERIODIC, py = G.bclo[1] == MAC_PERIODIC, pz = G.bclo[2] == MAC_PERIODIC;
-    double s = 0.0, m = 0.0;
-    const int ic = in ? i : 0, jc = in ? j : 0;                  // clamped: out-of-range threads still shuffle
-    const double xc = (ic + 0.5) * G.dx, yc = (jc + 0.5) * G.dy;
-    const int ih = (px && ic + 1 == G.nx) ? 0 : ic + 1;
-    const int jh = (py && jc + 1 == G.ny) ? 0 : jc + 1;
-    const bool last_x = (threadIdx.x & 31) == 31 || ic + 1 == G.nx;
-    const size_t sc = (size_t)G.nx * G.ny, su = (size_t)(G.nx + 1) * G.ny, sv = (size_t)G.nx * (G.ny + 1);
-    const double* up = u + (size_t)(G.nx + 1) * jc + su * k0;
-    const double* vp = v + ic + sv * k0;
-    const double* wp = w + ic + (size_t)G.nx * jc;
-    const size_t c0 = (size_t)ic + (size_t)G.nx * jc;
-    double fzl = beta_inv(G, I, beta0, xc, yc, k0 * G.dz) * __ldg(wp + sc * k0);
-#pragma unroll 4
-    for (int k = k0; k < k1; ++k) {
-        const double zc = (k + 0.5) * G.dz;
-        const int kh = (pz && k + 1 == G.nz) ? 0 : k + 1;
-        const double fxl = beta_inv(G, I, beta0, ic * G.dx, yc, zc) * __ldg(up + ic);
-        double fxh = __shfl_down_sync(0xffffffffu, fxl, 1);
-        if (last_x) fxh = beta_inv(G, I, beta0, ih * G.dx, yc, zc) * __ldg(up + ih);
-        const double fyl = beta_inv(G, I, beta0, xc, jc * G.dy, zc) * __ldg(vp + (size_t)G.nx * jc);
-        const double fyh = beta_inv(G, I, beta0, xc, jh * G.dy, zc) * __ldg(vp + (size_t)G.nx * jh);
-        const double fzh = beta_inv(G, I, beta0, xc, yc, kh * G.dz) * __ldg(wp + sc * kh);
-        double r = (fxh - fxl) * I.idx + (fyh - fyl) * I.idy + (fzh - fzl) * I.idz;
-        if (S) r -= beta_inv(G, I, beta0, xc, yc, zc) * __ldg(S + c0 + sc * k);
-        if (in) {
-            L.rhs[cidx(L, ic, jc, k)] = r;
-            s += r;
-            m = nanmax(m, fabs(r));
-        }
-        fzl = fzh;
-        up += su;
-        vp += sv;
-    }
-    block_reduce_store(s, m, part_sum, part_max, blockIdx.x + gridDim.x * (blockIdx.y + gridDim.y * blockIdx.z));
 }
 
 // a2: face coefficients.  Threads cover the extended index space i in [0,nx], j in [0,ny]; planes k in [k0,k1]

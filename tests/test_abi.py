@@ -39,7 +39,7 @@ def test_workspace_query_and_validation(mac):
     # level 0: phi, phi2, rhs + three face arrays; all levels ~ 8/7 of that (+ periodic image columns / rows
     # on the TMA levels, + 2 MB of reduction scratch)
     cells = 128 ** 3
-    assert 6 * cells * 8 < need < 8 * cells * 8
+    assert 6 * cells * 8 < need < 8.5 * cells * 8          # (four image columns / rows per side for the two-sweep kernel)
     d2 = mac.make_desc((128, 128, 128), (1 / 128,) * 3, (0, 0, 1), (0, 0, 1), host_staging=1)
     assert mac.workspace_bytes(d2) > need + 6 * cells * 8
 
