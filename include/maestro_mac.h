@@ -8,13 +8,14 @@
  *
  * so that the corrected face velocities satisfy the low Mach number divergence constraint
  *        div(beta0 U) = beta0 (S - (1/(Gamma1bar p0)) dp0/dt)      PAPER.md:49  (Sec. 2, Eq. 6)
- * (the dp0/dt term is folded into S by the caller).  The coefficient beta0/rho is the weighting of
+ * (the dp0/dt term is folded into S by the caller, or registered as a profile with
+ * maestro_mac_set_dpdt_term).  The coefficient beta0/rho is the weighting of
  * the pressure term (beta0/rho) grad(pi/beta0) of PAPER.md:35 (Sec. 2, Eq. 2); beta0, rho0 are the
  * one-dimensional base state of PAPER.md:29,39,45 (Eq. 4-5); (*) is solved by geometric multigrid
  * V-cycles ("multigrid linear solvers for the pressure projection steps", "second order projection
  * method", Sec. 3).  The paper gives no discretisation; the one used here is stated in
  * DESIGN.md ("Readings") and SURVEY.md Sec. 8(c): 7-point variable-coefficient operator, arithmetic
- * face densities, red-black Gauss-Seidel V(nu_pre,nu_post), 8-cell-mean restriction, cell-centred
+ * (or, desc.rho_mean = 1, harmonic) face densities, red-black Gauss-Seidel V(nu_pre,nu_post), 8-cell-mean restriction, cell-centred
  * trilinear prolongation, BiCGStab on the coarsest level, max-norm stopping test.
  *
  * LAYOUT (all arrays x-fastest, fp64, DEVICE memory unless stated otherwise)

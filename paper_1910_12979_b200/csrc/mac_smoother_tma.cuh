@@ -11,8 +11,10 @@
 // the "phi = 0 and a_f = 0 outside the domain" convention of the folded coefficients
 // (mac_common.cuh).  Arithmetic, marching order and results are those of fused::step.
 //
-// Used for levels whose x and y sides are not periodic (TMA cannot wrap); periodic levels keep the
-// cp.async kernel.  z may be periodic (the plane coordinate is wrapped by the issuing thread).
+// TMA cannot wrap: a level that is periodic in x and / or y carries periodic image columns / rows of
+// every array (mac_common.cuh "Ghosts"), which the box loads read like any halo; z may be periodic
+// (the plane coordinate is wrapped by the issuing thread).  One sweep per launch: the default path runs
+// pairs of sweeps through mac_smoother_t2.cuh and uses this kernel for a remaining single sweep.
 #pragma once
 #include <cuda.h>
 

@@ -1,6 +1,8 @@
 // maestro_mac.cu -- host side of the C ABI declared in include/maestro_mac.h.
 // Validates descriptors, builds the level hierarchy, carves the caller's workspace, and drives the
-// kernels of mac_kernels.cuh / mac_smoother.cuh on the caller's stream.  No device allocation here.
+// kernels on the caller's stream: mac_setup.cuh (assembly pass), mac_smoother_t2.cuh / _tma.cuh /
+// mac_smoother.cuh (smoothers), mac_tail.cuh (coarse tail), mac_kernels.cuh (transfers, bottom solve,
+// correction, reductions), mac_base.cuh (base state).  No device allocation here.
 #include "maestro_mac.h"
 
 #include <cuda_runtime.h>
