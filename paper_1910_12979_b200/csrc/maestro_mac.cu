@@ -282,8 +282,12 @@ int do_coefficients(maestro_mac_handle* H, const double* beta0, const double* rh
     if (H->d.smoother != 1 && rho) {
         const int zc = 16;
         dim3 gg((G.nx + 64) / 64, (G.ny + 4) / 4, (G.nz + zc - 1) / zc);
-        k_setup<true, false><<<gg, dim3(64, 4), 0, s>>>(G, dev_geo_inv(H), dev_level(H, 0), beta0, rho, nullptr, nullptr, nullptr,
-                                                        nullptr, nullptr, zc, H->flags, nullptr, nullptr);
+        if (H->d.rho_mean)
+            k_setup<true, false, true><<<gg, dim3(64, 4), 0, s>>>(G, dev_geo_inv(H), dev_level(H, 0), beta0, rho, nullptr, nullptr,
+                                                                  nullptr, nullptr, nullptr, zc, H->flags, nullptr, nullptr);
+        else
+            k_setup<true, false, false><<<gg, dim3(64, 4), 0, s>>>(G, dev_geo_inv(H), dev_level(H, 0), beta0, rho, nullptr, nullptr,
+                                                                   nullptr, nullptr, nullptr, zc, H->flags, nullptr, nullptr);
     } else if (H->d.smoother != 1) {
         const int zc = 16;
         dim3 gg((G.nx + 64) / 64, (G.ny + 4) / 4, (G.nz + zc) / zc);
@@ -322,8 +326,12 @@ int do_rhs(maestro_mac_handle* H, const double* beta0, const double* u, const do
         int zc;
         const dim3 gg = setup_grid(G, &zc);
         nb = (int)(gg.x * gg.y * gg.z);
-        k_setup<false, true><<<gg, dim3(64, 4), 0, s>>>(G, dev_geo_inv(H), dev_level(H, 0), beta0, nullptr, u, v, w, S, H->dpdt_term,
-                                                        zc, H->flags, H->part_sum, H->part_max);
+        if (H->dpdt_term)
+            k_setup<false, true, true><<<gg, dim3(64, 4), 0, s>>>(G, dev_geo_inv(H), dev_level(H, 0), beta0, nullptr, u, v, w, S,
+                                                                  H->dpdt_term, zc, H->flags, H->part_sum, H->part_max);
+        else
+            k_setup<false, true, false><<<gg, dim3(64, 4), 0, s>>>(G, dev_geo_inv(H), dev_level(H, 0), beta0, nullptr, u, v, w, S,
+                                                                   nullptr, zc, H->flags, H->part_sum, H->part_max);
     } else {
         int rows = G.ny * G.nz;
         nb = red_blocks(rows);
@@ -342,8 +350,12 @@ int do_setup_fused(maestro_mac_handle* H, const double* beta0, const double* rho
     CUDA_OK(cudaMemsetAsync(H->flags, 0, 16 * sizeof(int), s));
     int zc;
     const dim3 gg = setup_grid(G, &zc);
-    k_setup<true, true><<<gg, dim3(64, 4), 0, s>>>(G, dev_geo_inv(H), dev_level(H, 0), beta0, rho, u, v, w, S, H->dpdt_term, zc,
-                                                   H->flags, H->part_sum, H->part_max);
+    if (H->d.rho_mean || H->dpdt_term)
+        k_setup<true, true, true><<<gg, dim3(64, 4), 0, s>>>(G, dev_geo_inv(H), dev_level(H, 0), beta0, rho, u, v, w, S,
+                                                             H->dpdt_term, zc, H->flags, H->part_sum, H->part_max);
+    else
+        k_setup<true, true, false><<<gg, dim3(64, 4), 0, s>>>(G, dev_geo_inv(H), dev_level(H, 0), beta0, rho, u, v, w, S, nullptr,
+                                                              zc, H->flags, H->part_sum, H->part_max);
     LAUNCHED(H);
     int rc;
     if ((rc = do_coarsen(H, s)) != 0) return rc;
