@@ -166,7 +166,7 @@ def run_reference(a):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return 0
-    ns = a.cpu_sample_n or (128 if a.steps + a.warmup <= 4 else 64)
+    ns = a.cpu_sample_n or 128                 # one projection at 128^3 is about 1 s on 16 cores
     ns = min(ns, a.n)
     for _ in range(a.warmup):
         cpu_oracle_run(a.config, ns)
@@ -336,7 +336,7 @@ def run_ours(a):
 
     cpu = None
     if rank == 0 and world == 1 and not a.no_cpu_baseline:
-        ns = a.cpu_sample_n or min(128, a.n)
+        ns = a.cpu_sample_n or min(256, a.n)   # about 10 s of CPU work for the 512^3 workload
         dt, cyc, cells, threads, nu_o = cpu_oracle_run(a.config, ns)
         cpu = {"value": cells * nu_o * cyc / dt, "unit": UNIT, "cores": threads, "kind": "oracle",
                "sample": f"{a.config} at {ns}^3 (same recipe as the {a.n}^3 workload), one full projection, "
