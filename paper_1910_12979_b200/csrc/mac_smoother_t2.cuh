@@ -247,12 +247,17 @@ __device__ __forceinline__ void march(const Th& T, int ks, int ke, const CUtenso
 #undef MAC_T2_STAGE
 }
 
+// Work decomposition of one launch (host: t2_plan).  704 tiles on 148 SMs are 4.76 waves of whole columns: the
+// first nfull tiles (whole waves) march all of z, the remaining tiles are cut into nsplit z-chunks each so that the
+// last, partial wave is spread over every SM.  nfull = 0: every tile is cut into nsplit chunks.
+struct T2Plan { int tiles_x, tiles, nfull, nsplit, zchunk, ncta; };
+
 // NORM: additionally writes, per CTA, max |rhs - L phi_in| over the red cells to part_max[linear CTA index]
 template <int LA, bool NORM>
 __global__ void __launch_bounds__(NT, 1)
 k_rbgs_t2(const __grid_constant__ CUtensorMap tm_phi, const __grid_constant__ CUtensorMap tm_rhs,
           const __grid_constant__ CUtensorMap tm_ax, const __grid_constant__ CUtensorMap tm_ay,
-          const __grid_constant__ CUtensorMap tm_az, LevelDev L, double* __restrict__ pout, int zchunk,
+          const __grid_constant__ CUtensorMap tm_az, LevelDev L, double* __restrict__ pout, T2Plan plan,
           double* __restrict__ part_max)
 {
     using G = Cfg<LA>;
@@ -266,8 +271,16 @@ k_rbgs_t2(const __grid_constant__ CUtensorMap tm_phi, const __grid_constant__ CU
     const int lane = threadIdx.x;
     // a warp holds two rows; they must share their parity (the colour role is warp-uniform)
     const int ty = 4 * ((int)threadIdx.y >> 2) + (((int)threadIdx.y >> 1) & 1) + 2 * ((int)threadIdx.y & 1);
-    const int x0 = blockIdx.x * kTX, y0 = blockIdx.y * kTY;
-    const int k0 = blockIdx.z * zchunk, k1 = min(k0 + zchunk, L.nz);
+    // linear CTA index -> (tile, z range): the first plan.nfull tiles march the whole column, the others a chunk each
+    int tile = blockIdx.x, k0 = 0, k1 = L.nz;
+    if (tile >= plan.nfull) {
+        const int q = tile - plan.nfull, rem = plan.tiles - plan.nfull, c = q / rem;
+        tile = plan.nfull + (q - c * rem);
+        k0 = c * plan.zchunk;
+        k1 = min(k0 + plan.zchunk, L.nz);
+    }
+    const int tyi = tile / plan.tiles_x;
+    const int x0 = (tile - tyi * plan.tiles_x) * kTX, y0 = tyi * kTY;
     const int gi = x0 - HALO + 2 * lane, gj = y0 - HALO + ty;
     // ghost columns / rows of a periodic level hold valid images: they are recomputed like any halo cell
     const bool col_ok = gi >= -L.gx && gi < L.nx + L.gx && gj >= -L.gy && gj < L.ny + L.gy;
@@ -330,7 +343,7 @@ k_rbgs_t2(const __grid_constant__ CUtensorMap tm_phi, const __grid_constant__ CU
         if (tid == 0) {
             double m = sh_max[0];
             for (int q = 1; q < NT / 32; ++q) m = nanmax(m, sh_max[q]);
-            part_max[blockIdx.x + gridDim.x * (blockIdx.y + gridDim.y * blockIdx.z)] = m;
+            part_max[blockIdx.x] = m;
         }
     }
 }
@@ -361,22 +374,27 @@ static inline bool t2_level_ok(const LevelDev& L)
     return true;
 }
 
-static inline dim3 t2_sweep_grid(const LevelDev& L, int* zchunk_out)
+static inline t2::T2Plan t2_plan(const LevelDev& L)
 {
-    const int tiles_x = (L.nx + t2::kTX - 1) / t2::kTX, tiles_y = (L.ny + t2::kTY - 1) / t2::kTY;
-    // chunk count that minimises waves x (planes per chunk + the 6 redone planes + pipeline fill)
-    const int tiles = tiles_x * tiles_y;
-    long best = -1; int bn = 1;
-    const int maxchunk = L.nz >= 32 ? L.nz / 16 : 1;
-    for (int n = 1; n <= maxchunk; ++n) {
-        const int zc = (L.nz + n - 1) / n;
-        const int nn = (L.nz + zc - 1) / zc;
-        const long waves = ((long)tiles * nn + 147) / 148;
-        const long cost = waves * (zc + 10);
-        if (best < 0 || cost < best) { best = cost; bn = nn; }
+    t2::T2Plan P;
+    P.tiles_x = (L.nx + t2::kTX - 1) / t2::kTX;
+    P.tiles = P.tiles_x * ((L.ny + t2::kTY - 1) / t2::kTY);
+    const int S = 148, maxchunk = L.nz >= 32 ? L.nz / 16 : 1;
+    // cost in marching steps of the slowest SM: rounds x (planes per chunk + the 6 redone planes + pipeline fill)
+    long best = -1;
+    P.nfull = 0; P.nsplit = 1;
+    for (int full = 0; full <= (P.tiles / S) * S; full += S) {          // whole waves of whole columns, then chunks
+        const int rem = P.tiles - full;
+        for (int n = 1; n <= maxchunk; ++n) {
+            const int zc = (L.nz + n - 1) / n, nn = (L.nz + zc - 1) / zc;
+            const long cost = (long)(full / S) * (L.nz + 10) + (((long)rem * nn + S - 1) / S) * (zc + 10);
+            if (best < 0 || cost < best) { best = cost; P.nfull = full; P.nsplit = rem > 0 ? nn : 1; }
+            if (rem == 0) break;
+        }
     }
-    if (zchunk_out) *zchunk_out = (L.nz + bn - 1) / bn;
-    return dim3(tiles_x, tiles_y, bn);
+    P.zchunk = (L.nz + P.nsplit - 1) / P.nsplit;
+    P.ncta = P.nfull + (P.tiles - P.nfull) * P.nsplit;
+    return P;
 }
 
 // Two fused sweeps: reads `in_is_phi2 ? phi2 : phi` through T (maps built for the 32 x 24 tile), writes phi_out.
@@ -385,15 +403,15 @@ static inline int launch_t2_sweep(const TmaLevelMaps& T, bool in_is_phi2, double
                                   double* part_max = nullptr, int max_parts = 0, int* nparts = nullptr)
 {
     using namespace t2;
-    int zchunk;
-    const dim3 grid = t2_sweep_grid(L, &zchunk);
+    const T2Plan plan = t2_plan(L);
+    const dim3 grid(plan.ncta, 1, 1);
     const CUtensorMap& tin = in_is_phi2 ? T.phi2 : T.phi;
     const size_t sm = Cfg<MAC_T2_LA>::kSmem;
     if (part_max) {
         if ((long)grid.x * grid.y * grid.z > max_parts) return -1;
         *nparts = (int)(grid.x * grid.y * grid.z);
-        k_rbgs_t2<MAC_T2_LA, true><<<grid, dim3(LN, TYE), sm, s>>>(tin, T.rhs, T.ax, T.ay, T.az, L, phi_out, zchunk, part_max);
+        k_rbgs_t2<MAC_T2_LA, true><<<grid, dim3(LN, TYE), sm, s>>>(tin, T.rhs, T.ax, T.ay, T.az, L, phi_out, plan, part_max);
     } else
-        k_rbgs_t2<MAC_T2_LA, false><<<grid, dim3(LN, TYE), sm, s>>>(tin, T.rhs, T.ax, T.ay, T.az, L, phi_out, zchunk, nullptr);
+        k_rbgs_t2<MAC_T2_LA, false><<<grid, dim3(LN, TYE), sm, s>>>(tin, T.rhs, T.ax, T.ay, T.az, L, phi_out, plan, nullptr);
     return cudaPeekAtLastError() == cudaSuccess ? 0 : -1;
 }

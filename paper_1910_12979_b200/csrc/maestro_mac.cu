@@ -576,8 +576,7 @@ bool fused_norm_ok(const maestro_mac_handle* H)
     const dim3 g = tma_sweep_grid(dev_level(H, 0), 0, nullptr);
     if ((long)g.x * g.y * g.z > kMaxParts) return false;
     if (t2_ok(H, 0)) {
-        const dim3 g2 = t2_sweep_grid(dev_level(H, 0), nullptr);
-        if ((long)g2.x * g2.y * g2.z > kMaxParts) return false;
+        if (t2_plan(dev_level(H, 0)).ncta > kMaxParts) return false;
     }
     return true;
 }
