@@ -41,7 +41,7 @@
 
 namespace t2 {
 
-using fused::Coef; using fused::pick; using fused::put;
+using fused::pick; using fused::put;
 using tma::mbar_init; using tma::mbar_expect_tx; using tma::mbar_wait; using tma::tma_load_3d; using tma::smem_u32;
 
 constexpr int LN = 16, TYE = 24, NT = LN * TYE;      // 16 pairs x 24 rows = 384 threads
@@ -69,6 +69,11 @@ template <bool X> __device__ __forceinline__ double ldc(const unsigned char* p, 
 {
     return *reinterpret_cast<const double*>(p + dy * kRow + dl * 16 + (X ? 0 : 8));
 }
+
+struct Coef {                                // coefficients of one plane for a column pair, in registers, and the
+    double2 ax; double ax2; double2 ays, ayn, az, rhs;   // reciprocals of the two diagonals, which sweep 1 computes
+    double2 rdg;                             // and sweep 2 reuses (same coefficients, two steps later)
+};
 
 struct Th {                                  // per-thread constants
     unsigned char* phi0;                     // own slot of phi stage 0
@@ -106,13 +111,28 @@ template <bool X> __device__ __forceinline__ Lat lat_ex(const unsigned char* pe)
 
 // Gauss-Seidel update of column X of the pair in one plane.  l: lateral neighbours, other: the pair's other cell,
 // C: the plane's coefficients, az_up: low z faces of the plane above, d_ / u_: vertical neighbours (u_ is on the
-// dependent chain, see fused::gs_value).
-template <bool X>
-__device__ __forceinline__ double gs_cell(const Lat& l, double other, const Coef& C, const double2& az_up,
+// dependent chain, see fused::gs_value, whose arithmetic this is).  FIRST: sweep 1 forms the reciprocal of the
+// diagonal (seed + 2 Newton steps) and leaves it in C.rdg; sweep 2 meets the same diagonal and reuses it.
+template <bool X, bool FIRST>
+__device__ __forceinline__ double gs_cell(const Lat& l, double other, Coef& C, const double2& az_up,
                                           double d_, double u_, double& a, double& dg)
 {
-    return fused::gs_value(X ? C.ax.x : C.ax.y, X ? C.ax.y : C.ax2, pick<X>(C.ays), pick<X>(C.ayn), pick<X>(C.az),
-                           pick<X>(az_up), pick<X>(C.rhs), X ? l.we : other, X ? other : l.we, l.s, l.n, d_, u_, a, dg);
+    const double axw = X ? C.ax.x : C.ax.y, axe = X ? C.ax.y : C.ax2;
+    const double ays = pick<X>(C.ays), ayn = pick<X>(C.ayn), azd = pick<X>(C.az), azu = pick<X>(az_up);
+    const double w_ = X ? l.we : other, e_ = X ? other : l.we;
+    const double t = (fma(axe, e_, axw * w_) + fma(ayn, l.n, ays * l.s)) + fma(azd, d_, -pick<X>(C.rhs));
+    a = fma(azu, u_, t);
+    double r;
+    if (FIRST) {
+        dg = ((axw + axe) + (ays + ayn)) + (azd + azu);
+        asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(dg));
+        r = fma(fma(-dg, r, 1.0), r, r);
+        r = fma(fma(-dg, r, 1.0), r, r);
+        put<X>(C.rdg, r);
+    } else {
+        r = pick<X>(C.rdg);
+    }
+    return a * r;
 }
 
 // issue the five box loads of plane p (unwrapped) into the phi stage at byte offset op / coefficient stage at oc
@@ -142,7 +162,7 @@ template <bool X, int W, bool NORM>
 __device__ __forceinline__ void step(const Th& T, int kk, const unsigned char* s0, const unsigned char* sP,
                                      const unsigned char* cI, const unsigned char* cP, double* __restrict__ out,
                                      double2& Pn, double2& Pm1, double2& Pm2, double2& Pm3, double2& Pm4, double2& azn,
-                                     Coef& CUR, const Coef& S1, const Coef& S2, const Coef& S3, double& vmax, bool& vnan)
+                                     Coef& CUR, Coef& S1, Coef& S2, Coef& S3, double& vmax, bool& vnan)
 {
     constexpr int R = 1 - W;
     const bool v0 = (unsigned)(kk - T.lo[0]) <= T.span[0], v1 = (unsigned)(kk - T.lo[1]) <= T.span[1];
@@ -162,7 +182,7 @@ __device__ __forceinline__ void step(const Th& T, int kk, const unsigned char* s
     const Lat l3 = lat_ex<X>(T.ex0 + (EX_RB + R) * kEx);              // sweep-2 red neighbours in plane kk-3
     double a, dg;
     // (1) sweep 1, red cells of plane kk
-    const double n0 = gs_cell<X>(l0, pick<!X>(P0), CUR, azn, pick<X>(Pm1), pick<X>(Pn), a, dg);
+    const double n0 = gs_cell<X, true>(l0, pick<!X>(P0), CUR, azn, pick<X>(Pm1), pick<X>(Pn), a, dg);
     if (NORM) {                                       // |rhs - (sum - phi_0 dg)| of the input; a NaN sets the sign of vmax
         const double rr = fabs(fma(pick<X>(P0), dg, -a));
         const bool on = T.own && (unsigned)(kk - T.nlo) <= T.nspan;
@@ -171,13 +191,13 @@ __device__ __forceinline__ void step(const Th& T, int kk, const unsigned char* s
     }
     put<X>(P0, ((X ? T.ra_x : T.ra_y) && v0) ? n0 : pick<X>(P0));
     // (2) sweep 1, black cells of plane kk-1
-    const double n1 = gs_cell<X>(l1, pick<!X>(Pm1), S1, CUR.az, pick<X>(Pm2), pick<X>(P0), a, dg);
+    const double n1 = gs_cell<X, true>(l1, pick<!X>(Pm1), S1, CUR.az, pick<X>(Pm2), pick<X>(P0), a, dg);
     put<X>(Pm1, (T.ba && v1) ? n1 : pick<X>(Pm1));
     // (3) sweep 2, red cells of plane kk-2
-    const double n2 = gs_cell<X>(l2, pick<!X>(Pm2), S2, S1.az, pick<X>(Pm3), pick<X>(Pm1), a, dg);
+    const double n2 = gs_cell<X, false>(l2, pick<!X>(Pm2), S2, S1.az, pick<X>(Pm3), pick<X>(Pm1), a, dg);
     put<X>(Pm2, ((X ? T.rb_x : T.rb_y) && v2) ? n2 : pick<X>(Pm2));
     // (4) sweep 2, black cells of plane kk-3; the plane is finished
-    const double n3 = gs_cell<X>(l3, pick<!X>(Pm3), S3, S2.az, pick<X>(Pm4), pick<X>(Pm2), a, dg);
+    const double n3 = gs_cell<X, false>(l3, pick<!X>(Pm3), S3, S2.az, pick<X>(Pm4), pick<X>(Pm2), a, dg);
     *reinterpret_cast<double*>(T.ex0 + (EX_RA + W) * kEx) = pick<X>(P0);
     *reinterpret_cast<double*>(T.ex0 + (EX_BA + W) * kEx) = pick<X>(Pm1);
     *reinterpret_cast<double*>(T.ex0 + (EX_RB + W) * kEx) = pick<X>(Pm2);
@@ -196,7 +216,7 @@ __device__ __forceinline__ void stage(const Th& T, int kk, int ke, unsigned par,
                                       const CUtensorMap* tm_az, unsigned phi_ring, unsigned coef_ring, unsigned bar0,
                                       bool producer, int cx, int cy, int nz, bool perz, double* __restrict__ out,
                                       double2& Pn, double2& Pm1, double2& Pm2, double2& Pm3, double2& Pm4, double2& azn,
-                                      Coef& CUR, const Coef& S1, const Coef& S2, const Coef& S3, double& vmax, bool& vnan)
+                                      Coef& CUR, Coef& S1, Coef& S2, Coef& S3, double& vmax, bool& vnan)
 {
     using G = Cfg<LA>;
     static_assert(G::NP == 4 && G::NC == 4 && LA == 2, "the unrolled march assumes 4 stages per ring");
@@ -223,7 +243,7 @@ __device__ __forceinline__ void march(const Th& T, int ks, int ke, const CUtenso
     const double2 z2 = make_double2(0.0, 0.0);
     double2 Pm1, Pm2 = z2, Pm3 = z2, Pm4 = z2;
     Coef cA, cB, cC, cD;
-    cB.ax = cB.ays = cB.ayn = cB.az = cB.rhs = z2; cB.ax2 = 0.0;
+    cB.ax = cB.ays = cB.ayn = cB.az = cB.rhs = cB.rdg = z2; cB.ax2 = 0.0;
     cC = cB; cD = cB;
     // the prologue issued planes ks-1 .. ks+LA into stages 0 .. LA+1 of both rings (phase 0 of their barriers)
     mbar_wait(bar0 + 0, 0);
