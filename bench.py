@@ -237,7 +237,7 @@ def run_ours(a):
 
     wl = W.by_name(a.config, a.n)                     # seeded, synthetic; identical on every rank (replicas)
     nu = wl.nu_pre + wl.nu_post
-    P = mac.MacProjector(mac.desc_from_workload(wl, smoother=a.smoother, host_staging=0 if a.no_e2e else 1), device=dev)
+    P = mac.MacProjector(mac.desc_from_workload(wl, smoother=a.smoother, host_staging=0 if a.no_e2e else 1, timing=1), device=dev)
     dv = mac.to_device(wl, dev)
     pristine = [dv[k].clone() for k in ("u", "v", "w")]
     phi = torch.empty(wl.rho.shape, dtype=torch.float64, device=dev)

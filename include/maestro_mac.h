@@ -69,13 +69,17 @@ typedef struct {
     int nr;                   /* base-state samples */
     double dr;                /* sample spacing; samples at (m + 1/2) dr */
     double center[3];         /* spherical only */
-    int nu_pre, nu_post;      /* RBGS sweeps per level, default 2, 2 (0 = default) */
-    int max_cycles;           /* default 100 (0 = default), at most 128 are recorded in stats */
-    double rel_tol;           /* on ||r||inf / ||rhs||inf ; < 0 = default 1e-10 ; 0 = run exactly
-                                 max_cycles cycles without a stop test */
-    int coarsest_n;           /* default 4 (0 = default) */
-    int bottom_max_iter;      /* BiCGStab iterations, default 100 (0 = default) */
-    double bottom_rel_tol;    /* on ||r||2 / ||f||2, default 1e-8 (<= 0 = default) */
+    /* Defaulting rules.  maestro_mac_default_desc() fills every member with its default; a caller that builds
+       the struct by hand gets the default of a member by writing the stand-in value named below.  Values are
+       otherwise taken literally; anything else out of range is ERR_ARG. */
+    int nu_pre, nu_post;      /* RBGS sweeps per level before / after the coarse correction, default 2, 2;
+                                 either may be 0, both 0 is ERR_ARG (a V-cycle without smoothing) */
+    int max_cycles;           /* default 100 (0 stands for the default); at most 128 are recorded in stats */
+    double rel_tol;           /* on ||r||inf / ||rhs||inf ; < 0 stands for the default 1e-10 ; 0 = run exactly
+                                 max_cycles cycles without a stop test (with max_cycles = 0 that is 100 cycles) */
+    int coarsest_n;           /* default 4 (0 stands for the default) */
+    int bottom_max_iter;      /* BiCGStab iterations, default 100 (0 stands for the default) */
+    double bottom_rel_tol;    /* on ||r||2 / ||f||2, default 1e-8 (<= 0 stands for the default) */
     int prolongation;         /* 0 = cell-centred trilinear (default), 1 = piecewise constant */
     int host_staging;         /* 1 = reserve device staging in the workspace so that
                                  maestro_mac_project_host() can be used */
@@ -99,6 +103,9 @@ typedef struct {
     int rho_mean;             /* density on a face from the two cells it separates, in the coefficient
                                  beta0/rho_face and in the correction (1/rho_face) G phi alike:
                                  0 = arithmetic mean of rho (default), 1 = harmonic (mean of 1/rho). */
+    int timing;               /* 1 = bracket every level-0 smoother launch with a CUDA event pair on the call's
+                                 stream (stats.ms_smooth0 ...; bench.py's roofline); 0 (default) = no per-launch
+                                 events on the hot path */
 } maestro_mac_desc;
 
 typedef struct {
@@ -111,8 +118,8 @@ typedef struct {
     float ms_vcycles;         /* all cycles including the stop tests */
     float ms_correct;         /* mean shift, velocity correction, phi copy-out */
     int gpu_launches;         /* kernels launched by this call */
-    float ms_smooth0;         /* summed device time of the level-0 smoother launches that were timed
-                                 (one CUDA event pair per launch, on the call's stream) */
+    float ms_smooth0;         /* desc.timing = 1: summed device time of the level-0 smoother launches that were
+                                 timed (one CUDA event pair per launch, on the call's stream); else 0 */
     int smooth0_launches;     /* level-0 smoother launches of this call */
     int smooth0_timed;        /* how many of them ms_smooth0 covers (at most 512) */
     int smooth0_sweeps_timed; /* sweeps those launches applied (a two-sweep launch counts 2) */
@@ -148,13 +155,29 @@ int maestro_mac_setup(const maestro_mac_desc *desc, void *workspace, size_t work
  *   phi          device [nx*ny*nz], out, or NULL.
  *   stats        HOST, out, or NULL.
  * u, v, w, phi, rho, S must not overlap each other or the workspace.  One in-flight call per
- * handle.  The call synchronises the stream (it reads the stop test after every cycle) unless
- * rel_tol == 0.  rhs == 0 returns OK with cycles = 0, phi = 0 and the velocities untouched.
+ * handle.
+ * SYNCHRONISATION.  With rel_tol > 0, or with stats != NULL, the call synchronises the stream: once after
+ * the assembly pass (it reads ||rhs||inf and the non-finite flags), after every cycle when rel_tol > 0
+ * (the stop test), and at the end.  rhs == 0 then returns OK with cycles = 0, phi = 0 and the velocities
+ * untouched.  With rel_tol == 0 AND stats == NULL the call is ASYNCHRONOUS: it enqueues the assembly,
+ * exactly max_cycles cycles and the correction on the stream and returns OK without synchronising; a
+ * zero rhs runs its cycles on zeros (phi = 0, velocities unchanged bit for bit), and non-finite input is
+ * not detected by the call itself -- maestro_mac_status() reports it.
  * Returns OK, NOT_CONVERGED, ERR_ARG, ERR_CUDA or ERR_NONFINITE.
  */
 int maestro_mac_project(maestro_mac_handle *h, const double *beta0, const double *rho0,
                         const double *rho, double *u, double *v, double *w, const double *S,
                         double *phi, maestro_mac_stats *stats, void *cuda_stream);
+
+/*
+ * maestro_mac_status: completes an asynchronous maestro_mac_project() call (rel_tol == 0, stats == NULL):
+ * synchronises `cuda_stream` (the stream of that call), returns ERR_NONFINITE if the assembly pass flagged
+ * a non-finite rhs or a rho <= 0 (the outputs are then garbage), else OK, and fills *stats (HOST, may be
+ * NULL) as the synchronous call would have (with stats != NULL it launches one residual-norm pass for
+ * res_norm_inf).  After a synchronous call it returns OK and the stats of that call without touching the
+ * stream.  Returns OK, ERR_ARG, ERR_CUDA or ERR_NONFINITE.
+ */
+int maestro_mac_status(maestro_mac_handle *h, maestro_mac_stats *stats, void *cuda_stream);
 
 /*
  * maestro_mac_project_host: the same call with HOST buffers (pinned memory recommended): copies
@@ -209,6 +232,13 @@ enum { MAESTRO_MAC_ARR_PHI = 0, MAESTRO_MAC_ARR_RHS = 1, MAESTRO_MAC_ARR_BX = 2,
        MAESTRO_MAC_ARR_BY = 3, MAESTRO_MAC_ARR_BZ = 4 };
 
 int maestro_mac_num_levels(const maestro_mac_handle *h);
+/* Launch plan of the smoother on a level (host only; for tests that must know which decomposition they hit):
+ *   info[0] kernel (enum below), info[1] lateral tiles, info[2] tiles that march the whole z column (two-sweep
+ *   kernel: the whole waves), info[3] z-chunks per remaining tile, info[4] planes per chunk, info[5] CTAs of one
+ *   launch, info[6], info[7] periodic image columns / rows per side of the level's arrays. */
+enum { MAESTRO_MAC_KERNEL_COLOR = 0, MAESTRO_MAC_KERNEL_FUSED = 1, MAESTRO_MAC_KERNEL_TMA = 2,
+       MAESTRO_MAC_KERNEL_T2 = 3, MAESTRO_MAC_KERNEL_TAIL = 4, MAESTRO_MAC_KERNEL_BOTTOM = 5 };
+int maestro_mac_level_plan(const maestro_mac_handle *h, int level, int info[8]);
 /* n[3] cells and h[3] spacing of a level */
 int maestro_mac_level_dims(const maestro_mac_handle *h, int level, int n[3], double hh[3]);
 /* Copy a level array to / from a caller DEVICE buffer in the public layout (cells, or the face

@@ -325,7 +325,7 @@ static inline int smoother_configure()
 }
 
 // One fused sweep: reads phi_in, writes phi_out (distinct buffers).
-static inline int launch_fused_sweep(const double* phi_in, double* phi_out, const LevelDev& L, cudaStream_t s)
+static inline int launch_fused_sweep(const double* phi_in, double* phi_out, const LevelDev& L, int sms, cudaStream_t s)
 {
     using namespace fused;
     constexpr int LN = 16, kTX = 2 * LN - 4;
@@ -336,7 +336,7 @@ static inline int launch_fused_sweep(const double* phi_in, double* phi_out, cons
     // enough z-chunks for a few CTAs per SM, but chunks of at least 16 planes (each chunk recomputes
     // 2 red planes and restages 4)
     const int tiles = tiles_x * tiles_y;
-    int nchunk = (8 * 148 + tiles - 1) / tiles;
+    int nchunk = (8 * sms + tiles - 1) / tiles;
     int maxchunk = (L.nz + 15) / 16;
     if (nchunk > maxchunk) nchunk = maxchunk;
     if (nchunk < 1) nchunk = 1;

@@ -394,12 +394,12 @@ static inline bool t2_level_ok(const LevelDev& L)
     return true;
 }
 
-static inline t2::T2Plan t2_plan(const LevelDev& L)
+static inline t2::T2Plan t2_plan(const LevelDev& L, int sms)
 {
     t2::T2Plan P;
     P.tiles_x = (L.nx + t2::kTX - 1) / t2::kTX;
     P.tiles = P.tiles_x * ((L.ny + t2::kTY - 1) / t2::kTY);
-    const int S = 148, maxchunk = L.nz >= 32 ? L.nz / 16 : 1;
+    const int S = sms, maxchunk = L.nz >= 32 ? L.nz / 16 : 1;
     // cost in marching steps of the slowest SM: rounds x (planes per chunk + the 6 redone planes + pipeline fill)
     long best = -1;
     P.nfull = 0; P.nsplit = 1;
@@ -419,11 +419,11 @@ static inline t2::T2Plan t2_plan(const LevelDev& L)
 
 // Two fused sweeps: reads `in_is_phi2 ? phi2 : phi` through T (maps built for the 32 x 24 tile), writes phi_out.
 // part_max != NULL: also per-CTA maxima of the input's red-cell residual; *nparts receives their count.
-static inline int launch_t2_sweep(const TmaLevelMaps& T, bool in_is_phi2, double* phi_out, const LevelDev& L, cudaStream_t s,
+static inline int launch_t2_sweep(const TmaLevelMaps& T, bool in_is_phi2, double* phi_out, const LevelDev& L, int sms, cudaStream_t s,
                                   double* part_max = nullptr, int max_parts = 0, int* nparts = nullptr)
 {
     using namespace t2;
-    const T2Plan plan = t2_plan(L);
+    const T2Plan plan = t2_plan(L, sms);
     const dim3 grid(plan.ncta, 1, 1);
     const CUtensorMap& tin = in_is_phi2 ? T.phi2 : T.phi;
     const size_t sm = Cfg<MAC_T2_LA>::kSmem;

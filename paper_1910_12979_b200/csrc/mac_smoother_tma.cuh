@@ -310,13 +310,13 @@ static inline void tma_pick_chunks(int tiles, int nz, int slots, int* nchunk_out
 }
 
 // grid of one TMA sweep of level L (variant 0: 64x16 tile, 1: 32x16 tile)
-static inline dim3 tma_sweep_grid(const LevelDev& L, int variant, int* zchunk_out)
+static inline dim3 tma_sweep_grid(const LevelDev& L, int variant, int sms, int* zchunk_out)
 {
     const int LN = variant == 0 ? 32 : 16;
     const int kTX = 2 * LN - 4, TY = 12;
     const int tiles_x = (L.nx + kTX - 1) / kTX, tiles_y = (L.ny + TY - 1) / TY;
     int nchunk, zchunk;
-    tma_pick_chunks(tiles_x * tiles_y, L.nz, variant == 0 ? 148 : 296, &nchunk, &zchunk);
+    tma_pick_chunks(tiles_x * tiles_y, L.nz, variant == 0 ? sms : 2 * sms, &nchunk, &zchunk);
     if (zchunk_out) *zchunk_out = zchunk;
     return dim3(tiles_x, tiles_y, nchunk);
 }
@@ -325,11 +325,11 @@ static inline dim3 tma_sweep_grid(const LevelDev& L, int variant, int* zchunk_ou
 // part_max != NULL (variant 0 only): also write per-CTA maxima of the input's red-cell residual; *nparts
 // receives their count.
 static inline int launch_tma_sweep(const TmaLevelMaps& T, bool in_is_phi2, double* phi_out, const LevelDev& L, int variant,
-                                   cudaStream_t s, double* part_max = nullptr, int max_parts = 0, int* nparts = nullptr)
+                                   int sms, cudaStream_t s, double* part_max = nullptr, int max_parts = 0, int* nparts = nullptr)
 {
     using namespace tma;
     int zchunk;
-    const dim3 grid = tma_sweep_grid(L, variant, &zchunk);
+    const dim3 grid = tma_sweep_grid(L, variant, sms, &zchunk);
     const CUtensorMap& tin = in_is_phi2 ? T.phi2 : T.phi;
     if (part_max) {
         if (variant != 0 || (long)grid.x * grid.y * grid.z > max_parts) return -1;
@@ -489,12 +489,12 @@ static inline int tma_resid_configure()
 
 // mode: tma::RES_RESTRICT and/or tma::RES_NORM.  Returns the number of CTAs (= partial maxima written), or -1.
 static inline int launch_tma_resid(const TmaLevelMaps& T, bool in_is_phi2, const LevelDev& L, const LevelDev& Cc,
-                                   double* part_max, int max_parts, int mode, cudaStream_t s)
+                                   double* part_max, int max_parts, int mode, int sms, cudaStream_t s)
 {
     using namespace tma;
     const int tiles_x = (L.nx + 59) / 60, tiles_y = (L.ny + 13) / 14;
     int nchunk, zchunk;
-    tma_pick_chunks(tiles_x * tiles_y, L.nz, 148, &nchunk, &zchunk);
+    tma_pick_chunks(tiles_x * tiles_y, L.nz, sms, &nchunk, &zchunk);
     zchunk = (zchunk + 1) & ~1;                               // chunks start on even planes (coarse cells are not split)
     nchunk = (L.nz + zchunk - 1) / zchunk;
     while ((long)tiles_x * tiles_y * nchunk > max_parts && nchunk > 1) {

@@ -24,7 +24,7 @@
 namespace {
 
 constexpr int kMaxLevels = 32;
-constexpr int kRedBlocks = 148 * 8;       // blocks of the row-walking reduction kernels
+constexpr int kRedBlocksPerSm = 8;        // blocks per SM of the row-walking reduction kernels
 constexpr int kMaxParts = 131072;         // capacity of the partial-reduction arrays
 constexpr int kBottomMax = 4096;          // largest coarsest level (unknowns)
 constexpr size_t kBottomSmem = 200 * 1024; // bottom-solver vectors live in shared memory up to this size
@@ -60,7 +60,7 @@ struct maestro_mac_handle {
     size_t tail_smem;
     TailArgs tail;                 // prepared by plan_tail; level pointers are filled in at launch
     // scratch carved from the workspace
-    double *part_sum, *part_max;   // kRedBlocks each
+    double *part_sum, *part_max;   // kMaxParts each
     double *scal;                  // device scalars: [0] sum, [1] max (k_reduce_final output) ...
     double *bottom_vecs;           // 6 * bottom unknowns
     int *flags;                    // [0] bad rho, [1] bottom iterations
@@ -71,6 +71,10 @@ struct maestro_mac_handle {
     int *host_flags;               // pinned, 4 ints
     cudaEvent_t ev[4];
     int launches;
+    int sms;                       // multiprocessors of the device (cudaDevAttrMultiProcessorCount at setup)
+    int red_blocks;                // kRedBlocksPerSm * sms
+    int deferred;                  // the last project call returned without synchronising (maestro_mac_status reports it)
+    maestro_mac_stats last;        // stats of the last project call as far as the host knows them
     // level-0 smoother timing: one event pair per launch, summed after the final synchronise
     cudaEvent_t* sm_ev;            // 2 * kSmoothEvents events, or NULL
     int sm_used;                   // pairs recorded by the current call
@@ -99,7 +103,7 @@ int validate_and_default(const maestro_mac_desc* in, maestro_mac_desc* d)
     if (d->nr <= 0 || !(d->dr > 0.0) || !std::isfinite(d->dr)) return MAESTRO_MAC_ERR_ARG;
     if (d->nu_pre < 0 || d->nu_post < 0 || d->max_cycles < 0 || d->coarsest_n < 0 || d->bottom_max_iter < 0)
         return MAESTRO_MAC_ERR_ARG;
-    if (d->nu_pre == 0 && d->nu_post == 0) { d->nu_pre = 2; d->nu_post = 2; }
+    if (d->nu_pre == 0 && d->nu_post == 0) return MAESTRO_MAC_ERR_ARG;   // a V-cycle without smoothing (the defaults come from maestro_mac_default_desc)
     if (d->max_cycles == 0) d->max_cycles = 100;
     if (d->rel_tol < 0.0) d->rel_tol = 1e-10;
     if (!std::isfinite(d->rel_tol)) return MAESTRO_MAC_ERR_ARG;
@@ -111,6 +115,7 @@ int validate_and_default(const maestro_mac_desc* in, maestro_mac_desc* d)
     if (d->smoother < 0 || d->smoother > 4) return MAESTRO_MAC_ERR_ARG;   // 4: one sweep per pass everywhere
     if (d->stop_test != 0 && d->stop_test != 1) return MAESTRO_MAC_ERR_ARG;
     if (d->rho_mean != 0 && d->rho_mean != 1) return MAESTRO_MAC_ERR_ARG;
+    if (d->timing != 0 && d->timing != 1) return MAESTRO_MAC_ERR_ARG;
     return MAESTRO_MAC_OK;
 }
 
@@ -141,7 +146,10 @@ int build_levels(const maestro_mac_desc& d, Level* lev, int* nlev)
     int l = 0;
     for (;;) {
         // levels that run the TMA-staged kernels carry periodic image columns / rows (TMA cannot wrap)
-        const bool tma_level = (d.smoother == 0 || d.smoother == 3 || d.smoother == 4) && n[0] >= 60 && (n[0] & 1) == 0 && n[1] >= 4;
+        // (a periodic axis must hold both image strips apart: n >= 2 x ghost width, else the level keeps the plain layout)
+        const int gw = d.smoother == 0 ? t2::HALO : 2;
+        const bool per_ok = (d.bc_lo[0] != MAESTRO_MAC_PERIODIC || n[0] >= 2 * gw) && (d.bc_lo[1] != MAESTRO_MAC_PERIODIC || n[1] >= 2 * gw);
+        const bool tma_level = (d.smoother == 0 || d.smoother == 3 || d.smoother == 4) && n[0] >= 60 && (n[0] & 1) == 0 && n[1] >= 4 && per_ok;
         bool can = l + 1 < kMaxLevels;
         for (int a = 0; a < 3; ++a)
             if ((n[a] & 1) || n[a] / 2 < d.coarsest_n) can = false;
@@ -244,7 +252,7 @@ void dims3(int ex, int ey, int ez, dim3* grid, dim3* block)
 #define CUDA_OK(call) do { if ((call) != cudaSuccess) return MAESTRO_MAC_ERR_CUDA; } while (0)
 #define LAUNCHED(H) do { ++(H)->launches; if (cudaPeekAtLastError() != cudaSuccess) return MAESTRO_MAC_ERR_CUDA; } while (0)
 
-int red_blocks(int rows) { return rows < kRedBlocks ? rows : kRedBlocks; }
+int red_blocks(const maestro_mac_handle* H, int rows) { return rows < H->red_blocks ? rows : H->red_blocks; }
 
 enum { GH_PHI = 1, GH_RHS = 2, GH_AX = 4, GH_AY = 8, GH_AZ = 16 };
 
@@ -334,7 +342,7 @@ int do_rhs(maestro_mac_handle* H, const double* beta0, const double* u, const do
                                                                    nullptr, zc, H->flags, H->part_sum, H->part_max);
     } else {
         int rows = G.ny * G.nz;
-        nb = red_blocks(rows);
+        nb = red_blocks(H, rows);
         int bt = G.nx >= 256 ? 256 : (G.nx >= 128 ? 128 : 64);
         k_rhs<<<nb, bt, 0, s>>>(G, dev_level(H, 0), beta0, u, v, w, S, H->dpdt_term, H->part_sum, H->part_max);
     }
@@ -370,9 +378,9 @@ int do_rhs_finish(maestro_mac_handle* H, int nb, cudaStream_t s)
     LAUNCHED(H);
     if (H->singular) {
         CUDA_OK(cudaMemcpyAsync(H->scal + 2, H->scal, sizeof(double), cudaMemcpyDeviceToDevice, s));
-        k_shift_mean<<<kRedBlocks, 256, 0, s>>>(dev_level(H, 0), L0.rhs, H->scal + 2, 1.0 / (double)L0.ncell, H->part_sum, H->part_max);
+        k_shift_mean<<<H->red_blocks, 256, 0, s>>>(dev_level(H, 0), L0.rhs, H->scal + 2, 1.0 / (double)L0.ncell, H->part_sum, H->part_max);
         LAUNCHED(H);
-        k_reduce_final<<<1, 1024, 0, s>>>(H->part_sum, H->part_max, kRedBlocks, H->scal);
+        k_reduce_final<<<1, 1024, 0, s>>>(H->part_sum, H->part_max, H->red_blocks, H->scal);
         LAUNCHED(H);
     } else {
         CUDA_OK(cudaMemsetAsync(H->scal + 2, 0, sizeof(double), s));
@@ -392,7 +400,7 @@ int do_sweep(maestro_mac_handle* H, int l, cudaStream_t s, int* norm_parts = nul
     const int sm = H->d.smoother;
     const int tv = ((sm == 0 || sm == 4) && L.nx >= 60) ? 0 : (sm == 3 ? 1 : -1);   // TMA tile variant, or -1
     if (tv >= 0 && H->lev[l].tma[tv].ok) {
-        int rc = launch_tma_sweep(H->lev[l].tma[tv], H->lev[l].phi != H->lev[l].phi_a, H->lev[l].phi2, L, tv, s,
+        int rc = launch_tma_sweep(H->lev[l].tma[tv], H->lev[l].phi != H->lev[l].phi_a, H->lev[l].phi2, L, tv, H->sms, s,
                                   norm_parts ? H->part_max : nullptr, kMaxParts, norm_parts);
         if (rc != 0) return MAESTRO_MAC_ERR_CUDA;
         ++H->launches;
@@ -400,7 +408,7 @@ int do_sweep(maestro_mac_handle* H, int l, cudaStream_t s, int* norm_parts = nul
     } else if (norm_parts) {
         return MAESTRO_MAC_ERR_ARG;                                           // callers check fused_norm_ok first
     } else if (sm != 1 && fused_sweep_supported(L)) {
-        int rc = launch_fused_sweep(H->lev[l].phi, H->lev[l].phi2, L, s);
+        int rc = launch_fused_sweep(H->lev[l].phi, H->lev[l].phi2, L, H->sms, s);
         if (rc != 0) return MAESTRO_MAC_ERR_CUDA;
         ++H->launches;
         // the fused sweep ping-pongs: result is in phi2; swap the level's buffers
@@ -430,7 +438,7 @@ int do_sweep2(maestro_mac_handle* H, int l, cudaStream_t s, int* norm_parts = nu
     const bool timed = l == 0 && H->sm_ev && H->sm_used < kSmoothEvents;
     if (l == 0) ++H->sm_launches;
     if (timed) CUDA_OK(cudaEventRecord(H->sm_ev[2 * H->sm_used], s));
-    if (launch_t2_sweep(Lv.tma[2], Lv.phi != Lv.phi_a, Lv.phi2, dev_level(H, l), s, norm_parts ? H->part_max : nullptr,
+    if (launch_t2_sweep(Lv.tma[2], Lv.phi != Lv.phi_a, Lv.phi2, dev_level(H, l), H->sms, s, norm_parts ? H->part_max : nullptr,
                         kMaxParts, norm_parts) != 0)
         return MAESTRO_MAC_ERR_CUDA;
     ++H->launches;
@@ -464,7 +472,7 @@ int do_residual_restrict(maestro_mac_handle* H, int l, cudaStream_t s)
     if (tma_aux(H, l)) {
         Level& F = H->lev[l];
         int n = launch_tma_resid(F.tma[0], F.phi != F.phi_a, dev_level(H, l), dev_level(H, l + 1),
-                                 H->part_max, kMaxParts, tma::RES_RESTRICT, s);
+                                 H->part_max, kMaxParts, tma::RES_RESTRICT, H->sms, s);
         if (n < 0) return MAESTRO_MAC_ERR_CUDA;
         ++H->launches;
         return MAESTRO_MAC_OK;
@@ -573,10 +581,10 @@ bool fused_norm_ok(const maestro_mac_handle* H)
     const Level& L0 = H->lev[0];
     if (H->d.stop_test != 0 || (H->d.smoother != 0 && H->d.smoother != 4) || H->nlev < 2 || H->d.nu_pre < 1 || H->d.nu_post < 1) return false;
     if (!L0.tma[0].ok || L0.n[0] < 60) return false;
-    const dim3 g = tma_sweep_grid(dev_level(H, 0), 0, nullptr);
+    const dim3 g = tma_sweep_grid(dev_level(H, 0), 0, H->sms, nullptr);
     if ((long)g.x * g.y * g.z > kMaxParts) return false;
     if (t2_ok(H, 0)) {
-        if (t2_plan(dev_level(H, 0)).ncta > kMaxParts) return false;
+        if (t2_plan(dev_level(H, 0), H->sms).ncta > kMaxParts) return false;
     }
     return true;
 }
@@ -607,7 +615,7 @@ int do_residual_norm(maestro_mac_handle* H, int l, cudaStream_t s)
     LevelDev L = dev_level(H, l);
     if (tma_aux(H, l)) {
         Level& F = H->lev[l];
-        int n = launch_tma_resid(F.tma[0], F.phi != F.phi_a, L, L, H->part_max, kMaxParts, tma::RES_NORM, s);
+        int n = launch_tma_resid(F.tma[0], F.phi != F.phi_a, L, L, H->part_max, kMaxParts, tma::RES_NORM, H->sms, s);
         if (n < 0) return MAESTRO_MAC_ERR_CUDA;
         ++H->launches;
         k_reduce_final<<<1, 1024, 0, s>>>(H->part_sum, H->part_max, n, H->scal + 3);
@@ -615,7 +623,7 @@ int do_residual_norm(maestro_mac_handle* H, int l, cudaStream_t s)
         return MAESTRO_MAC_OK;
     }
     int rows = L.ny * L.nz;
-    int nb = red_blocks(rows);
+    int nb = red_blocks(H, rows);
     int bt = L.nx >= 256 ? 256 : (L.nx >= 128 ? 128 : 64);
     k_residual_norm<<<nb, bt, 0, s>>>(L, H->part_sum, H->part_max);
     LAUNCHED(H);
@@ -697,7 +705,15 @@ extern "C" int maestro_mac_setup(const maestro_mac_desc* desc, void* workspace, 
     for (int e = 0; ok && e < 4; ++e) ok = cudaEventCreate(&H->ev[e]) == cudaSuccess;
     H->sm_ev = nullptr;
     H->sm_used = H->sm_launches = H->sm_sweeps = 0;
-    if (ok) {
+    {
+        int dev = 0, sms = 0;
+        ok = ok && cudaGetDevice(&dev) == cudaSuccess && cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && sms > 0;
+        H->sms = ok ? sms : 1;
+        H->red_blocks = kRedBlocksPerSm * H->sms;
+        if (H->red_blocks > kMaxParts) H->red_blocks = kMaxParts;
+    }
+    H->deferred = 0;
+    if (ok && H->d.timing) {                         // per-launch event pairs of the level-0 smoother: only on request
         H->sm_ev = (cudaEvent_t*)std::calloc(2 * kSmoothEvents, sizeof(cudaEvent_t));
         ok = H->sm_ev != nullptr;
         for (int e = 0; ok && e < 2 * kSmoothEvents; ++e) ok = cudaEventCreate(&H->sm_ev[e]) == cudaSuccess;
@@ -739,6 +755,25 @@ extern "C" int maestro_mac_free(maestro_mac_handle* H)
     return MAESTRO_MAC_OK;
 }
 
+// Fills the timing members of st after the stream has been synchronised.
+static void collect_timings(maestro_mac_handle* H, maestro_mac_stats& st)
+{
+    st.bottom_iters_total = H->host_flags[1];
+    cudaEventElapsedTime(&st.ms_setup_kernels, H->ev[0], H->ev[1]);
+    cudaEventElapsedTime(&st.ms_vcycles, H->ev[1], H->ev[2]);
+    cudaEventElapsedTime(&st.ms_correct, H->ev[2], H->ev[3]);
+    st.smooth0_launches = H->sm_launches;
+    st.smooth0_timed = H->sm_used;
+    st.smooth0_sweeps_timed = H->sm_sweeps;
+    double acc = 0.0;
+    for (int q = 0; q < H->sm_used; ++q) {
+        float ms = 0.0f;
+        cudaEventElapsedTime(&ms, H->sm_ev[2 * q], H->sm_ev[2 * q + 1]);
+        acc += ms;
+    }
+    st.ms_smooth0 = (float)acc;
+}
+
 extern "C" int maestro_mac_project(maestro_mac_handle* H, const double* beta0, const double* rho0,
                                    const double* rho, double* u, double* v, double* w, const double* S,
                                    double* phi, maestro_mac_stats* stats, void* cuda_stream)
@@ -755,9 +790,13 @@ extern "C" int maestro_mac_project(maestro_mac_handle* H, const double* beta0, c
     st.levels = H->nlev;
     H->launches = 0;
     H->sm_used = H->sm_launches = H->sm_sweeps = 0;
+    H->deferred = 0;
     int rc;
     int result = MAESTRO_MAC_OK;
     Level& L0 = H->lev[0];
+    // rel_tol == 0 without stats: nothing the host must read.  The call enqueues everything and returns; the
+    // non-finite check is deferred to maestro_mac_status() and a zero rhs simply runs its (trivial) cycles.
+    const bool async = d.rel_tol == 0.0 && !stats;
 
     CUDA_OK(cudaEventRecord(H->ev[0], s));
     if (rho && d.smoother != 1) {
@@ -770,15 +809,18 @@ extern "C" int maestro_mac_project(maestro_mac_handle* H, const double* beta0, c
     CUDA_OK(cudaMemcpyAsync(H->host_flags, H->flags, sizeof(int), cudaMemcpyDeviceToHost, s));
     CUDA_OK(cudaMemsetAsync(L0.phi - L0.off_c, 0, L0.acell * sizeof(double), s));   // A16: phi = 0 (ghosts too)
     CUDA_OK(cudaEventRecord(H->ev[1], s));
-    CUDA_OK(cudaStreamSynchronize(s));
-    st.rhs_norm_inf = H->host_scal[1];
-    st.rhs_mean_removed = H->singular ? H->host_scal[2] / (double)L0.ncell : 0.0;
-    const bool bad = H->host_flags[0] != 0 || !std::isfinite(st.rhs_norm_inf) || !std::isfinite(H->host_scal[0]);
-    if (bad) {
-        if (stats) *stats = st;
-        return MAESTRO_MAC_ERR_NONFINITE;
+    bool trivial = false;
+    if (!async) {
+        CUDA_OK(cudaStreamSynchronize(s));
+        st.rhs_norm_inf = H->host_scal[1];
+        st.rhs_mean_removed = H->singular ? H->host_scal[2] / (double)L0.ncell : 0.0;
+        const bool bad = H->host_flags[0] != 0 || !std::isfinite(st.rhs_norm_inf) || !std::isfinite(H->host_scal[0]);
+        if (bad) {
+            if (stats) *stats = st;
+            return MAESTRO_MAC_ERR_NONFINITE;
+        }
+        trivial = st.rhs_norm_inf == 0.0;
     }
-    const bool trivial = st.rhs_norm_inf == 0.0;
     if (!trivial) {
         result = d.rel_tol > 0.0 ? MAESTRO_MAC_NOT_CONVERGED : MAESTRO_MAC_OK;
         if (d.rel_tol > 0.0) {
@@ -816,11 +858,11 @@ extern "C" int maestro_mac_project(maestro_mac_handle* H, const double* beta0, c
     CUDA_OK(cudaEventRecord(H->ev[2], s));
     if (!trivial && result != MAESTRO_MAC_ERR_NONFINITE) {
         if (H->singular) {   // A10: zero-mean phi
-            k_sum<<<kRedBlocks, 256, 0, s>>>(dev_level(H, 0), H->lev[0].phi, H->part_sum, H->part_max);
+            k_sum<<<H->red_blocks, 256, 0, s>>>(dev_level(H, 0), H->lev[0].phi, H->part_sum, H->part_max);
             LAUNCHED(H);
-            k_reduce_final<<<1, 1024, 0, s>>>(H->part_sum, H->part_max, kRedBlocks, H->scal + 6);
+            k_reduce_final<<<1, 1024, 0, s>>>(H->part_sum, H->part_max, H->red_blocks, H->scal + 6);
             LAUNCHED(H);
-            k_shift_mean<<<kRedBlocks, 256, 0, s>>>(dev_level(H, 0), H->lev[0].phi, H->scal + 6, 1.0 / (double)L0.ncell, H->part_sum, H->part_max);
+            k_shift_mean<<<H->red_blocks, 256, 0, s>>>(dev_level(H, 0), H->lev[0].phi, H->scal + 6, 1.0 / (double)L0.ncell, H->part_sum, H->part_max);
             LAUNCHED(H);
         }
         if ((rc = do_correct(H, H->lev[0].phi, rho0, rho, u, v, w, s)) != 0) return rc;
@@ -836,31 +878,52 @@ extern "C" int maestro_mac_project(maestro_mac_handle* H, const double* beta0, c
         }
     }
     CUDA_OK(cudaEventRecord(H->ev[3], s));
-    if (stats || d.rel_tol > 0.0) {
-        CUDA_OK(cudaMemcpyAsync(H->host_flags + 1, H->flags + 1, sizeof(int), cudaMemcpyDeviceToHost, s));
-        CUDA_OK(cudaStreamSynchronize(s));
-        st.bottom_iters_total = H->host_flags[1];
-        cudaEventElapsedTime(&st.ms_setup_kernels, H->ev[0], H->ev[1]);
-        cudaEventElapsedTime(&st.ms_vcycles, H->ev[1], H->ev[2]);
-        cudaEventElapsedTime(&st.ms_correct, H->ev[2], H->ev[3]);
-        st.smooth0_launches = H->sm_launches;
-        st.smooth0_timed = H->sm_used;
-        st.smooth0_sweeps_timed = H->sm_sweeps;
-        double acc = 0.0;
-        for (int q = 0; q < H->sm_used; ++q) {
-            float ms = 0.0f;
-            cudaEventElapsedTime(&ms, H->sm_ev[2 * q], H->sm_ev[2 * q + 1]);
-            acc += ms;
-        }
-        st.ms_smooth0 = (float)acc;
-        if (d.rel_tol == 0.0 && !trivial) {   // fixed-cycle run: report the final residual too
-            if ((rc = do_residual_norm(H, 0, s)) != 0) return rc;
-            CUDA_OK(cudaMemcpyAsync(H->host_scal + 4, H->scal + 4, sizeof(double), cudaMemcpyDeviceToHost, s));
-            CUDA_OK(cudaStreamSynchronize(s));
-            st.res_norm_inf = H->host_scal[4];
-        }
-    }
+    CUDA_OK(cudaMemcpyAsync(H->host_flags + 1, H->flags + 1, sizeof(int), cudaMemcpyDeviceToHost, s));
     st.gpu_launches = H->launches;
+    if (async) {                                   // nothing was read back: maestro_mac_status() completes the picture
+        H->deferred = 1;
+        H->last = st;
+        return MAESTRO_MAC_OK;
+    }
+    CUDA_OK(cudaStreamSynchronize(s));
+    collect_timings(H, st);
+    if (d.rel_tol == 0.0 && !trivial) {   // fixed-cycle run: report the final residual too
+        if ((rc = do_residual_norm(H, 0, s)) != 0) return rc;
+        CUDA_OK(cudaMemcpyAsync(H->host_scal + 4, H->scal + 4, sizeof(double), cudaMemcpyDeviceToHost, s));
+        CUDA_OK(cudaStreamSynchronize(s));
+        st.res_norm_inf = H->host_scal[4];
+        st.gpu_launches = H->launches;
+    }
+    H->last = st;
+    if (stats) *stats = st;
+    return result;
+}
+
+extern "C" int maestro_mac_status(maestro_mac_handle* H, maestro_mac_stats* stats, void* cuda_stream)
+{
+    if (!H) return MAESTRO_MAC_ERR_ARG;
+    cudaStream_t s = (cudaStream_t)cuda_stream;
+    if (!H->deferred) {
+        if (stats) *stats = H->last;
+        return MAESTRO_MAC_OK;
+    }
+    CUDA_OK(cudaStreamSynchronize(s));
+    H->deferred = 0;
+    maestro_mac_stats st = H->last;
+    st.rhs_norm_inf = H->host_scal[1];
+    st.rhs_mean_removed = H->singular ? H->host_scal[2] / (double)H->lev[0].ncell : 0.0;
+    collect_timings(H, st);
+    int result = MAESTRO_MAC_OK;
+    if (H->host_flags[0] != 0 || !std::isfinite(st.rhs_norm_inf) || !std::isfinite(H->host_scal[0])) result = MAESTRO_MAC_ERR_NONFINITE;
+    else if (stats) {                              // the final residual, as the synchronous fixed-cycle call reports it
+        int rc;
+        if ((rc = do_residual_norm(H, 0, s)) != 0) return rc;
+        CUDA_OK(cudaMemcpyAsync(H->host_scal + 4, H->scal + 4, sizeof(double), cudaMemcpyDeviceToHost, s));
+        CUDA_OK(cudaStreamSynchronize(s));
+        st.res_norm_inf = H->host_scal[4];
+        st.gpu_launches = H->launches;
+    }
+    H->last = st;
     if (stats) *stats = st;
     return result;
 }
@@ -912,7 +975,7 @@ extern "C" int maestro_mac_lateral_average(maestro_mac_handle* H, const double* 
     CUDA_OK(cudaMemsetAsync(H->part_sum, 0, H->d.nr * sizeof(double), s));
     CUDA_OK(cudaMemsetAsync(cnt, 0, H->d.nr * sizeof(unsigned long long), s));
     const int rows = H->d.ny * H->d.nz;
-    k_lateral_sum<<<rows < 148 * 16 ? rows : 148 * 16, 256, 0, s>>>(dev_geo(H), rho, H->part_sum, cnt);
+    k_lateral_sum<<<rows < H->sms * 16 ? rows : H->sms * 16, 256, 0, s>>>(dev_geo(H), rho, H->part_sum, cnt);
     LAUNCHED(H);
     k_average_finish<<<1, 256, 0, s>>>(H->d.nr, H->part_sum, cnt, rho0);
     LAUNCHED(H);
@@ -1042,4 +1105,30 @@ extern "C" int maestro_mac_step_correct(maestro_mac_handle* H, const double* rho
 {
     if (!H || !u || !v || !w || (!rho && !rho0)) return MAESTRO_MAC_ERR_ARG;
     return do_correct(H, H->lev[0].phi, rho0, rho, u, v, w, (cudaStream_t)cuda_stream);
+}
+
+extern "C" int maestro_mac_level_plan(const maestro_mac_handle* H, int level, int info[8])
+{
+    if (!H || !info || level < 0 || level >= H->nlev) return MAESTRO_MAC_ERR_ARG;
+    const Level& L = H->lev[level];
+    const LevelDev D = dev_level(H, level);
+    for (int q = 0; q < 8; ++q) info[q] = 0;
+    info[6] = L.gx; info[7] = L.gy;
+    const int sm = H->d.smoother;
+    if (level == H->nlev - 1 && H->nlev > 1) { info[0] = MAESTRO_MAC_KERNEL_BOTTOM; return MAESTRO_MAC_OK; }
+    if (H->tail_start >= 0 && level >= H->tail_start) { info[0] = MAESTRO_MAC_KERNEL_TAIL; return MAESTRO_MAC_OK; }
+    if (t2_ok(H, level)) {
+        const t2::T2Plan P = t2_plan(D, H->sms);
+        info[0] = MAESTRO_MAC_KERNEL_T2; info[1] = P.tiles; info[2] = P.nfull; info[3] = P.nsplit; info[4] = P.zchunk; info[5] = P.ncta;
+        return MAESTRO_MAC_OK;
+    }
+    const int tv = ((sm == 0 || sm == 4) && D.nx >= 60) ? 0 : (sm == 3 ? 1 : -1);
+    if (tv >= 0 && L.tma[tv].ok) {
+        int zc = 0;
+        const dim3 g = tma_sweep_grid(D, tv, H->sms, &zc);
+        info[0] = MAESTRO_MAC_KERNEL_TMA; info[1] = (int)(g.x * g.y); info[3] = (int)g.z; info[4] = zc; info[5] = (int)(g.x * g.y * g.z);
+        return MAESTRO_MAC_OK;
+    }
+    info[0] = (sm != 1 && fused_sweep_supported(D)) ? MAESTRO_MAC_KERNEL_FUSED : MAESTRO_MAC_KERNEL_COLOR;
+    return MAESTRO_MAC_OK;
 }

@@ -26,6 +26,7 @@ EXPORTS = [
     "maestro_mac_step_residual_restrict", "maestro_mac_step_prolong", "maestro_mac_step_bottom",
     "maestro_mac_step_vcycle", "maestro_mac_step_residual_norm", "maestro_mac_step_correct",
     "maestro_mac_base_state", "maestro_mac_set_dpdt_term", "maestro_mac_lateral_average",
+    "maestro_mac_status", "maestro_mac_level_plan",
 ]
 
 
@@ -37,7 +38,7 @@ class Desc(C.Structure):
                 ("max_cycles", C.c_int), ("rel_tol", C.c_double), ("coarsest_n", C.c_int),
                 ("bottom_max_iter", C.c_int), ("bottom_rel_tol", C.c_double),
                 ("prolongation", C.c_int), ("host_staging", C.c_int), ("smoother", C.c_int),
-                ("stop_test", C.c_int), ("rho_mean", C.c_int)]
+                ("stop_test", C.c_int), ("rho_mean", C.c_int), ("timing", C.c_int)]
 
 
 class Stats(C.Structure):
@@ -95,6 +96,8 @@ def lib():
         L.maestro_mac_base_state.argtypes = [C.c_int, _VP, _VP, _VP, _VP, _VP, _VP, _VP]
         L.maestro_mac_set_dpdt_term.argtypes = [_VP, _VP]
         L.maestro_mac_lateral_average.argtypes = [_VP, _VP, _VP, _VP]
+        L.maestro_mac_status.argtypes = [_VP, C.POINTER(Stats), _VP]
+        L.maestro_mac_level_plan.argtypes = [_VP, C.c_int, C.POINTER(C.c_int * 8)]
         for name in EXPORTS:
             if name != "maestro_mac_default_desc":
                 getattr(L, name).restype = C.c_int
@@ -111,7 +114,7 @@ class MacError(RuntimeError):
 def make_desc(n, dx, bc_lo, bc_hi, geometry=PLANAR, nr=None, dr=None, center=(0.0, 0.0, 0.0),
               nu_pre=2, nu_post=2, max_cycles=100, rel_tol=1e-10, coarsest_n=4,
               bottom_max_iter=100, bottom_rel_tol=1e-8, prolongation=0, host_staging=0,
-              smoother=0, stop_test=0, rho_mean=0) -> Desc:
+              smoother=0, stop_test=0, rho_mean=0, timing=0) -> Desc:
     d = Desc()
     lib().maestro_mac_default_desc(C.byref(d))
     d.nx, d.ny, d.nz = (int(x) for x in n)
@@ -125,6 +128,7 @@ def make_desc(n, dx, bc_lo, bc_hi, geometry=PLANAR, nr=None, dr=None, center=(0.
     d.prolongation, d.host_staging, d.smoother = int(prolongation), int(host_staging), int(smoother)
     d.stop_test = int(stop_test)
     d.rho_mean = int(rho_mean)
+    d.timing = int(timing)
     return d
 
 
@@ -199,6 +203,12 @@ class MacProjector:
                                        _stream())
         return rc, (st.as_dict() if want_stats else None)
 
+    def status(self, want_stats=True):
+        """Completes an asynchronous project call (rel_tol == 0, want_stats=False).  Returns (status, stats | None)."""
+        st = Stats()
+        rc = lib().maestro_mac_status(self._h, C.byref(st) if want_stats else None, _stream())
+        return rc, (st.as_dict() if want_stats else None)
+
     def project_host(self, beta0, rho0, rho, u, v, w, S=None, phi=None, want_stats=True):
         """Host (pinned) tensors; includes the host<->device copies."""
         st = Stats()
@@ -220,6 +230,15 @@ class MacProjector:
         n, h = (C.c_int * 3)(), (C.c_double * 3)()
         self._ck(lib().maestro_mac_level_dims(self._h, level, C.byref(n), C.byref(h)), "level_dims")
         return tuple(n), tuple(h)
+
+    KERNELS = ("color", "fused", "tma", "t2", "tail", "bottom")
+
+    def level_plan(self, level):
+        """Launch plan of the smoother on a level (maestro_mac_level_plan)."""
+        info = (C.c_int * 8)()
+        self._ck(lib().maestro_mac_level_plan(self._h, level, C.byref(info)), "level_plan")
+        return dict(kernel=self.KERNELS[info[0]], tiles=info[1], nfull=info[2], nsplit=info[3], zchunk=info[4],
+                    ncta=info[5], gx=info[6], gy=info[7])
 
     def level_shape(self, level, which):
         (nx, ny, nz), _ = self.level_dims(level)

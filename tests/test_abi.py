@@ -60,7 +60,15 @@ def test_workspace_query_and_validation(mac):
     assert rc_of(bad) == mac.ERR_ARG
     bad = mac.make_desc((34, 34, 34), (1 / 34,) * 3, (0, 0, 1), (0, 0, 1))      # 17^3 bottom > 4096
     assert rc_of(bad) == mac.ERR_UNSUPPORTED
+    bad = mac.make_desc((64, 64, 64), (1 / 64,) * 3, (0, 0, 1), (0, 0, 1), nu_pre=0, nu_post=0)   # no smoothing at all
+    assert rc_of(bad) == mac.ERR_ARG
+    ok = mac.make_desc((64, 64, 64), (1 / 64,) * 3, (0, 0, 1), (0, 0, 1), nu_pre=0, nu_post=3)    # taken literally
+    assert rc_of(ok) == mac.ERR_WORKSPACE
+    bad = mac.make_desc((64, 64, 64), (1 / 64,) * 3, (0, 0, 1), (0, 0, 1), timing=2)
+    assert rc_of(bad) == mac.ERR_ARG
     assert mac.lib().maestro_mac_setup(None, None, 0, None, None) == mac.ERR_ARG
+    assert mac.lib().maestro_mac_status(None, None, None) == mac.ERR_ARG
+    assert mac.lib().maestro_mac_level_plan(None, 0, None) == mac.ERR_ARG
     assert mac.lib().maestro_mac_free(None) == mac.OK
     assert mac.lib().maestro_mac_num_levels(None) == mac.ERR_ARG
 

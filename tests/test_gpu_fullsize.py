@@ -69,7 +69,18 @@ def test_kernels_at_full_size(oracle, mac, full):
     phi = rng.standard_normal(O.cell_shape(g))
     P.level_set(0, mac.ARR_PHI, tt(phi))
     assert P.step_residual_norm(0) == pytest.approx(O.norm_inf(O.residual(g, *bf, phi, rhs)), rel=1e-12)
-    P.step_smooth(0, 1)
+    # the launch decomposition bench.py times: the two-sweep kernel with whole-column tiles for the whole waves and
+    # z-chunks for the last, partial wave (592 + 112 x 5 CTAs on 148 SMs), then a pair plus a single sweep
+    plan = P.level_plan(0)
+    assert plan["kernel"] == "t2" and plan["nfull"] > 0 and plan["nsplit"] > 1 and plan["tiles"] == 704, plan
+    P.step_smooth(0, 2)
+    O.rbgs_sweep(g, *bf, rhs, phi); O.rbgs_sweep(g, *bf, rhs, phi)
+    assert close(P.level_get(0, mac.ARR_PHI), phi)
+    P.step_smooth(0, 3)
+    for _ in range(3):
+        O.rbgs_sweep(g, *bf, rhs, phi)
+    assert close(P.level_get(0, mac.ARR_PHI), phi)
+    P.step_smooth(0, 1)                               # the single-sweep kernel alone
     O.rbgs_sweep(g, *bf, rhs, phi)
     assert close(P.level_get(0, mac.ARR_PHI), phi)
     P.step_residual_restrict(0)
@@ -114,3 +125,22 @@ def test_projection_properties_at_full_size(oracle, mac, full):
     for got, ref in ((un, ru), (vn, rv), (wn, rw)):
         assert np.abs(got - ref).max() <= KERNEL_TOL * np.abs(ref).max()
     assert np.array_equal(un[:, :, 0], wl.u[:, :, 0]) and np.array_equal(wn[-1], wl.w[-1])
+
+
+def test_end_to_end_parity_at_full_size(oracle, mac, full):
+    """The whole 512^3 projection of bench.py's default line against the oracle (about a minute and 15 GB on the
+    host): same cycle count, same residual history, relative L2 <= 1e-10 in phi, u, v, w (north_star's bar)."""
+    import torch
+    from helpers import oracle_project, rel_l2
+    O, wl, P, dv = oracle, full["wl"], full["P"], full["dv"]
+    ref = oracle_project(O, wl)
+    K = ref["stats"]["cycles"]
+    u, v, w = tt(wl.u), tt(wl.v), tt(wl.w)
+    phi = torch.full(wl.rho.shape, float("nan"), dtype=torch.float64, device="cuda")
+    rc, st = P.project(dv["beta0"], dv["rho0"], dv["rho"], u, v, w, dv["S"], phi)
+    assert rc == 0 and ref["status"] == 0
+    assert st["cycles"] == K, (st["cycles"], K)
+    assert np.allclose(st["res_history"], ref["stats"]["res_history"][:K], rtol=1e-3)
+    assert st["rhs_norm_inf"] == pytest.approx(ref["stats"]["rhs_norm_inf"], rel=1e-12)
+    for key, got in (("phi", phi), ("u", u), ("v", v), ("w", w)):
+        assert rel_l2(got.cpu().numpy(), ref[key]) <= 1e-10, key

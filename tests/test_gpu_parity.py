@@ -280,6 +280,50 @@ def test_project_host_matches_device_path(oracle, mac):
     P.close()
 
 
+def test_asynchronous_fixed_cycle_call(oracle, mac):
+    """rel_tol = 0 and stats = NULL: the call returns without synchronising; maestro_mac_status() completes it with
+    the same results and stats as the synchronous fixed-cycle call, and reports non-finite input."""
+    import torch
+    wl = W.config2(N=32)
+    ref = gpu_project(mac, wl, rel_tol=0.0, max_cycles=4)
+    P = mac.MacProjector(mac.desc_from_workload(wl, rel_tol=0.0, max_cycles=4))
+    dv = mac.to_device(wl)
+    phi = torch.empty(wl.rho.shape, dtype=torch.float64, device="cuda")
+    rc, st = P.project(dv["beta0"], dv["rho0"], dv["rho"], dv["u"], dv["v"], dv["w"], dv["S"], phi, want_stats=False)
+    assert rc == 0 and st is None
+    rc, st = P.status()
+    assert rc == 0 and st["cycles"] == 4
+    assert st["rhs_norm_inf"] == ref["stats"]["rhs_norm_inf"] and st["res_norm_inf"] == ref["stats"]["res_norm_inf"]
+    assert np.array_equal(phi.cpu().numpy(), ref["phi"]) and np.array_equal(dv["u"].cpu().numpy(), ref["u"])
+    rc2, st2 = P.status()                          # idempotent: the stats of the last call, no work
+    assert rc2 == 0 and st2["cycles"] == 4
+    # zero rhs: the cycles run on zeros, the velocities stay bit for bit
+    z = W.config1(N=16); z.u[:] = 0; z.v[:] = 0; z.w[:] = 0; z.u[3, 4, 5] = -0.0
+    Pz = mac.MacProjector(mac.desc_from_workload(z, rel_tol=0.0, max_cycles=2))
+    dz = mac.to_device(z)
+    phiz = torch.full(z.rho.shape, float("nan"), dtype=torch.float64, device="cuda")
+    rc, _ = Pz.project(dz["beta0"], dz["rho0"], dz["rho"], dz["u"], dz["v"], dz["w"], None, phiz, want_stats=False)
+    assert rc == 0 and Pz.status(want_stats=False)[0] == 0
+    assert float(phiz.abs().max()) == 0.0 and np.array_equal(dz["u"].cpu().numpy(), z.u)
+    Pz.close()
+    # non-finite input surfaces in maestro_mac_status
+    bad = W.config2(N=32); bad.rho[1, 2, 3] = -1.0
+    db = mac.to_device(bad)
+    rc, _ = P.project(db["beta0"], db["rho0"], db["rho"], db["u"], db["v"], db["w"], db["S"], None, want_stats=False)
+    assert rc == 0
+    assert P.status()[0] == mac.ERR_NONFINITE
+    P.close()
+
+
+def test_per_launch_timing_is_opt_in(mac):
+    wl = W.config3(N=64, variant="D")
+    off, on = gpu_project(mac, wl), gpu_project(mac, wl, timing=1)
+    assert off["stats"]["smooth0_timed"] == 0 and off["stats"]["ms_smooth0"] == 0.0
+    assert off["stats"]["smooth0_launches"] == on["stats"]["smooth0_launches"] > 0
+    assert on["stats"]["smooth0_timed"] == on["stats"]["smooth0_launches"] and on["stats"]["ms_smooth0"] > 0.0
+    assert np.array_equal(off["phi"], on["phi"])
+
+
 def test_deterministic_across_runs(mac):
     wl = W.config2(N=32)
     a, b = gpu_project(mac, wl), gpu_project(mac, wl)
@@ -317,8 +361,8 @@ T2_CASES = [
 
 @pytest.mark.parametrize("case", range(len(T2_CASES)))
 def test_two_sweep_kernel_equals_two_single_sweeps(oracle, mac, case):
-    """k_rbgs_t2 (two sweeps per pass, smoother 4) is bit-identical to two launches of the single-sweep TMA kernel
-    (smoother 0) and matches two oracle sweeps; sizes span several tiles, a ragged tail and several z-chunks."""
+    """k_rbgs_t2 (two sweeps per pass, smoother 0) is bit-identical to two launches of the single-sweep TMA kernel
+    (smoother 4) and matches two oracle sweeps; sizes span several tiles, a ragged tail and several z-chunks."""
     O = oracle
     wl = W.mixed_bc_case(**T2_CASES[case])
     g, b, mg = oracle_structs(O, wl)
@@ -374,7 +418,7 @@ def test_harmonic_face_density_variant(oracle, mac, name, N, smoother):
         assert rel_l2(got[key], ref[key]) <= E2E_TOL, key
 
 
-@pytest.mark.parametrize("nu_pre,nu_post", [(1, 1), (3, 1), (1, 2), (4, 3)])
+@pytest.mark.parametrize("nu_pre,nu_post", [(1, 1), (3, 1), (1, 2), (4, 3), (0, 3), (2, 0)])
 @pytest.mark.parametrize("name,N", [("1", 64), ("4D", 64)])
 def test_sweep_counts_other_than_two(oracle, mac, name, N, nu_pre, nu_post):
     """Pairs of sweeps run through the two-sweep kernel, a remaining one through the single-sweep kernel, and the
