@@ -8,9 +8,10 @@ face coefficients -> coarsening -> rhs -> V-cycles to 1e-10 -> velocity correcti
 Prints ONE JSON line (rank 0).  `value` is level-0 cell-updates/s over the whole projection,
 N^3 (nu_pre + nu_post) cycles / t(project), inputs resident in HBM (SURVEY.md Sec. 8(d));
 `e2e` is the same metric through maestro_mac_project_host() with pinned HOST buffers, host<->device
-copies inside the timed region.  `roofline` is the level-0 fused red-black smoother (k_rbgs_t2, two sweeps per launch): 48 B/cell/sweep
- x the cell-sweeps of a launch over the mean device time of its launches, timed by CUDA event pairs inside
-the library on the call's stream during the timed steps.  Multi-GPU: replicas only:
+copies inside the timed region.  `roofline` is the level-0 fused red-black smoother (k_rbgs_t2: the two sweeps of a smoothing step in
+ONE pass over HBM): `achieved` = the bytes that pass must move (48 B per cell per launch: read phi, rhs, ax, ay, az, write phi;
+DESIGN.md Sec. 6) over the mean device time of its launches, timed by CUDA event pairs inside the library on the call's stream
+during the timed steps (desc.timing = 1); `per_sweep_*` restate it in SURVEY.md Sec. 8(d)'s per-sweep unit (48 B per cell per SWEEP).  Multi-GPU: replicas only:
 every rank projects its own copy; value = all ranks' units / max-over-ranks time.
 """
 from __future__ import annotations
@@ -45,6 +46,7 @@ def parse_args():
     ap.add_argument("--smoother", type=int, default=0, help="0 two sweeps per HBM pass, TMA staging (default); 1 two-pass reference; 2 fused, cp.async staging; 3 fused, TMA 32x16 tile; 4 one sweep per pass, TMA staging")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-other-configs", action="store_true", help="skip the millisecond-scale configs 1, 2, 3N")
     ap.add_argument("--cpu-sample-n", type=int, default=0, help="cells per side of the oracle sample (0 = auto)")
     return ap.parse_args()
 
@@ -136,12 +138,40 @@ class ClockSampler:
         return res
 
 
-def cpu_oracle_run(config: str, n: int):
-    """One projection by the oracle on the host cores.  Returns (seconds, cycles, cells, threads)."""
+def cpu_model():
+    try:
+        with open("/proc/cpuinfo") as f:
+            for line in f:
+                if line.lower().startswith("model name"):
+                    return line.split(":", 1)[1].strip()
+    except Exception:
+        pass
+    return "unknown"
+
+
+def host_mem_available_gb():
+    try:
+        with open("/proc/meminfo") as f:
+            for line in f:
+                if line.startswith("MemAvailable"):
+                    return float(line.split()[1]) / 1e6
+    except Exception:
+        pass
+    return 0.0
+
+
+def cpu_oracle_run(config: str, n: int, threads: int = 0, wl=None):
+    """One projection by the oracle on the host cores (threads = 0: all of them).  Returns (seconds, cycles, cells,
+    threads used, sweeps per cycle)."""
     from oracle import mac_oracle as O
     from paper_1910_12979_b200 import workloads as W
     O.build()
-    wl = W.by_name(config, n)
+    if threads > 0:
+        O.set_num_threads(threads)
+    else:
+        O.set_num_threads(os.cpu_count() or 1)
+    if wl is None:
+        wl = W.by_name(config, n)
     g = O.make_grid(wl.n, wl.dx, wl.bc_lo, wl.bc_hi)
     b = O.make_base(wl.geometry, wl.nr, wl.dr, wl.center)
     mg = O.make_mg(nu_pre=wl.nu_pre, nu_post=wl.nu_post, max_cycles=wl.max_cycles, rel_tol=wl.rel_tol)
@@ -166,7 +196,7 @@ def run_reference(a):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return 0
-    ns = a.cpu_sample_n or 128                 # one projection at 128^3 is about 1 s on 16 cores
+    ns = a.cpu_sample_n or 256                 # one projection at 256^3 is about 8 s on 16 cores
     ns = min(ns, a.n)
     for _ in range(a.warmup):
         cpu_oracle_run(a.config, ns)
@@ -182,8 +212,10 @@ def run_reference(a):
         "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": a.gpus, "steps": a.steps,
         "warmup": a.warmup, "ms_per_step": 1e3 * tot / max(a.steps, 1), "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": workload_label(a.config, a.n), "sample": sample},
-        "cpu_baseline": {"value": val, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": sample},
+        "config": {"workload": workload_label(a.config, a.n) + f"; the reference arm times the oracle on the {ns}^3 instance of it",
+                   "sample": sample, "same_config": ns == a.n},
+        "cpu_baseline": {"value": val, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": sample,
+                         "nproc": os.cpu_count(), "cpu_model": cpu_model()},
         "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
     }
@@ -290,15 +322,23 @@ def run_ours(a):
         # algorithmic bytes per launch = 48 B per cell per sweep x the cell-sweeps one launch
         # processes; the two-sweep kernel moves half of that through HBM (temporal blocking), so its fraction of the
         # per-sweep roofline can exceed 1 -- `one_pass_bytes` / `frac_one_pass` state what it must move at least
-        alg = SMOOTHER_BYTES_PER_CELL * wl.ncells * sweeps
-        ach = alg / (per_launch_ms * 1e-3) / 1e9
+        # `achieved`: what ONE launch must move -- it reads phi, rhs, ax, ay, az and writes phi once, whatever the number
+        # of sweeps it applies: 48 B per cell per launch.  This is the physically bounded figure
+        # (<= the copy peak).  `per_sweep_*`: SURVEY.md Sec. 8(d)'s unit, 48 B per cell per SWEEP, x the sweeps of a
+        # launch; for the two-sweep kernel it can exceed the peak because temporal blocking halves the HBM traffic.
         one_pass = SMOOTHER_BYTES_PER_CELL * wl.ncells
+        ach = one_pass / (per_launch_ms * 1e-3) / 1e9
+        per_sweep = SMOOTHER_BYTES_PER_CELL * wl.ncells * sweeps / (per_launch_ms * 1e-3) / 1e9
+        traffic = ncu_traffic(kname, a.n)
         roof = {"bound": "hbm", "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
-                "traffic": ncu_traffic(kname, a.n), "kernel": kname + " level 0",
-                "algorithmic_bytes_per_launch": alg, "sweeps_per_launch": sweeps,
+                "traffic": traffic, "traffic_source": "ncu --set full capture of this kernel, profiles/roofline_traffic.md (offline, not a live counter)",
+                "kernel": kname + " level 0",
+                "algorithmic_bytes_per_launch": one_pass, "sweeps_per_launch": sweeps,
                 "avg_launch_ms": per_launch_ms, "launches_timed": sm_n, "peak_source": peak_src,
                 "frac_of_8000_nominal": ach / 8000.0,
-                "one_pass_bytes": one_pass, "frac_one_pass": one_pass / (per_launch_ms * 1e-3) / 1e9 / peak,
+                "dram_traffic_gbs": (traffic / (per_launch_ms * 1e-3) / 1e9) if traffic else None,
+                "per_sweep_achieved": per_sweep, "per_sweep_frac": per_sweep / peak, "per_sweep_frac_of_8000_nominal": per_sweep / 8000.0,
+                "limiter": "see profiles/ (ncu): issue slots and fp64 dependency latency at 12 warps per SM, not DRAM",
                 "share_of_step": sm_ms / (t_dev * 1e3) if t_dev > 0 else None}
 
     # end to end through the host-buffer entry point
@@ -334,13 +374,51 @@ def run_ours(a):
     del dv, pristine, phi
     torch.cuda.empty_cache()
 
+    # the latency-bound configs of BASELINE.json, a few milliseconds each (parity-test cases, not the bench line)
+    others = []
+    if rank == 0 and world == 1 and not a.no_other_configs:
+        for cfg, n_o in (("1", 32), ("2", 128), ("3N", 256)):
+            wo = W.by_name(cfg, n_o)
+            Po = mac.MacProjector(mac.desc_from_workload(wo), device=dev)
+            do = mac.to_device(wo, dev)
+            keep = [do[k].clone() for k in ("u", "v", "w")]
+            tms, st_o = [], None
+            for it in range(3 + 10):
+                for t, p in zip((do["u"], do["v"], do["w"]), keep):
+                    t.copy_(p)
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                e0.record()
+                rc, st_o = Po.project(do["beta0"], do["rho0"], do["rho"], do["u"], do["v"], do["w"], do["S"], None)
+                e1.record()
+                torch.cuda.synchronize()
+                if rc != 0:
+                    raise RuntimeError(f"config {cfg}: maestro_mac_project returned {rc}")
+                if it >= 3:
+                    tms.append(e0.elapsed_time(e1))
+            others.append({"config": cfg, "n": n_o, "ms_per_projection": statistics.median(tms), "cycles": st_o["cycles"],
+                           "launches": st_o["gpu_launches"], "timing": "median of 10 after 3 warm-ups, CUDA events"})
+            Po.close()
+            del do, keep, wo
+        torch.cuda.empty_cache()
+
     cpu = None
     if rank == 0 and world == 1 and not a.no_cpu_baseline:
-        ns = a.cpu_sample_n or min(256, a.n)   # about 10 s of CPU work for the 512^3 workload
-        dt, cyc, cells, threads, nu_o = cpu_oracle_run(a.config, ns)
+        # the oracle as it stands on the SAME inputs (one whole projection, all host cores) when the host has the
+        # memory (about 15 GB at 512^3, a minute on 16 cores), else on the 256^3 instance of the workload; plus a
+        # one-thread figure on a bounded sample (SURVEY.md Sec. 8(d) asks for both)
+        ns = a.cpu_sample_n or (a.n if host_mem_available_gb() > 18.0 * (a.n / 512.0) ** 3 + 8.0 else min(256, a.n))
+        same = ns == a.n
+        dt, cyc, cells, threads, nu_o = cpu_oracle_run(a.config, ns, wl=wl if same else None)
+        n1 = min(128, a.n)
+        dt1, cyc1, cells1, _, nu1 = cpu_oracle_run(a.config, n1, threads=1)
         cpu = {"value": cells * nu_o * cyc / dt, "unit": UNIT, "cores": threads, "kind": "oracle",
-               "sample": f"{a.config} at {ns}^3 (same recipe as the {a.n}^3 workload), one full projection, "
-                         f"{cyc} cycles, {dt:.1f} s"}
+               "sample": (f"the whole workload: {a.config} at {ns}^3, the same inputs, one full projection, " if same else
+                          f"{a.config} at {ns}^3 (same recipe as the {a.n}^3 workload), one full projection, ")
+                         + f"{cyc} cycles, {dt:.1f} s",
+               "same_config": same, "seconds": dt, "cycles": cyc,
+               "one_thread": {"value": cells1 * nu1 * cyc1 / dt1, "unit": UNIT, "cores": 1,
+                              "sample": f"{a.config} at {n1}^3, one full projection, {cyc1} cycles, {dt1:.1f} s"},
+               "nproc": os.cpu_count(), "cpu_model": cpu_model()}
 
     if rank == 0:
         line = {
@@ -361,6 +439,7 @@ def run_ours(a):
             "final_rel_residual": stats[-1]["res_history"][-1] if stats[-1]["res_history"] else None,
             "wall_s_timed_region": t_wall,
             "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "roofline": roof, "cpu_baseline": cpu,
+            "other_configs": others,
         }
         print(json.dumps(line), flush=True)
     if world > 1:

@@ -91,7 +91,9 @@ typedef struct {
                                  1 = reference two-pass (one kernel per colour);
                                  2 = fused single pass, cp.async staging on every level;
                                  3 = fused single pass, TMA staging with the 32x16 tile.
-                                 Same arithmetic, same results. */
+                                 Same arithmetic, same results.  0 is the product path; 4 is its one-sweep-per-pass
+                                 form; 1, 2, 3 are kept as independent cross-checks for the parity tests (three
+                                 further implementations of the same sweep) and are not tuned. */
     int stop_test;            /* how ||rhs - L phi||inf is obtained after each cycle:
                                  0 = default: where the level-0 TMA smoother runs (smoother 0, nu_pre >= 1,
                                      nu_post >= 1) the test rides on the first pre-sweep of the NEXT cycle,

@@ -637,13 +637,6 @@ int do_correct(maestro_mac_handle* H, const double* phi, const double* rho0, con
 {
     GeoDev G = dev_geo(H);
     dim3 g, b;
-    if (rho && H->d.smoother == 2) {      // column-marching form: measured slower than one thread per face index
-        const int zc = 16;
-        dim3 gg((G.nx + 64) / 64, (G.ny + 4) / 4, (G.nz + zc - 1) / zc);
-        k_correct2<<<gg, dim3(64, 4), 0, s>>>(G, dev_geo_inv(H), dev_level(H, 0), phi, rho, u, v, w, zc);
-        LAUNCHED(H);
-        return MAESTRO_MAC_OK;
-    }
     dims3(G.nx + 1, G.ny + 1, G.nz + 1, &g, &b);
     k_correct<<<g, b, 0, s>>>(G, dev_level(H, 0), phi, rho, rho0, u, v, w);
     LAUNCHED(H);
