@@ -17,6 +17,8 @@ import numpy as np
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _LIB_PATH = os.path.join(_HERE, "libmac_oracle.so")
 _SRC = os.path.join(_HERE, "mac_oracle.c")
+_SRCS = [_SRC, os.path.join(_HERE, "nodal_oracle.c")]          # one library: MAC projection + nodal projection
+_HDRS = [os.path.join(_HERE, "mac_oracle.h"), os.path.join(_HERE, "nodal_oracle.h")]
 
 PERIODIC, WALL, OUTFLOW = 0, 1, 2
 PLANAR, SPHERICAL = 0, 1
@@ -24,12 +26,11 @@ PLANAR, SPHERICAL = 0, 1
 
 def build(force: bool = False) -> str:
     """Compile the oracle with gcc (-O2, OpenMP on independent loops only)."""
-    hdr = os.path.join(_HERE, "mac_oracle.h")
     if (not force and os.path.exists(_LIB_PATH)
-            and os.path.getmtime(_LIB_PATH) >= max(os.path.getmtime(_SRC), os.path.getmtime(hdr))):
+            and os.path.getmtime(_LIB_PATH) >= max(os.path.getmtime(p) for p in _SRCS + _HDRS)):
         return _LIB_PATH
     cmd = ["gcc", "-O2", "-std=c99", "-fopenmp", "-fPIC", "-shared", "-ffp-contract=off",
-           "-Wall", "-Wextra", "-o", _LIB_PATH, _SRC, "-lm"]
+           "-Wall", "-Wextra", "-o", _LIB_PATH, *_SRCS, "-lm"]
     subprocess.run(cmd, check=True, cwd=_HERE)
     return _LIB_PATH
 

@@ -326,3 +326,12 @@ def mixed_bc_case(n=(16, 8, 12), seed: int = 7, bc_lo=(OUTFLOW, WALL, PERIODIC),
     _close_faces(u, v, w, bc_lo, bc_hi)
     return Workload("mixed_bc", tuple(n), dx, tuple(bc_lo), tuple(bc_hi), geometry, nr, dr, center,
                     beta0, rho0, rho, u, v, w, S, seed=seed)
+
+
+def cell_centred(wl: Workload):
+    """Cell-centred velocities for the end-of-step (nodal) projection from a workload's face velocities: the mean of
+    the two faces of a cell per axis (input construction only).  Returns (uc, vc, wc), each [nz, ny, nx]."""
+    uc = np.ascontiguousarray(0.5 * (wl.u[:, :, :-1] + wl.u[:, :, 1:]))
+    vc = np.ascontiguousarray(0.5 * (wl.v[:, :-1, :] + wl.v[:, 1:, :]))
+    wc = np.ascontiguousarray(0.5 * (wl.w[:-1, :, :] + wl.w[1:, :, :]))
+    return uc, vc, wc
