@@ -108,6 +108,9 @@ typedef struct {
     int timing;               /* 1 = bracket every level-0 smoother launch with a CUDA event pair on the call's
                                  stream (stats.ms_smooth0 ...; bench.py's roofline); 0 (default) = no per-launch
                                  events on the hot path */
+    int nodal;                /* 1 = also reserve the level arrays of the end-of-step (nodal) projection in the
+                                 workspace so that maestro_mac_nodal_project() can be used (adds about 4/6 of the
+                                 MAC projection's workspace); 0 (default) = MAC projection only */
 } maestro_mac_desc;
 
 typedef struct {
@@ -221,6 +224,32 @@ int maestro_mac_lateral_average(maestro_mac_handle *h, const double *rho, double
  */
 int maestro_mac_set_dpdt_term(maestro_mac_handle *h, const double *dpdt_term);
 
+/*
+ * maestro_mac_nodal_project: the OTHER projection of the "second order projection method" with "multigrid linear
+ * solvers for the pressure projection steps" (Sec. 3): the end-of-step projection of the CELL-CENTRED
+ * velocity.  It enforces the same constraint div(beta0 U) = beta0 (S - ...) (Eq. 6; the dp0/dt term
+ * folded into S) with the same weighting sigma = beta0/rho of the pressure term (Eq. 2) on the same base
+ * state, with phi on the NODES of the grid.  The paper describes neither projection; the readings (N1..N10):
+ * trilinear finite-element (27-point) operator  (L phi)_a = -(1/V) sum_c sigma_c int_c grad psi_a . grad phi,
+ * rhs_a = (D(beta0 U))_a - (M(beta0 S))_a with the finite-element divergence D and the lumped source M (mean over the
+ * cells around the node), U <- U - (1/rho) G phi with G the cell-mean gradient (D = -G^T; an approximate projection
+ * in the sense of Almgren, Bell and Szymczak); WALL sides natural, OUTFLOW sides phi = 0 on the boundary nodes,
+ * periodic sides node n = node 0; no OUTFLOW side: the uniform volumetric source m = sum(rhs)/cells is removed
+ * (stats.rhs_mean_removed) and phi has zero volume-weighted mean; V(nu_pre, nu_post) cycles of Jacobi sweeps
+ * (omega = sum_d h_d^-2 / (3 max_d h_d^-2), 1 for cubic cells) on the MAC projection's cell hierarchy with coarse
+ * sigma = mean of the 8 children, trilinear prolongation P, restriction P^T / 8, BiCGStab on the coarsest level, stop
+ * on ||rhs - L phi||inf <= rel_tol ||rhs||inf over the unknowns.
+ *   beta0, rho0   device [nr]; rho device [nx*ny*nz] or NULL (rho := rho0 at cell centres); S device cells or NULL.
+ *   uc, vc, wc    device CELL arrays [nx*ny*nz], in/out.
+ *   phi           device NODE array [(nx+1)*(ny+1)*(nz+1)], idx = i + (nx+1)*(j + (ny+1)*k), out, or NULL; OUTFLOW
+ *                 nodes hold 0, on a periodic axis entry n equals entry 0.
+ *   stats         HOST, out, or NULL.
+ * Needs desc.nodal = 1 (else ERR_ARG).  Synchronises the stream like maestro_mac_project with stats.  Same return codes.
+ */
+int maestro_mac_nodal_project(maestro_mac_handle *h, const double *beta0, const double *rho0, const double *rho,
+                              double *uc, double *vc, double *wc, const double *S, double *phi,
+                              maestro_mac_stats *stats, void *cuda_stream);
+
 /* Release the handle (host memory, pinned words, events).  NULL is a no-op.  Returns OK. */
 int maestro_mac_free(maestro_mac_handle *h);
 
@@ -272,6 +301,28 @@ int maestro_mac_step_residual_norm(maestro_mac_handle *h, int level, double *nor
 /* a10: velocity correction from the level-0 phi */
 int maestro_mac_step_correct(maestro_mac_handle *h, const double *rho0, const double *rho,
                              double *u, double *v, double *w, void *cuda_stream);
+
+/* ---- step API of the nodal projection (desc.nodal = 1): the individual kernels on the handle's nodal level arrays.
+ * Node arrays hold (nx+1)(ny+1)(nz+1) values of the level; SIGMA is a cell array.  level_get(PHI) applies the node
+ * rules (OUTFLOW nodes 0, periodic entry n = entry 0); the kernels never read those entries. */
+enum { MAESTRO_MAC_NODAL_PHI = 0, MAESTRO_MAC_NODAL_RHS = 1, MAESTRO_MAC_NODAL_SIGMA = 2 };
+int maestro_mac_nodal_level_get(maestro_mac_handle *h, int level, int which, double *dst, void *cuda_stream);
+int maestro_mac_nodal_level_set(maestro_mac_handle *h, int level, int which, const double *src, void *cuda_stream);
+/* sigma = beta0(r_cell)/rho on level 0 and its coarsening to every level (also stages beta0 at the cell centres for a
+ * following maestro_mac_nodal_step_rhs) */
+int maestro_mac_nodal_step_sigma(maestro_mac_handle *h, const double *beta0, const double *rho0, const double *rho,
+                                 void *cuda_stream);
+/* rhs on level 0 (uniform source removed if singular); call right after maestro_mac_nodal_step_sigma; synchronises */
+int maestro_mac_nodal_step_rhs(maestro_mac_handle *h, const double *uc, const double *vc, const double *wc,
+                               const double *S, double *rhs_norm_inf, double *mean_removed, void *cuda_stream);
+int maestro_mac_nodal_step_smooth(maestro_mac_handle *h, int level, int nsweeps, void *cuda_stream);      /* Jacobi */
+int maestro_mac_nodal_step_residual_restrict(maestro_mac_handle *h, int level, void *cuda_stream);
+int maestro_mac_nodal_step_prolong(maestro_mac_handle *h, int level, void *cuda_stream);
+int maestro_mac_nodal_step_bottom(maestro_mac_handle *h, void *cuda_stream);
+int maestro_mac_nodal_step_vcycle(maestro_mac_handle *h, void *cuda_stream);
+int maestro_mac_nodal_step_residual_norm(maestro_mac_handle *h, int level, double *norm_inf, void *cuda_stream);
+int maestro_mac_nodal_step_correct(maestro_mac_handle *h, const double *rho0, const double *rho, double *uc,
+                                   double *vc, double *wc, void *cuda_stream);
 
 #ifdef __cplusplus
 }

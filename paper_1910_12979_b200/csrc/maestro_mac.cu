@@ -20,6 +20,7 @@
 #include "mac_smoother_t2.cuh"
 #include "mac_tail.cuh"
 #include "mac_base.cuh"
+#include "mac_nodal.cuh"
 
 namespace {
 
@@ -48,6 +49,14 @@ struct Staging {
     double *beta0, *rho0, *rho, *u, *v, *w, *S, *phi;
 };
 
+struct NodHost {                   // one level of the nodal projection (desc.nodal = 1)
+    int n[3];
+    double h[3];
+    size_t nnode, ncell;
+    double *phi, *phi2, *rhs;      // node arrays, (nx+1)(ny+1)(nz+1)
+    double *sigma;                 // cell array
+};
+
 }  // namespace
 
 struct maestro_mac_handle {
@@ -66,6 +75,9 @@ struct maestro_mac_handle {
     int *flags;                    // [0] bad rho, [1] bottom iterations
     Staging st;
     bool has_staging;
+    NodHost nod[kMaxLevels];       // nodal projection: level arrays (valid when has_nodal)
+    double* nod_vecs;              // 6 BiCGStab vectors over the nodes of the coarsest level
+    bool has_nodal;
     // host side
     double *host_scal;             // pinned, 8 doubles
     int *host_flags;               // pinned, 4 ints
@@ -116,6 +128,7 @@ int validate_and_default(const maestro_mac_desc* in, maestro_mac_desc* d)
     if (d->stop_test != 0 && d->stop_test != 1) return MAESTRO_MAC_ERR_ARG;
     if (d->rho_mean != 0 && d->rho_mean != 1) return MAESTRO_MAC_ERR_ARG;
     if (d->timing != 0 && d->timing != 1) return MAESTRO_MAC_ERR_ARG;
+    if (d->nodal != 0 && d->nodal != 1) return MAESTRO_MAC_ERR_ARG;
     return MAESTRO_MAC_OK;
 }
 
@@ -189,6 +202,21 @@ size_t carve(maestro_mac_handle* H, char* base)
     H->scal = (double*)take(16, 8);
     H->bottom_vecs = (double*)take(6 * H->lev[H->nlev - 1].ncell, 8);
     H->flags = (int*)take(16, 4);
+    H->has_nodal = H->d.nodal == 1;
+    H->nod_vecs = nullptr;
+    if (H->has_nodal) {
+        for (int l = 0; l < H->nlev; ++l) {
+            NodHost& N = H->nod[l];
+            for (int a = 0; a < 3; ++a) { N.n[a] = H->lev[l].n[a]; N.h[a] = H->lev[l].h[a]; }
+            N.nnode = (size_t)(N.n[0] + 1) * (N.n[1] + 1) * (N.n[2] + 1);
+            N.ncell = H->lev[l].ncell;
+            N.phi = (double*)take(N.nnode, 8);
+            N.phi2 = (double*)take(N.nnode, 8);
+            N.rhs = (double*)take(N.nnode, 8);
+            N.sigma = (double*)take(N.ncell, 8);
+        }
+        H->nod_vecs = (double*)take(6 * H->nod[H->nlev - 1].nnode, 8);
+    }
     H->has_staging = H->d.host_staging == 1;
     if (H->has_staging) {
         const maestro_mac_desc& d = H->d;
@@ -1125,3 +1153,5 @@ extern "C" int maestro_mac_level_plan(const maestro_mac_handle* H, int level, in
     info[0] = (sm != 1 && fused_sweep_supported(D)) ? MAESTRO_MAC_KERNEL_FUSED : MAESTRO_MAC_KERNEL_COLOR;
     return MAESTRO_MAC_OK;
 }
+
+#include "maestro_nodal.inl"

@@ -1,0 +1,407 @@
+// maestro_nodal.inl -- host side of the nodal (end-of-step) projection entry points of include/maestro_mac.h.
+// Included at the end of maestro_mac.cu (it uses the handle, the reduction helpers and the launch macros there).
+// Kernels: mac_nodal.cuh.  Readings N1..N10: DESIGN.md.
+
+namespace {
+
+NodLevel dev_nod(const maestro_mac_handle* H, int l)
+{
+    const NodHost& N = H->nod[l];
+    NodLevel D;
+    D.nx = N.n[0]; D.ny = N.n[1]; D.nz = N.n[2];
+    double g[3], gsum = 0.0, gmax = 0.0;
+    for (int a = 0; a < 3; ++a) {
+        D.bclo[a] = H->d.bc_lo[a]; D.bchi[a] = H->d.bc_hi[a];
+        g[a] = 1.0 / (N.h[a] * N.h[a]);
+        gsum += g[a];
+        if (g[a] > gmax) gmax = g[a];
+    }
+    for (int cls = 0; cls < 8; ++cls) {            // N2: K_ab / V for the 8 same / other-corner classes
+        double w = 0.0;
+        for (int d = 0; d < 3; ++d) {
+            double t = ((cls >> d) & 1 ? -1.0 : 1.0) * g[d];
+            for (int e = 0; e < 3; ++e)
+                if (e != d) t *= ((cls >> e) & 1) ? (1.0 / 6.0) : (1.0 / 3.0);
+            w += t;
+        }
+        D.w[cls] = w;
+    }
+    D.omega = gsum / (3.0 * gmax);                 // N7
+    D.phi = N.phi; D.phi2 = N.phi2; D.rhs = N.rhs; D.sigma = N.sigma;
+    return D;
+}
+
+void nod_dims(int ex, int ey, int ez, dim3* grid, dim3* block) { dims3(ex, ey, ez, grid, block); }
+
+// grid of a node kernel that also leaves one partial per block: planes per block chosen so that the partials fit
+void nod_dims_red(int ex, int ey, int ez, dim3* grid, dim3* block, int* zper)
+{
+    dims3(ex, ey, ez, grid, block);
+    int zp = 1;
+    while ((long)grid->x * grid->y * ((ez + zp - 1) / zp) > kMaxParts) zp *= 2;
+    grid->z = (ez + zp - 1) / zp;
+    *zper = zp;
+}
+
+// folds nb block partials into scal[off] (sum) and scal[off + 1] (max)
+int nod_fold(maestro_mac_handle* H, int nb, int off, cudaStream_t s)
+{
+    k_reduce_final<<<1, 1024, 0, s>>>(H->part_sum, H->part_max, nb, H->scal + off);
+    LAUNCHED(H);
+    return MAESTRO_MAC_OK;
+}
+
+int nod_do_sigma(maestro_mac_handle* H, const double* beta0, const double* rho0, const double* rho, cudaStream_t s)
+{
+    dim3 g, b;
+    const GeoDev G = dev_geo(H);
+    CUDA_OK(cudaMemsetAsync(H->flags, 0, 16 * sizeof(int), s));
+    nod_dims(G.nx, G.ny, G.nz, &g, &b);
+    // beta0 at the cell centres goes to level 0's second phi buffer (free until the first sweep); the rhs reads it
+    k_nod_sigma<<<g, b, 0, s>>>(G, beta0, rho, rho0, H->nod[0].sigma, H->nod[0].phi2, H->flags);
+    LAUNCHED(H);
+    for (int l = 0; l + 1 < H->nlev; ++l) {
+        const NodLevel C = dev_nod(H, l + 1);
+        nod_dims(C.nx, C.ny, C.nz, &g, &b);
+        k_nod_coarsen_sigma<<<g, b, 0, s>>>(dev_nod(H, l), C);
+        LAUNCHED(H);
+    }
+    return MAESTRO_MAC_OK;
+}
+
+// rhs on level 0 (after nod_do_sigma of the same call); scal[0..1] = sum, max of the final rhs, scal[2] = removed sum
+int nod_do_rhs(maestro_mac_handle* H, const double* u, const double* v, const double* w, const double* S, cudaStream_t s)
+{
+    const NodLevel L = dev_nod(H, 0);
+    dim3 g, b;
+    int zper;
+    nod_dims_red(L.nx + 1, L.ny + 1, L.nz + 1, &g, &b, &zper);
+    const int nb = (int)(g.x * g.y * g.z);
+    const double* hh = H->nod[0].h;
+    k_nod_rhs<<<g, b, 0, s>>>(L, 1.0 / (4.0 * hh[0]), 1.0 / (4.0 * hh[1]), 1.0 / (4.0 * hh[2]), H->nod[0].phi2, u, v, w, S,
+                              H->part_sum, H->part_max, zper);
+    LAUNCHED(H);
+    int rc;
+    if ((rc = nod_fold(H, nb, 0, s)) != 0) return rc;
+    if (H->singular) {                             // N5: remove the uniform volumetric source m = sum / cells
+        CUDA_OK(cudaMemcpyAsync(H->scal + 2, H->scal, sizeof(double), cudaMemcpyDeviceToDevice, s));
+        k_nod_shift<true, false><<<g, b, 0, s>>>(L, L.rhs, H->scal + 2, 1.0 / (double)H->nod[0].ncell, H->part_sum, H->part_max, zper);
+        LAUNCHED(H);
+        if ((rc = nod_fold(H, nb, 0, s)) != 0) return rc;
+    } else {
+        CUDA_OK(cudaMemsetAsync(H->scal + 2, 0, sizeof(double), s));
+    }
+    return MAESTRO_MAC_OK;
+}
+
+// One Jacobi sweep on level l (phi -> phi2, then the roles swap unless swap == false).  norm_parts != NULL: the sweep
+// also leaves block maxima of |rhs - L phi_in| in part_max and their count in *norm_parts.
+int nod_do_jacobi(maestro_mac_handle* H, int l, cudaStream_t s, int* norm_parts = nullptr, bool swap = true)
+{
+    const NodLevel L = dev_nod(H, l);
+    dim3 g, b;
+    int zper;
+    nod_dims_red(L.nx + 1, L.ny + 1, L.nz + 1, &g, &b, &zper);
+    if (norm_parts) {
+        *norm_parts = (int)(g.x * g.y * g.z);
+        k_nod_jacobi<true><<<g, b, 0, s>>>(L, L.phi, L.phi2, H->part_max, zper);
+    } else
+        k_nod_jacobi<false><<<g, b, 0, s>>>(L, L.phi, L.phi2, nullptr, zper);
+    LAUNCHED(H);
+    if (swap) { double* t = H->nod[l].phi; H->nod[l].phi = H->nod[l].phi2; H->nod[l].phi2 = t; }
+    return MAESTRO_MAC_OK;
+}
+
+int nod_do_smooth(maestro_mac_handle* H, int l, int nsweeps, cudaStream_t s)
+{
+    for (int q = 0; q < nsweeps; ++q) {
+        const int rc = nod_do_jacobi(H, l, s);
+        if (rc != 0) return rc;
+    }
+    return MAESTRO_MAC_OK;
+}
+
+// rhs[l+1] = (1/8) P^T (rhs[l] - L phi[l]), phi[l+1] = 0; the residual passes through phi2[l]
+int nod_do_residual_restrict(maestro_mac_handle* H, int l, cudaStream_t s)
+{
+    const NodLevel F = dev_nod(H, l), C = dev_nod(H, l + 1);
+    dim3 g, b;
+    int zper;
+    nod_dims_red(F.nx + 1, F.ny + 1, F.nz + 1, &g, &b, &zper);
+    k_nod_residual<<<g, b, 0, s>>>(F, F.phi, F.phi2, H->part_sum, H->part_max, zper);
+    LAUNCHED(H);
+    nod_dims(C.nx + 1, C.ny + 1, C.nz + 1, &g, &b);
+    k_nod_restrict<<<g, b, 0, s>>>(F, C, F.phi2);
+    LAUNCHED(H);
+    return MAESTRO_MAC_OK;
+}
+
+int nod_do_prolong(maestro_mac_handle* H, int l, cudaStream_t s)
+{
+    const NodLevel F = dev_nod(H, l);
+    dim3 g, b;
+    nod_dims(F.nx + 1, F.ny + 1, F.nz + 1, &g, &b);
+    k_nod_prolong_add<<<g, b, 0, s>>>(F, dev_nod(H, l + 1));
+    LAUNCHED(H);
+    return MAESTRO_MAC_OK;
+}
+
+int nod_do_bottom(maestro_mac_handle* H, cudaStream_t s)
+{
+    const int l = H->nlev - 1;
+    const int nb = (int)H->nod[l].nnode;
+    const int threads = nb >= 1024 ? 1024 : ((nb + 31) / 32) * 32;
+    k_nod_bottom<<<1, threads, 0, s>>>(dev_nod(H, l), H->nod_vecs, H->d.bottom_max_iter, H->d.bottom_rel_tol, H->singular, H->flags + 1);
+    LAUNCHED(H);
+    return MAESTRO_MAC_OK;
+}
+
+int nod_do_vcycle(maestro_mac_handle* H, cudaStream_t s, int pre_done = 0)
+{
+    int rc;
+    const int last = H->nlev - 1;
+    for (int l = 0; l < last; ++l) {
+        if ((rc = nod_do_smooth(H, l, H->d.nu_pre - (l == 0 ? pre_done : 0), s)) != 0) return rc;
+        if ((rc = nod_do_residual_restrict(H, l, s)) != 0) return rc;
+    }
+    if ((rc = nod_do_bottom(H, s)) != 0) return rc;
+    for (int l = last - 1; l >= 0; --l) {
+        if ((rc = nod_do_prolong(H, l, s)) != 0) return rc;
+        if ((rc = nod_do_smooth(H, l, H->d.nu_post, s)) != 0) return rc;
+    }
+    return MAESTRO_MAC_OK;
+}
+
+// max |rhs - L phi| over the unknowns of level l into scal[4]
+int nod_do_residual_norm(maestro_mac_handle* H, int l, cudaStream_t s)
+{
+    const NodLevel L = dev_nod(H, l);
+    dim3 g, b;
+    int zper;
+    nod_dims_red(L.nx + 1, L.ny + 1, L.nz + 1, &g, &b, &zper);
+    k_nod_residual<<<g, b, 0, s>>>(L, L.phi, nullptr, H->part_sum, H->part_max, zper);
+    LAUNCHED(H);
+    return nod_fold(H, (int)(g.x * g.y * g.z), 3, s);
+}
+
+int nod_do_correct(maestro_mac_handle* H, const double* phi, const double* rho0, const double* rho, double* u, double* v,
+                   double* w, cudaStream_t s)
+{
+    const NodLevel L = dev_nod(H, 0);
+    dim3 g, b;
+    nod_dims(L.nx, L.ny, L.nz, &g, &b);
+    const double* hh = H->nod[0].h;
+    k_nod_correct<<<g, b, 0, s>>>(L, dev_geo(H), 1.0 / (4.0 * hh[0]), 1.0 / (4.0 * hh[1]), 1.0 / (4.0 * hh[2]), phi, rho, rho0, u, v, w);
+    LAUNCHED(H);
+    return MAESTRO_MAC_OK;
+}
+
+}  // namespace
+
+extern "C" int maestro_mac_nodal_project(maestro_mac_handle* H, const double* beta0, const double* rho0, const double* rho,
+                                         double* uc, double* vc, double* wc, const double* S, double* phi,
+                                         maestro_mac_stats* stats, void* cuda_stream)
+{
+    if (!H || !H->has_nodal || !beta0 || !uc || !vc || !wc || (!rho && !rho0)) return MAESTRO_MAC_ERR_ARG;
+    if (uc == vc || uc == wc || vc == wc || (phi && (phi == uc || phi == vc || phi == wc || phi == rho || phi == S)))
+        return MAESTRO_MAC_ERR_ARG;
+    cudaStream_t s = (cudaStream_t)cuda_stream;
+    const maestro_mac_desc& d = H->d;
+    maestro_mac_stats st;
+    std::memset(&st, 0, sizeof(st));
+    st.singular = H->singular;
+    st.levels = H->nlev;
+    H->launches = 0;
+    H->sm_used = H->sm_launches = H->sm_sweeps = 0;
+    H->deferred = 0;
+    int rc, result = MAESTRO_MAC_OK;
+    NodHost& N0 = H->nod[0];
+
+    CUDA_OK(cudaEventRecord(H->ev[0], s));
+    if ((rc = nod_do_sigma(H, beta0, rho0, rho, s)) != 0) return rc;
+    if ((rc = nod_do_rhs(H, uc, vc, wc, S, s)) != 0) return rc;
+    CUDA_OK(cudaMemcpyAsync(H->host_scal, H->scal, 3 * sizeof(double), cudaMemcpyDeviceToHost, s));
+    CUDA_OK(cudaMemcpyAsync(H->host_flags, H->flags, sizeof(int), cudaMemcpyDeviceToHost, s));
+    CUDA_OK(cudaMemsetAsync(N0.phi, 0, N0.nnode * sizeof(double), s));      // N9: phi = 0
+    CUDA_OK(cudaEventRecord(H->ev[1], s));
+    CUDA_OK(cudaStreamSynchronize(s));
+    st.rhs_norm_inf = H->host_scal[1];
+    st.rhs_mean_removed = H->singular ? H->host_scal[2] / (double)N0.ncell : 0.0;
+    if (H->host_flags[0] != 0 || !std::isfinite(st.rhs_norm_inf) || !std::isfinite(H->host_scal[0])) {
+        if (stats) *stats = st;
+        return MAESTRO_MAC_ERR_NONFINITE;
+    }
+    const bool trivial = st.rhs_norm_inf == 0.0;
+    if (!trivial) {
+        result = d.rel_tol > 0.0 ? MAESTRO_MAC_NOT_CONVERGED : MAESTRO_MAC_OK;
+        if (d.rel_tol > 0.0) {
+            // the Jacobi sweep forms rhs - L phi of its input: the stop test rides on the first pre-sweep of the next cycle
+            const bool ride = d.stop_test == 0 && d.nu_pre >= 1 && H->nlev >= 2;
+            int pre_done = 0;
+            while (st.cycles < d.max_cycles) {
+                if ((rc = nod_do_vcycle(H, s, pre_done)) != 0) return rc;
+                pre_done = 0;
+                const bool spec = ride && st.cycles + 1 < d.max_cycles;
+                if (spec) {
+                    int nparts = 0;
+                    if ((rc = nod_do_jacobi(H, 0, s, &nparts, false)) != 0) return rc;
+                    if ((rc = nod_fold(H, nparts, 3, s)) != 0) return rc;
+                } else if ((rc = nod_do_residual_norm(H, 0, s)) != 0) return rc;
+                CUDA_OK(cudaMemcpyAsync(H->host_scal + 4, H->scal + 4, sizeof(double), cudaMemcpyDeviceToHost, s));
+                CUDA_OK(cudaStreamSynchronize(s));
+                st.res_norm_inf = H->host_scal[4];
+                const double rel = st.res_norm_inf / st.rhs_norm_inf;
+                if (st.cycles < 128) st.res_history[st.cycles] = rel;
+                ++st.cycles;
+                if (rel != rel) { result = MAESTRO_MAC_ERR_NONFINITE; break; }
+                if (rel <= d.rel_tol) { result = MAESTRO_MAC_OK; break; }
+                if (spec) {
+                    double* t = N0.phi; N0.phi = N0.phi2; N0.phi2 = t;
+                    pre_done = 1;
+                }
+            }
+        } else {
+            for (; st.cycles < d.max_cycles; ++st.cycles)
+                if ((rc = nod_do_vcycle(H, s)) != 0) return rc;
+        }
+    }
+    CUDA_OK(cudaEventRecord(H->ev[2], s));
+    const NodLevel L0 = dev_nod(H, 0);
+    dim3 g, b;
+    if (!trivial && result != MAESTRO_MAC_ERR_NONFINITE) {
+        if (H->singular) {                         // N5: zero w-weighted mean
+            int zper;
+            nod_dims_red(L0.nx + 1, L0.ny + 1, L0.nz + 1, &g, &b, &zper);
+            const int nb = (int)(g.x * g.y * g.z);
+            k_nod_shift<false, true><<<g, b, 0, s>>>(L0, L0.phi, nullptr, 0.0, H->part_sum, H->part_max, zper);
+            LAUNCHED(H);
+            if ((rc = nod_fold(H, nb, 6, s)) != 0) return rc;
+            k_nod_shift<false, false><<<g, b, 0, s>>>(L0, L0.phi, H->scal + 6, 1.0 / (double)N0.ncell, H->part_sum, H->part_max, zper);
+            LAUNCHED(H);
+        }
+        if ((rc = nod_do_correct(H, L0.phi, rho0, rho, uc, vc, wc, s)) != 0) return rc;
+    }
+    nod_dims(L0.nx + 1, L0.ny + 1, L0.nz + 1, &g, &b);
+    if (phi) {
+        k_nod_export<<<g, b, 0, s>>>(L0, L0.phi, phi);
+        LAUNCHED(H);
+    }
+    CUDA_OK(cudaEventRecord(H->ev[3], s));
+    CUDA_OK(cudaMemcpyAsync(H->host_flags + 1, H->flags + 1, sizeof(int), cudaMemcpyDeviceToHost, s));
+    CUDA_OK(cudaStreamSynchronize(s));
+    collect_timings(H, st);
+    if (d.rel_tol == 0.0 && !trivial) {
+        if ((rc = nod_do_residual_norm(H, 0, s)) != 0) return rc;
+        CUDA_OK(cudaMemcpyAsync(H->host_scal + 4, H->scal + 4, sizeof(double), cudaMemcpyDeviceToHost, s));
+        CUDA_OK(cudaStreamSynchronize(s));
+        st.res_norm_inf = H->host_scal[4];
+    }
+    st.gpu_launches = H->launches;
+    H->last = st;
+    if (stats) *stats = st;
+    return result;
+}
+
+// ---- step API of the nodal projection ---------------------------------------------------------------------------
+
+extern "C" int maestro_mac_nodal_level_get(maestro_mac_handle* H, int level, int which, double* dst, void* cuda_stream)
+{
+    if (!H || !H->has_nodal || !dst || level < 0 || level >= H->nlev) return MAESTRO_MAC_ERR_ARG;
+    cudaStream_t s = (cudaStream_t)cuda_stream;
+    const NodHost& N = H->nod[level];
+    if (which == MAESTRO_MAC_NODAL_SIGMA) {
+        CUDA_OK(cudaMemcpyAsync(dst, N.sigma, N.ncell * sizeof(double), cudaMemcpyDeviceToDevice, s));
+        return MAESTRO_MAC_OK;
+    }
+    if (which != MAESTRO_MAC_NODAL_PHI && which != MAESTRO_MAC_NODAL_RHS) return MAESTRO_MAC_ERR_ARG;
+    const NodLevel L = dev_nod(H, level);
+    dim3 g, b;
+    nod_dims(L.nx + 1, L.ny + 1, L.nz + 1, &g, &b);
+    if (which == MAESTRO_MAC_NODAL_PHI) {          // exported with the node rules applied
+        k_nod_export<<<g, b, 0, s>>>(L, L.phi, dst);
+        LAUNCHED(H);
+    } else
+        CUDA_OK(cudaMemcpyAsync(dst, N.rhs, N.nnode * sizeof(double), cudaMemcpyDeviceToDevice, s));
+    return MAESTRO_MAC_OK;
+}
+
+extern "C" int maestro_mac_nodal_level_set(maestro_mac_handle* H, int level, int which, const double* src, void* cuda_stream)
+{
+    if (!H || !H->has_nodal || !src || level < 0 || level >= H->nlev) return MAESTRO_MAC_ERR_ARG;
+    cudaStream_t s = (cudaStream_t)cuda_stream;
+    const NodHost& N = H->nod[level];
+    double* dst = which == MAESTRO_MAC_NODAL_PHI ? N.phi : (which == MAESTRO_MAC_NODAL_RHS ? N.rhs : (which == MAESTRO_MAC_NODAL_SIGMA ? N.sigma : nullptr));
+    if (!dst) return MAESTRO_MAC_ERR_ARG;
+    CUDA_OK(cudaMemcpyAsync(dst, src, (which == MAESTRO_MAC_NODAL_SIGMA ? N.ncell : N.nnode) * sizeof(double), cudaMemcpyDeviceToDevice, s));
+    return MAESTRO_MAC_OK;
+}
+
+extern "C" int maestro_mac_nodal_step_sigma(maestro_mac_handle* H, const double* beta0, const double* rho0, const double* rho,
+                                            void* cuda_stream)
+{
+    if (!H || !H->has_nodal || !beta0 || (!rho && !rho0)) return MAESTRO_MAC_ERR_ARG;
+    return nod_do_sigma(H, beta0, rho0, rho, (cudaStream_t)cuda_stream);
+}
+
+extern "C" int maestro_mac_nodal_step_rhs(maestro_mac_handle* H, const double* uc, const double* vc, const double* wc,
+                                          const double* S, double* rhs_norm_inf, double* mean_removed, void* cuda_stream)
+{
+    if (!H || !H->has_nodal || !uc || !vc || !wc) return MAESTRO_MAC_ERR_ARG;
+    cudaStream_t s = (cudaStream_t)cuda_stream;
+    const int rc = nod_do_rhs(H, uc, vc, wc, S, s);
+    if (rc != 0) return rc;
+    CUDA_OK(cudaMemcpyAsync(H->host_scal, H->scal, 3 * sizeof(double), cudaMemcpyDeviceToHost, s));
+    CUDA_OK(cudaStreamSynchronize(s));
+    if (rhs_norm_inf) *rhs_norm_inf = H->host_scal[1];
+    if (mean_removed) *mean_removed = H->singular ? H->host_scal[2] / (double)H->nod[0].ncell : 0.0;
+    return MAESTRO_MAC_OK;
+}
+
+extern "C" int maestro_mac_nodal_step_smooth(maestro_mac_handle* H, int level, int nsweeps, void* cuda_stream)
+{
+    if (!H || !H->has_nodal || level < 0 || level >= H->nlev || nsweeps < 0) return MAESTRO_MAC_ERR_ARG;
+    return nod_do_smooth(H, level, nsweeps, (cudaStream_t)cuda_stream);
+}
+
+extern "C" int maestro_mac_nodal_step_residual_restrict(maestro_mac_handle* H, int level, void* cuda_stream)
+{
+    if (!H || !H->has_nodal || level < 0 || level + 1 >= H->nlev) return MAESTRO_MAC_ERR_ARG;
+    return nod_do_residual_restrict(H, level, (cudaStream_t)cuda_stream);
+}
+
+extern "C" int maestro_mac_nodal_step_prolong(maestro_mac_handle* H, int level, void* cuda_stream)
+{
+    if (!H || !H->has_nodal || level < 0 || level + 1 >= H->nlev) return MAESTRO_MAC_ERR_ARG;
+    return nod_do_prolong(H, level, (cudaStream_t)cuda_stream);
+}
+
+extern "C" int maestro_mac_nodal_step_bottom(maestro_mac_handle* H, void* cuda_stream)
+{
+    if (!H || !H->has_nodal) return MAESTRO_MAC_ERR_ARG;
+    return nod_do_bottom(H, (cudaStream_t)cuda_stream);
+}
+
+extern "C" int maestro_mac_nodal_step_vcycle(maestro_mac_handle* H, void* cuda_stream)
+{
+    if (!H || !H->has_nodal) return MAESTRO_MAC_ERR_ARG;
+    return nod_do_vcycle(H, (cudaStream_t)cuda_stream);
+}
+
+extern "C" int maestro_mac_nodal_step_residual_norm(maestro_mac_handle* H, int level, double* norm_inf, void* cuda_stream)
+{
+    if (!H || !H->has_nodal || level < 0 || level >= H->nlev || !norm_inf) return MAESTRO_MAC_ERR_ARG;
+    cudaStream_t s = (cudaStream_t)cuda_stream;
+    const int rc = nod_do_residual_norm(H, level, s);
+    if (rc != 0) return rc;
+    CUDA_OK(cudaMemcpyAsync(H->host_scal + 4, H->scal + 4, sizeof(double), cudaMemcpyDeviceToHost, s));
+    CUDA_OK(cudaStreamSynchronize(s));
+    *norm_inf = H->host_scal[4];
+    return MAESTRO_MAC_OK;
+}
+
+extern "C" int maestro_mac_nodal_step_correct(maestro_mac_handle* H, const double* rho0, const double* rho, double* uc,
+                                              double* vc, double* wc, void* cuda_stream)
+{
+    if (!H || !H->has_nodal || !uc || !vc || !wc || (!rho && !rho0)) return MAESTRO_MAC_ERR_ARG;
+    return nod_do_correct(H, H->nod[0].phi, rho0, rho, uc, vc, wc, (cudaStream_t)cuda_stream);
+}

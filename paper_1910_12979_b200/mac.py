@@ -27,7 +27,12 @@ EXPORTS = [
     "maestro_mac_step_vcycle", "maestro_mac_step_residual_norm", "maestro_mac_step_correct",
     "maestro_mac_base_state", "maestro_mac_set_dpdt_term", "maestro_mac_lateral_average",
     "maestro_mac_status", "maestro_mac_level_plan",
+    "maestro_mac_nodal_project", "maestro_mac_nodal_level_get", "maestro_mac_nodal_level_set",
+    "maestro_mac_nodal_step_sigma", "maestro_mac_nodal_step_rhs", "maestro_mac_nodal_step_smooth",
+    "maestro_mac_nodal_step_residual_restrict", "maestro_mac_nodal_step_prolong", "maestro_mac_nodal_step_bottom",
+    "maestro_mac_nodal_step_vcycle", "maestro_mac_nodal_step_residual_norm", "maestro_mac_nodal_step_correct",
 ]
+NODAL_PHI, NODAL_RHS, NODAL_SIGMA = 0, 1, 2
 
 
 class Desc(C.Structure):
@@ -38,7 +43,7 @@ class Desc(C.Structure):
                 ("max_cycles", C.c_int), ("rel_tol", C.c_double), ("coarsest_n", C.c_int),
                 ("bottom_max_iter", C.c_int), ("bottom_rel_tol", C.c_double),
                 ("prolongation", C.c_int), ("host_staging", C.c_int), ("smoother", C.c_int),
-                ("stop_test", C.c_int), ("rho_mean", C.c_int), ("timing", C.c_int)]
+                ("stop_test", C.c_int), ("rho_mean", C.c_int), ("timing", C.c_int), ("nodal", C.c_int)]
 
 
 class Stats(C.Structure):
@@ -98,6 +103,18 @@ def lib():
         L.maestro_mac_lateral_average.argtypes = [_VP, _VP, _VP, _VP]
         L.maestro_mac_status.argtypes = [_VP, C.POINTER(Stats), _VP]
         L.maestro_mac_level_plan.argtypes = [_VP, C.c_int, C.POINTER(C.c_int * 8)]
+        L.maestro_mac_nodal_project.argtypes = proj
+        L.maestro_mac_nodal_level_get.argtypes = [_VP, C.c_int, C.c_int, _VP, _VP]
+        L.maestro_mac_nodal_level_set.argtypes = [_VP, C.c_int, C.c_int, _VP, _VP]
+        L.maestro_mac_nodal_step_sigma.argtypes = [_VP, _VP, _VP, _VP, _VP]
+        L.maestro_mac_nodal_step_rhs.argtypes = [_VP, _VP, _VP, _VP, _VP, C.POINTER(C.c_double), C.POINTER(C.c_double), _VP]
+        L.maestro_mac_nodal_step_smooth.argtypes = [_VP, C.c_int, C.c_int, _VP]
+        L.maestro_mac_nodal_step_residual_restrict.argtypes = [_VP, C.c_int, _VP]
+        L.maestro_mac_nodal_step_prolong.argtypes = [_VP, C.c_int, _VP]
+        L.maestro_mac_nodal_step_bottom.argtypes = [_VP, _VP]
+        L.maestro_mac_nodal_step_vcycle.argtypes = [_VP, _VP]
+        L.maestro_mac_nodal_step_residual_norm.argtypes = [_VP, C.c_int, C.POINTER(C.c_double), _VP]
+        L.maestro_mac_nodal_step_correct.argtypes = [_VP, _VP, _VP, _VP, _VP, _VP, _VP]
         for name in EXPORTS:
             if name != "maestro_mac_default_desc":
                 getattr(L, name).restype = C.c_int
@@ -114,7 +131,7 @@ class MacError(RuntimeError):
 def make_desc(n, dx, bc_lo, bc_hi, geometry=PLANAR, nr=None, dr=None, center=(0.0, 0.0, 0.0),
               nu_pre=2, nu_post=2, max_cycles=100, rel_tol=1e-10, coarsest_n=4,
               bottom_max_iter=100, bottom_rel_tol=1e-8, prolongation=0, host_staging=0,
-              smoother=0, stop_test=0, rho_mean=0, timing=0) -> Desc:
+              smoother=0, stop_test=0, rho_mean=0, timing=0, nodal=0) -> Desc:
     d = Desc()
     lib().maestro_mac_default_desc(C.byref(d))
     d.nx, d.ny, d.nz = (int(x) for x in n)
@@ -129,6 +146,7 @@ def make_desc(n, dx, bc_lo, bc_hi, geometry=PLANAR, nr=None, dr=None, center=(0.
     d.stop_test = int(stop_test)
     d.rho_mean = int(rho_mean)
     d.timing = int(timing)
+    d.nodal = int(nodal)
     return d
 
 
@@ -295,6 +313,61 @@ class MacProjector:
         """Register (or clear, q = None) the profile (1/(Gamma1bar p0)) dp0/dt of PAPER.md:49 Eq. 6."""
         self._dpdt_keepalive = q
         self._ck(lib().maestro_mac_set_dpdt_term(self._h, _ptr(q)), "set_dpdt_term")
+
+    # ---- nodal (end-of-step) projection: desc.nodal = 1 ----------------------------------------
+    def nodal_project(self, beta0, rho0, rho, uc, vc, wc, S=None, phi=None, want_stats=True):
+        """Device tensors; uc, vc, wc (CELL arrays) corrected in place; phi: node array or None."""
+        st = Stats()
+        rc = lib().maestro_mac_nodal_project(self._h, _ptr(beta0), _ptr(rho0), _ptr(rho), _ptr(uc), _ptr(vc), _ptr(wc),
+                                             _ptr(S), _ptr(phi), C.byref(st) if want_stats else None, _stream())
+        return rc, (st.as_dict() if want_stats else None)
+
+    def nodal_shape(self, level, which):
+        (nx, ny, nz), _ = self.level_dims(level)
+        return (nz, ny, nx) if which == NODAL_SIGMA else (nz + 1, ny + 1, nx + 1)
+
+    def nodal_get(self, level, which):
+        import torch
+        out = torch.empty(self.nodal_shape(level, which), dtype=torch.float64, device=self.device)
+        self._ck(lib().maestro_mac_nodal_level_get(self._h, level, which, _ptr(out), _stream()), "nodal_level_get")
+        return out
+
+    def nodal_set(self, level, which, src):
+        assert tuple(src.shape) == self.nodal_shape(level, which)
+        self._ck(lib().maestro_mac_nodal_level_set(self._h, level, which, _ptr(src), _stream()), "nodal_level_set")
+
+    def nodal_step_sigma(self, beta0, rho0, rho):
+        self._ck(lib().maestro_mac_nodal_step_sigma(self._h, _ptr(beta0), _ptr(rho0), _ptr(rho), _stream()), "nodal_step_sigma")
+
+    def nodal_step_rhs(self, uc, vc, wc, S=None):
+        nrm, mean = C.c_double(0), C.c_double(0)
+        self._ck(lib().maestro_mac_nodal_step_rhs(self._h, _ptr(uc), _ptr(vc), _ptr(wc), _ptr(S), C.byref(nrm), C.byref(mean),
+                                                  _stream()), "nodal_step_rhs")
+        return nrm.value, mean.value
+
+    def nodal_step_smooth(self, level, nsweeps=1):
+        self._ck(lib().maestro_mac_nodal_step_smooth(self._h, level, nsweeps, _stream()), "nodal_step_smooth")
+
+    def nodal_step_residual_restrict(self, level):
+        self._ck(lib().maestro_mac_nodal_step_residual_restrict(self._h, level, _stream()), "nodal_step_residual_restrict")
+
+    def nodal_step_prolong(self, level):
+        self._ck(lib().maestro_mac_nodal_step_prolong(self._h, level, _stream()), "nodal_step_prolong")
+
+    def nodal_step_bottom(self):
+        self._ck(lib().maestro_mac_nodal_step_bottom(self._h, _stream()), "nodal_step_bottom")
+
+    def nodal_step_vcycle(self):
+        self._ck(lib().maestro_mac_nodal_step_vcycle(self._h, _stream()), "nodal_step_vcycle")
+
+    def nodal_step_residual_norm(self, level=0):
+        nrm = C.c_double(0)
+        self._ck(lib().maestro_mac_nodal_step_residual_norm(self._h, level, C.byref(nrm), _stream()), "nodal_step_residual_norm")
+        return nrm.value
+
+    def nodal_step_correct(self, rho0, rho, uc, vc, wc):
+        self._ck(lib().maestro_mac_nodal_step_correct(self._h, _ptr(rho0), _ptr(rho), _ptr(uc), _ptr(vc), _ptr(wc), _stream()),
+                 "nodal_step_correct")
 
     def step_correct(self, rho0, rho, u, v, w):
         self._ck(lib().maestro_mac_step_correct(self._h, _ptr(rho0), _ptr(rho), _ptr(u), _ptr(v), _ptr(w), _stream()), "step_correct")
