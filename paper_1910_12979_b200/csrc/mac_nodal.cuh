@@ -2,21 +2,28 @@
 // "second order projection method ... multigrid linear solvers for the pressure projection steps"; weighting
 // beta0/rho of PAPER.md:35 Eq. 2, constraint of PAPER.md:49 Eq. 6).  Readings N1..N10 of DESIGN.md.
 //
-// phi lives on the nodes, (nx+1)(ny+1)(nz+1) values (idx = i + (nx+1)(j + (ny+1)k)); sigma = beta0/rho, the
-// velocities, rho and S are cell arrays in the public cell layout (idx = i + nx (j + ny k), no ghosts).
-// Operator: the trilinear (Q1) finite-element form of div(sigma grad phi) divided by the cell volume,
+// phi lives on the nodes, sigma = beta0/rho on the cells; the velocities, rho and S are cell arrays in the public cell
+// layout (idx = i + nx (j + ny k)).  Operator: the trilinear (Q1) finite-element form of div(sigma grad phi) divided by
+// the cell volume,
 //     (L phi)_a = -sum_c sigma_c sum_b (K^c_ab / V) phi_b
-// over the up to 8 cells c around node a and their 8 corners b.  K^c_ab / V depends only on whether b is the
-// same corner as a or the other one along each axis (8 classes): w[cls] = sum_d g_d k_d prod_{e != d} m_e,
-// g_d = 1/h_d^2, k = +1 same / -1 other, m = 1/3 same / 1/6 other.  A neighbour node b at offset (dx, dy, dz)
-// in {-1,0,1}^3 therefore enters with  -w[cls(dx,dy,dz)] * T(dx,dy,dz),  T = the sum of sigma over the cells
-// that contain both a and b: 19 additions expand the 8 sigmas to the 27 sums, 27 + 8 fused multiply-adds form
-// L phi.  Node rules (N4): OUTFLOW nodes count as 0 and are not unknowns; on a periodic axis node n is node 0
-// (the arrays keep n+1 entries; the kernels never read entry n and write it only when the result is exported);
-// cells outside a non-periodic boundary do not exist (sigma := 0).
-// Smoother: Jacobi (order-free: reproducible, one HBM pass per sweep, 32 B per node: sigma, phi, rhs in, phi out),
-// ping-pong between phi and phi2; the sweep can emit max |rhs - L phi_in|, so the stop test of a cycle rides on the
-// first pre-smoothing sweep of the next one at no extra pass.
+// over the up to 8 cells c around node a and their 8 corners b.  K^c_ab / V depends only on whether b is the same
+// corner as a or the other one along each axis (8 classes): w[cls] = sum_d g_d k_d prod_{e != d} m_e, g_d = 1/h_d^2,
+// k = +1 same / -1 other, m = 1/3 same / 1/6 other.  A neighbour node b at offset (dx, dy, dz) in {-1,0,1}^3 therefore
+// enters with  -w[cls(dx,dy,dz)] * T(dx,dy,dz),  T = the sum of sigma over the cells that contain both a and b.
+//
+// Internal layout of a level (x fastest; pointers address the interior origin, index 0):
+//   node arrays phi, phi2, rhs : idx = i + NX (j + NY k),  NX = nx + 3, NY = ny + 3, i in [-1, nx + 1]  (one ghost node per side)
+//   sigma (cells)              : idx = i + CX (j + CY k),  CX = nx + 2, CY = ny + 2, i in [-1, nx]      (one ghost cell per side)
+// Node rules (N4) expressed in that layout, so that the operator needs no boundary branches:
+//   * a cell outside a non-periodic boundary has sigma = 0 (its ghost entry): the terms of cells that do not exist vanish
+//     whatever (finite) value the ghost nodes hold; on periodic axes ghost cells and ghost nodes hold periodic images;
+//   * OUTFLOW nodes hold 0 and are not unknowns; on a periodic axis node n is the image of node 0 and not an unknown.
+// The z-marching operator pass (k_nod_march) relies on the ghosts of its input: every kernel whose phi output a later
+// pass reads writes the images as well (Jacobi output, prolongation), level_set fills them (k_nod_phi_ghosts).
+// Everything else reads through the rules (nod_val, nod_operator_generic) and ignores the ghosts.
+// Smoother: Jacobi (order-free: reproducible; one HBM pass per sweep, 32 B per node: sigma, phi, rhs in, phi out),
+// ping-pong between phi and phi2; the sweep can emit max |rhs - L phi_in|, so the stop test of a cycle rides on the first
+// pre-smoothing sweep of the next one at no extra pass.
 #pragma once
 #include "mac_kernels.cuh"
 
@@ -25,17 +32,21 @@ struct NodLevel {
     int bclo[3], bchi[3];
     double w[8];                    // class weights; bit 0 / 1 / 2: the other corner along x / y / z
     double omega;                   // Jacobi damping (N7)
-    double *phi, *phi2, *rhs;       // node arrays
-    double *sigma;                  // cell array
+    double *phi, *phi2, *rhs;       // node arrays (interior origin)
+    double *sigma;                  // cell array (interior origin)
 };
 
-__device__ __forceinline__ size_t nod_idx(const NodLevel& L, int i, int j, int k)
+__device__ __forceinline__ long long nod_idx(const NodLevel& L, int i, int j, int k)
 {
-    return (size_t)((long long)i + (long long)(L.nx + 1) * ((long long)j + (long long)(L.ny + 1) * (long long)k));
+    return (long long)i + (long long)(L.nx + 3) * ((long long)j + (long long)(L.ny + 3) * (long long)k);
 }
-__device__ __forceinline__ size_t nod_cidx(const NodLevel& L, int i, int j, int k)
+__device__ __forceinline__ long long nod_cidx(const NodLevel& L, int i, int j, int k)
 {
-    return (size_t)((long long)i + (long long)L.nx * ((long long)j + (long long)L.ny * (long long)k));
+    return (long long)i + (long long)(L.nx + 2) * ((long long)j + (long long)(L.ny + 2) * (long long)k);
+}
+__device__ __forceinline__ size_t pub_cidx(const NodLevel& L, int i, int j, int k)      // public cell layout
+{
+    return (size_t)i + (size_t)L.nx * ((size_t)j + (size_t)L.ny * (size_t)k);
 }
 
 // kind of node index t along axis d (N4): 0 unknown, 1 OUTFLOW node, 2 periodic duplicate
@@ -53,9 +64,44 @@ __device__ __forceinline__ int nod_kind(const NodLevel& L, int i, int j, int k)
     if (a == 1 || b == 1 || c == 1) return 1;
     return (a == 2 || b == 2 || c == 2) ? 2 : 0;
 }
+// offset (in index units along the axis) of the periodic image of unknown node t that the ghost layout stores: node 0
+// is also node n, node 1 also node n + 1, node n - 1 also node -1; 0 = none.  (Levels that are smoothed have n >= 4.)
+__device__ __forceinline__ int nod_image(const NodLevel& L, int d, int t)
+{
+    const int n = d == 0 ? L.nx : (d == 1 ? L.ny : L.nz);
+    if (L.bclo[d] != MAC_PERIODIC) return 0;
+    return t <= 1 ? n : (t == n - 1 ? -n : 0);
+}
+// store v at node q of array a and at its periodic images (ix, iy, iz: image offsets along the axes, 0 = none)
+__device__ __forceinline__ void nod_store_images(const NodLevel& L, double* __restrict__ a, long long q, double v, int ix,
+                                                 int iy, int iz)
+{
+    a[q] = v;
+    if (ix | iy | iz) {
+        const long long sy = L.nx + 3, sz = sy * (L.ny + 3);
+        const long long ox = ix, oy = (long long)iy * sy, oz = (long long)iz * sz;
+        if (ix) a[q + ox] = v;
+        if (iy) { a[q + oy] = v; if (ix) a[q + ox + oy] = v; }
+        if (iz) {
+            a[q + oz] = v;
+            if (ix) a[q + ox + oz] = v;
+            if (iy) { a[q + oy + oz] = v; if (ix) a[q + ox + oy + oz] = v; }
+        }
+    }
+}
 
-// One axis of the 27-point neighbourhood of an unknown node t: stored indices of the nodes t-1, t, t+1 (-1: the
-// value counts as 0: no such node, or an OUTFLOW node) and of the cells t-1, t (-1: no such cell).
+// value of a nodal array at node (I, J, K), 0 <= index <= n, under the node rules (OUTFLOW 0, periodic node n = node 0)
+__device__ __forceinline__ double nod_val(const NodLevel& L, const double* __restrict__ a, int I, int J, int K)
+{
+    if (nod_kind(L, I, J, K) == 1) return 0.0;
+    if (L.bclo[0] == MAC_PERIODIC && I == L.nx) I = 0;
+    if (L.bclo[1] == MAC_PERIODIC && J == L.ny) J = 0;
+    if (L.bclo[2] == MAC_PERIODIC && K == L.nz) K = 0;
+    return a[nod_idx(L, I, J, K)];
+}
+
+// One axis of the 27-point neighbourhood of an unknown node t: stored indices of the nodes t-1, t, t+1 (-2: the value
+// counts as 0: no such node, or an OUTFLOW node) and of the cells t-1, t (-2: no such cell).
 struct NodAxis { int nd[3]; int cl[2]; };
 __device__ __forceinline__ NodAxis nod_axis(const NodLevel& L, int d, int t)
 {
@@ -63,62 +109,41 @@ __device__ __forceinline__ NodAxis nod_axis(const NodLevel& L, int d, int t)
     const bool per = L.bclo[d] == MAC_PERIODIC;
     NodAxis A;
     A.nd[1] = t;
-    A.nd[0] = t > 0 ? t - 1 : (per ? n - 1 : -1);
-    A.nd[2] = t < n ? (t + 1 == n && per ? 0 : t + 1) : -1;
-    A.cl[0] = t > 0 ? t - 1 : (per ? n - 1 : -1);
-    A.cl[1] = t < n ? t : -1;
+    A.nd[0] = t > 0 ? t - 1 : (per ? n - 1 : -2);
+    A.nd[2] = t < n ? (t + 1 == n && per ? 0 : t + 1) : -2;
+    A.cl[0] = t > 0 ? t - 1 : (per ? n - 1 : -2);
+    A.cl[1] = t < n ? t : -2;
     if (!per) {                                       // OUTFLOW nodes count as 0
-        if (A.nd[0] == 0 && L.bclo[d] == MAC_OUTFLOW) A.nd[0] = -1;
-        if (A.nd[2] == n && L.bchi[d] == MAC_OUTFLOW) A.nd[2] = -1;
+        if (A.nd[0] == 0 && L.bclo[d] == MAC_OUTFLOW) A.nd[0] = -2;
+        if (A.nd[2] == n && L.bchi[d] == MAC_OUTFLOW) A.nd[2] = -2;
     }
     return A;
 }
 
-// L phi and the diagonal at the unknown node (i, j, k).  FAST: every neighbour node and cell exists and none is an
-// OUTFLOW node (all but a surface layer of nodes): plain strided loads.
-template <bool FAST>
-__device__ __forceinline__ void nod_operator(const NodLevel& L, const double* __restrict__ phi, int i, int j, int k,
-                                             double& lphi, double& diag)
+// L phi at the unknown node (i, j, k) through the node rules, one node at a time: the form that does not rely on
+// ghost entries (bottom solver).
+__device__ __forceinline__ double nod_operator_generic(const NodLevel& L, const double* __restrict__ phi, int i, int j, int k)
 {
     double p[3][3][3], s[2][2][2];
-    if (FAST) {
-        const long long px = 1, py = L.nx + 1, pz = (long long)(L.nx + 1) * (L.ny + 1);
-        const double* q = phi + nod_idx(L, i, j, k);
+    const NodAxis X = nod_axis(L, 0, i), Y = nod_axis(L, 1, j), Z = nod_axis(L, 2, k);
 #pragma unroll
-        for (int c = 0; c < 3; ++c)
+    for (int c = 0; c < 3; ++c)
 #pragma unroll
-            for (int b = 0; b < 3; ++b)
+        for (int b = 0; b < 3; ++b)
 #pragma unroll
-                for (int a = 0; a < 3; ++a) p[c][b][a] = q[(a - 1) * px + (b - 1) * py + (c - 1) * pz];
-        const long long cy = L.nx, cz = (long long)L.nx * L.ny;
-        const double* sg = L.sigma + nod_cidx(L, i - 1, j - 1, k - 1);
+            for (int a = 0; a < 3; ++a) {
+                const bool ok = X.nd[a] >= 0 && Y.nd[b] >= 0 && Z.nd[c] >= 0;
+                p[c][b][a] = ok ? phi[nod_idx(L, X.nd[a], Y.nd[b], Z.nd[c])] : 0.0;
+            }
 #pragma unroll
-        for (int c = 0; c < 2; ++c)
+    for (int c = 0; c < 2; ++c)
 #pragma unroll
-            for (int b = 0; b < 2; ++b)
+        for (int b = 0; b < 2; ++b)
 #pragma unroll
-                for (int a = 0; a < 2; ++a) s[c][b][a] = __ldg(sg + a + b * cy + c * cz);
-    } else {
-        const NodAxis X = nod_axis(L, 0, i), Y = nod_axis(L, 1, j), Z = nod_axis(L, 2, k);
-#pragma unroll
-        for (int c = 0; c < 3; ++c)
-#pragma unroll
-            for (int b = 0; b < 3; ++b)
-#pragma unroll
-                for (int a = 0; a < 3; ++a) {
-                    const bool ok = X.nd[a] >= 0 && Y.nd[b] >= 0 && Z.nd[c] >= 0;
-                    p[c][b][a] = ok ? phi[nod_idx(L, X.nd[a], Y.nd[b], Z.nd[c])] : 0.0;
-                }
-#pragma unroll
-        for (int c = 0; c < 2; ++c)
-#pragma unroll
-            for (int b = 0; b < 2; ++b)
-#pragma unroll
-                for (int a = 0; a < 2; ++a) {
-                    const bool ok = X.cl[a] >= 0 && Y.cl[b] >= 0 && Z.cl[c] >= 0;
-                    s[c][b][a] = ok ? __ldg(L.sigma + nod_cidx(L, X.cl[a], Y.cl[b], Z.cl[c])) : 0.0;
-                }
-    }
+            for (int a = 0; a < 2; ++a) {
+                const bool ok = X.cl[a] >= 0 && Y.cl[b] >= 0 && Z.cl[c] >= 0;
+                s[c][b][a] = ok ? __ldg(L.sigma + nod_cidx(L, X.cl[a], Y.cl[b], Z.cl[c])) : 0.0;
+            }
     // T(dx,dy,dz): sigma summed over the cells that contain the node and its neighbour: expand x, then y, then z
     double tx[2][2][3], ty[2][3][3], t[3][3][3];
 #pragma unroll
@@ -146,28 +171,73 @@ __device__ __forceinline__ void nod_operator(const NodLevel& L, const double* __
     double sum = 0.0;
 #pragma unroll
     for (int q = 7; q >= 0; --q) sum = fma(L.w[q], acc[q], sum);
-    lphi = -sum;
-    diag = -(L.w[0] * t[1][1][1]);
+    return -sum;
 }
 
-__device__ __forceinline__ bool nod_fast(const NodLevel& L, int i, int j, int k)
-{
-    return i >= 2 && i <= L.nx - 2 && j >= 2 && j <= L.ny - 2 && k >= 2 && k <= L.nz - 2;
-}
-
-// ---- N3: sigma = beta0(r_cell) / rho, beta0 at the cell centres (bcell, scratch for the rhs), rho check ------
+// ---- ghosts -----------------------------------------------------------------------------------------------------
+// sigma ghost cells: periodic images, 0 outside a non-periodic boundary.  One thread per cell of the extended array.
 __global__ void __launch_bounds__(256)
-k_nod_sigma(GeoDev G, const double* __restrict__ beta0, const double* __restrict__ rho, const double* __restrict__ rho0,
-            double* __restrict__ sigma, double* __restrict__ bcell, int* __restrict__ flags)
+k_nod_sig_ghosts(NodLevel L)
+{
+    const int i = (int)(blockIdx.x * blockDim.x + threadIdx.x) - 1, j = (int)(blockIdx.y * blockDim.y + threadIdx.y) - 1,
+              k = (int)blockIdx.z - 1;
+    if (i > L.nx || j > L.ny) return;
+    const bool gi = i < 0 || i >= L.nx, gj = j < 0 || j >= L.ny, gk = k < 0 || k >= L.nz;
+    if (!(gi || gj || gk)) return;
+    const bool zero = (gi && L.bclo[0] != MAC_PERIODIC) || (gj && L.bclo[1] != MAC_PERIODIC) || (gk && L.bclo[2] != MAC_PERIODIC);
+    const int si = gi ? (i < 0 ? i + L.nx : i - L.nx) : i, sj = gj ? (j < 0 ? j + L.ny : j - L.ny) : j,
+              sk = gk ? (k < 0 ? k + L.nz : k - L.nz) : k;
+    L.sigma[nod_cidx(L, i, j, k)] = zero ? 0.0 : L.sigma[nod_cidx(L, si, sj, sk)];
+}
+
+// nodal array a: OUTFLOW nodes := 0, periodic images (nodes -1, n, n+1) := their source, ghosts outside a non-periodic
+// boundary := 0.  One thread per node of the extended array.
+__global__ void __launch_bounds__(256)
+k_nod_phi_ghosts(NodLevel L, double* __restrict__ a)
+{
+    const int i = (int)(blockIdx.x * blockDim.x + threadIdx.x) - 1, j = (int)(blockIdx.y * blockDim.y + threadIdx.y) - 1,
+              k = (int)blockIdx.z - 1;
+    if (i > L.nx + 1 || j > L.ny + 1) return;
+    int id[3] = {i, j, k};
+    bool zero = false, moved = false;
+#pragma unroll
+    for (int d = 0; d < 3; ++d) {
+        const int n = d == 0 ? L.nx : (d == 1 ? L.ny : L.nz), t = id[d];
+        if (L.bclo[d] == MAC_PERIODIC) {
+            if (t < 0) { id[d] = t + n; moved = true; } else if (t >= n) { id[d] = t - n; moved = true; }
+        } else if (t < 0 || t > n || nod_axis_kind(L, d, t) == 1) zero = true;
+    }
+    if (zero) a[nod_idx(L, i, j, k)] = 0.0;
+    else if (moved) a[nod_idx(L, i, j, k)] = a[nod_idx(L, id[0], id[1], id[2])];
+}
+
+// internal <-> public layout of a level array (step API).  node: (nx+1)(ny+1)(nz+1) values, else cells.  to_public
+// with rules applies the node rules to a nodal array (OUTFLOW 0, periodic entry n = entry 0).
+__global__ void __launch_bounds__(256)
+k_nod_copy(NodLevel L, double* __restrict__ internal, double* __restrict__ pub, int node, int to_public, int rules)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y * blockDim.y + threadIdx.y, k = blockIdx.z;
+    const int ex = L.nx + node, ey = L.ny + node;
+    if (i >= ex || j >= ey) return;
+    const size_t p = (size_t)i + (size_t)ex * ((size_t)j + (size_t)ey * (size_t)k);
+    const long long q = node ? nod_idx(L, i, j, k) : nod_cidx(L, i, j, k);
+    if (to_public) pub[p] = (node && rules) ? nod_val(L, internal, i, j, k) : internal[q];
+    else internal[q] = pub[p];
+}
+
+// ---- N3: sigma = beta0(r_cell) / rho, beta0 at the cell centres (bcell, public cell layout, scratch for the rhs) ---
+__global__ void __launch_bounds__(256)
+k_nod_sigma(GeoDev G, NodLevel L, const double* __restrict__ beta0, const double* __restrict__ rho,
+            const double* __restrict__ rho0, double* __restrict__ bcell, int* __restrict__ flags)
 {
     const int i = blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y * blockDim.y + threadIdx.y, k = blockIdx.z;
     if (i >= G.nx || j >= G.ny) return;
-    const size_t c = (size_t)i + (size_t)G.nx * ((size_t)j + (size_t)G.ny * k);
+    const size_t c = pub_cidx(L, i, j, k);
     const double r = radius(G, (i + 0.5) * G.dx, (j + 0.5) * G.dy, (k + 0.5) * G.dz);
     const double b = profile_eval(beta0, G.nr, G.dr, r);
     const double rh = rho ? __ldg(rho + c) : profile_eval(rho0, G.nr, G.dr, r);
     if (!(rh > 0.0) || !(rh <= 1.79769313486231570e308)) atomicOr(flags, 1);
-    sigma[c] = b / rh;
+    L.sigma[nod_cidx(L, i, j, k)] = b / rh;
     bcell[c] = b;
 }
 
@@ -197,28 +267,28 @@ k_nod_rhs(NodLevel L, double i4hx, double i4hy, double i4hz, const double* __res
     const bool in = i <= L.nx && j <= L.ny;
     double rsum = 0.0, rmax = 0.0;
     for (int k = blockIdx.z * zper; k < min((int)(blockIdx.z + 1) * zper, L.nz + 1); ++k) {
-    double r = 0.0;
-    if (in && nod_kind(L, i, j, k) == 0) {
-        const NodAxis X = nod_axis(L, 0, i), Y = nod_axis(L, 1, j), Z = nod_axis(L, 2, k);
+        double r = 0.0;
+        if (in && nod_kind(L, i, j, k) == 0) {
+            const NodAxis X = nod_axis(L, 0, i), Y = nod_axis(L, 1, j), Z = nod_axis(L, 2, k);
 #pragma unroll
-        for (int c = 0; c < 2; ++c)
+            for (int c = 0; c < 2; ++c)
 #pragma unroll
-            for (int b = 0; b < 2; ++b)
+                for (int b = 0; b < 2; ++b)
 #pragma unroll
-                for (int a = 0; a < 2; ++a) {
-                    if (X.cl[a] < 0 || Y.cl[b] < 0 || Z.cl[c] < 0) continue;
-                    const size_t q = nod_cidx(L, X.cl[a], Y.cl[b], Z.cl[c]);
-                    const double bc = bcell[q];
-                    // the node is the HIGH corner of the cell at offset -1 (a == 0): -(2 s - 1) = -1
-                    r -= (a == 0 ? 1.0 : -1.0) * (bc * __ldg(u + q)) * i4hx;
-                    r -= (b == 0 ? 1.0 : -1.0) * (bc * __ldg(v + q)) * i4hy;
-                    r -= (c == 0 ? 1.0 : -1.0) * (bc * __ldg(w + q)) * i4hz;
-                    if (S) r -= 0.125 * (bc * __ldg(S + q));
-                }
-    }
-    if (in) L.rhs[nod_idx(L, i, j, k)] = r;
-    rsum += r;
-    rmax = nanmax(rmax, fabs(r));
+                    for (int a = 0; a < 2; ++a) {
+                        if (X.cl[a] < 0 || Y.cl[b] < 0 || Z.cl[c] < 0) continue;
+                        const size_t q = pub_cidx(L, X.cl[a], Y.cl[b], Z.cl[c]);
+                        const double bc = bcell[q];
+                        // the node is the HIGH corner of the cell at offset -1 (a == 0): -(2 s - 1) = -1
+                        r -= (a == 0 ? 1.0 : -1.0) * (bc * __ldg(u + q)) * i4hx;
+                        r -= (b == 0 ? 1.0 : -1.0) * (bc * __ldg(v + q)) * i4hy;
+                        r -= (c == 0 ? 1.0 : -1.0) * (bc * __ldg(w + q)) * i4hz;
+                        if (S) r -= 0.125 * (bc * __ldg(S + q));
+                    }
+        }
+        if (in) L.rhs[nod_idx(L, i, j, k)] = r;
+        rsum += r;
+        rmax = nanmax(rmax, fabs(r));
     }
     block_reduce_store(rsum, rmax, part_sum, part_max, blockIdx.x + gridDim.x * (blockIdx.y + gridDim.y * blockIdx.z));
 }
@@ -232,7 +302,7 @@ __device__ __forceinline__ double nod_weight(const NodLevel& L, int i, int j, in
 }
 
 // a[node] -= (scal[0] * inv_cells) * (WEIGHTED ? w_a : 1) at the unknowns; block partials of sum (of w_a a_a when
-// WSUM) and max |a| afterwards.  shift == NULL: only the reductions.
+// WSUM) and max |a| afterwards.  scal == NULL: only the reductions.
 template <bool WEIGHTED, bool WSUM>
 __global__ void __launch_bounds__(256)
 k_nod_shift(NodLevel L, double* __restrict__ a, const double* __restrict__ scal, double inv_cells,
@@ -241,79 +311,130 @@ k_nod_shift(NodLevel L, double* __restrict__ a, const double* __restrict__ scal,
     const int i = blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y * blockDim.y + threadIdx.y;
     double s = 0.0, m = 0.0;
     for (int k = blockIdx.z * zper; k < min((int)(blockIdx.z + 1) * zper, L.nz + 1); ++k)
-    if (i <= L.nx && j <= L.ny && nod_kind(L, i, j, k) == 0) {
-        const size_t q = nod_idx(L, i, j, k);
-        const double wa = (WEIGHTED || WSUM) ? nod_weight(L, i, j, k) : 1.0;
-        double val = a[q];
-        if (scal) {
-            val -= (scal[0] * inv_cells) * (WEIGHTED ? wa : 1.0);
-            a[q] = val;
+        if (i <= L.nx && j <= L.ny && nod_kind(L, i, j, k) == 0) {
+            const long long q = nod_idx(L, i, j, k);
+            const double wa = (WEIGHTED || WSUM) ? nod_weight(L, i, j, k) : 1.0;
+            double val = a[q];
+            if (scal) {
+                val -= (scal[0] * inv_cells) * (WEIGHTED ? wa : 1.0);
+                a[q] = val;
+            }
+            s += WSUM ? wa * val : val;
+            m = nanmax(m, fabs(val));
         }
-        s += WSUM ? wa * val : val;
-        m = nanmax(m, fabs(val));
-    }
     block_reduce_store(s, m, part_sum, part_max, blockIdx.x + gridDim.x * (blockIdx.y + gridDim.y * blockIdx.z));
 }
 
-// ---- N7: one Jacobi sweep pin -> pout (distinct buffers); NORM: block partials of max |rhs - L phi_in| ---------
-template <bool NORM>
-__global__ void __launch_bounds__(256)
-k_nod_jacobi(NodLevel L, const double* __restrict__ pin, double* __restrict__ pout, double* __restrict__ part_max, int zper)
+// ---- N7 / residual: the operator pass, marching in z ------------------------------------------------------------
+// MODE bit 0 (NOD_JACOBI): out = pin + omega (rhs - L pin) / L_aa (one Jacobi sweep, pin -> out, distinct buffers; the
+// periodic images of out are written too); bit 1 (NOD_RESID): out = rhs - L pin (out may be NULL; no images: the
+// restriction reads through the rules); bit 2 (NOD_NORM): block partials of max |rhs - L pin| over the unknowns in
+// part_max[linear block index].  OUTFLOW nodes receive 0.
+//
+// A thread owns a node column (i, j) and marches a chunk of planes.  It keeps the 3 x 3 phi values of planes k-1, k, k+1
+// and the expanded sigma sums of the cell planes below and above in registers, so a plane costs 9 phi loads, 4 sigma
+// loads, rhs and the store (the lateral neighbours come from L1: a block's tile re-reads a one-node ring), 5 additions
+// for the new sigma sums and 54 multiply-adds:
+//     L phi = -sum_{dx,dy} [ Tlo (w_o phi_{k-1} + w_s phi_k) + Tup (w_o phi_{k+1} + w_s phi_k) ],
+// w_s / w_o = the class weight with the same / the other corner along z.  The ghost layout makes every node interior.
+// The march is unrolled six-fold (period 3 of the phi planes x period 2 of the sigma planes) so that nothing moves
+// between registers.
+enum { NOD_JACOBI = 1, NOD_RESID = 2, NOD_NORM = 4 };
+
+struct NodPlane { double v[3][3]; };               // [dy][dx]
+
+__device__ __forceinline__ void nod_load_phi(NodPlane& P, const double* __restrict__ q, long long py)
 {
-    const int i = blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y * blockDim.y + threadIdx.y;
-    double rabs = 0.0;
-    for (int k = blockIdx.z * zper; k < min((int)(blockIdx.z + 1) * zper, L.nz + 1); ++k)
+#pragma unroll
+    for (int b = 0; b < 3; ++b)
+#pragma unroll
+        for (int a = 0; a < 3; ++a) P.v[b][a] = q[(a - 1) + (b - 1) * py];
+}
+// the 2 x 2 sigmas of a cell plane around the node column, expanded to the 3 x 3 sums over the cells shared with each
+// lateral neighbour
+__device__ __forceinline__ void nod_load_sig(NodPlane& T, const double* __restrict__ sg, long long cy)
+{
+    const double s00 = __ldg(sg), s01 = __ldg(sg + 1), s10 = __ldg(sg + cy), s11 = __ldg(sg + cy + 1);
+    T.v[0][0] = s00; T.v[0][1] = s00 + s01; T.v[0][2] = s01;
+    T.v[2][0] = s10; T.v[2][1] = s10 + s11; T.v[2][2] = s11;
+    T.v[1][0] = s00 + s10; T.v[1][1] = T.v[0][1] + T.v[2][1]; T.v[1][2] = s01 + s11;
+}
+
+template <int MODE>
+__global__ void __launch_bounds__(256, 2)
+k_nod_march(NodLevel L, const double* __restrict__ pin, double* __restrict__ out, double* __restrict__ part_max, int zchunk)
+{
+    const int i = blockIdx.x * 32 + threadIdx.x, j = blockIdx.y * 8 + threadIdx.y;
+    const int k0 = blockIdx.z * zchunk, k1 = min(k0 + zchunk, L.nz + 1);
+    const int ic = min(i, L.nx), jc = min(j, L.ny);               // threads beyond the grid march a valid column and store nothing
+    int kxy = 3;                                                  // lateral kind: 0 unknown, 1 OUTFLOW, 2 duplicate, 3 outside
     if (i <= L.nx && j <= L.ny) {
-        const size_t q = nod_idx(L, i, j, k);
-        double out = 0.0;
-        if (nod_kind(L, i, j, k) == 0) {
-            double lp, dg;
-            if (nod_fast(L, i, j, k)) nod_operator<true>(L, pin, i, j, k, lp, dg);
-            else nod_operator<false>(L, pin, i, j, k, lp, dg);
-            const double r = L.rhs[q] - lp;
-            rabs = nanmax(rabs, fabs(r));
-            out = pin[q] + L.omega * r / dg;
-        }
-        pout[q] = out;
+        const int ka = nod_axis_kind(L, 0, i), kb = nod_axis_kind(L, 1, j);
+        kxy = (ka == 1 || kb == 1) ? 1 : ((ka == 2 || kb == 2) ? 2 : 0);
     }
-    if (NORM) {
+    const int ix = kxy == 0 ? nod_image(L, 0, i) : 0, iy = kxy == 0 ? nod_image(L, 1, j) : 0;
+    double rmax = 0.0;
+    const long long py = L.nx + 3, pz = py * (L.ny + 3), cy = L.nx + 2, cz = cy * (L.ny + 2);
+    const double* q = pin + nod_idx(L, ic, jc, k0);
+    const double* sg = L.sigma + nod_cidx(L, ic - 1, jc - 1, k0 - 1);
+    long long qo = nod_idx(L, ic, jc, k0);
+    NodPlane P[3], T[2];
+    nod_load_phi(P[0], q - pz, py);
+    nod_load_phi(P[1], q, py);
+    nod_load_sig(T[0], sg, cy);
+#pragma unroll 1
+    for (int k = k0; k < k1; k += 6) {
+#pragma unroll
+        for (int u = 0; u < 6; ++u) {
+            if (k + u >= k1) break;
+            NodPlane& Pm = P[u % 3];                     // planes k-1, k, k+1 and the cell planes below / above
+            NodPlane& Pc = P[(u + 1) % 3];
+            NodPlane& Pp = P[(u + 2) % 3];
+            NodPlane& Tlo = T[u % 2];
+            NodPlane& Tup = T[(u + 1) % 2];
+            nod_load_phi(Pp, q + pz, py);
+            nod_load_sig(Tup, sg + cz, cy);
+            const double rh = L.rhs[qo];
+            double acc0 = 0.0, acc1 = 0.0;
+#pragma unroll
+            for (int b = 0; b < 3; ++b)
+#pragma unroll
+                for (int a = 0; a < 3; ++a) {
+                    const int cl = (a != 1 ? 1 : 0) | (b != 1 ? 2 : 0);
+                    const double sc = L.w[cl] * Pc.v[b][a];
+                    acc0 = fma(Tlo.v[b][a], fma(L.w[4 + cl], Pm.v[b][a], sc), acc0);
+                    acc1 = fma(Tup.v[b][a], fma(L.w[4 + cl], Pp.v[b][a], sc), acc1);
+                }
+            const int kz = nod_axis_kind(L, 2, k + u);
+            if (kxy == 0 && kz == 0) {
+                const double r = rh + (acc0 + acc1);                          // rhs - L phi, L phi = -(acc0 + acc1)
+                if (MODE & NOD_NORM) rmax = nanmax(rmax, fabs(r));
+                if (MODE & NOD_JACOBI) {
+                    const double dg = -(L.w[0] * (Tlo.v[1][1] + Tup.v[1][1]));
+                    nod_store_images(L, out, qo, Pc.v[1][1] + L.omega * r / dg, ix, iy, nod_image(L, 2, k + u));
+                } else if (out) out[qo] = r;
+            } else if (kxy <= 1 && (kxy == 1 || kz == 1) && out) {
+                out[qo] = 0.0;                                                // OUTFLOW node
+            }
+            q += pz; sg += cz; qo += pz;
+        }
+    }
+    if (MODE & NOD_NORM) {
         __shared__ double sh[8];
-        const int tid = threadIdx.x + blockDim.x * threadIdx.y;
-        rabs = warp_nanmax(rabs);
-        if ((tid & 31) == 0) sh[tid >> 5] = rabs;
+        const int tid = threadIdx.x + 32 * threadIdx.y;
+        rmax = warp_nanmax(rmax);
+        if ((tid & 31) == 0) sh[tid >> 5] = rmax;
         __syncthreads();
         if (tid == 0) {
             double m = sh[0];
-            for (int q = 1; q < (int)(blockDim.x * blockDim.y + 31) / 32; ++q) m = nanmax(m, sh[q]);
+            for (int qq = 1; qq < 8; ++qq) m = nanmax(m, sh[qq]);
             part_max[blockIdx.x + gridDim.x * (blockIdx.y + gridDim.y * blockIdx.z)] = m;
         }
     }
 }
 
-// ---- residual r = rhs - L phi at the unknowns, 0 elsewhere (res may be NULL); block partials of max |r| ---------
-__global__ void __launch_bounds__(256)
-k_nod_residual(NodLevel L, const double* __restrict__ phi, double* __restrict__ res, double* __restrict__ part_sum,
-               double* __restrict__ part_max, int zper)
-{
-    const int i = blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y * blockDim.y + threadIdx.y;
-    double rmax = 0.0;
-    for (int k = blockIdx.z * zper; k < min((int)(blockIdx.z + 1) * zper, L.nz + 1); ++k)
-    if (i <= L.nx && j <= L.ny) {
-        double r = 0.0;
-        const size_t q = nod_idx(L, i, j, k);
-        if (nod_kind(L, i, j, k) == 0) {
-            double lp, dg;
-            if (nod_fast(L, i, j, k)) nod_operator<true>(L, phi, i, j, k, lp, dg);
-            else nod_operator<false>(L, phi, i, j, k, lp, dg);
-            r = L.rhs[q] - lp;
-        }
-        if (res) res[q] = r;
-        rmax = nanmax(rmax, fabs(r));
-    }
-    block_reduce_store(0.0, rmax, part_sum, part_max, blockIdx.x + gridDim.x * (blockIdx.y + gridDim.y * blockIdx.z));
-}
-
-// ---- N6: coarse rhs = (1/8) P^T res (weights 1, 1/2 per axis over the 27 fine nodes), coarse phi = 0 -----------
+// ---- N6: coarse rhs = (1/8) P^T res (weights 1, 1/2 per axis over the 27 fine nodes); the coarse phi is zeroed by
+// the host (whole array, ghosts included) -----------------------------------------------------------------------
 __global__ void __launch_bounds__(256)
 k_nod_restrict(NodLevel F, NodLevel C, const double* __restrict__ res)
 {
@@ -323,15 +444,15 @@ k_nod_restrict(NodLevel F, NodLevel C, const double* __restrict__ res)
     if (nod_kind(C, I, J, K) == 0) {
         int fi[3], fj[3], fk[3];
 #pragma unroll
-        for (int o = 0; o < 3; ++o) {                 // fine node 2 T + (o - 1) per axis, wrapped, or -1
+        for (int o = 0; o < 3; ++o) {                 // fine node 2 T + (o - 1) per axis, wrapped, or -2
             int t = 2 * I + o - 1;
-            if (F.bclo[0] == MAC_PERIODIC) { if (t < 0) t += F.nx; if (t >= F.nx) t -= F.nx; } else if (t < 0 || t > F.nx) t = -1;
+            if (F.bclo[0] == MAC_PERIODIC) { if (t < 0) t += F.nx; if (t >= F.nx) t -= F.nx; } else if (t < 0 || t > F.nx) t = -2;
             fi[o] = t;
             t = 2 * J + o - 1;
-            if (F.bclo[1] == MAC_PERIODIC) { if (t < 0) t += F.ny; if (t >= F.ny) t -= F.ny; } else if (t < 0 || t > F.ny) t = -1;
+            if (F.bclo[1] == MAC_PERIODIC) { if (t < 0) t += F.ny; if (t >= F.ny) t -= F.ny; } else if (t < 0 || t > F.ny) t = -2;
             fj[o] = t;
             t = 2 * K + o - 1;
-            if (F.bclo[2] == MAC_PERIODIC) { if (t < 0) t += F.nz; if (t >= F.nz) t -= F.nz; } else if (t < 0 || t > F.nz) t = -1;
+            if (F.bclo[2] == MAC_PERIODIC) { if (t < 0) t += F.nz; if (t >= F.nz) t -= F.nz; } else if (t < 0 || t > F.nz) t = -2;
             fk[o] = t;
         }
 #pragma unroll
@@ -346,22 +467,10 @@ k_nod_restrict(NodLevel F, NodLevel C, const double* __restrict__ res)
                 }
         s *= 0.125;
     }
-    const size_t q = nod_idx(C, I, J, K);
-    C.rhs[q] = s;
-    C.phi[q] = 0.0;
+    C.rhs[nod_idx(C, I, J, K)] = s;
 }
 
-// value of a coarse nodal array at node (I, J, K) under the node rules (OUTFLOW 0, periodic node n = node 0)
-__device__ __forceinline__ double nod_val(const NodLevel& L, const double* __restrict__ a, int I, int J, int K)
-{
-    if (nod_kind(L, I, J, K) == 1) return 0.0;
-    if (L.bclo[0] == MAC_PERIODIC && I == L.nx) I = 0;
-    if (L.bclo[1] == MAC_PERIODIC && J == L.ny) J = 0;
-    if (L.bclo[2] == MAC_PERIODIC && K == L.nz) K = 0;
-    return a[nod_idx(L, I, J, K)];
-}
-
-// ---- N6: phi_f += P e_c at the fine unknowns (trilinear: weights 1, 1/2, 1/4, 1/8) -----------------------------
+// ---- N6: phi_f += P e_c at the fine unknowns (trilinear: weights 1, 1/2, 1/4, 1/8), images included --------------
 __global__ void __launch_bounds__(256)
 k_nod_prolong_add(NodLevel F, NodLevel C)
 {
@@ -373,7 +482,8 @@ k_nod_prolong_add(NodLevel F, NodLevel C)
     for (int c = 0; c <= ok; ++c)
         for (int b = 0; b <= oj; ++b)
             for (int a = 0; a <= oi; ++a) s += wt * nod_val(C, C.phi, I + a, J + b, K + c);
-    F.phi[nod_idx(F, i, j, k)] += s;
+    const long long q = nod_idx(F, i, j, k);
+    nod_store_images(F, F.phi, q, F.phi[q] + s, nod_image(F, 0, i), nod_image(F, 1, j), nod_image(F, 2, k));
 }
 
 // ---- N10: U <- U - (1/rho) G phi, G the cell-mean gradient (mean of the 4 edge differences per axis) -----------
@@ -402,56 +512,50 @@ k_nod_correct(NodLevel L, GeoDev G, double i4hx, double i4hy, double i4hz, const
                 gy += (b ? 1.0 : -1.0) * p[c][b][a] * i4hy;
                 gz += (c ? 1.0 : -1.0) * p[c][b][a] * i4hz;
             }
-    const size_t q = nod_cidx(L, i, j, k);
+    const size_t q = pub_cidx(L, i, j, k);
     const double rh = rho ? __ldg(rho + q) : profile_eval(rho0, G.nr, G.dr, radius(G, (i + 0.5) * G.dx, (j + 0.5) * G.dy, (k + 0.5) * G.dz));
     u[q] -= gx / rh;
     v[q] -= gy / rh;
     w[q] -= gz / rh;
 }
 
-// export: OUTFLOW nodes 0, periodic duplicates equal their image; src and dst may be the same array
-__global__ void __launch_bounds__(256)
-k_nod_export(NodLevel L, const double* __restrict__ src, double* __restrict__ dst)
+// ---- N8: bottom solve, unpreconditioned BiCGStab on the unknowns of the coarsest level (one thread block).  The
+// iterate x is the level's phi; the six work vectors are arrays in the same internal layout (interior origins vec0 +
+// m * vstride), global memory -- the level is tiny and L1/L2-resident; entries of OUTFLOW nodes and periodic
+// duplicates stay 0.  Same algorithm and stopping rule as the MAC bottom solver (reading A15).
+struct NodBottomIdx { int i, j, k; long long q; bool active; };
+__device__ __forceinline__ NodBottomIdx nod_bottom_idx(const NodLevel& L, int c)
 {
-    const int i = blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y * blockDim.y + threadIdx.y, k = blockIdx.z;
-    if (i > L.nx || j > L.ny) return;
-    dst[nod_idx(L, i, j, k)] = nod_val(L, src, i, j, k);
-}
-
-// ---- N8: bottom solve, unpreconditioned BiCGStab on the unknowns of the coarsest level (one thread block, vectors
-// over ALL nodes of the level in global memory -- the level is tiny and L1/L2-resident; entries of OUTFLOW nodes and
-// periodic duplicates stay 0).  Same algorithm and stopping rule as the MAC bottom solver (reading A15).
-__device__ __forceinline__ double nod_matvec_at(const NodLevel& L, const double* __restrict__ x, int c, bool active)
-{
-    if (!active) return 0.0;
+    NodBottomIdx B;
     const int px = L.nx + 1, py = L.ny + 1;
-    const int i = c % px, j = (c / px) % py, k = c / (px * py);
-    double lp, dg;
-    nod_operator<false>(L, x, i, j, k, lp, dg);
-    return lp;
+    B.i = c % px; B.j = (c / px) % py; B.k = c / (px * py);
+    B.q = nod_idx(L, B.i, B.j, B.k);
+    B.active = nod_kind(L, B.i, B.j, B.k) == 0;
+    return B;
 }
 
 __global__ void __launch_bounds__(1024)
-k_nod_bottom(NodLevel L, double* __restrict__ vecs, int maxit, double tol, int singular, int* __restrict__ iters_accum)
+k_nod_bottom(NodLevel L, double* __restrict__ vec0, long long vstride, int maxit, double tol, int singular,
+             int* __restrict__ iters_accum)
 {
     __shared__ double sh[64];
     const int nb = (L.nx + 1) * (L.ny + 1) * (L.nz + 1), nt = blockDim.x, tid = threadIdx.x;
-    double *x = L.phi, *r = vecs, *rhat = vecs + nb, *p = vecs + 2 * (size_t)nb, *v = vecs + 3 * (size_t)nb,
-           *s = vecs + 4 * (size_t)nb, *t = vecs + 5 * (size_t)nb;
+    double *x = L.phi, *r = vec0, *rhat = vec0 + vstride, *p = vec0 + 2 * vstride, *v = vec0 + 3 * vstride,
+           *s = vec0 + 4 * vstride, *t = vec0 + 5 * vstride;
     const double* f = L.rhs;
-    auto active = [&](int c) {
-        const int px = L.nx + 1, py = L.ny + 1;
-        return nod_kind(L, c % px, (c / px) % py, c / (px * py)) == 0;
-    };
+#define NOD_FOR_NODES for (int c = tid; c < nb; c += nt)
     double cnt = 0.0, fs = 0.0;
-    for (int c = tid; c < nb; c += nt)
-        if (active(c)) { cnt += 1.0; fs += f[c]; }
+    NOD_FOR_NODES {
+        const NodBottomIdx B = nod_bottom_idx(L, c);
+        if (B.active) { cnt += 1.0; fs += f[B.q]; }
+    }
     const Dot2 q0 = block_dot2(cnt, fs, sh, nt);
     const double nunk = q0.a, fm = singular ? q0.b / q0.a : 0.0;
     double rr = 0.0;
-    for (int c = tid; c < nb; c += nt) {
-        const double fv = active(c) ? f[c] - fm : 0.0;
-        r[c] = fv; rhat[c] = fv; p[c] = 0.0; v[c] = 0.0; x[c] = 0.0;
+    NOD_FOR_NODES {
+        const NodBottomIdx B = nod_bottom_idx(L, c);
+        const double fv = B.active ? f[B.q] - fm : 0.0;
+        r[B.q] = fv; rhat[B.q] = fv; p[B.q] = 0.0; v[B.q] = 0.0; s[B.q] = 0.0; x[B.q] = 0.0;
         rr += fv * fv;
     }
     rr = block_dot2(rr, 0.0, sh, nt).a;
@@ -463,52 +567,67 @@ k_nod_bottom(NodLevel L, double* __restrict__ vecs, int maxit, double tol, int s
         while (it < maxit && rr > stop2) {
             if (rho == 0.0) break;
             const double beta = it == 0 ? 0.0 : (rho / rho_old) * (alpha / omega);
-            for (int c = tid; c < nb; c += nt) p[c] = r[c] + beta * (p[c] - omega * v[c]);
+            NOD_FOR_NODES { const long long q = nod_bottom_idx(L, c).q; p[q] = r[q] + beta * (p[q] - omega * v[q]); }
             group_sync(nt);
             double d = 0.0;
-            for (int c = tid; c < nb; c += nt) { const double y = nod_matvec_at(L, p, c, active(c)); v[c] = y; d += rhat[c] * y; }
+            NOD_FOR_NODES {
+                const NodBottomIdx B = nod_bottom_idx(L, c);
+                const double y = B.active ? nod_operator_generic(L, p, B.i, B.j, B.k) : 0.0;
+                v[B.q] = y;
+                d += rhat[B.q] * y;
+            }
             d = block_dot2(d, 0.0, sh, nt).a;
             if (d == 0.0) break;
             alpha = rho / d;
             double ss = 0.0;
-            for (int c = tid; c < nb; c += nt) { const double y = r[c] - alpha * v[c]; s[c] = y; ss += y * y; }
+            NOD_FOR_NODES { const long long q = nod_bottom_idx(L, c).q; const double y = r[q] - alpha * v[q]; s[q] = y; ss += y * y; }
             ss = block_dot2(ss, 0.0, sh, nt).a;
             ++it;
             if (ss <= stop2) {
-                for (int c = tid; c < nb; c += nt) x[c] += alpha * p[c];
+                NOD_FOR_NODES { const long long q = nod_bottom_idx(L, c).q; x[q] += alpha * p[q]; }
                 rr = ss;
                 break;
             }
             double ts = 0.0, tt = 0.0;
-            for (int c = tid; c < nb; c += nt) { const double y = nod_matvec_at(L, s, c, active(c)); t[c] = y; ts += y * s[c]; tt += y * y; }
-            Dot2 q = block_dot2(ts, tt, sh, nt);
-            if (q.b == 0.0) {
-                for (int c = tid; c < nb; c += nt) x[c] += alpha * p[c];
+            NOD_FOR_NODES {
+                const NodBottomIdx B = nod_bottom_idx(L, c);
+                const double y = B.active ? nod_operator_generic(L, s, B.i, B.j, B.k) : 0.0;
+                t[B.q] = y;
+                ts += y * s[B.q];
+                tt += y * y;
+            }
+            Dot2 qd = block_dot2(ts, tt, sh, nt);
+            if (qd.b == 0.0) {
+                NOD_FOR_NODES { const long long q = nod_bottom_idx(L, c).q; x[q] += alpha * p[q]; }
                 break;
             }
-            omega = q.a / q.b;
+            omega = qd.a / qd.b;
             double r2 = 0.0, hr = 0.0;
-            for (int c = tid; c < nb; c += nt) {
-                x[c] += alpha * p[c] + omega * s[c];
-                const double y = s[c] - omega * t[c];
-                r[c] = y;
+            NOD_FOR_NODES {
+                const long long q = nod_bottom_idx(L, c).q;
+                x[q] += alpha * p[q] + omega * s[q];
+                const double y = s[q] - omega * t[q];
+                r[q] = y;
                 r2 += y * y;
-                hr += rhat[c] * y;
+                hr += rhat[q] * y;
             }
-            q = block_dot2(r2, hr, sh, nt);
-            rr = q.a;
+            qd = block_dot2(r2, hr, sh, nt);
+            rr = qd.a;
             rho_old = rho;
-            rho = q.b;
+            rho = qd.b;
             if (omega == 0.0) break;
         }
     }
     if (singular) {                                // zero plain mean over the unknowns (N8)
         group_sync(nt);
         double a = 0.0;
-        for (int c = tid; c < nb; c += nt) a += x[c];
+        NOD_FOR_NODES a += x[nod_bottom_idx(L, c).q];
         const double xm = block_dot2(a, 0.0, sh, nt).a / nunk;
-        for (int c = tid; c < nb; c += nt)
-            if (active(c)) x[c] -= xm;
+        NOD_FOR_NODES {
+            const NodBottomIdx B = nod_bottom_idx(L, c);
+            if (B.active) x[B.q] -= xm;
+        }
     }
+#undef NOD_FOR_NODES
     if (tid == 0 && iters_accum) *iters_accum += it;
 }

@@ -208,10 +208,11 @@ __device__ __forceinline__ void step(const Th& T, int kk, const unsigned char* s
     Pm4 = Pm3; Pm3 = Pm2; Pm2 = Pm1; Pm1 = P0;
 }
 
-// Stage J (0 .. 3) of the four-fold unrolled march: plane kk sits in stage (1 + J) % 4 of both rings, so every
-// shared-memory offset is a compile-time constant.
+// Step J (0 .. 3) of the four-fold unrolled march (the unrolling keeps the four rotating coefficient sets in fixed
+// registers).  Plane kk sits in stage s0 of both rings, plane kk+1 in the next one; the rings have NS = LA + 2 stages, so
+// their period is independent of the unrolling and the stage offsets are runtime values (two integer operations a step).
 template <int LA, int J, bool X, bool NORM>
-__device__ __forceinline__ void stage(const Th& T, int kk, int ke, unsigned par, const CUtensorMap* tm_phi,
+__device__ __forceinline__ void stage(const Th& T, int kk, int ke, unsigned& s0, unsigned& phase, const CUtensorMap* tm_phi,
                                       const CUtensorMap* tm_rhs, const CUtensorMap* tm_ax, const CUtensorMap* tm_ay,
                                       const CUtensorMap* tm_az, unsigned phi_ring, unsigned coef_ring, unsigned bar0,
                                       bool producer, int cx, int cy, int nz, bool perz, double* __restrict__ out,
@@ -219,18 +220,22 @@ __device__ __forceinline__ void stage(const Th& T, int kk, int ke, unsigned par,
                                       Coef& CUR, Coef& S1, Coef& S2, Coef& S3, double& vmax, bool& vnan)
 {
     using G = Cfg<LA>;
-    static_assert(G::NP == 4 && G::NC == 4 && LA == 2, "the unrolled march assumes 4 stages per ring");
-    constexpr int i0 = (1 + J) % 4, iP = (2 + J) % 4, iN = J % 4;
-    // plane kk+1 (barrier iP) has landed: a barrier is reused every 4 steps, its parity flips with every reuse
-    mbar_wait(bar0 + 8 * iP, (par + (J >= 2 ? 1u : 0u)) & 1u);
+    constexpr unsigned NS = G::NP;
+    static_assert(G::NP == G::NC, "both rings have the same depth");
+    const unsigned sP = s0 + 1 == NS ? 0u : s0 + 1;            // stage of plane kk+1
+    const unsigned sN = s0 == 0 ? NS - 1 : s0 - 1;             // stage plane kk-1 vacated: receives plane kk+1+LA
+    // plane kk+1 has landed: a barrier is reused every NS steps, its parity flips with every reuse
+    mbar_wait(bar0 + 8 * sP, (phase >> sP) & 1u);
+    phase ^= 1u << sP;
     __syncthreads();                                           // every thread has finished step kk-1
     if (producer && kk + 1 + LA <= ke + 1) {                   // never leave a load in flight at exit
         asm volatile("fence.proxy.async.shared::cta;\n" ::: "memory");
-        issue_plane<LA>(tm_phi, tm_rhs, tm_ax, tm_ay, tm_az, phi_ring, coef_ring, bar0, iN * kPl, iN * G::kCoef,
+        issue_plane<LA>(tm_phi, tm_rhs, tm_ax, tm_ay, tm_az, phi_ring, coef_ring, bar0, sN * kPl, sN * G::kCoef,
                         kk + 1 + LA, nz, perz, cx, cy);
     }
-    step<X, J & 1, NORM>(T, kk, T.phi0 + i0 * kPl, T.phi0 + iP * kPl, T.coef0 + i0 * G::kCoef, T.coef0 + iP * G::kCoef,
+    step<X, J & 1, NORM>(T, kk, T.phi0 + s0 * kPl, T.phi0 + sP * kPl, T.coef0 + s0 * G::kCoef, T.coef0 + sP * G::kCoef,
                          out, Pn, Pm1, Pm2, Pm3, Pm4, azn, CUR, S1, S2, S3, vmax, vnan);
+    s0 = sP;
 }
 
 template <int LA, bool REDX0, bool NORM>
@@ -251,14 +256,14 @@ __device__ __forceinline__ void march(const Th& T, int ks, int ke, const CUtenso
     Pm1 = ldp(T.phi0);
     double2 Pn = ldp(T.phi0 + kPl);
     double2 azn = ldp(T.coef0 + G::kCoef + C_AZ * kPl);
-    unsigned par = 0;
+    unsigned s0 = 1, phase = 3u;                               // plane ks sits in stage 1; stages 0 and 1 have completed phase 0
 #define MAC_T2_STAGE(J, XX, CUR, S1, S2, S3)                                                                          \
     if (kk > ke) break;                                                                                               \
-    stage<LA, J, XX, NORM>(T, kk, ke, par, tm_phi, tm_rhs, tm_ax, tm_ay, tm_az, phi_ring, coef_ring, bar0, producer,  \
+    stage<LA, J, XX, NORM>(T, kk, ke, s0, phase, tm_phi, tm_rhs, tm_ax, tm_ay, tm_az, phi_ring, coef_ring, bar0, producer,  \
                            cx, cy, nz, perz, out, Pn, Pm1, Pm2, Pm3, Pm4, azn, CUR, S1, S2, S3, vmax, vnan);                \
     out += out_stride; ++kk;
 #pragma unroll 1
-    for (int kk = ks; kk <= ke; par ^= 1u) {
+    for (int kk = ks; kk <= ke;) {
         MAC_T2_STAGE(0, REDX0, cA, cD, cC, cB)
         MAC_T2_STAGE(1, !REDX0, cB, cA, cD, cC)
         MAC_T2_STAGE(2, REDX0, cC, cB, cA, cD)

@@ -49,12 +49,14 @@ struct Staging {
     double *beta0, *rho0, *rho, *u, *v, *w, *S, *phi;
 };
 
-struct NodHost {                   // one level of the nodal projection (desc.nodal = 1)
+struct NodHost {                   // one level of the nodal projection (desc.nodal = 1); layout: mac_nodal.cuh
     int n[3];
     double h[3];
-    size_t nnode, ncell;
-    double *phi, *phi2, *rhs;      // node arrays, (nx+1)(ny+1)(nz+1)
-    double *sigma;                 // cell array
+    size_t nnode, ncell;           // nodes (nx+1)(ny+1)(nz+1) and cells of the level
+    size_t anode, acell;           // allocated entries: one ghost node / ghost cell per side
+    size_t onode, ocell;           // entries from an allocation's base to the interior origin
+    double *phi, *phi2, *rhs;      // node arrays (interior origins)
+    double *sigma;                 // cell array (interior origin)
 };
 
 }  // namespace
@@ -210,12 +212,17 @@ size_t carve(maestro_mac_handle* H, char* base)
             for (int a = 0; a < 3; ++a) { N.n[a] = H->lev[l].n[a]; N.h[a] = H->lev[l].h[a]; }
             N.nnode = (size_t)(N.n[0] + 1) * (N.n[1] + 1) * (N.n[2] + 1);
             N.ncell = H->lev[l].ncell;
-            N.phi = (double*)take(N.nnode, 8);
-            N.phi2 = (double*)take(N.nnode, 8);
-            N.rhs = (double*)take(N.nnode, 8);
-            N.sigma = (double*)take(N.ncell, 8);
+            N.anode = (size_t)(N.n[0] + 3) * (N.n[1] + 3) * (N.n[2] + 3);
+            N.acell = (size_t)(N.n[0] + 2) * (N.n[1] + 2) * (N.n[2] + 2);
+            N.onode = 1 + (size_t)(N.n[0] + 3) * (1 + (size_t)(N.n[1] + 3));
+            N.ocell = 1 + (size_t)(N.n[0] + 2) * (1 + (size_t)(N.n[1] + 2));
+            auto at = [&](void* b, size_t o) -> double* { return b ? (double*)b + o : nullptr; };
+            N.phi = at(take(N.anode, 8), N.onode);
+            N.phi2 = at(take(N.anode, 8), N.onode);
+            N.rhs = at(take(N.anode, 8), N.onode);
+            N.sigma = at(take(N.acell, 8), N.ocell);
         }
-        H->nod_vecs = (double*)take(6 * H->nod[H->nlev - 1].nnode, 8);
+        H->nod_vecs = (double*)take(6 * H->nod[H->nlev - 1].anode, 8);
     }
     H->has_staging = H->d.host_staging == 1;
     if (H->has_staging) {

@@ -43,11 +43,61 @@ void nod_dims_red(int ex, int ey, int ez, dim3* grid, dim3* block, int* zper)
     *zper = zp;
 }
 
+// grid of the z-marching operator pass (k_nod_march, 32 x 8 node tiles): enough z-chunks for a few blocks per SM, chunks
+// of at least 16 planes (a chunk reloads two planes), and at most kMaxParts blocks (one partial maximum each)
+dim3 nod_march_grid(const maestro_mac_handle* H, const NodLevel& L, int* zchunk)
+{
+    const int tx = (L.nx + 1 + 31) / 32, ty = (L.ny + 1 + 7) / 8, nzn = L.nz + 1;
+    int nchunk = (6 * H->sms + tx * ty - 1) / (tx * ty);
+    const int maxchunk = (nzn + 15) / 16;
+    if (nchunk > maxchunk) nchunk = maxchunk;
+    if (nchunk < 1) nchunk = 1;
+    int zc = (nzn + nchunk - 1) / nchunk;
+    while ((long)tx * ty * ((nzn + zc - 1) / zc) > kMaxParts) zc *= 2;
+    *zchunk = zc;
+    return dim3(tx, ty, (nzn + zc - 1) / zc);
+}
+
 // folds nb block partials into scal[off] (sum) and scal[off + 1] (max)
 int nod_fold(maestro_mac_handle* H, int nb, int off, cudaStream_t s)
 {
     k_reduce_final<<<1, 1024, 0, s>>>(H->part_sum, H->part_max, nb, H->scal + off);
     LAUNCHED(H);
+    return MAESTRO_MAC_OK;
+}
+
+// beta0 at the cell centres of level 0 in the public cell layout: staged in level 0's second phi buffer (allocation
+// base; (nx+3)(ny+3)(nz+3) >= nx ny nz entries), which is free between nod_do_sigma and the first sweep
+double* nod_bcell(const maestro_mac_handle* H) { return H->nod[0].phi2 - H->nod[0].onode; }
+
+int nod_sig_ghosts(maestro_mac_handle* H, int l, cudaStream_t s)
+{
+    const NodLevel L = dev_nod(H, l);
+    dim3 g, b;
+    nod_dims(L.nx + 2, L.ny + 2, L.nz + 2, &g, &b);
+    k_nod_sig_ghosts<<<g, b, 0, s>>>(L);
+    LAUNCHED(H);
+    return MAESTRO_MAC_OK;
+}
+
+int nod_phi_ghosts(maestro_mac_handle* H, int l, double* a, cudaStream_t s)
+{
+    const NodLevel L = dev_nod(H, l);
+    dim3 g, b;
+    nod_dims(L.nx + 3, L.ny + 3, L.nz + 3, &g, &b);
+    k_nod_phi_ghosts<<<g, b, 0, s>>>(L, a);
+    LAUNCHED(H);
+    return MAESTRO_MAC_OK;
+}
+
+// every nodal phi buffer := 0, ghosts included (they must hold finite values: the operator multiplies them by sigma = 0)
+int nod_zero_phi(maestro_mac_handle* H, cudaStream_t s)
+{
+    for (int l = 0; l < H->nlev; ++l) {
+        const NodHost& N = H->nod[l];
+        CUDA_OK(cudaMemsetAsync(N.phi - N.onode, 0, N.anode * sizeof(double), s));
+        CUDA_OK(cudaMemsetAsync(N.phi2 - N.onode, 0, N.anode * sizeof(double), s));
+    }
     return MAESTRO_MAC_OK;
 }
 
@@ -57,14 +107,16 @@ int nod_do_sigma(maestro_mac_handle* H, const double* beta0, const double* rho0,
     const GeoDev G = dev_geo(H);
     CUDA_OK(cudaMemsetAsync(H->flags, 0, 16 * sizeof(int), s));
     nod_dims(G.nx, G.ny, G.nz, &g, &b);
-    // beta0 at the cell centres goes to level 0's second phi buffer (free until the first sweep); the rhs reads it
-    k_nod_sigma<<<g, b, 0, s>>>(G, beta0, rho, rho0, H->nod[0].sigma, H->nod[0].phi2, H->flags);
+    k_nod_sigma<<<g, b, 0, s>>>(G, dev_nod(H, 0), beta0, rho, rho0, nod_bcell(H), H->flags);
     LAUNCHED(H);
+    int rc;
+    if ((rc = nod_sig_ghosts(H, 0, s)) != 0) return rc;
     for (int l = 0; l + 1 < H->nlev; ++l) {
         const NodLevel C = dev_nod(H, l + 1);
         nod_dims(C.nx, C.ny, C.nz, &g, &b);
         k_nod_coarsen_sigma<<<g, b, 0, s>>>(dev_nod(H, l), C);
         LAUNCHED(H);
+        if ((rc = nod_sig_ghosts(H, l + 1, s)) != 0) return rc;
     }
     return MAESTRO_MAC_OK;
 }
@@ -78,7 +130,7 @@ int nod_do_rhs(maestro_mac_handle* H, const double* u, const double* v, const do
     nod_dims_red(L.nx + 1, L.ny + 1, L.nz + 1, &g, &b, &zper);
     const int nb = (int)(g.x * g.y * g.z);
     const double* hh = H->nod[0].h;
-    k_nod_rhs<<<g, b, 0, s>>>(L, 1.0 / (4.0 * hh[0]), 1.0 / (4.0 * hh[1]), 1.0 / (4.0 * hh[2]), H->nod[0].phi2, u, v, w, S,
+    k_nod_rhs<<<g, b, 0, s>>>(L, 1.0 / (4.0 * hh[0]), 1.0 / (4.0 * hh[1]), 1.0 / (4.0 * hh[2]), nod_bcell(H), u, v, w, S,
                               H->part_sum, H->part_max, zper);
     LAUNCHED(H);
     int rc;
@@ -99,14 +151,13 @@ int nod_do_rhs(maestro_mac_handle* H, const double* u, const double* v, const do
 int nod_do_jacobi(maestro_mac_handle* H, int l, cudaStream_t s, int* norm_parts = nullptr, bool swap = true)
 {
     const NodLevel L = dev_nod(H, l);
-    dim3 g, b;
-    int zper;
-    nod_dims_red(L.nx + 1, L.ny + 1, L.nz + 1, &g, &b, &zper);
+    int zchunk;
+    const dim3 g = nod_march_grid(H, L, &zchunk);
     if (norm_parts) {
         *norm_parts = (int)(g.x * g.y * g.z);
-        k_nod_jacobi<true><<<g, b, 0, s>>>(L, L.phi, L.phi2, H->part_max, zper);
+        k_nod_march<NOD_JACOBI | NOD_NORM><<<g, dim3(32, 8), 0, s>>>(L, L.phi, L.phi2, H->part_max, zchunk);
     } else
-        k_nod_jacobi<false><<<g, b, 0, s>>>(L, L.phi, L.phi2, nullptr, zper);
+        k_nod_march<NOD_JACOBI><<<g, dim3(32, 8), 0, s>>>(L, L.phi, L.phi2, nullptr, zchunk);
     LAUNCHED(H);
     if (swap) { double* t = H->nod[l].phi; H->nod[l].phi = H->nod[l].phi2; H->nod[l].phi2 = t; }
     return MAESTRO_MAC_OK;
@@ -126,13 +177,14 @@ int nod_do_residual_restrict(maestro_mac_handle* H, int l, cudaStream_t s)
 {
     const NodLevel F = dev_nod(H, l), C = dev_nod(H, l + 1);
     dim3 g, b;
-    int zper;
-    nod_dims_red(F.nx + 1, F.ny + 1, F.nz + 1, &g, &b, &zper);
-    k_nod_residual<<<g, b, 0, s>>>(F, F.phi, F.phi2, H->part_sum, H->part_max, zper);
+    int zchunk;
+    g = nod_march_grid(H, F, &zchunk);
+    k_nod_march<NOD_RESID><<<g, dim3(32, 8), 0, s>>>(F, F.phi, F.phi2, nullptr, zchunk);
     LAUNCHED(H);
     nod_dims(C.nx + 1, C.ny + 1, C.nz + 1, &g, &b);
     k_nod_restrict<<<g, b, 0, s>>>(F, C, F.phi2);
     LAUNCHED(H);
+    CUDA_OK(cudaMemsetAsync(H->nod[l + 1].phi - H->nod[l + 1].onode, 0, H->nod[l + 1].anode * sizeof(double), s));   // coarse phi = 0
     return MAESTRO_MAC_OK;
 }
 
@@ -151,7 +203,8 @@ int nod_do_bottom(maestro_mac_handle* H, cudaStream_t s)
     const int l = H->nlev - 1;
     const int nb = (int)H->nod[l].nnode;
     const int threads = nb >= 1024 ? 1024 : ((nb + 31) / 32) * 32;
-    k_nod_bottom<<<1, threads, 0, s>>>(dev_nod(H, l), H->nod_vecs, H->d.bottom_max_iter, H->d.bottom_rel_tol, H->singular, H->flags + 1);
+    k_nod_bottom<<<1, threads, 0, s>>>(dev_nod(H, l), H->nod_vecs + H->nod[l].onode, (long long)H->nod[l].anode, H->d.bottom_max_iter,
+                                      H->d.bottom_rel_tol, H->singular, H->flags + 1);
     LAUNCHED(H);
     return MAESTRO_MAC_OK;
 }
@@ -176,10 +229,9 @@ int nod_do_vcycle(maestro_mac_handle* H, cudaStream_t s, int pre_done = 0)
 int nod_do_residual_norm(maestro_mac_handle* H, int l, cudaStream_t s)
 {
     const NodLevel L = dev_nod(H, l);
-    dim3 g, b;
-    int zper;
-    nod_dims_red(L.nx + 1, L.ny + 1, L.nz + 1, &g, &b, &zper);
-    k_nod_residual<<<g, b, 0, s>>>(L, L.phi, nullptr, H->part_sum, H->part_max, zper);
+    int zchunk;
+    const dim3 g = nod_march_grid(H, L, &zchunk);
+    k_nod_march<NOD_RESID | NOD_NORM><<<g, dim3(32, 8), 0, s>>>(L, L.phi, nullptr, H->part_max, zchunk);
     LAUNCHED(H);
     return nod_fold(H, (int)(g.x * g.y * g.z), 3, s);
 }
@@ -222,7 +274,7 @@ extern "C" int maestro_mac_nodal_project(maestro_mac_handle* H, const double* be
     if ((rc = nod_do_rhs(H, uc, vc, wc, S, s)) != 0) return rc;
     CUDA_OK(cudaMemcpyAsync(H->host_scal, H->scal, 3 * sizeof(double), cudaMemcpyDeviceToHost, s));
     CUDA_OK(cudaMemcpyAsync(H->host_flags, H->flags, sizeof(int), cudaMemcpyDeviceToHost, s));
-    CUDA_OK(cudaMemsetAsync(N0.phi, 0, N0.nnode * sizeof(double), s));      // N9: phi = 0
+    if ((rc = nod_zero_phi(H, s)) != 0) return rc;                          // N9: phi = 0 (and finite ghosts everywhere)
     CUDA_OK(cudaEventRecord(H->ev[1], s));
     CUDA_OK(cudaStreamSynchronize(s));
     st.rhs_norm_inf = H->host_scal[1];
@@ -283,7 +335,7 @@ extern "C" int maestro_mac_nodal_project(maestro_mac_handle* H, const double* be
     }
     nod_dims(L0.nx + 1, L0.ny + 1, L0.nz + 1, &g, &b);
     if (phi) {
-        k_nod_export<<<g, b, 0, s>>>(L0, L0.phi, phi);
+        k_nod_copy<<<g, b, 0, s>>>(L0, L0.phi, phi, 1, 1, 1);
         LAUNCHED(H);
     }
     CUDA_OK(cudaEventRecord(H->ev[3], s));
@@ -291,6 +343,7 @@ extern "C" int maestro_mac_nodal_project(maestro_mac_handle* H, const double* be
     CUDA_OK(cudaStreamSynchronize(s));
     collect_timings(H, st);
     if (d.rel_tol == 0.0 && !trivial) {
+        if (H->singular && (rc = nod_phi_ghosts(H, 0, H->nod[0].phi, s)) != 0) return rc;   // the mean shift left the images stale
         if ((rc = nod_do_residual_norm(H, 0, s)) != 0) return rc;
         CUDA_OK(cudaMemcpyAsync(H->host_scal + 4, H->scal + 4, sizeof(double), cudaMemcpyDeviceToHost, s));
         CUDA_OK(cudaStreamSynchronize(s));
@@ -304,36 +357,35 @@ extern "C" int maestro_mac_nodal_project(maestro_mac_handle* H, const double* be
 
 // ---- step API of the nodal projection ---------------------------------------------------------------------------
 
+static int nod_level_copy(maestro_mac_handle* H, int level, int which, double* pub, int to_public, cudaStream_t s)
+{
+    if (!H || !H->has_nodal || !pub || level < 0 || level >= H->nlev) return MAESTRO_MAC_ERR_ARG;
+    const NodLevel L = dev_nod(H, level);
+    double* internal = which == MAESTRO_MAC_NODAL_PHI ? L.phi : (which == MAESTRO_MAC_NODAL_RHS ? L.rhs : (which == MAESTRO_MAC_NODAL_SIGMA ? L.sigma : nullptr));
+    if (!internal) return MAESTRO_MAC_ERR_ARG;
+    const int node = which == MAESTRO_MAC_NODAL_SIGMA ? 0 : 1;
+    dim3 g, b;
+    nod_dims(L.nx + node, L.ny + node, L.nz + node, &g, &b);
+    k_nod_copy<<<g, b, 0, s>>>(L, internal, pub, node, to_public, which == MAESTRO_MAC_NODAL_PHI ? 1 : 0);
+    LAUNCHED(H);
+    if (to_public) return MAESTRO_MAC_OK;
+    if (which == MAESTRO_MAC_NODAL_SIGMA) return nod_sig_ghosts(H, level, s);
+    if (which == MAESTRO_MAC_NODAL_PHI) {          // the second buffer must hold finite ghosts too (see nod_zero_phi)
+        const NodHost& N = H->nod[level];
+        CUDA_OK(cudaMemsetAsync(N.phi2 - N.onode, 0, N.anode * sizeof(double), s));
+        return nod_phi_ghosts(H, level, internal, s);
+    }
+    return MAESTRO_MAC_OK;
+}
+
 extern "C" int maestro_mac_nodal_level_get(maestro_mac_handle* H, int level, int which, double* dst, void* cuda_stream)
 {
-    if (!H || !H->has_nodal || !dst || level < 0 || level >= H->nlev) return MAESTRO_MAC_ERR_ARG;
-    cudaStream_t s = (cudaStream_t)cuda_stream;
-    const NodHost& N = H->nod[level];
-    if (which == MAESTRO_MAC_NODAL_SIGMA) {
-        CUDA_OK(cudaMemcpyAsync(dst, N.sigma, N.ncell * sizeof(double), cudaMemcpyDeviceToDevice, s));
-        return MAESTRO_MAC_OK;
-    }
-    if (which != MAESTRO_MAC_NODAL_PHI && which != MAESTRO_MAC_NODAL_RHS) return MAESTRO_MAC_ERR_ARG;
-    const NodLevel L = dev_nod(H, level);
-    dim3 g, b;
-    nod_dims(L.nx + 1, L.ny + 1, L.nz + 1, &g, &b);
-    if (which == MAESTRO_MAC_NODAL_PHI) {          // exported with the node rules applied
-        k_nod_export<<<g, b, 0, s>>>(L, L.phi, dst);
-        LAUNCHED(H);
-    } else
-        CUDA_OK(cudaMemcpyAsync(dst, N.rhs, N.nnode * sizeof(double), cudaMemcpyDeviceToDevice, s));
-    return MAESTRO_MAC_OK;
+    return nod_level_copy(H, level, which, dst, 1, (cudaStream_t)cuda_stream);
 }
 
 extern "C" int maestro_mac_nodal_level_set(maestro_mac_handle* H, int level, int which, const double* src, void* cuda_stream)
 {
-    if (!H || !H->has_nodal || !src || level < 0 || level >= H->nlev) return MAESTRO_MAC_ERR_ARG;
-    cudaStream_t s = (cudaStream_t)cuda_stream;
-    const NodHost& N = H->nod[level];
-    double* dst = which == MAESTRO_MAC_NODAL_PHI ? N.phi : (which == MAESTRO_MAC_NODAL_RHS ? N.rhs : (which == MAESTRO_MAC_NODAL_SIGMA ? N.sigma : nullptr));
-    if (!dst) return MAESTRO_MAC_ERR_ARG;
-    CUDA_OK(cudaMemcpyAsync(dst, src, (which == MAESTRO_MAC_NODAL_SIGMA ? N.ncell : N.nnode) * sizeof(double), cudaMemcpyDeviceToDevice, s));
-    return MAESTRO_MAC_OK;
+    return nod_level_copy(H, level, which, const_cast<double*>(src), 0, (cudaStream_t)cuda_stream);
 }
 
 extern "C" int maestro_mac_nodal_step_sigma(maestro_mac_handle* H, const double* beta0, const double* rho0, const double* rho,
