@@ -12,8 +12,11 @@
 // enters with  -w[cls(dx,dy,dz)] * T(dx,dy,dz),  T = the sum of sigma over the cells that contain both a and b.
 //
 // Internal layout of a level (x fastest; pointers address the interior origin, index 0):
-//   node arrays phi, phi2, rhs : idx = i + NX (j + NY k),  NX = nx + 3, NY = ny + 3, i in [-1, nx + 1]  (one ghost node per side)
-//   sigma (cells)              : idx = i + CX (j + CY k),  CX = nx + 2, CY = ny + 2, i in [-1, nx]      (one ghost cell per side)
+//   node arrays phi, phi2, rhs : idx = i + NX (j + NY k),  NX = nx + 4, NY = ny + 3, i in [-1, nx + 1]  (one ghost node per side)
+//   sigma (cells)              : idx = i + CX (j + CY k),  CX = nx + 4, CY = ny + 2, i in [-1, nx]      (one ghost cell per side)
+//   Rows start TWO entries before index 0 (one unused pad entry, then the ghost) and the row pitches are even: TMA wants
+//   16-byte multiples for the pitch AND for the first entry of a box, and the boxes of k_nod_march start at the even
+//   entries x0 - 2 (phi, sigma) and x0 (rhs) of a row.
 // Node rules (N4) expressed in that layout, so that the operator needs no boundary branches:
 //   * a cell outside a non-periodic boundary has sigma = 0 (its ghost entry): the terms of cells that do not exist vanish
 //     whatever (finite) value the ghost nodes hold; on periodic axes ghost cells and ghost nodes hold periodic images;
@@ -26,9 +29,13 @@
 // pre-smoothing sweep of the next one at no extra pass.
 #pragma once
 #include "mac_kernels.cuh"
+#include "mac_setup.cuh"
+#include "mac_smoother_tma.cuh"
 
 struct NodLevel {
     int nx, ny, nz;                 // cells
+    int NX, NY, CX, CY;             // pitches: nodes per row / rows per plane, cells per row / rows per plane (ghosts and
+                                    // one pad entry: row pitches are even, i.e. multiples of 16 bytes, as TMA wants)
     int bclo[3], bchi[3];
     double w[8];                    // class weights; bit 0 / 1 / 2: the other corner along x / y / z
     double omega;                   // Jacobi damping (N7)
@@ -38,11 +45,11 @@ struct NodLevel {
 
 __device__ __forceinline__ long long nod_idx(const NodLevel& L, int i, int j, int k)
 {
-    return (long long)i + (long long)(L.nx + 3) * ((long long)j + (long long)(L.ny + 3) * (long long)k);
+    return (long long)i + (long long)L.NX * ((long long)j + (long long)L.NY * (long long)k);
 }
 __device__ __forceinline__ long long nod_cidx(const NodLevel& L, int i, int j, int k)
 {
-    return (long long)i + (long long)(L.nx + 2) * ((long long)j + (long long)(L.ny + 2) * (long long)k);
+    return (long long)i + (long long)L.CX * ((long long)j + (long long)L.CY * (long long)k);
 }
 __device__ __forceinline__ size_t pub_cidx(const NodLevel& L, int i, int j, int k)      // public cell layout
 {
@@ -78,7 +85,7 @@ __device__ __forceinline__ void nod_store_images(const NodLevel& L, double* __re
 {
     a[q] = v;
     if (ix | iy | iz) {
-        const long long sy = L.nx + 3, sz = sy * (L.ny + 3);
+        const long long sy = L.NX, sz = sy * L.NY;
         const long long ox = ix, oy = (long long)iy * sy, oz = (long long)iz * sz;
         if (ix) a[q + ox] = v;
         if (iy) { a[q + oy] = v; if (ix) a[q + ox + oy] = v; }
@@ -360,13 +367,35 @@ __device__ __forceinline__ void nod_load_sig(NodPlane& T, const double* __restri
     T.v[1][0] = s00 + s10; T.v[1][1] = T.v[0][1] + T.v[2][1]; T.v[1][2] = s01 + s11;
 }
 
+// Staging: the planes a step consumes (phi plane k+1 of the tile plus a one-node ring, the sigma cell plane k, the
+// rhs plane k) are brought into shared memory by TMA box loads (cp.async.bulk.tensor.3d, one elected thread, an
+// mbarrier per stage; no per-thread address arithmetic) three steps ahead (ring of four stages, 7.25 KB each), so the
+// DRAM latency is off the marching step and the step itself reads shared memory only.  The ghost layout keeps every
+// box inside the arrays except beyond the last tile, where the hardware fills zeros that only threads outside the
+// grid read.
+namespace nodm {
+constexpr int TX = 32, TY = 8, NS = 4, LA = 3;
+constexpr int BW = TX + 4;                                            // box width of phi / sigma: entries x0-2 .. x0+33 of a row
+constexpr int kPhi = 2944, kSig = 2688, kRhs = 2048;                  // bytes per stage (128-byte multiples)
+constexpr int kStage = kPhi + kSig + kRhs;
+constexpr unsigned kTx = (TY + 2) * BW * 8 + (TY + 1) * BW * 8 + TY * TX * 8;   // bytes landing per stage
+static_assert((TY + 2) * BW * 8 <= kPhi && (TY + 1) * BW * 8 <= kSig, "stage layout");
+}  // namespace nodm
+
 template <int MODE>
 __global__ void __launch_bounds__(256, 2)
-k_nod_march(NodLevel L, const double* __restrict__ pin, double* __restrict__ out, double* __restrict__ part_max, int zchunk)
+k_nod_march(const __grid_constant__ CUtensorMap tm_phi, const __grid_constant__ CUtensorMap tm_sig,
+            const __grid_constant__ CUtensorMap tm_rhs, NodLevel L, const double* __restrict__ pin, double* __restrict__ out,
+            double* __restrict__ part_max, int zchunk)
 {
-    const int i = blockIdx.x * 32 + threadIdx.x, j = blockIdx.y * 8 + threadIdx.y;
+    using namespace nodm;
+    using tma::mbar_init; using tma::mbar_expect_tx; using tma::mbar_wait; using tma::tma_load_3d; using tma::smem_u32;
+    __shared__ __align__(128) unsigned char ring[NS * kStage];
+    __shared__ __align__(8) unsigned long long bars[NS];
+    const int tx = threadIdx.x, ty = threadIdx.y, tid = tx + TX * ty;
+    const int x0 = blockIdx.x * TX, y0 = blockIdx.y * TY;
+    const int i = x0 + tx, j = y0 + ty;
     const int k0 = blockIdx.z * zchunk, k1 = min(k0 + zchunk, L.nz + 1);
-    const int ic = min(i, L.nx), jc = min(j, L.ny);               // threads beyond the grid march a valid column and store nothing
     int kxy = 3;                                                  // lateral kind: 0 unknown, 1 OUTFLOW, 2 duplicate, 3 outside
     if (i <= L.nx && j <= L.ny) {
         const int ka = nod_axis_kind(L, 0, i), kb = nod_axis_kind(L, 1, j);
@@ -374,14 +403,40 @@ k_nod_march(NodLevel L, const double* __restrict__ pin, double* __restrict__ out
     }
     const int ix = kxy == 0 ? nod_image(L, 0, i) : 0, iy = kxy == 0 ? nod_image(L, 1, j) : 0;
     double rmax = 0.0;
-    const long long py = L.nx + 3, pz = py * (L.ny + 3), cy = L.nx + 2, cz = cy * (L.ny + 2);
-    const double* q = pin + nod_idx(L, ic, jc, k0);
-    const double* sg = L.sigma + nod_cidx(L, ic - 1, jc - 1, k0 - 1);
-    long long qo = nod_idx(L, ic, jc, k0);
+    const long long py = L.NX, pz = py * L.NY, cy = L.CX;
+    const unsigned ring0 = smem_u32(ring), bar0 = smem_u32(bars);
+    const bool producer = tid == 0;
+    // stage of step k: phi plane k+1 (box origin: node (x0-2, y0-1)), cell plane k (cell (x0-2, y0-1)), rhs plane k (node
+    // (x0, y0)); tensor-map coordinates count from the allocation origin: entry -2 of a row, row -1, plane -1
+    auto issue = [&](int k) {
+        if (k < k1) {
+            const unsigned s = (unsigned)(k - k0) & (NS - 1), d = ring0 + s * kStage, bar = bar0 + 8 * s;
+            mbar_expect_tx(bar, kTx);
+            tma_load_3d(d, &tm_phi, bar, x0, y0, k + 2);
+            tma_load_3d(d + kPhi, &tm_sig, bar, x0, y0, k + 1);
+            tma_load_3d(d + kPhi + kSig, &tm_rhs, bar, x0 + 2, y0 + 1, k + 1);
+        }
+    };
+    static_assert(NS == 4 && LA == 3, "ring arithmetic below");
+    if (producer) {
+        for (int q = 0; q < NS; ++q) mbar_init(bar0 + 8 * q, 1);
+        asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
+        asm volatile("fence.proxy.async.shared::cta;\n" ::: "memory");
+        for (int q = 0; q < LA; ++q) issue(k0 + q);
+    }
+    // planes k0-1, k0 and the cell plane k0-1 directly (once per chunk)
+    const int ic = min(i, L.nx), jc = min(j, L.ny);
     NodPlane P[3], T[2];
-    nod_load_phi(P[0], q - pz, py);
-    nod_load_phi(P[1], q, py);
-    nod_load_sig(T[0], sg, cy);
+    {
+        const double* q = pin + nod_idx(L, ic, jc, k0);
+        nod_load_phi(P[0], q - pz, py);
+        nod_load_phi(P[1], q, py);
+        nod_load_sig(T[0], L.sigma + nod_cidx(L, ic - 1, jc - 1, k0 - 1), cy);
+    }
+    __syncthreads();                                              // barrier inits visible before anyone waits
+    long long qo = nod_idx(L, ic, jc, k0);
+    const unsigned char* mine = ring + (ty * BW + tx + 1) * 8;    // node (i-1, j-1) of the phi box = cell (i-1, j-1) of the sigma box
+    unsigned phase = 0;
 #pragma unroll 1
     for (int k = k0; k < k1; k += 6) {
 #pragma unroll
@@ -392,9 +447,27 @@ k_nod_march(NodLevel L, const double* __restrict__ pin, double* __restrict__ out
             NodPlane& Pp = P[(u + 2) % 3];
             NodPlane& Tlo = T[u % 2];
             NodPlane& Tup = T[(u + 1) % 2];
-            nod_load_phi(Pp, q + pz, py);
-            nod_load_sig(Tup, sg + cz, cy);
-            const double rh = L.rhs[qo];
+            const unsigned s = (unsigned)(k + u - k0) & (NS - 1);
+            mbar_wait(bar0 + 8 * s, (phase >> s) & 1u);  // the stage of this step has landed
+            phase ^= 1u << s;
+            __syncthreads();                             // every thread has finished step k-1: its stage can be refilled
+            if (producer) {
+                asm volatile("fence.proxy.async.shared::cta;\n" ::: "memory");
+                issue(k + u + LA);
+            }
+            const double* sphi = reinterpret_cast<const double*>(mine + s * kStage);
+            const double* ssig = reinterpret_cast<const double*>(mine + s * kStage + kPhi);
+#pragma unroll
+            for (int b = 0; b < 3; ++b)
+#pragma unroll
+                for (int a = 0; a < 3; ++a) Pp.v[b][a] = sphi[b * BW + a];
+            {
+                const double s00 = ssig[0], s01 = ssig[1], s10 = ssig[BW], s11 = ssig[BW + 1];
+                Tup.v[0][0] = s00; Tup.v[0][1] = s00 + s01; Tup.v[0][2] = s01;
+                Tup.v[2][0] = s10; Tup.v[2][1] = s10 + s11; Tup.v[2][2] = s11;
+                Tup.v[1][0] = s00 + s10; Tup.v[1][1] = Tup.v[0][1] + Tup.v[2][1]; Tup.v[1][2] = s01 + s11;
+            }
+            const double rh = *reinterpret_cast<const double*>(ring + s * kStage + kPhi + kSig + tid * 8);
             double acc0 = 0.0, acc1 = 0.0;
 #pragma unroll
             for (int b = 0; b < 3; ++b)
@@ -410,18 +483,17 @@ k_nod_march(NodLevel L, const double* __restrict__ pin, double* __restrict__ out
                 const double r = rh + (acc0 + acc1);                          // rhs - L phi, L phi = -(acc0 + acc1)
                 if (MODE & NOD_NORM) rmax = nanmax(rmax, fabs(r));
                 if (MODE & NOD_JACOBI) {
-                    const double dg = -(L.w[0] * (Tlo.v[1][1] + Tup.v[1][1]));
-                    nod_store_images(L, out, qo, Pc.v[1][1] + L.omega * r / dg, ix, iy, nod_image(L, 2, k + u));
+                    const double ndg = L.w[0] * (Tlo.v[1][1] + Tup.v[1][1]);  // -L_aa > 0
+                    nod_store_images(L, out, qo, Pc.v[1][1] - fast_div_pos(L.omega * r, ndg), ix, iy, nod_image(L, 2, k + u));
                 } else if (out) out[qo] = r;
             } else if (kxy <= 1 && (kxy == 1 || kz == 1) && out) {
                 out[qo] = 0.0;                                                // OUTFLOW node
             }
-            q += pz; sg += cz; qo += pz;
+            qo += pz;
         }
     }
     if (MODE & NOD_NORM) {
         __shared__ double sh[8];
-        const int tid = threadIdx.x + 32 * threadIdx.y;
         rmax = warp_nanmax(rmax);
         if ((tid & 31) == 0) sh[tid >> 5] = rmax;
         __syncthreads();

@@ -55,8 +55,12 @@ struct NodHost {                   // one level of the nodal projection (desc.no
     size_t nnode, ncell;           // nodes (nx+1)(ny+1)(nz+1) and cells of the level
     size_t anode, acell;           // allocated entries: one ghost node / ghost cell per side
     size_t onode, ocell;           // entries from an allocation's base to the interior origin
+    int NX, NY, CX, CY;            // row pitches (even: 16-byte multiples) and rows per plane of the node / cell arrays
     double *phi, *phi2, *rhs;      // node arrays (interior origins)
     double *sigma;                 // cell array (interior origin)
+    double* phi_a;                 // the buffer `phi` pointed to at carve time (tensor map tm_phi; tm_phi2 is its partner)
+    CUtensorMap tm_phi, tm_phi2, tm_rhs, tm_sig;   // box loads of k_nod_march: 36 x 10 nodes, 36 x 9 cells, 32 x 8 nodes
+    int tma_ok;
 };
 
 }  // namespace
@@ -212,12 +216,15 @@ size_t carve(maestro_mac_handle* H, char* base)
             for (int a = 0; a < 3; ++a) { N.n[a] = H->lev[l].n[a]; N.h[a] = H->lev[l].h[a]; }
             N.nnode = (size_t)(N.n[0] + 1) * (N.n[1] + 1) * (N.n[2] + 1);
             N.ncell = H->lev[l].ncell;
-            N.anode = (size_t)(N.n[0] + 3) * (N.n[1] + 3) * (N.n[2] + 3);
-            N.acell = (size_t)(N.n[0] + 2) * (N.n[1] + 2) * (N.n[2] + 2);
-            N.onode = 1 + (size_t)(N.n[0] + 3) * (1 + (size_t)(N.n[1] + 3));
-            N.ocell = 1 + (size_t)(N.n[0] + 2) * (1 + (size_t)(N.n[1] + 2));
+            N.NX = (N.n[0] + 4 + 1) & ~1; N.NY = N.n[1] + 3;     // rows: pad, ghost, nodes 0..nx, ghost
+            N.CX = (N.n[0] + 3 + 1) & ~1; N.CY = N.n[1] + 2;     // rows: pad, ghost, cells 0..nx-1, ghost
+            N.anode = (size_t)N.NX * N.NY * (N.n[2] + 3);
+            N.acell = (size_t)N.CX * N.CY * (N.n[2] + 2);
+            N.onode = 2 + (size_t)N.NX * (1 + (size_t)N.NY);
+            N.ocell = 2 + (size_t)N.CX * (1 + (size_t)N.CY);
             auto at = [&](void* b, size_t o) -> double* { return b ? (double*)b + o : nullptr; };
             N.phi = at(take(N.anode, 8), N.onode);
+            N.phi_a = N.phi;
             N.phi2 = at(take(N.anode, 8), N.onode);
             N.rhs = at(take(N.anode, 8), N.onode);
             N.sigma = at(take(N.acell, 8), N.ocell);
@@ -758,6 +765,16 @@ extern "C" int maestro_mac_setup(const maestro_mac_desc* desc, void* workspace, 
             tma_build_maps(&H->lev[l].tma[2], D, t2::LN, t2::TYE);
             // a level laid out with periodic images has no other smoother: its tensor maps must exist
             if ((D.gx || D.gy) && !H->lev[l].tma[H->d.smoother == 3 ? 1 : 0].ok) ok = false;
+        }
+    if (ok && H->has_nodal)
+        for (int l = 0; l < H->nlev; ++l) {          // tensor maps of k_nod_march (Jacobi sweeps, residuals)
+            NodHost& N = H->nod[l];
+            const uint64_t nzn = (uint64_t)N.n[2] + 3, nzc = (uint64_t)N.n[2] + 2;
+            N.tma_ok = tma_encode3(&N.tm_phi, N.phi - N.onode, N.NX, N.NY, nzn, N.NX, N.NY, nodm::BW, nodm::TY + 2) &&
+                       tma_encode3(&N.tm_phi2, N.phi2 - N.onode, N.NX, N.NY, nzn, N.NX, N.NY, nodm::BW, nodm::TY + 2) &&
+                       tma_encode3(&N.tm_rhs, N.rhs - N.onode, N.NX, N.NY, nzn, N.NX, N.NY, nodm::TX, nodm::TY) &&
+                       tma_encode3(&N.tm_sig, N.sigma - N.ocell, N.CX, N.CY, nzc, N.CX, N.CY, nodm::BW, nodm::TY + 1);
+            if (!N.tma_ok) ok = false;
         }
     if (!ok) {
         maestro_mac_free(H);

@@ -9,6 +9,7 @@ NodLevel dev_nod(const maestro_mac_handle* H, int l)
     const NodHost& N = H->nod[l];
     NodLevel D;
     D.nx = N.n[0]; D.ny = N.n[1]; D.nz = N.n[2];
+    D.NX = N.NX; D.NY = N.NY; D.CX = N.CX; D.CY = N.CY;
     double g[3], gsum = 0.0, gmax = 0.0;
     for (int a = 0; a < 3; ++a) {
         D.bclo[a] = H->d.bc_lo[a]; D.bchi[a] = H->d.bc_hi[a];
@@ -43,19 +44,24 @@ void nod_dims_red(int ex, int ey, int ez, dim3* grid, dim3* block, int* zper)
     *zper = zp;
 }
 
-// grid of the z-marching operator pass (k_nod_march, 32 x 8 node tiles): enough z-chunks for a few blocks per SM, chunks
-// of at least 16 planes (a chunk reloads two planes), and at most kMaxParts blocks (one partial maximum each)
+// grid of the z-marching operator pass (k_nod_march, 32 x 8 node tiles, two blocks per SM): the chunk count that
+// minimises waves x (planes per chunk + the planes a chunk loads directly), chunks of at least 16 planes, and at most
+// kMaxParts blocks (one partial maximum each)
 dim3 nod_march_grid(const maestro_mac_handle* H, const NodLevel& L, int* zchunk)
 {
     const int tx = (L.nx + 1 + 31) / 32, ty = (L.ny + 1 + 7) / 8, nzn = L.nz + 1;
-    int nchunk = (6 * H->sms + tx * ty - 1) / (tx * ty);
-    const int maxchunk = (nzn + 15) / 16;
-    if (nchunk > maxchunk) nchunk = maxchunk;
-    if (nchunk < 1) nchunk = 1;
-    int zc = (nzn + nchunk - 1) / nchunk;
-    while ((long)tx * ty * ((nzn + zc - 1) / zc) > kMaxParts) zc *= 2;
-    *zchunk = zc;
-    return dim3(tx, ty, (nzn + zc - 1) / zc);
+    const long slots = 2L * H->sms;
+    const int maxchunk = nzn >= 32 ? nzn / 16 : 1;
+    long best = -1;
+    int bz = nzn;
+    for (int n = 1; n <= maxchunk; ++n) {
+        const int zc = (nzn + n - 1) / n, nn = (nzn + zc - 1) / zc;
+        if ((long)tx * ty * nn > kMaxParts) break;
+        const long cost = (((long)tx * ty * nn + slots - 1) / slots) * (zc + 4);
+        if (best < 0 || cost < best) { best = cost; bz = zc; }
+    }
+    *zchunk = bz;
+    return dim3(tx, ty, (nzn + bz - 1) / bz);
 }
 
 // folds nb block partials into scal[off] (sum) and scal[off + 1] (max)
@@ -153,11 +159,13 @@ int nod_do_jacobi(maestro_mac_handle* H, int l, cudaStream_t s, int* norm_parts 
     const NodLevel L = dev_nod(H, l);
     int zchunk;
     const dim3 g = nod_march_grid(H, L, &zchunk);
+    const NodHost& N = H->nod[l];
+    const CUtensorMap& tin = N.phi == N.phi_a ? N.tm_phi : N.tm_phi2;
     if (norm_parts) {
         *norm_parts = (int)(g.x * g.y * g.z);
-        k_nod_march<NOD_JACOBI | NOD_NORM><<<g, dim3(32, 8), 0, s>>>(L, L.phi, L.phi2, H->part_max, zchunk);
+        k_nod_march<NOD_JACOBI | NOD_NORM><<<g, dim3(32, 8), 0, s>>>(tin, N.tm_sig, N.tm_rhs, L, L.phi, L.phi2, H->part_max, zchunk);
     } else
-        k_nod_march<NOD_JACOBI><<<g, dim3(32, 8), 0, s>>>(L, L.phi, L.phi2, nullptr, zchunk);
+        k_nod_march<NOD_JACOBI><<<g, dim3(32, 8), 0, s>>>(tin, N.tm_sig, N.tm_rhs, L, L.phi, L.phi2, nullptr, zchunk);
     LAUNCHED(H);
     if (swap) { double* t = H->nod[l].phi; H->nod[l].phi = H->nod[l].phi2; H->nod[l].phi2 = t; }
     return MAESTRO_MAC_OK;
@@ -179,7 +187,8 @@ int nod_do_residual_restrict(maestro_mac_handle* H, int l, cudaStream_t s)
     dim3 g, b;
     int zchunk;
     g = nod_march_grid(H, F, &zchunk);
-    k_nod_march<NOD_RESID><<<g, dim3(32, 8), 0, s>>>(F, F.phi, F.phi2, nullptr, zchunk);
+    const NodHost& N = H->nod[l];
+    k_nod_march<NOD_RESID><<<g, dim3(32, 8), 0, s>>>(N.phi == N.phi_a ? N.tm_phi : N.tm_phi2, N.tm_sig, N.tm_rhs, F, F.phi, F.phi2, nullptr, zchunk);
     LAUNCHED(H);
     nod_dims(C.nx + 1, C.ny + 1, C.nz + 1, &g, &b);
     k_nod_restrict<<<g, b, 0, s>>>(F, C, F.phi2);
@@ -231,7 +240,9 @@ int nod_do_residual_norm(maestro_mac_handle* H, int l, cudaStream_t s)
     const NodLevel L = dev_nod(H, l);
     int zchunk;
     const dim3 g = nod_march_grid(H, L, &zchunk);
-    k_nod_march<NOD_RESID | NOD_NORM><<<g, dim3(32, 8), 0, s>>>(L, L.phi, nullptr, H->part_max, zchunk);
+    const NodHost& N = H->nod[l];
+    k_nod_march<NOD_RESID | NOD_NORM><<<g, dim3(32, 8), 0, s>>>(N.phi == N.phi_a ? N.tm_phi : N.tm_phi2, N.tm_sig, N.tm_rhs, L, L.phi, nullptr,
+                                                                H->part_max, zchunk);
     LAUNCHED(H);
     return nod_fold(H, (int)(g.x * g.y * g.z), 3, s);
 }
