@@ -543,19 +543,54 @@ k_nod_restrict(NodLevel F, NodLevel C, const double* __restrict__ res)
 }
 
 // ---- N6: phi_f += P e_c at the fine unknowns (trilinear: weights 1, 1/2, 1/4, 1/8), images included --------------
+// One thread per COARSE node (I, J, K) adds the interpolant to the up to 8 fine nodes
+// (2I + a, 2J + b, 2K + c), a, b, c in {0, 1}: 8 coarse values (through the node rules) are shared by the 8 fine nodes,
+// the fine values move as 16-byte x pairs.  Per fine node: wt * (sum of the coarse corners it lies between).
 __global__ void __launch_bounds__(256)
-k_nod_prolong_add(NodLevel F, NodLevel C)
+k_nod_prolong_add2(NodLevel F, NodLevel C)
 {
-    const int i = blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y * blockDim.y + threadIdx.y, k = blockIdx.z;
-    if (i > F.nx || j > F.ny || nod_kind(F, i, j, k) != 0) return;
-    const int I = i >> 1, J = j >> 1, K = k >> 1, oi = i & 1, oj = j & 1, ok = k & 1;
-    const double wt = (oi ? 0.5 : 1.0) * (oj ? 0.5 : 1.0) * (ok ? 0.5 : 1.0);
-    double s = 0.0;
-    for (int c = 0; c <= ok; ++c)
-        for (int b = 0; b <= oj; ++b)
-            for (int a = 0; a <= oi; ++a) s += wt * nod_val(C, C.phi, I + a, J + b, K + c);
-    const long long q = nod_idx(F, i, j, k);
-    nod_store_images(F, F.phi, q, F.phi[q] + s, nod_image(F, 0, i), nod_image(F, 1, j), nod_image(F, 2, k));
+    const int I = blockIdx.x * blockDim.x + threadIdx.x, J = blockIdx.y * blockDim.y + threadIdx.y, K = blockIdx.z;
+    if (I > C.nx || J > C.ny) return;
+    double e[2][2][2];
+#pragma unroll
+    for (int c = 0; c < 2; ++c)
+#pragma unroll
+        for (int b = 0; b < 2; ++b)
+#pragma unroll
+            for (int a = 0; a < 2; ++a)
+                e[c][b][a] = (I + a <= C.nx && J + b <= C.ny && K + c <= C.nz) ? nod_val(C, C.phi, I + a, J + b, K + c) : 0.0;
+    const int i = 2 * I, j = 2 * J, k = 2 * K;
+    const bool x1 = i + 1 <= F.nx;
+#pragma unroll
+    for (int c = 0; c < 2; ++c) {
+        if (k + c > F.nz) continue;
+#pragma unroll
+        for (int b = 0; b < 2; ++b) {
+            if (j + b > F.ny) continue;
+            const long long q = nod_idx(F, i, j + b, k + c);
+            // fine node (i + a, j + b, k + c): weight 1/2 per odd axis, corners (0..a, 0..b, 0..c)
+            double s0 = 0.0, s1 = 0.0;
+            for (int cc = 0; cc <= c; ++cc)
+                for (int bb = 0; bb <= b; ++bb) {
+                    s0 += e[cc][bb][0];
+                    s1 += e[cc][bb][0];
+                    s1 += e[cc][bb][1];
+                }
+            const double wt = (b ? 0.5 : 1.0) * (c ? 0.5 : 1.0);
+            const int iy = nod_image(F, 1, j + b), iz = nod_image(F, 2, k + c);
+            const int k0 = nod_kind(F, i, j + b, k + c), k1 = x1 ? nod_kind(F, i + 1, j + b, k + c) : 3;
+            if (k0 == 0 && k1 == 0 && !(iy | iz) && nod_image(F, 0, i) == 0 && nod_image(F, 0, i + 1) == 0) {
+                double2* p2 = reinterpret_cast<double2*>(F.phi + q);          // node 2I sits at an even entry of its row
+                double2 v = *p2;
+                v.x += wt * s0;
+                v.y += (0.5 * wt) * s1;
+                *p2 = v;
+            } else {
+                if (k0 == 0) nod_store_images(F, F.phi, q, F.phi[q] + wt * s0, nod_image(F, 0, i), iy, iz);
+                if (k1 == 0) nod_store_images(F, F.phi, q + 1, F.phi[q + 1] + (0.5 * wt) * s1, nod_image(F, 0, i + 1), iy, iz);
+            }
+        }
+    }
 }
 
 // ---- N10: U <- U - (1/rho) G phi, G the cell-mean gradient (mean of the 4 edge differences per axis) -----------

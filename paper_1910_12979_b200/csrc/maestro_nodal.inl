@@ -199,10 +199,10 @@ int nod_do_residual_restrict(maestro_mac_handle* H, int l, cudaStream_t s)
 
 int nod_do_prolong(maestro_mac_handle* H, int l, cudaStream_t s)
 {
-    const NodLevel F = dev_nod(H, l);
+    const NodLevel F = dev_nod(H, l), C = dev_nod(H, l + 1);
     dim3 g, b;
-    nod_dims(F.nx + 1, F.ny + 1, F.nz + 1, &g, &b);
-    k_nod_prolong_add<<<g, b, 0, s>>>(F, dev_nod(H, l + 1));
+    nod_dims(C.nx + 1, C.ny + 1, C.nz + 1, &g, &b);
+    k_nod_prolong_add2<<<g, b, 0, s>>>(F, C);                       // one thread per coarse node
     LAUNCHED(H);
     return MAESTRO_MAC_OK;
 }
