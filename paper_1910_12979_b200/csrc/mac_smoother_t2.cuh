@@ -44,14 +44,26 @@ namespace t2 {
 using fused::pick; using fused::put;
 using tma::mbar_init; using tma::mbar_expect_tx; using tma::mbar_wait; using tma::tma_load_3d; using tma::smem_u32;
 
-constexpr int LN = 16, TYE = 24, NT = LN * TYE;      // 16 pairs x 24 rows = 384 threads
-constexpr int HALO = 4;
-constexpr int kTX = 2 * LN - 2 * HALO;               // 24 finished columns per tile
-constexpr int kTY = TYE - 2 * HALO;                  // 16 finished rows per tile
-constexpr int kRow = LN * 16;                        // bytes of one staged row
-constexpr int kPl = TYE * kRow;                      // bytes of one staged array plane
-constexpr int kPad = 512;                            // readable slack below the phi ring (masked lanes read row -1)
-enum { C_AX = 0, C_AY = 1, C_AZ = 2, C_RHS = 3, C_COUNT = 4 };
+constexpr int LN = 16, TYE = 24, NT = LN * TYE;      // 16 pairs x 24 rows = 384 threads: the COMPUTED cells (32 x 24)
+constexpr int HALO = 4;                              // cells a finished cell depends on laterally (periodic image width)
+// Only three of the four rings around a finished cell are COMPUTED (sweep-1 red / black, sweep-2 red); the fourth is
+// the old black value that sweep-1 red reads.  So the staged phi box is one cell wider than the computed tile on every
+// side (two in x, to keep box origins even: 16-byte aligned rows) and has no threads of its own, and a tile finishes
+// the computed cells that are >= 3 cells inside: 26 columns (x0-1 .. x0+24 for computed x0-4 .. x0+27) x 18 rows.
+constexpr int CH = 3;                                // computed rings
+constexpr int kTX = 2 * LN - 2 * CH;                 // 26 finished columns per tile: [x0 - 1, x0 + 25)
+constexpr int kTY = TYE - 2 * CH;                    // 18 finished rows per tile:    [y0, y0 + 18), thread row ty is row y0 - 3 + ty
+constexpr int SX = 2 * LN + 4, SY = TYE + 2;         // staged phi box: columns x0-6 .. x0+29, rows y0-4 .. y0+21
+constexpr int AXW = 2 * LN + 2;                      // staged ax box: faces x0-4 .. x0+29 (x0+28 is the last one read)
+constexpr int kRowP = SX * 8;                        // bytes of one staged phi row
+constexpr int kPlP = ((SY * kRowP + 127) / 128) * 128;   // bytes of one phi stage (128-byte multiple: TMA destinations)
+constexpr int kRow = LN * 16;                        // bytes of one staged row of ay, az, rhs (the computed columns)
+constexpr int kRowA = AXW * 8;                       // bytes of one staged row of ax
+constexpr int kPad = 512;                            // readable slack below the phi ring
+// one coefficient stage: ax (TYE rows), ay (TYE + 1 face rows), az, rhs (TYE rows); every array starts 128-byte aligned
+constexpr int O_AX = 0, O_AY = O_AX + TYE * kRowA, O_AZ = O_AY + (TYE + 1) * kRow, O_RHS = O_AZ + TYE * kRow;
+constexpr int kCoefStage = O_RHS + TYE * kRow;
+static_assert(O_AY % 128 == 0 && O_AZ % 128 == 0 && O_RHS % 128 == 0 && kCoefStage % 128 == 0, "TMA destinations are 128-byte aligned");
 constexpr int kExRow = LN * 8;                       // exchange plane: one double per pair, TYE + 2 rows (a pad row each side)
 constexpr int kEx = (TYE + 2) * kExRow;
 enum { EX_RA = 0, EX_BA = 2, EX_RB = 4 };            // sweep-1 red, sweep-1 black, sweep-2 red; two buffers each
@@ -59,15 +71,15 @@ enum { EX_RA = 0, EX_BA = 2, EX_RB = 4 };            // sweep-1 red, sweep-1 bla
 template <int LA>
 struct Cfg {
     static constexpr int NP = LA + 2, NC = LA + 2;   // planes k, k+1 resident + LA in flight
-    static constexpr int kCoef = C_COUNT * kPl;
-    static constexpr unsigned kTx = (unsigned)kRow * (TYE + (TYE - 1) + 3 * (TYE - 2));   // bytes landing per plane
-    static constexpr size_t kSmem = (size_t)kPad + (size_t)NP * kPl + (size_t)NC * kCoef + 6 * kEx + 8 * NP + 128;
+    static constexpr int kCoef = kCoefStage;
+    static constexpr unsigned kTx = (unsigned)(SY * kRowP + kCoefStage);   // bytes landing per plane
+    static constexpr size_t kSmem = (size_t)kPad + (size_t)NP * kPlP + (size_t)NC * kCoef + 6 * kEx + 8 * NP + 128;
 };
 
 __device__ __forceinline__ double2 ldp(const unsigned char* p) { return *reinterpret_cast<const double2*>(p); }
 template <bool X> __device__ __forceinline__ double ldc(const unsigned char* p, int dy, int dl)
 {
-    return *reinterpret_cast<const double*>(p + dy * kRow + dl * 16 + (X ? 0 : 8));
+    return *reinterpret_cast<const double*>(p + dy * kRowP + dl * 16 + (X ? 0 : 8));
 }
 
 struct Coef {                                // coefficients of one plane for a column pair, in registers, and the
@@ -77,9 +89,10 @@ struct Coef {                                // coefficients of one plane for a 
 
 struct Th {                                  // per-thread constants
     unsigned char* phi0;                     // own slot of phi stage 0
-    const unsigned char* coef0;              // own slot of coefficient stage 0, array C_AX
+    const unsigned char* coef0;              // own slot of coefficient stage 0 in the 32-column arrays (add O_AY, O_AZ, O_RHS)
+    const unsigned char* cax0;               // own slot of coefficient stage 0, array ax
     unsigned char* ex0;                      // own element of exchange buffer 0
-    bool ra_x, ra_y, ba, rb_x, rb_y, own;    // lateral validity of the four half-sweeps (x / y cell of the pair)
+    bool ra, ba_x, ba_y, rb, own_x, own_y;   // lateral validity of the four half-sweeps (x / y cell of the pair)
     long long img_x, img_y;                  // periodic images of the own pair (0 = none)
     // half-sweep h is applied at step kk iff (unsigned)(kk - lo[h]) <= span[h]: the planes it is wanted on
     // (sweep-1 red [k0-3, k1+2], black [k0-2, k1+1], sweep-2 red [k0-1, k1], black [k0, k1-1]) that exist
@@ -146,13 +159,13 @@ __device__ __forceinline__ void issue_plane(const CUtensorMap* tm_phi, const CUt
     if (perz) { if (p < 0) p += nz; else if (p >= nz) p -= nz; }
     const unsigned dp = phi_ring + op;
     const unsigned dc = coef_ring + oc;
-    const unsigned bar = bar0 + op / (kPl / 8);                                // barrier of phi stage op / kPl
+    const unsigned bar = bar0 + op / (kPlP / 8);                               // barrier of phi stage op / kPlP
     mbar_expect_tx(bar, G::kTx);
-    tma_load_3d(dp, tm_phi, bar, cx, cy, p);                                   // rows 0 .. TYE-1
-    tma_load_3d(dc + C_RHS * kPl + kRow, tm_rhs, bar, cx, cy + 1, p);          // rows 1 .. TYE-2
-    tma_load_3d(dc + C_AX * kPl + kRow, tm_ax, bar, cx, cy + 1, p);
-    tma_load_3d(dc + C_AZ * kPl + kRow, tm_az, bar, cx, cy + 1, p);
-    tma_load_3d(dc + C_AY * kPl + kRow, tm_ay, bar, cx, cy + 1, p);            // rows 1 .. TYE-1 (faces)
+    tma_load_3d(dp, tm_phi, bar, cx - 2, cy - 1, p);                           // SX x SY: one more ring (two columns in x)
+    tma_load_3d(dc + O_RHS, tm_rhs, bar, cx, cy, p);                           // the computed cells
+    tma_load_3d(dc + O_AX, tm_ax, bar, cx, cy, p);                             // AXW faces a row
+    tma_load_3d(dc + O_AZ, tm_az, bar, cx, cy, p);
+    tma_load_3d(dc + O_AY, tm_ay, bar, cx, cy, p);                             // TYE + 1 face rows
 }
 
 // One marching step at plane kk; X: the x column of the pair is red in plane kk; W: exchange buffers written by this
@@ -160,7 +173,8 @@ __device__ __forceinline__ void issue_plane(const CUtensorMap* tm_phi, const CUt
 // CUR receives the coefficients of plane kk; S1, S2, S3 hold those of planes kk-1, kk-2, kk-3.
 template <bool X, int W, bool NORM>
 __device__ __forceinline__ void step(const Th& T, int kk, const unsigned char* s0, const unsigned char* sP,
-                                     const unsigned char* cI, const unsigned char* cP, double* __restrict__ out,
+                                     const unsigned char* cI, const unsigned char* cP, const unsigned char* aI,
+                                     double* __restrict__ out,
                                      double2& Pn, double2& Pm1, double2& Pm2, double2& Pm3, double2& Pm4, double2& azn,
                                      Coef& CUR, Coef& S1, Coef& S2, Coef& S3, double& vmax, bool& vnan)
 {
@@ -170,12 +184,12 @@ __device__ __forceinline__ void step(const Th& T, int kk, const unsigned char* s
     double2 P0 = Pn;                                  // old phi of plane kk (staged read of the last step)
     CUR.az = azn;
     Pn = ldp(sP);                                     // old phi and low z faces of plane kk+1
-    azn = ldp(cP + C_AZ * kPl);
-    CUR.ax = ldp(cI + C_AX * kPl);
-    CUR.ax2 = *reinterpret_cast<const double*>(cI + C_AX * kPl + 16);
-    CUR.ays = ldp(cI + C_AY * kPl);
-    CUR.ayn = ldp(cI + C_AY * kPl + kRow);
-    CUR.rhs = ldp(cI + C_RHS * kPl);
+    azn = ldp(cP + O_AZ);
+    CUR.ax = ldp(aI);
+    CUR.ax2 = *reinterpret_cast<const double*>(aI + 16);
+    CUR.ays = ldp(cI + O_AY);
+    CUR.ayn = ldp(cI + O_AY + kRow);
+    CUR.rhs = ldp(cI + O_RHS);
     const Lat l0 = lat_load<X>(s0);                                   // old black neighbours in plane kk
     const Lat l1 = lat_ex<X>(T.ex0 + (EX_RA + R) * kEx);              // sweep-1 red neighbours in plane kk-1
     const Lat l2 = lat_ex<X>(T.ex0 + (EX_BA + R) * kEx);              // sweep-1 black neighbours in plane kk-2
@@ -185,25 +199,27 @@ __device__ __forceinline__ void step(const Th& T, int kk, const unsigned char* s
     const double n0 = gs_cell<X, true>(l0, pick<!X>(P0), CUR, azn, pick<X>(Pm1), pick<X>(Pn), a, dg);
     if (NORM) {                                       // |rhs - (sum - phi_0 dg)| of the input; a NaN sets the sign of vmax
         const double rr = fabs(fma(pick<X>(P0), dg, -a));
-        const bool on = T.own && (unsigned)(kk - T.nlo) <= T.nspan;
+        const bool on = (X ? T.own_x : T.own_y) && (unsigned)(kk - T.nlo) <= T.nspan;
         vmax = fmax(vmax, on ? rr : 0.0);             // (fmax drops NaNs: they are recorded separately)
         vnan = vnan || (on && rr != rr);
     }
-    put<X>(P0, ((X ? T.ra_x : T.ra_y) && v0) ? n0 : pick<X>(P0));
+    put<X>(P0, (T.ra && v0) ? n0 : pick<X>(P0));
     // (2) sweep 1, black cells of plane kk-1
     const double n1 = gs_cell<X, true>(l1, pick<!X>(Pm1), S1, CUR.az, pick<X>(Pm2), pick<X>(P0), a, dg);
-    put<X>(Pm1, (T.ba && v1) ? n1 : pick<X>(Pm1));
+    put<X>(Pm1, ((X ? T.ba_x : T.ba_y) && v1) ? n1 : pick<X>(Pm1));
     // (3) sweep 2, red cells of plane kk-2
     const double n2 = gs_cell<X, false>(l2, pick<!X>(Pm2), S2, S1.az, pick<X>(Pm3), pick<X>(Pm1), a, dg);
-    put<X>(Pm2, ((X ? T.rb_x : T.rb_y) && v2) ? n2 : pick<X>(Pm2));
+    put<X>(Pm2, (T.rb && v2) ? n2 : pick<X>(Pm2));
     // (4) sweep 2, black cells of plane kk-3; the plane is finished
     const double n3 = gs_cell<X, false>(l3, pick<!X>(Pm3), S3, S2.az, pick<X>(Pm4), pick<X>(Pm2), a, dg);
     *reinterpret_cast<double*>(T.ex0 + (EX_RA + W) * kEx) = pick<X>(P0);
     *reinterpret_cast<double*>(T.ex0 + (EX_BA + W) * kEx) = pick<X>(Pm1);
     *reinterpret_cast<double*>(T.ex0 + (EX_RB + W) * kEx) = pick<X>(Pm2);
-    if (T.own && v3) {
-        put<X>(Pm3, n3);
-        store_images(reinterpret_cast<double2*>(out), Pm3, T.img_x, T.img_y);
+    if (v3) {                                         // plane kk-3 leaves: the owned cells of the pair
+        if (X ? T.own_x : T.own_y) put<X>(Pm3, n3);
+        if (T.own_x && T.own_y) store_images(reinterpret_cast<double2*>(out), Pm3, T.img_x, T.img_y);
+        else if (T.own_x) store_images(out, Pm3.x, T.img_x, T.img_y);
+        else if (T.own_y) store_images(out + 1, Pm3.y, T.img_x, T.img_y);
     }
     Pm4 = Pm3; Pm3 = Pm2; Pm2 = Pm1; Pm1 = P0;
 }
@@ -230,11 +246,11 @@ __device__ __forceinline__ void stage(const Th& T, int kk, int ke, unsigned& s0,
     __syncthreads();                                           // every thread has finished step kk-1
     if (producer && kk + 1 + LA <= ke + 1) {                   // never leave a load in flight at exit
         asm volatile("fence.proxy.async.shared::cta;\n" ::: "memory");
-        issue_plane<LA>(tm_phi, tm_rhs, tm_ax, tm_ay, tm_az, phi_ring, coef_ring, bar0, sN * kPl, sN * G::kCoef,
+        issue_plane<LA>(tm_phi, tm_rhs, tm_ax, tm_ay, tm_az, phi_ring, coef_ring, bar0, sN * kPlP, sN * G::kCoef,
                         kk + 1 + LA, nz, perz, cx, cy);
     }
-    step<X, J & 1, NORM>(T, kk, T.phi0 + s0 * kPl, T.phi0 + sP * kPl, T.coef0 + s0 * G::kCoef, T.coef0 + sP * G::kCoef,
-                         out, Pn, Pm1, Pm2, Pm3, Pm4, azn, CUR, S1, S2, S3, vmax, vnan);
+    step<X, J & 1, NORM>(T, kk, T.phi0 + s0 * kPlP, T.phi0 + sP * kPlP, T.coef0 + s0 * G::kCoef, T.coef0 + sP * G::kCoef,
+                         T.cax0 + s0 * G::kCoef, out, Pn, Pm1, Pm2, Pm3, Pm4, azn, CUR, S1, S2, S3, vmax, vnan);
     s0 = sP;
 }
 
@@ -254,8 +270,8 @@ __device__ __forceinline__ void march(const Th& T, int ks, int ke, const CUtenso
     mbar_wait(bar0 + 0, 0);
     mbar_wait(bar0 + 8, 0);
     Pm1 = ldp(T.phi0);
-    double2 Pn = ldp(T.phi0 + kPl);
-    double2 azn = ldp(T.coef0 + G::kCoef + C_AZ * kPl);
+    double2 Pn = ldp(T.phi0 + kPlP);
+    double2 azn = ldp(T.coef0 + G::kCoef + O_AZ);
     unsigned s0 = 1, phase = 3u;                               // plane ks sits in stage 1; stages 0 and 1 have completed phase 0
 #define MAC_T2_STAGE(J, XX, CUR, S1, S2, S3)                                                                          \
     if (kk > ke) break;                                                                                               \
@@ -290,7 +306,7 @@ k_rbgs_t2(const __grid_constant__ CUtensorMap tm_phi, const __grid_constant__ CU
     unsigned char* smem_raw = smem_dyn + ((128u - (smem_u32(smem_dyn) & 127u)) & 127u);
     unsigned char* phi_gen = smem_raw + kPad;
     const unsigned phi_ring = smem_u32(phi_gen);
-    const unsigned coef_ring = phi_ring + G::NP * kPl;
+    const unsigned coef_ring = phi_ring + G::NP * kPlP;
     const unsigned bar0 = coef_ring + G::NC * G::kCoef + 6 * kEx;     // (the exchange buffers sit between the rings and the barriers)
 
     const int lane = threadIdx.x;
@@ -305,21 +321,24 @@ k_rbgs_t2(const __grid_constant__ CUtensorMap tm_phi, const __grid_constant__ CU
         k1 = min(k0 + plan.zchunk, L.nz);
     }
     const int tyi = tile / plan.tiles_x;
-    const int x0 = (tile - tyi * plan.tiles_x) * kTX, y0 = tyi * kTY;
-    const int gi = x0 - HALO + 2 * lane, gj = y0 - HALO + ty;
+    const int x0 = (tile - tyi * plan.tiles_x) * kTX, y0 = tyi * kTY;   // finished cells: [x0 - 1, x0 + 25) x [y0, y0 + 18)
+    const int gi = x0 - HALO + 2 * lane, gj = y0 - CH + ty;             // x cell of the own pair (gi is even), own row
     // ghost columns / rows of a periodic level hold valid images: they are recomputed like any halo cell
     const bool col_ok = gi >= -L.gx && gi < L.nx + L.gx && gj >= -L.gy && gj < L.ny + L.gy;
     const bool producer = threadIdx.x == 0 && threadIdx.y == 0;
 
+    // validity by distance from the edge of the computed tile: sweep-1 red everywhere (it reads the staged ring), then
+    // one ring less per half-sweep; columns x0-4 (x cell of lane 0) and x0+27 (y cell of lane 15) are the outermost
     Th T;
-    T.ra_x = col_ok && ty >= 1 && ty <= TYE - 2 && lane >= 1;
-    T.ra_y = col_ok && ty >= 1 && ty <= TYE - 2 && lane <= LN - 2;
-    T.ba = col_ok && ty >= 2 && ty <= TYE - 3 && lane >= 1 && lane <= LN - 2;
-    T.rb_x = col_ok && ty >= 3 && ty <= TYE - 4 && lane >= 2 && lane <= LN - 2;
-    T.rb_y = col_ok && ty >= 3 && ty <= TYE - 4 && lane >= 1 && lane <= LN - 3;
-    T.own = ty >= HALO && ty <= TYE - 1 - HALO && lane >= 2 && lane <= LN - 3 && gi < L.nx && gj < L.ny;
-    T.img_x = T.own ? image_dx(L, gi) : 0;
-    T.img_y = T.own ? image_dy(L, gj) : 0;
+    T.ra = col_ok;
+    T.ba_x = col_ok && ty >= 1 && ty <= TYE - 2 && lane >= 1;
+    T.ba_y = col_ok && ty >= 1 && ty <= TYE - 2 && lane <= LN - 2;
+    T.rb = col_ok && ty >= 2 && ty <= TYE - 3 && lane >= 1 && lane <= LN - 2;
+    const bool own_row = ty >= CH && ty <= TYE - 1 - CH && gj < L.ny && gi >= 0 && gi < L.nx;   // (the pair lies inside or outside as a whole)
+    T.own_x = own_row && lane >= 2 && lane <= LN - 2;
+    T.own_y = own_row && lane >= 1 && lane <= LN - 3;
+    T.img_x = own_row ? image_dx(L, gi) : 0;
+    T.img_y = own_row ? image_dy(L, gj) : 0;
     const bool perz = L.bclo[2] == MAC_PERIODIC;
     {
         const int wl[4] = {k0 - 3, k0 - 2, k0 - 1, k0}, wh[4] = {k1 + 2, k1 + 1, k1, k1 - 1};
@@ -332,11 +351,11 @@ k_rbgs_t2(const __grid_constant__ CUtensorMap tm_phi, const __grid_constant__ CU
         T.nlo = k0;
         T.nspan = (unsigned)(k1 - 1 - k0);
     }
-    const unsigned slot = (ty * LN + lane) * 16;
-    T.phi0 = phi_gen + slot;
-    T.coef0 = phi_gen + G::NP * kPl + slot;
-    T.ex0 = phi_gen + G::NP * kPl + G::NC * G::kCoef + ((ty + 1) * LN + lane) * 8;
-    const int cx0 = x0 - HALO + L.gx, cy0 = y0 - HALO + L.gy;     // tensor-map coordinates of the tile origin
+    T.phi0 = phi_gen + (ty + 1) * kRowP + 16 + lane * 16;         // the box starts one row and two columns before the computed tile
+    T.coef0 = phi_gen + G::NP * kPlP + ty * kRow + lane * 16;
+    T.cax0 = phi_gen + G::NP * kPlP + O_AX + ty * kRowA + lane * 16;
+    T.ex0 = phi_gen + G::NP * kPlP + G::NC * G::kCoef + ((ty + 1) * LN + lane) * 8;
+    const int cx0 = x0 - HALO + L.gx, cy0 = y0 - CH + L.gy;       // tensor-map coordinates of the computed tile's origin
 
     const int ks = k0 - 3;
     if (producer) {
@@ -344,13 +363,13 @@ k_rbgs_t2(const __grid_constant__ CUtensorMap tm_phi, const __grid_constant__ CU
         asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
         asm volatile("fence.proxy.async.shared::cta;\n" ::: "memory");
         for (int q = 0; q < LA + 2 && ks - 1 + q <= k1 + 3; ++q)
-            issue_plane<LA>(&tm_phi, &tm_rhs, &tm_ax, &tm_ay, &tm_az, phi_ring, coef_ring, bar0, q * kPl, q * G::kCoef, ks - 1 + q, L.nz,
+            issue_plane<LA>(&tm_phi, &tm_rhs, &tm_ax, &tm_ay, &tm_az, phi_ring, coef_ring, bar0, q * kPlP, q * G::kCoef, ks - 1 + q, L.nz,
                             perz, cx0, cy0);
     }
     __syncthreads();                                             // barrier inits visible before anyone waits
 
     const unsigned long long ostride = (unsigned long long)L.cx * L.ry;
-    double* out = pout + (T.own ? (long long)gi + (long long)L.cx * gj : 0) + (long long)(ks - 3) * (long long)ostride;
+    double* out = pout + (own_row ? (long long)gi + (long long)L.cx * gj : 0) + (long long)(ks - 3) * (long long)ostride;
     double vmax = 0.0;
     bool vnan = false;
     if (((gj + ks) & 1) == 0)
@@ -390,6 +409,26 @@ static inline int t2_smoother_configure()
     return 0;
 }
 
+// Tensor maps of the two-sweep kernel (Level::tma[2]): phi boxes carry the read-only ring (SX x SY), the coefficient
+// boxes cover the computed 32 x 24 cells (ax: AXW faces a row, ay: TYE + 1 face rows).  Coordinates as in tma_build_maps.
+static inline int t2_build_maps(TmaLevelMaps* T, const LevelDev& L)
+{
+    using namespace t2;
+    T->ok = 0;
+    if ((L.bclo[0] == MAC_PERIODIC && L.gx == 0) || (L.bclo[1] == MAC_PERIODIC && L.gy == 0)) return 0;   // cannot wrap
+    if ((L.nx & 1) || L.nx < 2 || (L.px & 1) || (L.cx & 1)) return 0;
+    const uint64_t ex = (uint64_t)L.nx + 2 * L.gx, ey = (uint64_t)L.ny + 2 * L.gy;
+    const long long oc = (long long)L.gx + (long long)L.cx * L.gy, oa = (long long)L.gx + (long long)L.px * L.gy;
+    bool ok = tma_encode3(&T->phi, L.phi - oc, ex, ey, L.nz, L.cx, L.ry, SX, SY) &&
+              tma_encode3(&T->phi2, L.phi2 - oc, ex, ey, L.nz, L.cx, L.ry, SX, SY) &&
+              tma_encode3(&T->rhs, L.rhs - oc, ex, ey, L.nz, L.cx, L.ry, 2 * LN, TYE) &&
+              tma_encode3(&T->ax, L.ax - oa, ex + 1, ey, L.nz, L.px, L.ry, AXW, TYE) &&
+              tma_encode3(&T->az, L.az - oc, ex, ey, (uint64_t)L.nz + 1, L.cx, L.ry, 2 * LN, TYE) &&
+              tma_encode3(&T->ay, L.ay - oc, ex, ey + 1, L.nz, L.cx, (uint64_t)L.ry + 1, 2 * LN, TYE + 1);
+    T->ok = ok ? 1 : 0;
+    return T->ok;
+}
+
 // the two-sweep kernel needs its 4-cell halo inside the periodic images and a few planes to march through
 static inline bool t2_level_ok(const LevelDev& L)
 {
@@ -402,7 +441,7 @@ static inline bool t2_level_ok(const LevelDev& L)
 static inline t2::T2Plan t2_plan(const LevelDev& L, int sms)
 {
     t2::T2Plan P;
-    P.tiles_x = (L.nx + t2::kTX - 1) / t2::kTX;
+    P.tiles_x = (L.nx + 1 + t2::kTX - 1) / t2::kTX;                   // tile t finishes columns [26 t - 1, 26 t + 25)
     P.tiles = P.tiles_x * ((L.ny + t2::kTY - 1) / t2::kTY);
     const int S = sms, maxchunk = L.nz >= 32 ? L.nz / 16 : 1;
     // cost in marching steps of the slowest SM: rounds x (planes per chunk + the 6 redone planes + pipeline fill)

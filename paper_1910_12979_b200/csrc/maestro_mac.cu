@@ -762,7 +762,7 @@ extern "C" int maestro_mac_setup(const maestro_mac_desc* desc, void* workspace, 
             LevelDev D = dev_level(H, l);
             tma_build_maps(&H->lev[l].tma[0], D, 32, 16);
             tma_build_maps(&H->lev[l].tma[1], D, 16, 16);
-            tma_build_maps(&H->lev[l].tma[2], D, t2::LN, t2::TYE);
+            t2_build_maps(&H->lev[l].tma[2], D);
             // a level laid out with periodic images has no other smoother: its tensor maps must exist
             if ((D.gx || D.gy) && !H->lev[l].tma[H->d.smoother == 3 ? 1 : 0].ok) ok = false;
         }

@@ -72,7 +72,7 @@ def test_kernels_at_full_size(oracle, mac, full):
     # the launch decomposition bench.py times: the two-sweep kernel with whole-column tiles for the whole waves and
     # z-chunks for the last, partial wave (592 + 112 x 5 CTAs on 148 SMs), then a pair plus a single sweep
     plan = P.level_plan(0)
-    assert plan["kernel"] == "t2" and plan["nfull"] > 0 and plan["nsplit"] > 1 and plan["tiles"] == 704, plan
+    assert plan["kernel"] == "t2" and plan["nfull"] > 0 and plan["nsplit"] > 1 and plan["tiles"] == 580, plan
     P.step_smooth(0, 2)
     O.rbgs_sweep(g, *bf, rhs, phi); O.rbgs_sweep(g, *bf, rhs, phi)
     assert close(P.level_get(0, mac.ARR_PHI), phi)

@@ -2,7 +2,7 @@
 element-wise parity of the default two-sweep smoother on a small level whose launch plan has whole-column tiles AND
 z-chunked tiles (the decomposition the 512^3 bench runs: more lateral tiles than SMs).
 
-At 256^3 level 0 has 11 x 16 = 176 tiles > 148 SMs, so k_rbgs_t2 runs 148 whole-column CTAs plus 28 tiles cut into
+At 256^3 level 0 has 10 x 15 = 150 tiles > 148 SMs, so k_rbgs_t2 runs 148 whole-column CTAs plus 2 tiles cut into
 z-chunks, and its NORM variant carries the stop test: a seam error between the two kinds of CTA would show here as a
 relative L2 difference far above 1e-10.  The oracle needs about 8 s per projection at this size.
 """
@@ -53,12 +53,12 @@ def test_end_to_end_parity_256(oracle, mac, name):
 
 
 MIXED_PLAN_CASES = [
-    # 13 x 13 = 169 tiles of 24 x 16 (ragged in x): one whole wave of whole-column tiles plus 21 tiles in z-chunks
-    dict(n=(304, 208, 32), bc_lo=(WALL, OUT, OUT), bc_hi=(OUT, WALL, WALL), geometry=W.SPHERICAL, seed=41),
-    # 16 x 12 = 192 tiles, periodic in x and y (image columns / rows), periodic z
+    # 13 x 12 = 156 tiles of 26 x 18 (ragged in x and y): one whole wave of whole-column tiles plus 8 tiles in z-chunks
+    dict(n=(336, 208, 64), bc_lo=(WALL, OUT, OUT), bc_hi=(OUT, WALL, WALL), geometry=W.SPHERICAL, seed=41),
+    # 15 x 11 = 165 tiles, periodic in x and y (image columns / rows), periodic z
     dict(n=(384, 192, 64), bc_lo=(PER, PER, PER), bc_hi=(PER, PER, PER), seed=42),
     # ragged in x and y: 15 x 11 = 165 tiles
-    dict(n=(344, 168, 32), bc_lo=(OUT, PER, WALL), bc_hi=(WALL, PER, OUT), seed=43),
+    dict(n=(368, 192, 64), bc_lo=(OUT, PER, WALL), bc_hi=(WALL, PER, OUT), seed=43),
 ]
 
 
@@ -100,7 +100,7 @@ def test_two_sweep_kernel_with_whole_column_and_chunked_tiles(oracle, mac, case)
 def test_riding_stop_test_with_mixed_plan(oracle, mac):
     """stop_test 0 (k_rbgs_t2 NORM variant on whole-column + chunked tiles) against stop_test 1 and the oracle."""
     wl = W.mixed_bc_case(**MIXED_PLAN_CASES[0])
-    wl.dx = (1.0 / 304,) * 3                      # cubic cells: point Gauss-Seidel multigrid converges as in the configs
+    wl.dx = (1.0 / 336,) * 3                      # cubic cells: point Gauss-Seidel multigrid converges as in the configs
     wl.dr = 0.5 * wl.dx[0]
     wl.nr = len(wl.beta0)
     a, b = gpu_project(mac, wl, stop_test=0), gpu_project(mac, wl, stop_test=1)
