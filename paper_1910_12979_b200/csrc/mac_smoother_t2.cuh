@@ -87,13 +87,18 @@ struct Coef {                                // coefficients of one plane for a 
     double2 rdg;                             // and sweep 2 reuses (same coefficients, two steps later)
 };
 
+// One bit per lateral condition, kept in ONE register that the compiler cannot rematerialise from (lane, row): each
+// update is then selected by a single bit test (the flags as separate bools were recomputed every step as chains of
+// five dependent selects on the critical path).
+enum { F_RA = 1, F_BA_X = 2, F_BA_Y = 4, F_RB = 8, F_OWN_X = 16, F_OWN_Y = 32, F_IMG = 64 };
+
 struct Th {                                  // per-thread constants
     unsigned char* phi0;                     // own slot of phi stage 0
     const unsigned char* coef0;              // own slot of coefficient stage 0 in the 32-column arrays (add O_AY, O_AZ, O_RHS)
     const unsigned char* cax0;               // own slot of coefficient stage 0, array ax
     unsigned char* ex0;                      // own element of exchange buffer 0
-    bool ra, ba_x, ba_y, rb, own_x, own_y;   // lateral validity of the four half-sweeps (x / y cell of the pair)
-    long long img_x, img_y;                  // periodic images of the own pair (0 = none)
+    unsigned fl;                             // lateral validity of the four half-sweeps (F_* bits; x / y cell of the pair)
+    long long img_x, img_y;                  // periodic images of the own pair (0 = none; F_IMG set iff one is not)
     // half-sweep h is applied at step kk iff (unsigned)(kk - lo[h]) <= span[h]: the planes it is wanted on
     // (sweep-1 red [k0-3, k1+2], black [k0-2, k1+1], sweep-2 red [k0-1, k1], black [k0, k1-1]) that exist
     int lo[4];
@@ -199,27 +204,31 @@ __device__ __forceinline__ void step(const Th& T, int kk, const unsigned char* s
     const double n0 = gs_cell<X, true>(l0, pick<!X>(P0), CUR, azn, pick<X>(Pm1), pick<X>(Pn), a, dg);
     if (NORM) {                                       // |rhs - (sum - phi_0 dg)| of the input; a NaN sets the sign of vmax
         const double rr = fabs(fma(pick<X>(P0), dg, -a));
-        const bool on = (X ? T.own_x : T.own_y) && (unsigned)(kk - T.nlo) <= T.nspan;
+        const bool on = (T.fl & (X ? F_OWN_X : F_OWN_Y)) && (unsigned)(kk - T.nlo) <= T.nspan;
         vmax = fmax(vmax, on ? rr : 0.0);             // (fmax drops NaNs: they are recorded separately)
         vnan = vnan || (on && rr != rr);
     }
-    put<X>(P0, (T.ra && v0) ? n0 : pick<X>(P0));
+    put<X>(P0, ((T.fl & F_RA) && v0) ? n0 : pick<X>(P0));
     // (2) sweep 1, black cells of plane kk-1
     const double n1 = gs_cell<X, true>(l1, pick<!X>(Pm1), S1, CUR.az, pick<X>(Pm2), pick<X>(P0), a, dg);
-    put<X>(Pm1, ((X ? T.ba_x : T.ba_y) && v1) ? n1 : pick<X>(Pm1));
+    put<X>(Pm1, ((T.fl & (X ? F_BA_X : F_BA_Y)) && v1) ? n1 : pick<X>(Pm1));
     // (3) sweep 2, red cells of plane kk-2
     const double n2 = gs_cell<X, false>(l2, pick<!X>(Pm2), S2, S1.az, pick<X>(Pm3), pick<X>(Pm1), a, dg);
-    put<X>(Pm2, (T.rb && v2) ? n2 : pick<X>(Pm2));
+    put<X>(Pm2, ((T.fl & F_RB) && v2) ? n2 : pick<X>(Pm2));
     // (4) sweep 2, black cells of plane kk-3; the plane is finished
     const double n3 = gs_cell<X, false>(l3, pick<!X>(Pm3), S3, S2.az, pick<X>(Pm4), pick<X>(Pm2), a, dg);
     *reinterpret_cast<double*>(T.ex0 + (EX_RA + W) * kEx) = pick<X>(P0);
     *reinterpret_cast<double*>(T.ex0 + (EX_BA + W) * kEx) = pick<X>(Pm1);
     *reinterpret_cast<double*>(T.ex0 + (EX_RB + W) * kEx) = pick<X>(Pm2);
-    if (v3) {                                         // plane kk-3 leaves: the owned cells of the pair
-        if (X ? T.own_x : T.own_y) put<X>(Pm3, n3);
-        if (T.own_x && T.own_y) store_images(reinterpret_cast<double2*>(out), Pm3, T.img_x, T.img_y);
-        else if (T.own_x) store_images(out, Pm3.x, T.img_x, T.img_y);
-        else if (T.own_y) store_images(out + 1, Pm3.y, T.img_x, T.img_y);
+    put<X>(Pm3, ((T.fl & (X ? F_OWN_X : F_OWN_Y)) && v3) ? n3 : pick<X>(Pm3));
+    if (v3) {                                         // plane kk-3 leaves: the owned cells of the pair (predicated stores)
+        if (T.fl & F_OWN_X) out[0] = Pm3.x;
+        if (T.fl & F_OWN_Y) out[1] = Pm3.y;
+        if (T.fl & F_IMG) {                           // periodic levels, tiles at the domain edge
+            const long long dx = T.img_x, dy = T.img_y;
+            if (T.fl & F_OWN_X) { if (dx) out[dx] = Pm3.x; if (dy) { out[dy] = Pm3.x; if (dx) out[dx + dy] = Pm3.x; } }
+            if (T.fl & F_OWN_Y) { if (dx) out[dx + 1] = Pm3.y; if (dy) { out[dy + 1] = Pm3.y; if (dx) out[dx + dy + 1] = Pm3.y; } }
+        }
     }
     Pm4 = Pm3; Pm3 = Pm2; Pm2 = Pm1; Pm1 = P0;
 }
@@ -330,15 +339,18 @@ k_rbgs_t2(const __grid_constant__ CUtensorMap tm_phi, const __grid_constant__ CU
     // validity by distance from the edge of the computed tile: sweep-1 red everywhere (it reads the staged ring), then
     // one ring less per half-sweep; columns x0-4 (x cell of lane 0) and x0+27 (y cell of lane 15) are the outermost
     Th T;
-    T.ra = col_ok;
-    T.ba_x = col_ok && ty >= 1 && ty <= TYE - 2 && lane >= 1;
-    T.ba_y = col_ok && ty >= 1 && ty <= TYE - 2 && lane <= LN - 2;
-    T.rb = col_ok && ty >= 2 && ty <= TYE - 3 && lane >= 1 && lane <= LN - 2;
-    const bool own_row = ty >= CH && ty <= TYE - 1 - CH && gj < L.ny && gi >= 0 && gi < L.nx;   // (the pair lies inside or outside as a whole)
-    T.own_x = own_row && lane >= 2 && lane <= LN - 2;
-    T.own_y = own_row && lane >= 1 && lane <= LN - 3;
-    T.img_x = own_row ? image_dx(L, gi) : 0;
+    const bool in_y = ty >= 1 && ty <= TYE - 2, own_row = ty >= CH && ty <= TYE - 1 - CH && gj < L.ny && gi >= 0 && gi < L.nx;
+    T.img_x = own_row ? image_dx(L, gi) : 0;          // (a pair lies inside or outside the domain as a whole)
     T.img_y = own_row ? image_dy(L, gj) : 0;
+    unsigned fl = 0;
+    if (col_ok) {
+        fl = F_RA | (in_y && lane >= 1 ? F_BA_X : 0) | (in_y && lane <= LN - 2 ? F_BA_Y : 0) |
+             (ty >= 2 && ty <= TYE - 3 && lane >= 1 && lane <= LN - 2 ? F_RB : 0) |
+             (own_row && lane >= 2 && lane <= LN - 2 ? F_OWN_X : 0) | (own_row && lane >= 1 && lane <= LN - 3 ? F_OWN_Y : 0);
+        if ((fl & (F_OWN_X | F_OWN_Y)) && (T.img_x | T.img_y)) fl |= F_IMG;
+    }
+    asm volatile("" : "+r"(fl));                      // opaque: keep the bits, do not recompute the conditions per step
+    T.fl = fl;
     const bool perz = L.bclo[2] == MAC_PERIODIC;
     {
         const int wl[4] = {k0 - 3, k0 - 2, k0 - 1, k0}, wh[4] = {k1 + 2, k1 + 1, k1, k1 - 1};
