@@ -93,12 +93,16 @@ struct Coef {                                // coefficients of one plane for a 
 enum { F_RA = 1, F_BA_X = 2, F_BA_Y = 4, F_RB = 8, F_OWN_X = 16, F_OWN_Y = 32, F_IMG = 64 };
 
 struct Th {                                  // per-thread constants
-    unsigned char* phi0;                     // own slot of phi stage 0
-    const unsigned char* coef0;              // own slot of coefficient stage 0 in the 32-column arrays (add O_AY, O_AZ, O_RHS)
-    const unsigned char* cax0;               // own slot of coefficient stage 0, array ax
-    unsigned char* ex0;                      // own element of exchange buffer 0
+    unsigned char* base;                     // start of the phi ring (CTA-uniform); the own slots are 32-bit offsets from it,
+    unsigned o_phi, o_cf, o_ax, o_ex;        // opaque to the compiler (else it recomputes them from (lane, row) every step):
+                                             // phi stage 0, coefficient stage 0 (32-column arrays: add O_AY, O_AZ, O_RHS),
+                                             // coefficient stage 0 array ax, exchange buffer 0
+    __device__ __forceinline__ unsigned char* phi0() const { return base + o_phi; }
+    __device__ __forceinline__ const unsigned char* coef0() const { return base + o_cf; }
+    __device__ __forceinline__ const unsigned char* cax0() const { return base + o_ax; }
+    __device__ __forceinline__ unsigned char* ex0() const { return base + o_ex; }
     unsigned fl;                             // lateral validity of the four half-sweeps (F_* bits; x / y cell of the pair)
-    long long img_x, img_y;                  // periodic images of the own pair (0 = none; F_IMG set iff one is not)
+    int img_x, img_y;                        // periodic images of the own pair (0 = none; F_IMG set iff one is not)
     // half-sweep h is applied at step kk iff (unsigned)(kk - lo[h]) <= span[h]: the planes it is wanted on
     // (sweep-1 red [k0-3, k1+2], black [k0-2, k1+1], sweep-2 red [k0-1, k1], black [k0, k1-1]) that exist
     int lo[4];
@@ -184,6 +188,8 @@ __device__ __forceinline__ void step(const Th& T, int kk, const unsigned char* s
                                      Coef& CUR, Coef& S1, Coef& S2, Coef& S3, double& vmax, bool& vnan)
 {
     constexpr int R = 1 - W;
+    unsigned fl = T.fl;
+    asm volatile("" : "+r"(fl));                      // (keeps the bit tests from being hoisted into one register each)
     const bool v0 = (unsigned)(kk - T.lo[0]) <= T.span[0], v1 = (unsigned)(kk - T.lo[1]) <= T.span[1];
     const bool v2 = (unsigned)(kk - T.lo[2]) <= T.span[2], v3 = (unsigned)(kk - T.lo[3]) <= T.span[3];
     double2 P0 = Pn;                                  // old phi of plane kk (staged read of the last step)
@@ -196,38 +202,38 @@ __device__ __forceinline__ void step(const Th& T, int kk, const unsigned char* s
     CUR.ayn = ldp(cI + O_AY + kRow);
     CUR.rhs = ldp(cI + O_RHS);
     const Lat l0 = lat_load<X>(s0);                                   // old black neighbours in plane kk
-    const Lat l1 = lat_ex<X>(T.ex0 + (EX_RA + R) * kEx);              // sweep-1 red neighbours in plane kk-1
-    const Lat l2 = lat_ex<X>(T.ex0 + (EX_BA + R) * kEx);              // sweep-1 black neighbours in plane kk-2
-    const Lat l3 = lat_ex<X>(T.ex0 + (EX_RB + R) * kEx);              // sweep-2 red neighbours in plane kk-3
+    const Lat l1 = lat_ex<X>(T.ex0() + (EX_RA + R) * kEx);              // sweep-1 red neighbours in plane kk-1
+    const Lat l2 = lat_ex<X>(T.ex0() + (EX_BA + R) * kEx);              // sweep-1 black neighbours in plane kk-2
+    const Lat l3 = lat_ex<X>(T.ex0() + (EX_RB + R) * kEx);              // sweep-2 red neighbours in plane kk-3
     double a, dg;
     // (1) sweep 1, red cells of plane kk
     const double n0 = gs_cell<X, true>(l0, pick<!X>(P0), CUR, azn, pick<X>(Pm1), pick<X>(Pn), a, dg);
     if (NORM) {                                       // |rhs - (sum - phi_0 dg)| of the input; a NaN sets the sign of vmax
         const double rr = fabs(fma(pick<X>(P0), dg, -a));
-        const bool on = (T.fl & (X ? F_OWN_X : F_OWN_Y)) && (unsigned)(kk - T.nlo) <= T.nspan;
+        const bool on = (fl & (X ? F_OWN_X : F_OWN_Y)) && (unsigned)(kk - T.nlo) <= T.nspan;
         vmax = fmax(vmax, on ? rr : 0.0);             // (fmax drops NaNs: they are recorded separately)
         vnan = vnan || (on && rr != rr);
     }
-    put<X>(P0, ((T.fl & F_RA) && v0) ? n0 : pick<X>(P0));
+    put<X>(P0, ((fl & F_RA) && v0) ? n0 : pick<X>(P0));
     // (2) sweep 1, black cells of plane kk-1
     const double n1 = gs_cell<X, true>(l1, pick<!X>(Pm1), S1, CUR.az, pick<X>(Pm2), pick<X>(P0), a, dg);
-    put<X>(Pm1, ((T.fl & (X ? F_BA_X : F_BA_Y)) && v1) ? n1 : pick<X>(Pm1));
+    put<X>(Pm1, ((fl & (X ? F_BA_X : F_BA_Y)) && v1) ? n1 : pick<X>(Pm1));
     // (3) sweep 2, red cells of plane kk-2
     const double n2 = gs_cell<X, false>(l2, pick<!X>(Pm2), S2, S1.az, pick<X>(Pm3), pick<X>(Pm1), a, dg);
-    put<X>(Pm2, ((T.fl & F_RB) && v2) ? n2 : pick<X>(Pm2));
+    put<X>(Pm2, ((fl & F_RB) && v2) ? n2 : pick<X>(Pm2));
     // (4) sweep 2, black cells of plane kk-3; the plane is finished
     const double n3 = gs_cell<X, false>(l3, pick<!X>(Pm3), S3, S2.az, pick<X>(Pm4), pick<X>(Pm2), a, dg);
-    *reinterpret_cast<double*>(T.ex0 + (EX_RA + W) * kEx) = pick<X>(P0);
-    *reinterpret_cast<double*>(T.ex0 + (EX_BA + W) * kEx) = pick<X>(Pm1);
-    *reinterpret_cast<double*>(T.ex0 + (EX_RB + W) * kEx) = pick<X>(Pm2);
-    put<X>(Pm3, ((T.fl & (X ? F_OWN_X : F_OWN_Y)) && v3) ? n3 : pick<X>(Pm3));
+    *reinterpret_cast<double*>(T.ex0() + (EX_RA + W) * kEx) = pick<X>(P0);
+    *reinterpret_cast<double*>(T.ex0() + (EX_BA + W) * kEx) = pick<X>(Pm1);
+    *reinterpret_cast<double*>(T.ex0() + (EX_RB + W) * kEx) = pick<X>(Pm2);
+    put<X>(Pm3, ((fl & (X ? F_OWN_X : F_OWN_Y)) && v3) ? n3 : pick<X>(Pm3));
     if (v3) {                                         // plane kk-3 leaves: the owned cells of the pair (predicated stores)
-        if (T.fl & F_OWN_X) out[0] = Pm3.x;
-        if (T.fl & F_OWN_Y) out[1] = Pm3.y;
-        if (T.fl & F_IMG) {                           // periodic levels, tiles at the domain edge
+        if (fl & F_OWN_X) out[0] = Pm3.x;
+        if (fl & F_OWN_Y) out[1] = Pm3.y;
+        if (fl & F_IMG) {                           // periodic levels, tiles at the domain edge
             const long long dx = T.img_x, dy = T.img_y;
-            if (T.fl & F_OWN_X) { if (dx) out[dx] = Pm3.x; if (dy) { out[dy] = Pm3.x; if (dx) out[dx + dy] = Pm3.x; } }
-            if (T.fl & F_OWN_Y) { if (dx) out[dx + 1] = Pm3.y; if (dy) { out[dy + 1] = Pm3.y; if (dx) out[dx + dy + 1] = Pm3.y; } }
+            if (fl & F_OWN_X) { if (dx) out[dx] = Pm3.x; if (dy) { out[dy] = Pm3.x; if (dx) out[dx + dy] = Pm3.x; } }
+            if (fl & F_OWN_Y) { if (dx) out[dx + 1] = Pm3.y; if (dy) { out[dy + 1] = Pm3.y; if (dx) out[dx + dy + 1] = Pm3.y; } }
         }
     }
     Pm4 = Pm3; Pm3 = Pm2; Pm2 = Pm1; Pm1 = P0;
@@ -258,8 +264,8 @@ __device__ __forceinline__ void stage(const Th& T, int kk, int ke, unsigned& s0,
         issue_plane<LA>(tm_phi, tm_rhs, tm_ax, tm_ay, tm_az, phi_ring, coef_ring, bar0, sN * kPlP, sN * G::kCoef,
                         kk + 1 + LA, nz, perz, cx, cy);
     }
-    step<X, J & 1, NORM>(T, kk, T.phi0 + s0 * kPlP, T.phi0 + sP * kPlP, T.coef0 + s0 * G::kCoef, T.coef0 + sP * G::kCoef,
-                         T.cax0 + s0 * G::kCoef, out, Pn, Pm1, Pm2, Pm3, Pm4, azn, CUR, S1, S2, S3, vmax, vnan);
+    step<X, J & 1, NORM>(T, kk, T.phi0() + s0 * kPlP, T.phi0() + sP * kPlP, T.coef0() + s0 * G::kCoef, T.coef0() + sP * G::kCoef,
+                         T.cax0() + s0 * G::kCoef, out, Pn, Pm1, Pm2, Pm3, Pm4, azn, CUR, S1, S2, S3, vmax, vnan);
     s0 = sP;
 }
 
@@ -278,9 +284,9 @@ __device__ __forceinline__ void march(const Th& T, int ks, int ke, const CUtenso
     // the prologue issued planes ks-1 .. ks+LA into stages 0 .. LA+1 of both rings (phase 0 of their barriers)
     mbar_wait(bar0 + 0, 0);
     mbar_wait(bar0 + 8, 0);
-    Pm1 = ldp(T.phi0);
-    double2 Pn = ldp(T.phi0 + kPlP);
-    double2 azn = ldp(T.coef0 + G::kCoef + O_AZ);
+    Pm1 = ldp(T.phi0());
+    double2 Pn = ldp(T.phi0() + kPlP);
+    double2 azn = ldp(T.coef0() + G::kCoef + O_AZ);
     unsigned s0 = 1, phase = 3u;                               // plane ks sits in stage 1; stages 0 and 1 have completed phase 0
 #define MAC_T2_STAGE(J, XX, CUR, S1, S2, S3)                                                                          \
     if (kk > ke) break;                                                                                               \
@@ -340,8 +346,8 @@ k_rbgs_t2(const __grid_constant__ CUtensorMap tm_phi, const __grid_constant__ CU
     // one ring less per half-sweep; columns x0-4 (x cell of lane 0) and x0+27 (y cell of lane 15) are the outermost
     Th T;
     const bool in_y = ty >= 1 && ty <= TYE - 2, own_row = ty >= CH && ty <= TYE - 1 - CH && gj < L.ny && gi >= 0 && gi < L.nx;
-    T.img_x = own_row ? image_dx(L, gi) : 0;          // (a pair lies inside or outside the domain as a whole)
-    T.img_y = own_row ? image_dy(L, gj) : 0;
+    T.img_x = own_row ? (int)image_dx(L, gi) : 0;     // (a pair lies inside or outside the domain as a whole; one plane of a
+    T.img_y = own_row ? (int)image_dy(L, gj) : 0;     // level has fewer than 2^31 cells: t2_level_ok)
     unsigned fl = 0;
     if (col_ok) {
         fl = F_RA | (in_y && lane >= 1 ? F_BA_X : 0) | (in_y && lane <= LN - 2 ? F_BA_Y : 0) |
@@ -363,10 +369,12 @@ k_rbgs_t2(const __grid_constant__ CUtensorMap tm_phi, const __grid_constant__ CU
         T.nlo = k0;
         T.nspan = (unsigned)(k1 - 1 - k0);
     }
-    T.phi0 = phi_gen + (ty + 1) * kRowP + 16 + lane * 16;         // the box starts one row and two columns before the computed tile
-    T.coef0 = phi_gen + G::NP * kPlP + ty * kRow + lane * 16;
-    T.cax0 = phi_gen + G::NP * kPlP + O_AX + ty * kRowA + lane * 16;
-    T.ex0 = phi_gen + G::NP * kPlP + G::NC * G::kCoef + ((ty + 1) * LN + lane) * 8;
+    T.base = phi_gen;
+    T.o_phi = (ty + 1) * kRowP + 16 + lane * 16;                  // the box starts one row and two columns before the computed tile
+    T.o_cf = G::NP * kPlP + ty * kRow + lane * 16;
+    T.o_ax = G::NP * kPlP + O_AX + ty * kRowA + lane * 16;
+    T.o_ex = G::NP * kPlP + G::NC * G::kCoef + ((ty + 1) * LN + lane) * 8;
+    asm volatile("" : "+r"(T.o_phi), "+r"(T.o_cf), "+r"(T.o_ax), "+r"(T.o_ex));
     const int cx0 = x0 - HALO + L.gx, cy0 = y0 - CH + L.gy;       // tensor-map coordinates of the computed tile's origin
 
     const int ks = k0 - 3;
@@ -445,6 +453,7 @@ static inline int t2_build_maps(TmaLevelMaps* T, const LevelDev& L)
 static inline bool t2_level_ok(const LevelDev& L)
 {
     if (L.nx < 48 || L.ny < 16 || L.nz < 8 || (L.nx & 1)) return false;
+    if ((long long)L.cx * L.ry >= (1ll << 31)) return false;         // image offsets are ints
     if (L.bclo[0] == MAC_PERIODIC && L.gx < t2::HALO) return false;
     if (L.bclo[1] == MAC_PERIODIC && L.gy < t2::HALO) return false;
     return true;
