@@ -7,8 +7,9 @@ face coefficients -> coarsening -> rhs -> V-cycles to 1e-10 -> velocity correcti
 
 Prints ONE JSON line (rank 0).  `value` is level-0 cell-updates/s over the whole projection,
 N^3 (nu_pre + nu_post) cycles / t(project), inputs resident in HBM (SURVEY.md Sec. 8(d));
-`e2e` is the same metric through maestro_mac_project_host() with pinned HOST buffers, host<->device
-copies inside the timed region.  `roofline` is the level-0 fused red-black smoother (k_rbgs_t2: the two sweeps of a smoothing step in
+`e2e` is the same metric through maestro_mac_project_host_seq() (K steps in one call, pinned HOST buffers, every step's
+u, v, w copied host -> device and back inside the timed region, overlapped with the neighbouring steps' projections; the
+unpipelined single call maestro_mac_project_host() is reported beside it).  `roofline` is the level-0 fused red-black smoother (k_rbgs_t2: the two sweeps of a smoothing step in
 ONE pass over HBM): `achieved` = the bytes that pass must move (48 B per cell per launch: read phi, rhs, ax, ay, az, write phi;
 DESIGN.md Sec. 6) over the mean device time of its launches, timed by CUDA event pairs inside the library on the call's stream
 during the timed steps (desc.timing = 1); `per_sweep_*` restate it in SURVEY.md Sec. 8(d)'s per-sweep unit (48 B per cell per SWEEP).  Multi-GPU: replicas only:
@@ -269,7 +270,7 @@ def run_ours(a):
 
     wl = W.by_name(a.config, a.n)                     # seeded, synthetic; identical on every rank (replicas)
     nu = wl.nu_pre + wl.nu_post
-    P = mac.MacProjector(mac.desc_from_workload(wl, smoother=a.smoother, host_staging=0 if a.no_e2e else 1, timing=1), device=dev)
+    P = mac.MacProjector(mac.desc_from_workload(wl, smoother=a.smoother, host_staging=0 if a.no_e2e else 3, timing=1), device=dev)
     dv = mac.to_device(wl, dev)
     pristine = [dv[k].clone() for k in ("u", "v", "w")]
     phi = torch.empty(wl.rho.shape, dtype=torch.float64, device=dev)
@@ -349,27 +350,54 @@ def run_ours(a):
         h0 = [torch.from_numpy(getattr(wl, k)) for k in ("u", "v", "w")]
         h2d = sum(hb[k].numel() * 8 for k in hb if hb[k] is not None)
         d2h = sum(hb[k].numel() * 8 for k in ("u", "v", "w"))
-        e_t, e_units = 0.0, 0
         n_e2e = a.steps
-        for k in range(1 + n_e2e):                  # one warm-up
+        # (i) the single call (maestro_mac_project_host): upload, project, download, one after the other
+        single_ms = None
+        for k in range(2):                          # one warm-up, one timed
             for t, p in zip((hb["u"], hb["v"], hb["w"]), h0):
                 t.copy_(p)
             barrier()
             t0 = time.perf_counter()
             rc, st = P.project_host(hb["beta0"], hb["rho0"], hb["rho"], hb["u"], hb["v"], hb["w"], hb["S"], None)
             torch.cuda.synchronize()
-            dt = time.perf_counter() - t0
+            single_ms = 1e3 * (time.perf_counter() - t0)
             if rc != 0:
                 raise RuntimeError(f"maestro_mac_project_host returned {rc}")
-            if k > 0:
-                e_t += dt
-                e_units += wl.ncells * nu * st["cycles"]
+        # (ii) the sequence call (maestro_mac_project_host_seq, config 5's pattern): K steps in ONE call; every step's
+        # u, v, w go host -> device and come back inside the timed region, overlapped with the neighbouring steps'
+        # projections; rho, S and the profiles go up once per call (their bytes are spread over the K steps below)
+        for t, p in zip((hb["u"], hb["v"], hb["w"]), h0):
+            t.copy_(p)
+        outs = [[torch.empty_like(hb[k]).pin_memory() for k in ("u", "v", "w")] for _ in range(3)]
+        uvw = 3 * [None]
+        for q, key in enumerate(("u", "v", "w")):
+            uvw[q] = ([hb[key]] * n_e2e, [outs[k % 3][q] for k in range(n_e2e)])
+        e_t, e_units = 0.0, 0
+        for rep_ in range(2):                       # a one-step warm-up call, then the timed call of K steps
+            K = 1 if rep_ == 0 else n_e2e
+            barrier()
+            t0 = time.perf_counter()
+            rc, sts = P.project_host_seq(hb["beta0"], hb["rho0"], hb["rho"], hb["S"], uvw[0][0][:K], uvw[1][0][:K], uvw[2][0][:K],
+                                         uvw[0][1][:K], uvw[1][1][:K], uvw[2][1][:K])
+            torch.cuda.synchronize()
+            dt = time.perf_counter() - t0
+            if rc != 0:
+                raise RuntimeError(f"maestro_mac_project_host_seq returned {rc}")
+            if rep_ == 1:
+                e_t = dt
+                e_units = sum(wl.ncells * nu * st["cycles"] for st in sts)
+        once = sum(hb[k].numel() * 8 for k in ("beta0", "rho0", "rho", "S") if hb[k] is not None)
+        h2d = d2h + once // n_e2e
         emax = torch.tensor([e_t], dtype=torch.float64, device=dev)
         if world > 1:
             dist.all_reduce(emax, op=dist.ReduceOp.MAX)
         e2e = {"value": world * e_units / float(emax.item()), "unit": UNIT, "h2d_bytes_per_step": h2d,
                "d2h_bytes_per_step": d2h, "ms_per_step": 1e3 * float(emax.item()) / n_e2e,
-               "api": "maestro_mac_project_host (pinned host buffers)"}
+               "api": "maestro_mac_project_host_seq: K steps in one call, pinned host buffers, every step's u, v, w copied in and "
+                      "out inside the timed region (overlapped with the neighbouring steps); rho, S, beta0, rho0 once per call",
+               "steps_in_call": n_e2e, "h2d_bytes_once_per_call": once,
+               "single_call_ms": single_ms, "single_call_api": "maestro_mac_project_host (nothing overlapped; all inputs sent)"}
+        del outs
     P.close()
     del dv, pristine, phi
     torch.cuda.empty_cache()

@@ -82,7 +82,12 @@ typedef struct {
     double bottom_rel_tol;    /* on ||r||2 / ||f||2, default 1e-8 (<= 0 stands for the default) */
     int prolongation;         /* 0 = cell-centred trilinear (default), 1 = piecewise constant */
     int host_staging;         /* 1 = reserve device staging in the workspace so that
-                                 maestro_mac_project_host() can be used */
+                                 maestro_mac_project_host() can be used;
+                                 2, 3 = that many staging sets of u, v, w, phi (and two copy streams):
+                                 maestro_mac_project_host_seq() overlaps the transfers of neighbouring steps.
+                                 With 2 sets the upload of step k+1 waits for the download of step k-1 (a step
+                                 costs max(projection, download + upload)); with 3 sets it does not
+                                 (max(projection, upload, download)) */
     int smoother;             /* 0 = default: fused red+black passes with planes staged by TMA where the level
                                      allows it (nx >= 60), else by cp.async; pairs of sweeps run as ONE pass
                                      over HBM (two-sweep kernel, temporal blocking) on levels of at least
@@ -193,6 +198,28 @@ int maestro_mac_status(maestro_mac_handle *h, maestro_mac_stats *stats, void *cu
 int maestro_mac_project_host(maestro_mac_handle *h, const double *beta0, const double *rho0,
                              const double *rho, double *u, double *v, double *w, const double *S,
                              double *phi, maestro_mac_stats *stats, void *cuda_stream);
+
+/*
+ * maestro_mac_project_host_seq: `nsteps` consecutive projections with HOST buffers, pipelined (BASELINE.json
+ * config 5: "10 consecutive projections with new U_edge each step"; the constraint of PAPER.md:49 Eq. 6 is
+ * enforced once per time step with the same base state and density).  beta0, rho0, rho, S (host; NULL
+ * conventions as above) are copied to the device ONCE and serve every step; for step k the face velocities are
+ * read from u_in[k], v_in[k], w_in[k] (host arrays of nsteps pointers) and the projected ones are written to
+ * u_out[k], v_out[k], w_out[k] (may equal the inputs), phi (when phi_out != NULL) to phi_out[k].
+ * While step k is projected on `cuda_stream`, the velocities of step k+1 travel host -> device and the results
+ * of step k-1 device -> host on the handle's two copy streams (staging sets used round robin, desc.host_staging = 2
+ * or 3), so
+ * every step's transfers happen inside the call but only the first upload and the last download are exposed.
+ * Host buffers must be page-locked for the copies to overlap, and must not be touched until the call returns
+ * (it returns after everything has completed).  stats: host array of nsteps entries, or NULL.
+ * Returns the first negative status met (the sequence stops there), else NOT_CONVERGED if any step returned it,
+ * else OK.  ERR_ARG if the handle was set up with host_staging < 2.
+ */
+int maestro_mac_project_host_seq(maestro_mac_handle *h, int nsteps, const double *beta0, const double *rho0,
+                                 const double *rho, const double *S,
+                                 const double *const *u_in, const double *const *v_in, const double *const *w_in,
+                                 double *const *u_out, double *const *v_out, double *const *w_out,
+                                 double *const *phi_out, maestro_mac_stats *stats, void *cuda_stream);
 
 /*
  * maestro_mac_base_state: the 1-D base-state quantities the projection consumes, from the thermodynamic

@@ -47,6 +47,7 @@ struct Level {
 
 struct Staging {
     double *beta0, *rho0, *rho, *u, *v, *w, *S, *phi;
+    double *ux[2], *vx[2], *wx[2], *phix[2];   // further sets of u, v, w, phi (desc.host_staging = 2, 3)
 };
 
 struct NodHost {                   // one level of the nodal projection (desc.nodal = 1); layout: mac_nodal.cuh
@@ -81,12 +82,16 @@ struct maestro_mac_handle {
     int *flags;                    // [0] bad rho, [1] bottom iterations
     Staging st;
     bool has_staging;
+    cudaStream_t cp_in, cp_out;    // copy streams of maestro_mac_project_host_seq (host_staging = 2), else NULL
+    cudaEvent_t ev_in[3], ev_done[3], ev_out[3];   // per staging set: upload complete, projection complete, download complete
     NodHost nod[kMaxLevels];       // nodal projection: level arrays (valid when has_nodal)
     double* nod_vecs;              // 6 BiCGStab vectors over the nodes of the coarsest level
     bool has_nodal;
     // host side
-    double *host_scal;             // pinned, 8 doubles
-    int *host_flags;               // pinned, 4 ints
+    double *host_scal;             // pinned and mapped, 8 doubles: kernels write the scalars the host reads (k_publish)
+    int *host_flags;               // pinned and mapped, 4 ints
+    double *host_scal_dev;         // the same two blocks as the device sees them (cudaHostGetDevicePointer)
+    int *host_flags_dev;
     cudaEvent_t ev[4];
     int launches;
     int sms;                       // multiprocessors of the device (cudaDevAttrMultiProcessorCount at setup)
@@ -129,7 +134,7 @@ int validate_and_default(const maestro_mac_desc* in, maestro_mac_desc* d)
     if (d->bottom_max_iter == 0) d->bottom_max_iter = 100;
     if (!(d->bottom_rel_tol > 0.0)) d->bottom_rel_tol = 1e-8;
     if (d->prolongation != 0 && d->prolongation != 1) return MAESTRO_MAC_ERR_ARG;
-    if (d->host_staging != 0 && d->host_staging != 1) return MAESTRO_MAC_ERR_ARG;
+    if (d->host_staging < 0 || d->host_staging > 3) return MAESTRO_MAC_ERR_ARG;
     if (d->smoother < 0 || d->smoother > 4) return MAESTRO_MAC_ERR_ARG;   // 4: one sweep per pass everywhere
     if (d->stop_test != 0 && d->stop_test != 1) return MAESTRO_MAC_ERR_ARG;
     if (d->rho_mean != 0 && d->rho_mean != 1) return MAESTRO_MAC_ERR_ARG;
@@ -231,7 +236,7 @@ size_t carve(maestro_mac_handle* H, char* base)
         }
         H->nod_vecs = (double*)take(6 * H->nod[H->nlev - 1].anode, 8);
     }
-    H->has_staging = H->d.host_staging == 1;
+    H->has_staging = H->d.host_staging >= 1;
     if (H->has_staging) {
         const maestro_mac_desc& d = H->d;
         size_t nc = (size_t)d.nx * d.ny * d.nz;
@@ -243,6 +248,14 @@ size_t carve(maestro_mac_handle* H, char* base)
         H->st.u = (double*)take((size_t)(d.nx + 1) * d.ny * d.nz, 8);
         H->st.v = (double*)take((size_t)d.nx * (d.ny + 1) * d.nz, 8);
         H->st.w = (double*)take((size_t)d.nx * d.ny * (d.nz + 1), 8);
+        for (int q = 0; q < 2; ++q) {
+            H->st.ux[q] = H->st.vx[q] = H->st.wx[q] = H->st.phix[q] = nullptr;
+            if (d.host_staging < q + 2) continue;
+            H->st.phix[q] = (double*)take(nc, 8);
+            H->st.ux[q] = (double*)take((size_t)(d.nx + 1) * d.ny * d.nz, 8);
+            H->st.vx[q] = (double*)take((size_t)d.nx * (d.ny + 1) * d.nz, 8);
+            H->st.wx[q] = (double*)take((size_t)d.nx * d.ny * (d.nz + 1), 8);
+        }
     }
     return align_up(off, 256);
 }
@@ -291,8 +304,36 @@ void dims3(int ex, int ey, int ez, dim3* grid, dim3* block)
     *grid = dim3((ex + bx - 1) / bx, (ey + by - 1) / by, ez);
 }
 
+// The scalars the host reads (norms, flags) are WRITTEN into mapped pinned memory by a one-thread kernel instead of
+// being fetched by cudaMemcpyAsync: a device-to-host copy queues on the copy engine behind whatever bulk download is
+// in flight (maestro_mac_project_host_seq overlaps those with the projection), and every V-cycle would wait for it.
+__global__ void k_publish(double* __restrict__ dst, const double* __restrict__ src, int n)
+{
+    for (int q = threadIdx.x; q < n; q += blockDim.x) dst[q] = src[q];
+    __threadfence_system();
+}
+__global__ void k_publish_int(int* __restrict__ dst, const int* __restrict__ src, int n)
+{
+    for (int q = threadIdx.x; q < n; q += blockDim.x) dst[q] = src[q];
+    __threadfence_system();
+}
+
 #define CUDA_OK(call) do { if ((call) != cudaSuccess) return MAESTRO_MAC_ERR_CUDA; } while (0)
 #define LAUNCHED(H) do { ++(H)->launches; if (cudaPeekAtLastError() != cudaSuccess) return MAESTRO_MAC_ERR_CUDA; } while (0)
+
+// host_scal[at .. at+n) <- scal[at .. at+n) / host_flags likewise, visible to the host after the stream is synchronised
+int publish_scal(maestro_mac_handle* H, int at, int n, cudaStream_t s)
+{
+    k_publish<<<1, 32, 0, s>>>(H->host_scal_dev + at, H->scal + at, n);
+    ++H->launches;
+    return cudaPeekAtLastError() == cudaSuccess ? MAESTRO_MAC_OK : MAESTRO_MAC_ERR_CUDA;
+}
+int publish_flags(maestro_mac_handle* H, int at, int n, cudaStream_t s)
+{
+    k_publish_int<<<1, 32, 0, s>>>(H->host_flags_dev + at, H->flags + at, n);
+    ++H->launches;
+    return cudaPeekAtLastError() == cudaSuccess ? MAESTRO_MAC_OK : MAESTRO_MAC_ERR_CUDA;
+}
 
 int red_blocks(const maestro_mac_handle* H, int rows) { return rows < H->red_blocks ? rows : H->red_blocks; }
 
@@ -419,7 +460,7 @@ int do_rhs_finish(maestro_mac_handle* H, int nb, cudaStream_t s)
     k_reduce_final<<<1, 1024, 0, s>>>(H->part_sum, H->part_max, nb, H->scal);
     LAUNCHED(H);
     if (H->singular) {
-        CUDA_OK(cudaMemcpyAsync(H->scal + 2, H->scal, sizeof(double), cudaMemcpyDeviceToDevice, s));
+        k_publish<<<1, 32, 0, s>>>(H->scal + 2, H->scal, 1);
         k_shift_mean<<<H->red_blocks, 256, 0, s>>>(dev_level(H, 0), L0.rhs, H->scal + 2, 1.0 / (double)L0.ncell, H->part_sum, H->part_max);
         LAUNCHED(H);
         k_reduce_final<<<1, 1024, 0, s>>>(H->part_sum, H->part_max, H->red_blocks, H->scal);
@@ -735,11 +776,23 @@ extern "C" int maestro_mac_setup(const maestro_mac_desc* desc, void* workspace, 
     H->host_scal = nullptr;
     H->host_flags = nullptr;
     for (int e = 0; e < 4; ++e) H->ev[e] = nullptr;
-    bool ok = cudaMallocHost((void**)&H->host_scal, 8 * sizeof(double)) == cudaSuccess &&
-              cudaMallocHost((void**)&H->host_flags, 4 * sizeof(int)) == cudaSuccess;
+    bool ok = cudaHostAlloc((void**)&H->host_scal, 8 * sizeof(double), cudaHostAllocMapped) == cudaSuccess &&
+              cudaHostAlloc((void**)&H->host_flags, 4 * sizeof(int), cudaHostAllocMapped) == cudaSuccess &&
+              cudaHostGetDevicePointer((void**)&H->host_scal_dev, H->host_scal, 0) == cudaSuccess &&
+              cudaHostGetDevicePointer((void**)&H->host_flags_dev, H->host_flags, 0) == cudaSuccess;
     for (int e = 0; ok && e < 4; ++e) ok = cudaEventCreate(&H->ev[e]) == cudaSuccess;
     H->sm_ev = nullptr;
     H->sm_used = H->sm_launches = H->sm_sweeps = 0;
+    H->cp_in = H->cp_out = nullptr;
+    for (int e = 0; e < 3; ++e) H->ev_in[e] = H->ev_done[e] = H->ev_out[e] = nullptr;
+    if (ok && H->d.host_staging >= 2) {
+        ok = cudaStreamCreateWithFlags(&H->cp_in, cudaStreamNonBlocking) == cudaSuccess &&
+             cudaStreamCreateWithFlags(&H->cp_out, cudaStreamNonBlocking) == cudaSuccess;
+        for (int e = 0; ok && e < 3; ++e)
+            ok = cudaEventCreateWithFlags(&H->ev_in[e], cudaEventDisableTiming) == cudaSuccess &&
+                 cudaEventCreateWithFlags(&H->ev_done[e], cudaEventDisableTiming) == cudaSuccess &&
+                 cudaEventCreateWithFlags(&H->ev_out[e], cudaEventDisableTiming) == cudaSuccess;
+    }
     {
         int dev = 0, sms = 0;
         ok = ok && cudaGetDevice(&dev) == cudaSuccess && cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && sms > 0;
@@ -791,6 +844,13 @@ extern "C" int maestro_mac_free(maestro_mac_handle* H)
     if (H->host_flags) cudaFreeHost(H->host_flags);
     for (int e = 0; e < 4; ++e)
         if (H->ev[e]) cudaEventDestroy(H->ev[e]);
+    if (H->cp_in) cudaStreamDestroy(H->cp_in);
+    if (H->cp_out) cudaStreamDestroy(H->cp_out);
+    for (int e = 0; e < 3; ++e) {
+        if (H->ev_in[e]) cudaEventDestroy(H->ev_in[e]);
+        if (H->ev_done[e]) cudaEventDestroy(H->ev_done[e]);
+        if (H->ev_out[e]) cudaEventDestroy(H->ev_out[e]);
+    }
     if (H->sm_ev) {
         for (int e = 0; e < 2 * kSmoothEvents; ++e)
             if (H->sm_ev[e]) cudaEventDestroy(H->sm_ev[e]);
@@ -850,8 +910,8 @@ extern "C" int maestro_mac_project(maestro_mac_handle* H, const double* beta0, c
         if ((rc = do_coefficients(H, beta0, rho0, rho, s)) != 0) return rc;
         if ((rc = do_rhs(H, beta0, u, v, w, S, s)) != 0) return rc;
     }
-    CUDA_OK(cudaMemcpyAsync(H->host_scal, H->scal, 3 * sizeof(double), cudaMemcpyDeviceToHost, s));
-    CUDA_OK(cudaMemcpyAsync(H->host_flags, H->flags, sizeof(int), cudaMemcpyDeviceToHost, s));
+    if (publish_scal(H, 0, 3, s) != 0) return MAESTRO_MAC_ERR_CUDA;
+    if (publish_flags(H, 0, 1, s) != 0) return MAESTRO_MAC_ERR_CUDA;
     CUDA_OK(cudaMemsetAsync(L0.phi - L0.off_c, 0, L0.acell * sizeof(double), s));   // A16: phi = 0 (ghosts too)
     CUDA_OK(cudaEventRecord(H->ev[1], s));
     bool trivial = false;
@@ -882,7 +942,7 @@ extern "C" int maestro_mac_project(maestro_mac_handle* H, const double* beta0, c
                     k_reduce_final<<<1, 1024, 0, s>>>(H->part_sum, H->part_max, nparts, H->scal + 3);
                     LAUNCHED(H);
                 } else if ((rc = do_residual_norm(H, 0, s)) != 0) return rc;
-                CUDA_OK(cudaMemcpyAsync(H->host_scal + 4, H->scal + 4, sizeof(double), cudaMemcpyDeviceToHost, s));
+                if (publish_scal(H, 4, 1, s) != 0) return MAESTRO_MAC_ERR_CUDA;
                 CUDA_OK(cudaStreamSynchronize(s));
                 st.res_norm_inf = H->host_scal[4];
                 const double rel = st.res_norm_inf / st.rhs_norm_inf;
@@ -923,7 +983,7 @@ extern "C" int maestro_mac_project(maestro_mac_handle* H, const double* beta0, c
         }
     }
     CUDA_OK(cudaEventRecord(H->ev[3], s));
-    CUDA_OK(cudaMemcpyAsync(H->host_flags + 1, H->flags + 1, sizeof(int), cudaMemcpyDeviceToHost, s));
+    if (publish_flags(H, 1, 1, s) != 0) return MAESTRO_MAC_ERR_CUDA;
     st.gpu_launches = H->launches;
     if (async) {                                   // nothing was read back: maestro_mac_status() completes the picture
         H->deferred = 1;
@@ -934,7 +994,7 @@ extern "C" int maestro_mac_project(maestro_mac_handle* H, const double* beta0, c
     collect_timings(H, st);
     if (d.rel_tol == 0.0 && !trivial) {   // fixed-cycle run: report the final residual too
         if ((rc = do_residual_norm(H, 0, s)) != 0) return rc;
-        CUDA_OK(cudaMemcpyAsync(H->host_scal + 4, H->scal + 4, sizeof(double), cudaMemcpyDeviceToHost, s));
+        if (publish_scal(H, 4, 1, s) != 0) return MAESTRO_MAC_ERR_CUDA;
         CUDA_OK(cudaStreamSynchronize(s));
         st.res_norm_inf = H->host_scal[4];
         st.gpu_launches = H->launches;
@@ -963,7 +1023,7 @@ extern "C" int maestro_mac_status(maestro_mac_handle* H, maestro_mac_stats* stat
     else if (stats) {                              // the final residual, as the synchronous fixed-cycle call reports it
         int rc;
         if ((rc = do_residual_norm(H, 0, s)) != 0) return rc;
-        CUDA_OK(cudaMemcpyAsync(H->host_scal + 4, H->scal + 4, sizeof(double), cudaMemcpyDeviceToHost, s));
+        if (publish_scal(H, 4, 1, s) != 0) return MAESTRO_MAC_ERR_CUDA;
         CUDA_OK(cudaStreamSynchronize(s));
         st.res_norm_inf = H->host_scal[4];
         st.gpu_launches = H->launches;
@@ -999,6 +1059,62 @@ extern "C" int maestro_mac_project_host(maestro_mac_handle* H, const double* bet
     if (phi) CUDA_OK(cudaMemcpyAsync(phi, T.phi, nc * sizeof(double), cudaMemcpyDeviceToHost, s));
     CUDA_OK(cudaStreamSynchronize(s));
     return rc;
+}
+
+extern "C" int maestro_mac_project_host_seq(maestro_mac_handle* H, int nsteps, const double* beta0, const double* rho0,
+                                            const double* rho, const double* S, const double* const* u_in,
+                                            const double* const* v_in, const double* const* w_in, double* const* u_out,
+                                            double* const* v_out, double* const* w_out, double* const* phi_out,
+                                            maestro_mac_stats* stats, void* cuda_stream)
+{
+    if (!H || !H->cp_in || nsteps < 0 || !beta0 || (!rho && !rho0) || !u_in || !v_in || !w_in || !u_out || !v_out || !w_out)
+        return MAESTRO_MAC_ERR_ARG;
+    for (int k = 0; k < nsteps; ++k)
+        if (!u_in[k] || !v_in[k] || !w_in[k] || !u_out[k] || !v_out[k] || !w_out[k] || (phi_out && !phi_out[k])) return MAESTRO_MAC_ERR_ARG;
+    cudaStream_t s = (cudaStream_t)cuda_stream;
+    const maestro_mac_desc& d = H->d;
+    const size_t nc = (size_t)d.nx * d.ny * d.nz;
+    const size_t nu = (size_t)(d.nx + 1) * d.ny * d.nz, nv = (size_t)d.nx * (d.ny + 1) * d.nz, nw = (size_t)d.nx * d.ny * (d.nz + 1);
+    Staging& T = H->st;
+    const int nset = d.host_staging;                // 2 or 3 sets of u, v, w, phi, used round robin
+    double* su[3] = {T.u, T.ux[0], T.ux[1]}; double* sv[3] = {T.v, T.vx[0], T.vx[1]};
+    double* sw[3] = {T.w, T.wx[0], T.wx[1]}; double* sp[3] = {T.phi, T.phix[0], T.phix[1]};
+    // the step-invariant inputs go first on the upload stream; the first velocity upload queues behind them
+    CUDA_OK(cudaMemcpyAsync(T.beta0, beta0, d.nr * sizeof(double), cudaMemcpyHostToDevice, H->cp_in));
+    if (rho0) CUDA_OK(cudaMemcpyAsync(T.rho0, rho0, d.nr * sizeof(double), cudaMemcpyHostToDevice, H->cp_in));
+    if (rho) CUDA_OK(cudaMemcpyAsync(T.rho, rho, nc * sizeof(double), cudaMemcpyHostToDevice, H->cp_in));
+    if (S) CUDA_OK(cudaMemcpyAsync(T.S, S, nc * sizeof(double), cudaMemcpyHostToDevice, H->cp_in));
+    auto upload = [&](int k) -> int {               // velocities of step k into set k % nset, once its last download is done
+        const int b = k % nset;
+        if (k >= nset) CUDA_OK(cudaStreamWaitEvent(H->cp_in, H->ev_out[b], 0));
+        CUDA_OK(cudaMemcpyAsync(su[b], u_in[k], nu * sizeof(double), cudaMemcpyHostToDevice, H->cp_in));
+        CUDA_OK(cudaMemcpyAsync(sv[b], v_in[k], nv * sizeof(double), cudaMemcpyHostToDevice, H->cp_in));
+        CUDA_OK(cudaMemcpyAsync(sw[b], w_in[k], nw * sizeof(double), cudaMemcpyHostToDevice, H->cp_in));
+        CUDA_OK(cudaEventRecord(H->ev_in[b], H->cp_in));
+        return MAESTRO_MAC_OK;
+    };
+    int rc, worst = MAESTRO_MAC_OK;
+    if (nsteps > 0 && (rc = upload(0)) != 0) return rc;
+    for (int k = 0; k < nsteps; ++k) {
+        const int b = k % nset;
+        if (k + 1 < nsteps && (rc = upload(k + 1)) != 0) return rc;      // travels while step k is projected
+        CUDA_OK(cudaStreamWaitEvent(s, H->ev_in[b], 0));
+        rc = maestro_mac_project(H, T.beta0, rho0 ? T.rho0 : nullptr, rho ? T.rho : nullptr, su[b], sv[b], sw[b],
+                                 S ? T.S : nullptr, phi_out ? sp[b] : nullptr, stats ? stats + k : nullptr, cuda_stream);
+        if (rc < 0) { worst = rc; break; }
+        if (rc == MAESTRO_MAC_NOT_CONVERGED) worst = rc;
+        CUDA_OK(cudaEventRecord(H->ev_done[b], s));
+        CUDA_OK(cudaStreamWaitEvent(H->cp_out, H->ev_done[b], 0));      // travels while step k+1 is projected
+        CUDA_OK(cudaMemcpyAsync(u_out[k], su[b], nu * sizeof(double), cudaMemcpyDeviceToHost, H->cp_out));
+        CUDA_OK(cudaMemcpyAsync(v_out[k], sv[b], nv * sizeof(double), cudaMemcpyDeviceToHost, H->cp_out));
+        CUDA_OK(cudaMemcpyAsync(w_out[k], sw[b], nw * sizeof(double), cudaMemcpyDeviceToHost, H->cp_out));
+        if (phi_out) CUDA_OK(cudaMemcpyAsync(phi_out[k], sp[b], nc * sizeof(double), cudaMemcpyDeviceToHost, H->cp_out));
+        CUDA_OK(cudaEventRecord(H->ev_out[b], H->cp_out));
+    }
+    CUDA_OK(cudaStreamSynchronize(H->cp_in));
+    CUDA_OK(cudaStreamSynchronize(H->cp_out));
+    CUDA_OK(cudaStreamSynchronize(s));
+    return worst;
 }
 
 // ---- base state ---------------------------------------------------
@@ -1094,7 +1210,7 @@ extern "C" int maestro_mac_step_rhs(maestro_mac_handle* H, const double* beta0, 
     cudaStream_t s = (cudaStream_t)cuda_stream;
     int rc = do_rhs(H, beta0, u, v, w, S, s);
     if (rc != 0) return rc;
-    CUDA_OK(cudaMemcpyAsync(H->host_scal, H->scal, 3 * sizeof(double), cudaMemcpyDeviceToHost, s));
+    if (publish_scal(H, 0, 3, s) != 0) return MAESTRO_MAC_ERR_CUDA;
     CUDA_OK(cudaStreamSynchronize(s));
     if (rhs_norm_inf) *rhs_norm_inf = H->host_scal[1];
     if (mean_removed) *mean_removed = H->singular ? H->host_scal[2] / (double)H->lev[0].ncell : 0.0;
@@ -1139,7 +1255,7 @@ extern "C" int maestro_mac_step_residual_norm(maestro_mac_handle* H, int level, 
     cudaStream_t s = (cudaStream_t)cuda_stream;
     int rc = do_residual_norm(H, level, s);
     if (rc != 0) return rc;
-    CUDA_OK(cudaMemcpyAsync(H->host_scal + 4, H->scal + 4, sizeof(double), cudaMemcpyDeviceToHost, s));
+    if (publish_scal(H, 4, 1, s) != 0) return MAESTRO_MAC_ERR_CUDA;
     CUDA_OK(cudaStreamSynchronize(s));
     *norm_inf = H->host_scal[4];
     return MAESTRO_MAC_OK;

@@ -142,7 +142,7 @@ int nod_do_rhs(maestro_mac_handle* H, const double* u, const double* v, const do
     int rc;
     if ((rc = nod_fold(H, nb, 0, s)) != 0) return rc;
     if (H->singular) {                             // N5: remove the uniform volumetric source m = sum / cells
-        CUDA_OK(cudaMemcpyAsync(H->scal + 2, H->scal, sizeof(double), cudaMemcpyDeviceToDevice, s));
+        k_publish<<<1, 32, 0, s>>>(H->scal + 2, H->scal, 1);
         k_nod_shift<true, false><<<g, b, 0, s>>>(L, L.rhs, H->scal + 2, 1.0 / (double)H->nod[0].ncell, H->part_sum, H->part_max, zper);
         LAUNCHED(H);
         if ((rc = nod_fold(H, nb, 0, s)) != 0) return rc;
@@ -283,8 +283,8 @@ extern "C" int maestro_mac_nodal_project(maestro_mac_handle* H, const double* be
     CUDA_OK(cudaEventRecord(H->ev[0], s));
     if ((rc = nod_do_sigma(H, beta0, rho0, rho, s)) != 0) return rc;
     if ((rc = nod_do_rhs(H, uc, vc, wc, S, s)) != 0) return rc;
-    CUDA_OK(cudaMemcpyAsync(H->host_scal, H->scal, 3 * sizeof(double), cudaMemcpyDeviceToHost, s));
-    CUDA_OK(cudaMemcpyAsync(H->host_flags, H->flags, sizeof(int), cudaMemcpyDeviceToHost, s));
+    if (publish_scal(H, 0, 3, s) != 0) return MAESTRO_MAC_ERR_CUDA;
+    if (publish_flags(H, 0, 1, s) != 0) return MAESTRO_MAC_ERR_CUDA;
     if ((rc = nod_zero_phi(H, s)) != 0) return rc;                          // N9: phi = 0 (and finite ghosts everywhere)
     CUDA_OK(cudaEventRecord(H->ev[1], s));
     CUDA_OK(cudaStreamSynchronize(s));
@@ -310,7 +310,7 @@ extern "C" int maestro_mac_nodal_project(maestro_mac_handle* H, const double* be
                     if ((rc = nod_do_jacobi(H, 0, s, &nparts, false)) != 0) return rc;
                     if ((rc = nod_fold(H, nparts, 3, s)) != 0) return rc;
                 } else if ((rc = nod_do_residual_norm(H, 0, s)) != 0) return rc;
-                CUDA_OK(cudaMemcpyAsync(H->host_scal + 4, H->scal + 4, sizeof(double), cudaMemcpyDeviceToHost, s));
+                if (publish_scal(H, 4, 1, s) != 0) return MAESTRO_MAC_ERR_CUDA;
                 CUDA_OK(cudaStreamSynchronize(s));
                 st.res_norm_inf = H->host_scal[4];
                 const double rel = st.res_norm_inf / st.rhs_norm_inf;
@@ -350,13 +350,13 @@ extern "C" int maestro_mac_nodal_project(maestro_mac_handle* H, const double* be
         LAUNCHED(H);
     }
     CUDA_OK(cudaEventRecord(H->ev[3], s));
-    CUDA_OK(cudaMemcpyAsync(H->host_flags + 1, H->flags + 1, sizeof(int), cudaMemcpyDeviceToHost, s));
+    if (publish_flags(H, 1, 1, s) != 0) return MAESTRO_MAC_ERR_CUDA;
     CUDA_OK(cudaStreamSynchronize(s));
     collect_timings(H, st);
     if (d.rel_tol == 0.0 && !trivial) {
         if (H->singular && (rc = nod_phi_ghosts(H, 0, H->nod[0].phi, s)) != 0) return rc;   // the mean shift left the images stale
         if ((rc = nod_do_residual_norm(H, 0, s)) != 0) return rc;
-        CUDA_OK(cudaMemcpyAsync(H->host_scal + 4, H->scal + 4, sizeof(double), cudaMemcpyDeviceToHost, s));
+        if (publish_scal(H, 4, 1, s) != 0) return MAESTRO_MAC_ERR_CUDA;
         CUDA_OK(cudaStreamSynchronize(s));
         st.res_norm_inf = H->host_scal[4];
     }
@@ -413,7 +413,7 @@ extern "C" int maestro_mac_nodal_step_rhs(maestro_mac_handle* H, const double* u
     cudaStream_t s = (cudaStream_t)cuda_stream;
     const int rc = nod_do_rhs(H, uc, vc, wc, S, s);
     if (rc != 0) return rc;
-    CUDA_OK(cudaMemcpyAsync(H->host_scal, H->scal, 3 * sizeof(double), cudaMemcpyDeviceToHost, s));
+    if (publish_scal(H, 0, 3, s) != 0) return MAESTRO_MAC_ERR_CUDA;
     CUDA_OK(cudaStreamSynchronize(s));
     if (rhs_norm_inf) *rhs_norm_inf = H->host_scal[1];
     if (mean_removed) *mean_removed = H->singular ? H->host_scal[2] / (double)H->nod[0].ncell : 0.0;
@@ -456,7 +456,7 @@ extern "C" int maestro_mac_nodal_step_residual_norm(maestro_mac_handle* H, int l
     cudaStream_t s = (cudaStream_t)cuda_stream;
     const int rc = nod_do_residual_norm(H, level, s);
     if (rc != 0) return rc;
-    CUDA_OK(cudaMemcpyAsync(H->host_scal + 4, H->scal + 4, sizeof(double), cudaMemcpyDeviceToHost, s));
+    if (publish_scal(H, 4, 1, s) != 0) return MAESTRO_MAC_ERR_CUDA;
     CUDA_OK(cudaStreamSynchronize(s));
     *norm_inf = H->host_scal[4];
     return MAESTRO_MAC_OK;

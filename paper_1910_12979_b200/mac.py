@@ -20,7 +20,7 @@ ARR_PHI, ARR_RHS, ARR_BX, ARR_BY, ARR_BZ = 0, 1, 2, 3, 4
 
 EXPORTS = [
     "maestro_mac_default_desc", "maestro_mac_setup", "maestro_mac_project",
-    "maestro_mac_project_host", "maestro_mac_free", "maestro_mac_num_levels",
+    "maestro_mac_project_host", "maestro_mac_project_host_seq", "maestro_mac_free", "maestro_mac_num_levels",
     "maestro_mac_level_dims", "maestro_mac_level_get", "maestro_mac_level_set",
     "maestro_mac_step_coefficients", "maestro_mac_step_rhs", "maestro_mac_step_smooth",
     "maestro_mac_step_residual_restrict", "maestro_mac_step_prolong", "maestro_mac_step_bottom",
@@ -84,6 +84,8 @@ def lib():
         proj = [_VP, _VP, _VP, _VP, _VP, _VP, _VP, _VP, _VP, C.POINTER(Stats), _VP]
         L.maestro_mac_project.argtypes = proj
         L.maestro_mac_project_host.argtypes = proj
+        L.maestro_mac_project_host_seq.argtypes = [_VP, C.c_int, _VP, _VP, _VP, _VP, _VP, _VP, _VP, _VP, _VP, _VP, _VP,
+                                                   C.POINTER(Stats), _VP]
         L.maestro_mac_free.argtypes = [_VP]
         L.maestro_mac_num_levels.argtypes = [_VP]
         L.maestro_mac_level_dims.argtypes = [_VP, C.c_int, C.POINTER(C.c_int * 3), C.POINTER(C.c_double * 3)]
@@ -234,6 +236,17 @@ class MacProjector:
                                             _ptr(v), _ptr(w), _ptr(S), _ptr(phi),
                                             C.byref(st) if want_stats else None, _stream())
         return rc, (st.as_dict() if want_stats else None)
+
+    def project_host_seq(self, beta0, rho0, rho, S, u_in, v_in, w_in, u_out, v_out, w_out, phi_out=None, want_stats=True):
+        """len(u_in) consecutive projections with host (pinned) tensors, transfers overlapped with the neighbouring
+        steps (maestro_mac_project_host_seq; needs host_staging=2).  u_in ... phi_out are lists of host tensors."""
+        n = len(u_in)
+        def arr(ts):
+            return (C.c_void_p * n)(*[_ptr(t) for t in ts]) if ts is not None else None
+        st = (Stats * n)() if want_stats else None
+        rc = lib().maestro_mac_project_host_seq(self._h, n, _ptr(beta0), _ptr(rho0), _ptr(rho), _ptr(S), arr(u_in), arr(v_in),
+                                                arr(w_in), arr(u_out), arr(v_out), arr(w_out), arr(phi_out), st, _stream())
+        return rc, ([x.as_dict() for x in st] if want_stats else None)
 
     # ---- step API ---------------------------------------------------------------------------
     def _ck(self, rc, where):

@@ -280,6 +280,54 @@ def test_project_host_matches_device_path(oracle, mac):
     P.close()
 
 
+@pytest.mark.parametrize("nset", [2, 3])
+def test_project_host_seq_pipelined(oracle, mac, nset):
+    """maestro_mac_project_host_seq (config 5's pattern: consecutive projections with a new U_edge each step, transfers
+    overlapped with the neighbouring steps): every step equals the one-at-a-time call bit for bit, with in-place and
+    separate output buffers, and the oracle on the step's own U_edge."""
+    import torch
+    steps = [W.config5(N=64, step=k) for k in range(5)]
+    wl = steps[0]
+    pin = lambda a: torch.from_numpy(a.copy()).pin_memory()
+    P = mac.MacProjector(mac.desc_from_workload(wl, host_staging=nset))
+    one = []
+    for sw in steps:                               # references: the single call, one step at a time
+        u, v, w, phi = pin(sw.u), pin(sw.v), pin(sw.w), torch.empty(wl.rho.shape, dtype=torch.float64).pin_memory()
+        rc, st = P.project_host(pin(wl.beta0), pin(wl.rho0), pin(wl.rho), u, v, w, pin(wl.S), phi)
+        assert rc == 0
+        one.append((u.numpy().copy(), v.numpy().copy(), w.numpy().copy(), phi.numpy().copy(), st["cycles"]))
+    ui, vi, wi = [pin(sw.u) for sw in steps], [pin(sw.v) for sw in steps], [pin(sw.w) for sw in steps]
+    uo = [torch.empty_like(t).pin_memory() for t in ui]
+    phis = [torch.empty(wl.rho.shape, dtype=torch.float64).pin_memory() for _ in steps]
+    # u in place, v and w into separate buffers (two of them, reused every other step, as bench.py does: checked at the end)
+    vo2, wo2 = [torch.empty_like(vi[0]).pin_memory() for _ in range(2)], [torch.empty_like(wi[0]).pin_memory() for _ in range(2)]
+    rc, sts = P.project_host_seq(pin(wl.beta0), pin(wl.rho0), pin(wl.rho), pin(wl.S), ui, vi, wi, ui,
+                                 [vo2[k & 1] for k in range(5)], [wo2[k & 1] for k in range(5)], phis)
+    assert rc == 0 and [st["cycles"] for st in sts] == [o[4] for o in one]
+    for k in range(5):
+        assert np.array_equal(ui[k].numpy(), one[k][0]) and np.array_equal(phis[k].numpy(), one[k][3]), k
+    for k in (3, 4):                               # the last writers of the two rotating buffers
+        assert np.array_equal(vo2[k & 1].numpy(), one[k][1]) and np.array_equal(wo2[k & 1].numpy(), one[k][2]), k
+    ref = oracle_project(oracle, steps[4])
+    assert ref["stats"]["cycles"] == one[4][4]
+    assert rel_l2(one[4][0], ref["u"]) <= E2E_TOL and rel_l2(one[4][3], ref["phi"]) <= E2E_TOL
+    # separate outputs for everything, inputs untouched
+    rc, sts = P.project_host_seq(pin(wl.beta0), pin(wl.rho0), pin(wl.rho), pin(wl.S), [pin(sw.u) for sw in steps[:2]],
+                                 vi[:2], wi[:2], uo[:2], [vo2[0], vo2[1]], [wo2[0], wo2[1]], None)
+    assert rc == 0
+    for k in range(2):
+        assert np.array_equal(uo[k].numpy(), one[k][0]) and np.array_equal(vo2[k].numpy(), one[k][1]), k
+        assert np.array_equal(vi[k].numpy(), steps[k].v)
+    # argument errors: no double staging; a NULL step pointer
+    rc, _ = P.project_host_seq(pin(wl.beta0), pin(wl.rho0), pin(wl.rho), pin(wl.S), [ui[0]], [vi[0]], [None], [ui[0]], [vo2[0]], [wo2[0]])
+    assert rc == mac.ERR_ARG
+    P.close()
+    P1 = mac.MacProjector(mac.desc_from_workload(wl, host_staging=1))
+    rc, _ = P1.project_host_seq(pin(wl.beta0), pin(wl.rho0), pin(wl.rho), pin(wl.S), [ui[0]], [vi[0]], [wi[0]], [uo[0]], [vo2[0]], [wo2[0]])
+    assert rc == mac.ERR_ARG
+    P1.close()
+
+
 def test_asynchronous_fixed_cycle_call(oracle, mac):
     """rel_tol = 0 and stats = NULL: the call returns without synchronising; maestro_mac_status() completes it with
     the same results and stats as the synchronous fixed-cycle call, and reports non-finite input."""
