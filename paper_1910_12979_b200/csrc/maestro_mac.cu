@@ -19,6 +19,7 @@
 #include "mac_smoother_tma.cuh"
 #include "mac_smoother_t2.cuh"
 #include "mac_tail.cuh"
+#include "mac_cluster.cuh"
 #include "mac_base.cuh"
 #include "mac_nodal.cuh"
 
@@ -75,6 +76,11 @@ struct maestro_mac_handle {
     int tail_start;                // first level of the one-launch coarse tail (k_coarse_tail), or -1
     size_t tail_smem;
     TailArgs tail;                 // prepared by plan_tail; level pointers are filled in at launch
+    size_t cl_smem;                // dynamic shared memory per block of the cluster kernel
+    int cl_start;                  // first level of the cluster kernel (k_cluster_vcycles: levels of <= 32^3 cells), or -1
+    clus::Args cl;                 // prepared by plan_tail; level pointers are filled in at launch
+    double *cl_scratch;            // device: the result block of a device-side solve (cycles, norm, flag, history)
+    double *host_hist, *host_hist_dev;   // mapped pinned copy of the result block (4 + 128 doubles)
     // scratch carved from the workspace
     double *part_sum, *part_max;   // kMaxParts each
     double *scal;                  // device scalars: [0] sum, [1] max (k_reduce_final output) ...
@@ -213,6 +219,7 @@ size_t carve(maestro_mac_handle* H, char* base)
     H->scal = (double*)take(16, 8);
     H->bottom_vecs = (double*)take(6 * H->lev[H->nlev - 1].ncell, 8);
     H->flags = (int*)take(16, 4);
+    H->cl_scratch = (double*)take(8 + 4 + 128, 8);
     H->has_nodal = H->d.nodal == 1;
     H->nod_vecs = nullptr;
     if (H->has_nodal) {
@@ -594,7 +601,53 @@ void plan_tail(maestro_mac_handle* H)
 {
     H->tail_start = -1;
     H->tail_smem = 0;
+    H->cl_start = -1;
     if (H->d.smoother == 1 || H->d.smoother == 2) return;
+    // the cluster kernel takes every level from the first one of at most 32^3 cells (plain layout) down to the bottom,
+    // if the slabs fit the blocks' shared memory and the bottom level is small enough for block 0
+    for (int t0 = 0; t0 + 1 < H->nlev && H->d.smoother == 0; ++t0) {
+        if (H->lev[t0].ncell > (size_t)clus::kMaxCells || H->nlev - t0 > clus::kMaxLevels) continue;
+        if (H->lev[t0].gx || H->lev[t0].gy) continue;
+        if (H->lev[H->nlev - 1].ncell > (size_t)clus::kMaxBottom) break;
+        clus::Args& A = H->cl;
+        A.nlev = H->nlev - t0;
+        size_t off = 0;
+        for (int q = 0; q < A.nlev; ++q) {
+            const Level& L = H->lev[t0 + q];
+            clus::Lev& V = A.V[q];
+            const bool bottom = q + 1 == A.nlev;
+            V.hx = (L.n[0] + 1) / 2;
+            V.mx = tail_magic(L.n[0]); V.mxy = tail_magic(L.n[0] * L.n[1]);
+            V.mhx = tail_magic(V.hx); V.mhxy = tail_magic(V.hx * L.n[1]);
+            V.ppc = bottom ? L.n[2] : (L.n[2] + clus::kCtas - 1) / clus::kCtas;
+            V.mppc = tail_magic(V.ppc);
+            const size_t pe = (size_t)L.n[0] * L.n[1];
+            V.o_phi = (int)off; off += pe * V.ppc;
+            V.o_rhs = (int)off; off += pe * V.ppc;
+            V.o_ax = V.o_ay = V.o_az = 0;
+            if (!bottom) {                                 // the bottom is solved by BiCGStab from the global coefficients
+                V.o_ax = (int)off; off += (size_t)(L.n[0] + 1) * L.n[1] * V.ppc;
+                V.o_ay = (int)off; off += (size_t)L.n[0] * (L.n[1] + 1) * V.ppc;
+                V.o_az = (int)off; off += pe * (V.ppc + 1);
+            }
+        }
+        A.o_vecs = (int)off;
+        if (H->lev[H->nlev - 1].ncell > (size_t)clus::kWarpBottom) off += 6 * H->lev[H->nlev - 1].ncell;
+        A.o_scr = (int)off;
+        {
+            size_t scr = 0;
+            for (int q = 1; q < A.nlev; ++q) {
+                const Level& L = H->lev[t0 + q];
+                const size_t own = (size_t)L.n[0] * L.n[1] * A.V[q].ppc * 8;
+                if (own > scr) scr = own;
+            }
+            off += scr;
+        }
+        if (off * sizeof(double) > clus::kSmemMax) continue;
+        H->cl_start = t0;
+        H->cl_smem = off * sizeof(double);
+        return;
+    }
     for (int t0 = 0; t0 + 1 < H->nlev; ++t0) {
         if (H->lev[t0].ncell > (size_t)kTailMaxCells || H->nlev - t0 > kTailMaxLevels) continue;
         if (H->lev[t0].gx || H->lev[t0].gy) continue;
@@ -642,6 +695,34 @@ int do_tail(maestro_mac_handle* H, cudaStream_t s)
     return MAESTRO_MAC_OK;
 }
 
+// levels cl_start .. coarsest in one launch of one cluster; solve: whole cycles with the stop test (cl_start == 0)
+int do_cluster(maestro_mac_handle* H, cudaStream_t s, int solve, int max_cycles, double rel_tol)
+{
+    clus::Args& A = H->cl;
+    for (int q = 0; q < A.nlev; ++q) A.V[q].L = dev_level(H, H->cl_start + q);
+    A.nu_pre = H->d.nu_pre; A.nu_post = H->d.nu_post;
+    A.maxit = H->d.bottom_max_iter; A.tol = H->d.bottom_rel_tol;
+    A.singular = H->singular; A.prolongation = H->d.prolongation;
+    A.solve = solve; A.max_cycles = max_cycles; A.rel_tol = rel_tol;
+    A.rhs_norm = H->scal + 1;
+    A.result = H->cl_scratch + 8;
+    A.iters_accum = H->flags + 1;
+    const size_t sm = H->cl_smem;
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(clus::kCtas, 1, 1);
+    cfg.blockDim = dim3(clus::kThreads, 1, 1);
+    cfg.dynamicSmemBytes = sm;
+    cfg.stream = s;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeClusterDimension;
+    at[0].val.clusterDim.x = clus::kCtas; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+    cfg.attrs = at;
+    cfg.numAttrs = 1;
+    if (cudaLaunchKernelEx(&cfg, clus::k_cluster_vcycles, A) != cudaSuccess) return MAESTRO_MAC_ERR_CUDA;
+    LAUNCHED(H);
+    return MAESTRO_MAC_OK;
+}
+
 int do_bottom(maestro_mac_handle* H, cudaStream_t s)
 {
     int l = H->nlev - 1;
@@ -679,12 +760,12 @@ int do_vcycle(maestro_mac_handle* H, cudaStream_t s, int pre_done = 0)
     int rc;
     // with a coarse tail the levels from tail_start down are one launch (pre_done only ever concerns a level-0
     // TMA sweep, i.e. a level far above the tail)
-    const int lend = H->tail_start >= 0 ? H->tail_start : H->nlev - 1;
+    const int lend = H->cl_start >= 0 ? H->cl_start : (H->tail_start >= 0 ? H->tail_start : H->nlev - 1);
     for (int l = 0; l < lend; ++l) {
         if ((rc = do_smooth(H, l, H->d.nu_pre - (l == 0 ? pre_done : 0), s)) != 0) return rc;
         if ((rc = do_residual_restrict(H, l, s)) != 0) return rc;
     }
-    if ((rc = H->tail_start >= 0 ? do_tail(H, s) : do_bottom(H, s)) != 0) return rc;
+    if ((rc = H->cl_start >= 0 ? do_cluster(H, s, 0, 1, 0.0) : (H->tail_start >= 0 ? do_tail(H, s) : do_bottom(H, s))) != 0) return rc;
     for (int l = lend - 1; l >= 0; --l) {
         if ((rc = do_prolong(H, l, s)) != 0) return rc;
         if ((rc = do_smooth(H, l, H->d.nu_post, s)) != 0) return rc;
@@ -775,11 +856,14 @@ extern "C" int maestro_mac_setup(const maestro_mac_desc* desc, void* workspace, 
         if (H->d.bc_lo[a] == MAESTRO_MAC_OUTFLOW || H->d.bc_hi[a] == MAESTRO_MAC_OUTFLOW) H->singular = 0;
     H->host_scal = nullptr;
     H->host_flags = nullptr;
+    H->host_hist = nullptr;
     for (int e = 0; e < 4; ++e) H->ev[e] = nullptr;
     bool ok = cudaHostAlloc((void**)&H->host_scal, 8 * sizeof(double), cudaHostAllocMapped) == cudaSuccess &&
               cudaHostAlloc((void**)&H->host_flags, 4 * sizeof(int), cudaHostAllocMapped) == cudaSuccess &&
               cudaHostGetDevicePointer((void**)&H->host_scal_dev, H->host_scal, 0) == cudaSuccess &&
-              cudaHostGetDevicePointer((void**)&H->host_flags_dev, H->host_flags, 0) == cudaSuccess;
+              cudaHostGetDevicePointer((void**)&H->host_flags_dev, H->host_flags, 0) == cudaSuccess &&
+              cudaHostAlloc((void**)&H->host_hist, (4 + 128) * sizeof(double), cudaHostAllocMapped) == cudaSuccess &&
+              cudaHostGetDevicePointer((void**)&H->host_hist_dev, H->host_hist, 0) == cudaSuccess;
     for (int e = 0; ok && e < 4; ++e) ok = cudaEventCreate(&H->ev[e]) == cudaSuccess;
     H->sm_ev = nullptr;
     H->sm_used = H->sm_launches = H->sm_sweeps = 0;
@@ -808,6 +892,8 @@ extern "C" int maestro_mac_setup(const maestro_mac_desc* desc, void* workspace, 
     }
     plan_tail(H);
     if (ok) ok = cudaFuncSetAttribute(k_coarse_tail, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kTailSmem) == cudaSuccess;
+    if (ok) ok = cudaFuncSetAttribute(clus::k_cluster_vcycles, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)clus::kSmemMax) == cudaSuccess;
+    if (ok) ok = cudaFuncSetAttribute(clus::k_cluster_vcycles, cudaFuncAttributeNonPortableClusterSizeAllowed, 1) == cudaSuccess;
     if (ok) ok = cudaFuncSetAttribute(k_bottom_bicgstab, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kBottomSmem) == cudaSuccess;
     if (ok) ok = smoother_configure() == 0 && tma_smoother_configure() == 0 && tma_resid_configure() == 0 && t2_smoother_configure() == 0;
     if (ok)
@@ -842,6 +928,7 @@ extern "C" int maestro_mac_free(maestro_mac_handle* H)
     if (!H) return MAESTRO_MAC_OK;
     if (H->host_scal) cudaFreeHost(H->host_scal);
     if (H->host_flags) cudaFreeHost(H->host_flags);
+    if (H->host_hist) cudaFreeHost(H->host_hist);
     for (int e = 0; e < 4; ++e)
         if (H->ev[e]) cudaEventDestroy(H->ev[e]);
     if (H->cp_in) cudaStreamDestroy(H->cp_in);
@@ -926,7 +1013,15 @@ extern "C" int maestro_mac_project(maestro_mac_handle* H, const double* beta0, c
         }
         trivial = st.rhs_norm_inf == 0.0;
     }
-    if (!trivial) {
+    // a problem whose level 0 already fits the cluster kernel is solved by ONE launch: cycles and stop test on the
+    // device, the host reads the cycle count and the residual history after the final synchronise
+    const bool device_solve = H->cl_start == 0;
+    if (!trivial && device_solve) {
+        if ((rc = do_cluster(H, s, 1, d.max_cycles, d.rel_tol > 0.0 ? d.rel_tol : -1.0)) != 0) return rc;
+        k_publish<<<1, 32, 0, s>>>(H->host_hist_dev, H->cl_scratch + 8, 4 + 128);
+        LAUNCHED(H);
+        if (d.rel_tol == 0.0) st.cycles = d.max_cycles;                       // (known without reading anything back)
+    } else if (!trivial) {
         result = d.rel_tol > 0.0 ? MAESTRO_MAC_NOT_CONVERGED : MAESTRO_MAC_OK;
         if (d.rel_tol > 0.0) {
             const bool ride = fused_norm_ok(H);
@@ -992,7 +1087,13 @@ extern "C" int maestro_mac_project(maestro_mac_handle* H, const double* beta0, c
     }
     CUDA_OK(cudaStreamSynchronize(s));
     collect_timings(H, st);
-    if (d.rel_tol == 0.0 && !trivial) {   // fixed-cycle run: report the final residual too
+    if (device_solve && !trivial) {
+        st.cycles = (int)H->host_hist[0];
+        st.res_norm_inf = H->host_hist[1];
+        for (int c = 0; c < st.cycles && c < 128; ++c) st.res_history[c] = H->host_hist[4 + c];
+        if (H->host_hist[2] != 0.0) result = MAESTRO_MAC_ERR_NONFINITE;       // (a NaN met during the cycles; results were written)
+        else if (d.rel_tol > 0.0) result = st.res_norm_inf <= d.rel_tol * st.rhs_norm_inf ? MAESTRO_MAC_OK : MAESTRO_MAC_NOT_CONVERGED;
+    } else if (d.rel_tol == 0.0 && !trivial) {   // fixed-cycle run: report the final residual too
         if ((rc = do_residual_norm(H, 0, s)) != 0) return rc;
         if (publish_scal(H, 4, 1, s) != 0) return MAESTRO_MAC_ERR_CUDA;
         CUDA_OK(cudaStreamSynchronize(s));

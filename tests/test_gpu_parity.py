@@ -341,7 +341,9 @@ def test_asynchronous_fixed_cycle_call(oracle, mac):
     assert rc == 0 and st is None
     rc, st = P.status()
     assert rc == 0 and st["cycles"] == 4
-    assert st["rhs_norm_inf"] == ref["stats"]["rhs_norm_inf"] and st["res_norm_inf"] == ref["stats"]["res_norm_inf"]
+    assert st["rhs_norm_inf"] == ref["stats"]["rhs_norm_inf"]
+    # (the synchronous call of a problem this small takes the norm inside k_cluster_vcycles, status() by k_residual_norm)
+    assert st["res_norm_inf"] == pytest.approx(ref["stats"]["res_norm_inf"], rel=1e-9)
     assert np.array_equal(phi.cpu().numpy(), ref["phi"]) and np.array_equal(dv["u"].cpu().numpy(), ref["u"])
     rc2, st2 = P.status()                          # idempotent: the stats of the last call, no work
     assert rc2 == 0 and st2["cycles"] == 4
