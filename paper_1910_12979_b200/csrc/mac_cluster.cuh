@@ -446,25 +446,16 @@ k_cluster_vcycles(const __grid_constant__ Args A)
     int done = 0;
     double res = 0.0;
     bool bad = false;
-#ifdef MAC_CL_TRACE
-    int tr = 0;
-#define TRACE() do { if (rank == 0 && threadIdx.x == 0 && cyc == 1 && tr < 60) A.result[4 + 64 + tr++] = (double)clock64(); } while (0)
-#else
-#define TRACE() do { } while (0)
-#endif
     for (int cyc = 0; cyc < ncyc; ++cyc) {
-        TRACE();
         for (int q = 0; q < last; ++q) {
             for (int sw = 0; sw < A.nu_pre; ++sw) {
                 color_pass(cl, sm, sV[q], 0, rank); cl.sync();
                 color_pass(cl, sm, sV[q], 1, rank); cl.sync();
             }
-            TRACE();
             residual_scatter(cl, sm, sV[q], sV[q + 1], A.o_scr, rank);
             cl.sync();
             restrict_gather(sm, sV[q + 1], A.o_scr, rank);
             cl.sync();
-            TRACE();
         }
         if (rank == 0) {                        // the bottom level lives here
             const Lev& V = sV[last];
@@ -485,17 +476,14 @@ k_cluster_vcycles(const __grid_constant__ Args A)
             }
         }
         cl.sync();
-        TRACE();
         for (int q = last - 1; q >= 0; --q) {
             prolong_add(cl, sm, sV[q], sV[q + 1], A.prolongation, rank);
             cl.sync();
-            TRACE();
             for (int sw = 0; sw < A.nu_post; ++sw) {
                 color_pass(cl, sm, sV[q], 0, rank); cl.sync();
                 color_pass(cl, sm, sV[q], 1, rank); cl.sync();
             }
         }
-        TRACE();
         if (!A.solve) break;
         // stop test on level 0 (O9): max-norm of the residual relative to ||rhs||inf
         double m = 0.0;
@@ -511,9 +499,7 @@ k_cluster_vcycles(const __grid_constant__ Args A)
                 }
             }
         }
-        TRACE();
         res = cluster_nanmax(cl, m, sh, slots, rank);
-        TRACE();
         const double rel = res / rnorm;
         if (rank == 0 && threadIdx.x == 0 && cyc < 128) A.result[4 + cyc] = rel;
         done = cyc + 1;
@@ -528,11 +514,7 @@ k_cluster_vcycles(const __grid_constant__ Args A)
         for (int q = threadIdx.x; q < n; q += kThreads) gp[q] = sm[V.o_phi + q];
     }
     if (A.solve && rank == 0 && threadIdx.x == 0) {
-#ifdef MAC_CL_TRACE
-        A.result[0] = 128.0;
-#else
         A.result[0] = (double)done;
-#endif
         A.result[1] = res;
         A.result[2] = bad ? 1.0 : 0.0;
     }
