@@ -339,7 +339,7 @@ def run_ours(a):
                 "frac_of_8000_nominal": ach / 8000.0,
                 "dram_traffic_gbs": (traffic / (per_launch_ms * 1e-3) / 1e9) if traffic else None,
                 "per_sweep_achieved": per_sweep, "per_sweep_frac": per_sweep / peak, "per_sweep_frac_of_8000_nominal": per_sweep / 8000.0,
-                "limiter": "see profiles/ (ncu): issue slots and fp64 dependency latency at 12 warps per SM, not DRAM",
+                "limiter": "see profiles/ (ncu): shared-memory pipe and fp64 dependency latency at 12 warps per SM (register-bound occupancy), not DRAM; the chip runs at its 1000 W power cap",
                 "share_of_step": sm_ms / (t_dev * 1e3) if t_dev > 0 else None}
 
     # end to end through the host-buffer entry point
@@ -427,6 +427,30 @@ def run_ours(a):
                            "launches": st_o["gpu_launches"], "timing": "median of 10 after 3 warm-ups, CUDA events"})
             Po.close()
             del do, keep, wo
+        torch.cuda.empty_cache()
+        # the end-of-step (nodal) projection of SURVEY.md Sec. 8(f) rank 3 on the 256^3 star (cell-centred velocities)
+        import numpy as _np
+        wo = W.by_name("3N", 256)
+        Po = mac.MacProjector(mac.desc_from_workload(wo, nodal=1), device=dev)
+        do = mac.to_device(wo, dev)
+        cc = [torch.from_numpy(_np.ascontiguousarray(x)).to(dev) for x in W.cell_centred(wo)]
+        tms, st_o = [], None
+        for it in range(2 + 5):
+            uc, vc, wc = (c.clone() for c in cc)
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            rc, st_o = Po.nodal_project(do["beta0"], do["rho0"], do["rho"], uc, vc, wc, do["S"], None)
+            e1.record()
+            torch.cuda.synchronize()
+            if rc != 0:
+                raise RuntimeError(f"nodal projection returned {rc}")
+            if it >= 2:
+                tms.append(e0.elapsed_time(e1))
+        others.append({"config": "3N, end-of-step nodal projection (maestro_mac_nodal_project)", "n": 256,
+                       "ms_per_projection": statistics.median(tms), "cycles": st_o["cycles"], "launches": st_o["gpu_launches"],
+                       "timing": "median of 5 after 2 warm-ups, CUDA events"})
+        Po.close()
+        del do, cc, wo
         torch.cuda.empty_cache()
 
     cpu = None

@@ -45,24 +45,42 @@ k_base_state(int nr, const double* __restrict__ rho0, const double* __restrict__
 // Sec. 8(f) rank 4).  Cell (i,j,k) belongs to sample m = min(nr-1, floor(r / dr)), r the radius of its
 // centre (planar: z).  The decision is an integer taken from floating point, so r and r / dr are formed
 // with exactly the oracle's operations (no FMA contraction, IEEE sqrt and division): both sides bin
-// every cell alike.  Sums and counts are accumulated with atomics (a warp whose cells share one sample
-// -- every warp in planar geometry -- reduces first and issues one), so the sums are exact up to the
-// order of additions; k_average_finish divides and fills samples without cells by linear interpolation
+// every cell alike.  k_average_finish divides and fills samples without cells by linear interpolation
 // in m (constant beyond the ends).
 // ------------------------------------------------------------------------------------------------
+// The sums are taken in a FIXED order, so the result is bit-reproducible from run to run (fp64 atomics are not): a block
+// walks a fixed set of rows; every warp owns a private set of bins in shared memory (no two warps ever add to the same
+// word); within a warp step the lanes that share a sample are found with __match_any_sync and their values are added
+// in lane order by the lowest lane; at the end the block folds its warps' bins in warp order into partial[block][m],
+// and k_average_finish folds the blocks in block order.  Shared memory: nwarp x nr x (8 + 4) bytes (dynamic); the host
+// picks nwarp so that it fits.
 __global__ void __launch_bounds__(256)
-k_lateral_sum(GeoDev G, const double* __restrict__ rho, double* __restrict__ sum, unsigned long long* __restrict__ cnt)
+k_lateral_sum(GeoDev G, const double* __restrict__ rho, double* __restrict__ part_sum, unsigned* __restrict__ part_cnt)
 {
+    extern __shared__ double lat_sm[];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarp = blockDim.x >> 5;
+    double* bsum = lat_sm + (size_t)warp * G.nr;                                  // this warp's bins
+    unsigned* cnt0 = reinterpret_cast<unsigned*>(lat_sm + (size_t)nwarp * G.nr);
+    unsigned* bcnt = cnt0 + (size_t)warp * G.nr;
+    for (int m = lane; m < G.nr; m += 32) { bsum[m] = 0.0; bcnt[m] = 0u; }
+    __syncwarp();
     const int nrows = G.ny * G.nz;
-    for (int row = blockIdx.x; row < nrows; row += gridDim.x) {
+    // rows in contiguous chunks per block: the assignment depends only on the launch shape
+    const int per_block = (nrows + gridDim.x - 1) / gridDim.x;
+    const int r0 = blockIdx.x * per_block, r1 = min(nrows, r0 + per_block);
+    for (int row = r0 + warp; row < r1; row += nwarp) {
         const int j = row % G.ny, k = row / G.ny;
         const double ay = __dsub_rn(__dmul_rn((double)j + 0.5, G.dy), G.cy), az = __dsub_rn(__dmul_rn((double)k + 0.5, G.dz), G.cz);
         const double zc = __dmul_rn((double)k + 0.5, G.dz);
         const double* __restrict__ p = rho + (size_t)G.nx * ((size_t)j + (size_t)G.ny * k);
-        for (int i0 = warp * 32; i0 < G.nx; i0 += nwarp * 32) {
+        double vq[4];
+        for (int i0 = 0; i0 < G.nx; i0 += 32) {
             const int i = i0 + lane;
             const bool on = i < G.nx;
+            if ((i0 & 127) == 0) {                                    // request the next four warp-rows of values at once
+#pragma unroll
+                for (int q = 0; q < 4; ++q) vq[q] = i + 32 * q < G.nx ? __ldg(p + i + 32 * q) : 0.0;
+            }
             double r = zc;
             if (G.geometry != 0) {
                 const double ax = __dsub_rn(__dmul_rn((double)i + 0.5, G.dx), G.cx);
@@ -70,25 +88,46 @@ k_lateral_sum(GeoDev G, const double* __restrict__ rho, double* __restrict__ sum
             }
             int m = (int)floor(__ddiv_rn(r, G.dr));
             m = max(0, min(m, G.nr - 1));
-            const double v = on ? __ldg(p + i) : 0.0;
-            const unsigned act = __ballot_sync(0xffffffffu, on);
-            const int m0 = __shfl_sync(0xffffffffu, m, 0);
-            if (__all_sync(0xffffffffu, !on || m == m0)) {           // one sample for the whole warp
-                const double s = warp_sum(v);
-                if (lane == 0) { atomicAdd(sum + m0, s); atomicAdd(cnt + m0, (unsigned long long)__popc(act)); }
-            } else if (on) {
-                atomicAdd(sum + m, v);
-                atomicAdd(cnt + m, 1ull);
+            const int qs = (i0 >> 5) & 3;
+            const double v = qs == 0 ? vq[0] : (qs == 1 ? vq[1] : (qs == 2 ? vq[2] : vq[3]));
+            const unsigned same = __match_any_sync(0xffffffffu, on ? m : -1 - lane);   // lanes of the same sample (idle lanes: alone)
+            if (same == 0xffffffffu) {                                // one sample for the whole warp (always, in planar geometry)
+                const double s = warp_sum(v);                         // fixed shuffle tree
+                if (lane == 0) { bsum[m] += s; bcnt[m] += 32u; }
+            } else {                                                  // the lowest lane of each group adds its values in lane order
+                double s = 0.0;
+                unsigned rest = same;
+                while (__any_sync(0xffffffffu, rest != 0u)) {
+                    const int src = rest ? __ffs(rest) - 1 : 0;
+                    const double t = __shfl_sync(0xffffffffu, v, src);
+                    if (rest) { s += t; rest &= rest - 1u; }
+                }
+                if (on && lane == __ffs(same) - 1) { bsum[m] += s; bcnt[m] += (unsigned)__popc(same); }
             }
+            __syncwarp();
         }
+    }
+    __syncthreads();
+    for (int m = threadIdx.x; m < G.nr; m += blockDim.x) {            // fold the warps in warp order
+        double s = 0.0;
+        unsigned c = 0u;
+        for (int w = 0; w < nwarp; ++w) { s += lat_sm[(size_t)w * G.nr + m]; c += cnt0[(size_t)w * G.nr + m]; }
+        part_sum[(size_t)blockIdx.x * G.nr + m] = s;
+        part_cnt[(size_t)blockIdx.x * G.nr + m] = c;
     }
 }
 
 __global__ void __launch_bounds__(256)
-k_average_finish(int nr, const double* __restrict__ sum, const unsigned long long* __restrict__ cnt, double* __restrict__ rho0)
+k_average_finish(int nr, int nblocks, const double* __restrict__ part_sum, const unsigned* __restrict__ part_cnt,
+                 unsigned long long* __restrict__ cnt, double* __restrict__ rho0)
 {
-    for (int m = threadIdx.x; m < nr; m += blockDim.x)
-        if (cnt[m] > 0) rho0[m] = sum[m] / (double)cnt[m];
+    for (int m = threadIdx.x; m < nr; m += blockDim.x) {              // fold the blocks in block order
+        double s = 0.0;
+        unsigned long long c = 0ull;
+        for (int b = 0; b < nblocks; ++b) { s += part_sum[(size_t)b * nr + m]; c += part_cnt[(size_t)b * nr + m]; }
+        cnt[m] = c;
+        if (c > 0) rho0[m] = s / (double)c;
+    }
     __syncthreads();
     if (threadIdx.x == 0) {                                          // samples without cells
         int prev = -1;

@@ -30,6 +30,8 @@ constexpr int kRedBlocksPerSm = 8;        // blocks per SM of the row-walking re
 constexpr int kMaxParts = 131072;         // capacity of the partial-reduction arrays
 constexpr int kBottomMax = 4096;          // largest coarsest level (unknowns)
 constexpr size_t kBottomSmem = 200 * 1024; // bottom-solver vectors live in shared memory up to this size
+constexpr int kLateralBlocks = 160;      // blocks of the lateral-average sum (one per SM, at most this many)
+constexpr size_t kLateralSmem = 200 * 1024;
 constexpr int kSmoothEvents = 512;        // level-0 smoother launches timed per call
 
 struct Level {
@@ -79,6 +81,7 @@ struct maestro_mac_handle {
     size_t cl_smem;                // dynamic shared memory per block of the cluster kernel
     int cl_start;                  // first level of the cluster kernel (k_cluster_vcycles: levels of <= 32^3 cells), or -1
     clus::Args cl;                 // prepared by plan_tail; level pointers are filled in at launch
+    double *lat_part;              // lateral average: kLateralBlocks x nr partial sums (doubles) and counts (unsigned), or NULL
     double *cl_scratch;            // device: the result block of a device-side solve (cycles, norm, flag, history)
     double *host_hist, *host_hist_dev;   // mapped pinned copy of the result block (4 + 128 doubles)
     // scratch carved from the workspace
@@ -220,6 +223,7 @@ size_t carve(maestro_mac_handle* H, char* base)
     H->bottom_vecs = (double*)take(6 * H->lev[H->nlev - 1].ncell, 8);
     H->flags = (int*)take(16, 4);
     H->cl_scratch = (double*)take(8 + 4 + 128, 8);
+    H->lat_part = (size_t)H->d.nr * 12 <= kLateralSmem ? (double*)take((size_t)kLateralBlocks * H->d.nr * 12 / 8 + 8, 8) : nullptr;
     H->has_nodal = H->d.nodal == 1;
     H->nod_vecs = nullptr;
     if (H->has_nodal) {
@@ -892,6 +896,7 @@ extern "C" int maestro_mac_setup(const maestro_mac_desc* desc, void* workspace, 
     }
     plan_tail(H);
     if (ok) ok = cudaFuncSetAttribute(k_coarse_tail, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kTailSmem) == cudaSuccess;
+    if (ok) ok = cudaFuncSetAttribute(k_lateral_sum, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kLateralSmem) == cudaSuccess;
     if (ok) ok = cudaFuncSetAttribute(clus::k_cluster_vcycles, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)clus::kSmemMax) == cudaSuccess;
     if (ok) ok = cudaFuncSetAttribute(clus::k_cluster_vcycles, cudaFuncAttributeNonPortableClusterSizeAllowed, 1) == cudaSuccess;
     if (ok) ok = cudaFuncSetAttribute(k_bottom_bicgstab, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kBottomSmem) == cudaSuccess;
@@ -1231,15 +1236,21 @@ extern "C" int maestro_mac_base_state(int nr, const double* rho0, const double* 
 extern "C" int maestro_mac_lateral_average(maestro_mac_handle* H, const double* rho, double* rho0, void* cuda_stream)
 {
     if (!H || !rho || !rho0) return MAESTRO_MAC_ERR_ARG;
-    if (H->d.nr > kMaxParts) return MAESTRO_MAC_ERR_UNSUPPORTED;
+    if (H->d.nr > kMaxParts || !H->lat_part) return MAESTRO_MAC_ERR_UNSUPPORTED;
     cudaStream_t s = (cudaStream_t)cuda_stream;
     unsigned long long* cnt = reinterpret_cast<unsigned long long*>(H->part_max);
-    CUDA_OK(cudaMemsetAsync(H->part_sum, 0, H->d.nr * sizeof(double), s));
-    CUDA_OK(cudaMemsetAsync(cnt, 0, H->d.nr * sizeof(unsigned long long), s));
-    const int rows = H->d.ny * H->d.nz;
-    k_lateral_sum<<<rows < H->sms * 16 ? rows : H->sms * 16, 256, 0, s>>>(dev_geo(H), rho, H->part_sum, cnt);
+    const int nr = H->d.nr, rows = H->d.ny * H->d.nz;
+    // as many warps per block as private bin sets fit in shared memory; blocks: one per SM, capped by the scratch
+    int nwarp = (int)(kLateralSmem / ((size_t)nr * 12));
+    if (nwarp < 1) return MAESTRO_MAC_ERR_UNSUPPORTED;
+    if (nwarp > 8) nwarp = 8;
+    int nb = H->sms < kLateralBlocks ? H->sms : kLateralBlocks;
+    if (nb > rows) nb = rows;
+    double* psum = H->lat_part;
+    unsigned* pcnt = reinterpret_cast<unsigned*>(H->lat_part + (size_t)kLateralBlocks * nr);
+    k_lateral_sum<<<nb, 32 * nwarp, (size_t)nwarp * nr * 12, s>>>(dev_geo(H), rho, psum, pcnt);
     LAUNCHED(H);
-    k_average_finish<<<1, 256, 0, s>>>(H->d.nr, H->part_sum, cnt, rho0);
+    k_average_finish<<<1, 256, 0, s>>>(nr, nb, psum, pcnt, cnt, rho0);
     LAUNCHED(H);
     return MAESTRO_MAC_OK;
 }
