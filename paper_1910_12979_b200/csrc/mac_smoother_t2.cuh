@@ -44,7 +44,10 @@ namespace t2 {
 using fused::pick; using fused::put;
 using tma::mbar_init; using tma::mbar_expect_tx; using tma::mbar_wait; using tma::tma_load_3d; using tma::smem_u32;
 
-constexpr int LN = 16, TYE = 24, NT = LN * TYE;      // 16 pairs x 24 rows = 384 threads: the COMPUTED cells (32 x 24)
+#ifndef MAC_T2_TYE
+#define MAC_T2_TYE 24                                // thread rows of a tile (a multiple of 4)
+#endif
+constexpr int LN = 16, TYE = MAC_T2_TYE, NT = LN * TYE;   // 16 pairs x 24 rows = 384 threads: the COMPUTED cells (32 x 24)
 constexpr int HALO = 4;                              // cells a finished cell depends on laterally (periodic image width)
 // Only three of the four rings around a finished cell are COMPUTED (sweep-1 red / black, sweep-2 red); the fourth is
 // the old black value that sweep-1 red reads.  So the staged phi box is one cell wider than the computed tile on every
@@ -81,6 +84,10 @@ template <bool X> __device__ __forceinline__ double ldc(const unsigned char* p, 
 {
     return *reinterpret_cast<const double*>(p + dy * kRowP + dl * 16 + (X ? 0 : 8));
 }
+
+// 24-row tiles keep the reciprocal diagonals of sweep 1 for sweep 2 (16 registers); taller tiles (more threads, fewer
+// registers each) form them again
+constexpr bool kKeepRdg = TYE <= 24;
 
 struct Coef {                                // coefficients of one plane for a column pair, in registers, and the
     double2 ax; double ax2; double2 ays, ayn, az, rhs;   // reciprocals of the two diagonals, which sweep 1 computes
@@ -150,7 +157,7 @@ __device__ __forceinline__ double gs_cell(const Lat& l, double other, Coef& C, c
         asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(dg));
         r = fma(fma(-dg, r, 1.0), r, r);
         r = fma(fma(-dg, r, 1.0), r, r);
-        put<X>(C.rdg, r);
+        if (kKeepRdg) put<X>(C.rdg, r);
     } else {
         r = pick<X>(C.rdg);
     }
@@ -219,10 +226,10 @@ __device__ __forceinline__ void step(const Th& T, int kk, const unsigned char* s
     const double n1 = gs_cell<X, true>(l1, pick<!X>(Pm1), S1, CUR.az, pick<X>(Pm2), pick<X>(P0), a, dg);
     put<X>(Pm1, ((fl & (X ? F_BA_X : F_BA_Y)) && v1) ? n1 : pick<X>(Pm1));
     // (3) sweep 2, red cells of plane kk-2
-    const double n2 = gs_cell<X, false>(l2, pick<!X>(Pm2), S2, S1.az, pick<X>(Pm3), pick<X>(Pm1), a, dg);
+    const double n2 = gs_cell<X, !kKeepRdg>(l2, pick<!X>(Pm2), S2, S1.az, pick<X>(Pm3), pick<X>(Pm1), a, dg);
     put<X>(Pm2, ((fl & F_RB) && v2) ? n2 : pick<X>(Pm2));
     // (4) sweep 2, black cells of plane kk-3; the plane is finished
-    const double n3 = gs_cell<X, false>(l3, pick<!X>(Pm3), S3, S2.az, pick<X>(Pm4), pick<X>(Pm2), a, dg);
+    const double n3 = gs_cell<X, !kKeepRdg>(l3, pick<!X>(Pm3), S3, S2.az, pick<X>(Pm4), pick<X>(Pm2), a, dg);
     *reinterpret_cast<double*>(T.ex0() + (EX_RA + W) * kEx) = pick<X>(P0);
     *reinterpret_cast<double*>(T.ex0() + (EX_BA + W) * kEx) = pick<X>(Pm1);
     *reinterpret_cast<double*>(T.ex0() + (EX_RB + W) * kEx) = pick<X>(Pm2);
