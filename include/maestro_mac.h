@@ -295,7 +295,8 @@ int maestro_mac_num_levels(const maestro_mac_handle *h);
  *   kernel: the whole waves), info[3] z-chunks per remaining tile, info[4] planes per chunk, info[5] CTAs of one
  *   launch, info[6], info[7] periodic image columns / rows per side of the level's arrays. */
 enum { MAESTRO_MAC_KERNEL_COLOR = 0, MAESTRO_MAC_KERNEL_FUSED = 1, MAESTRO_MAC_KERNEL_TMA = 2,
-       MAESTRO_MAC_KERNEL_T2 = 3, MAESTRO_MAC_KERNEL_TAIL = 4, MAESTRO_MAC_KERNEL_BOTTOM = 5 };
+       MAESTRO_MAC_KERNEL_T2 = 3, MAESTRO_MAC_KERNEL_TAIL = 4, MAESTRO_MAC_KERNEL_BOTTOM = 5,
+       MAESTRO_MAC_KERNEL_CLUSTER = 6 };   /* CLUSTER: the level is one of those k_cluster_vcycles walks in one launch */
 int maestro_mac_level_plan(const maestro_mac_handle *h, int level, int info[8]);
 /* n[3] cells and h[3] spacing of a level */
 int maestro_mac_level_dims(const maestro_mac_handle *h, int level, int n[3], double hh[3]);

@@ -601,7 +601,7 @@ int do_prolong(maestro_mac_handle* H, int l, cudaStream_t s)
 // which keep one launch per step on every level.
 unsigned tail_magic(int d) { return d <= 1 ? 0u : (unsigned)((1ull << 32) / (unsigned)d + 1ull); }
 
-void plan_tail(maestro_mac_handle* H)
+void plan_tail(maestro_mac_handle* H, bool allow_cluster = true)
 {
     H->tail_start = -1;
     H->tail_smem = 0;
@@ -609,7 +609,7 @@ void plan_tail(maestro_mac_handle* H)
     if (H->d.smoother == 1 || H->d.smoother == 2) return;
     // the cluster kernel takes every level from the first one of at most 32^3 cells (plain layout) down to the bottom,
     // if the slabs fit the blocks' shared memory and the bottom level is small enough for block 0
-    for (int t0 = 0; t0 + 1 < H->nlev && H->d.smoother == 0; ++t0) {
+    for (int t0 = 0; allow_cluster && t0 + 1 < H->nlev && H->d.smoother == 0; ++t0) {
         if (H->lev[t0].ncell > (size_t)clus::kMaxCells || H->nlev - t0 > clus::kMaxLevels) continue;
         if (H->lev[t0].gx || H->lev[t0].gy) continue;
         if (H->lev[H->nlev - 1].ncell > (size_t)clus::kMaxBottom) break;
@@ -899,6 +899,22 @@ extern "C" int maestro_mac_setup(const maestro_mac_desc* desc, void* workspace, 
     if (ok) ok = cudaFuncSetAttribute(k_lateral_sum, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kLateralSmem) == cudaSuccess;
     if (ok) ok = cudaFuncSetAttribute(clus::k_cluster_vcycles, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)clus::kSmemMax) == cudaSuccess;
     if (ok) ok = cudaFuncSetAttribute(clus::k_cluster_vcycles, cudaFuncAttributeNonPortableClusterSizeAllowed, 1) == cudaSuccess;
+    if (ok && H->cl_start >= 0) {                    // can this device place a 16-block cluster with that much shared memory?
+        cudaLaunchConfig_t cfg = {};
+        cfg.gridDim = dim3(clus::kCtas, 1, 1);
+        cfg.blockDim = dim3(clus::kThreads, 1, 1);
+        cfg.dynamicSmemBytes = H->cl_smem;
+        cudaLaunchAttribute at[1];
+        at[0].id = cudaLaunchAttributeClusterDimension;
+        at[0].val.clusterDim.x = clus::kCtas; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+        cfg.attrs = at;
+        cfg.numAttrs = 1;
+        int nclusters = 0;
+        if (cudaOccupancyMaxActiveClusters(&nclusters, clus::k_cluster_vcycles, &cfg) != cudaSuccess || nclusters < 1) {
+            (void)cudaGetLastError();
+            plan_tail(H, false);                     // no: the one-block tail (or one launch per step) takes the small levels
+        }
+    }
     if (ok) ok = cudaFuncSetAttribute(k_bottom_bicgstab, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kBottomSmem) == cudaSuccess;
     if (ok) ok = smoother_configure() == 0 && tma_smoother_configure() == 0 && tma_resid_configure() == 0 && t2_smoother_configure() == 0;
     if (ok)
@@ -1388,7 +1404,8 @@ extern "C" int maestro_mac_level_plan(const maestro_mac_handle* H, int level, in
     for (int q = 0; q < 8; ++q) info[q] = 0;
     info[6] = L.gx; info[7] = L.gy;
     const int sm = H->d.smoother;
-    if (level == H->nlev - 1 && H->nlev > 1) { info[0] = MAESTRO_MAC_KERNEL_BOTTOM; return MAESTRO_MAC_OK; }
+    if (level == H->nlev - 1 && H->nlev > 1 && H->cl_start < 0) { info[0] = MAESTRO_MAC_KERNEL_BOTTOM; return MAESTRO_MAC_OK; }
+    if (H->cl_start >= 0 && level >= H->cl_start) { info[0] = MAESTRO_MAC_KERNEL_CLUSTER; return MAESTRO_MAC_OK; }
     if (H->tail_start >= 0 && level >= H->tail_start) { info[0] = MAESTRO_MAC_KERNEL_TAIL; return MAESTRO_MAC_OK; }
     if (t2_ok(H, level)) {
         const t2::T2Plan P = t2_plan(D, H->sms);

@@ -262,7 +262,7 @@ class MacProjector:
         self._ck(lib().maestro_mac_level_dims(self._h, level, C.byref(n), C.byref(h)), "level_dims")
         return tuple(n), tuple(h)
 
-    KERNELS = ("color", "fused", "tma", "t2", "tail", "bottom")
+    KERNELS = ("color", "fused", "tma", "t2", "tail", "bottom", "cluster")
 
     def level_plan(self, level):
         """Launch plan of the smoother on a level (maestro_mac_level_plan)."""

@@ -328,6 +328,32 @@ def test_project_host_seq_pipelined(oracle, mac, nset):
     P1.close()
 
 
+@pytest.mark.parametrize("name,N", [("1", 32), ("2", 32), ("3D", 32), ("3N", 16)])
+def test_device_side_solve_of_small_problems(oracle, mac, name, N):
+    """A problem whose level 0 has at most 32^3 cells is solved by ONE launch of k_cluster_vcycles (cycles and stop test
+    on the device): same cycle count and residual history as the host-driven solve of
+    smoother 4 (one launch per step, k_coarse_tail, stop test read by the host every cycle), results equal up to the
+    bottom solver's rounding (one-warp BiCGStab there, block BiCGStab here), a handful of launches, and the oracle's result."""
+    wl = W.by_name(name, N)
+    P = mac.MacProjector(mac.desc_from_workload(wl))
+    assert P.level_plan(0)["kernel"] == "cluster", P.level_plan(0)
+    P.close()
+    a, b = gpu_project(mac, wl), gpu_project(mac, wl, smoother=4)
+    assert a["status"] == b["status"] == 0 and a["stats"]["cycles"] == b["stats"]["cycles"]
+    assert a["stats"]["gpu_launches"] <= 20 < b["stats"]["gpu_launches"]
+    assert np.allclose(a["stats"]["res_history"], b["stats"]["res_history"], rtol=1e-6)
+    for key in ("phi", "u", "v", "w"):
+        assert rel_l2(a[key], b[key]) <= 1e-12, key
+    ref = oracle_project(oracle, wl)
+    assert ref["stats"]["cycles"] == a["stats"]["cycles"]
+    for key in ("phi", "u", "v", "w"):
+        assert rel_l2(a[key], ref[key]) <= E2E_TOL, key
+    # fixed cycle count: the history is filled, the final norm reported
+    c = gpu_project(mac, wl, rel_tol=0.0, max_cycles=3)
+    assert c["status"] == 0 and c["stats"]["cycles"] == 3
+    assert np.allclose(c["stats"]["res_history"], a["stats"]["res_history"][:3], rtol=1e-12)
+
+
 def test_asynchronous_fixed_cycle_call(oracle, mac):
     """rel_tol = 0 and stats = NULL: the call returns without synchronising; maestro_mac_status() completes it with
     the same results and stats as the synchronous fixed-cycle call, and reports non-finite input."""
