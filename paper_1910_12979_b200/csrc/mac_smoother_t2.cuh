@@ -313,7 +313,7 @@ __device__ __forceinline__ void march(const Th& T, int ks, int ke, const CUtenso
 // Work decomposition of one launch (host: t2_plan).  704 tiles on 148 SMs are 4.76 waves of whole columns: the
 // first nfull tiles (whole waves) march all of z, the remaining tiles are cut into nsplit z-chunks each so that the
 // last, partial wave is spread over every SM.  nfull = 0: every tile is cut into nsplit chunks.
-struct T2Plan { int tiles_x, tiles, nfull, nsplit, zchunk, ncta; };
+struct T2Plan { int tiles_x, tiles, nfull, nsplit, zchunk, ncta, images; };   // images: the kernel stores the periodic images of phi itself
 
 // NORM: additionally writes, per CTA, max |rhs - L phi_in| over the red cells to part_max[linear CTA index]
 template <int LA, bool NORM>
@@ -360,7 +360,7 @@ k_rbgs_t2(const __grid_constant__ CUtensorMap tm_phi, const __grid_constant__ CU
         fl = F_RA | (in_y && lane >= 1 ? F_BA_X : 0) | (in_y && lane <= LN - 2 ? F_BA_Y : 0) |
              (ty >= 2 && ty <= TYE - 3 && lane >= 1 && lane <= LN - 2 ? F_RB : 0) |
              (own_row && lane >= 2 && lane <= LN - 2 ? F_OWN_X : 0) | (own_row && lane >= 1 && lane <= LN - 3 ? F_OWN_Y : 0);
-        if ((fl & (F_OWN_X | F_OWN_Y)) && (T.img_x | T.img_y)) fl |= F_IMG;
+        if (plan.images && (fl & (F_OWN_X | F_OWN_Y)) && (T.img_x | T.img_y)) fl |= F_IMG;
     }
     asm volatile("" : "+r"(fl));                      // opaque: keep the bits, do not recompute the conditions per step
     T.fl = fl;
@@ -423,6 +423,9 @@ k_rbgs_t2(const __grid_constant__ CUtensorMap tm_phi, const __grid_constant__ CU
 
 // ---- host side ---------------------------------------------------------------------------------
 
+#ifndef MAC_T2_IMAGES_BELOW
+#define MAC_T2_IMAGES_BELOW (1ll << 18)   // cells of a level below which the two-sweep kernel stores the periodic images itself
+#endif
 #ifndef MAC_T2_LA
 #define MAC_T2_LA 2                   // planes of TMA lookahead (4 stages per ring)
 #endif
@@ -486,11 +489,16 @@ static inline t2::T2Plan t2_plan(const LevelDev& L, int sms)
     }
     P.zchunk = (L.nz + P.nsplit - 1) / P.nsplit;
     P.ncta = P.nfull + (P.tiles - P.nfull) * P.nsplit;
+    // Periodic images of the output: written by the owning threads inside the kernel on small levels (no extra launch);
+    // on large ones by k_fill_ghosts after it -- measured at 512^3, the few divergent image stores of the edge tiles
+    // cost the launch 10 % (y) / 4 % (x), a separate pass over the image strips 1 %
+    P.images = (L.gx || L.gy) && (long long)L.nx * L.ny * L.nz < MAC_T2_IMAGES_BELOW ? 1 : 0;
     return P;
 }
 
 // Two fused sweeps: reads `in_is_phi2 ? phi2 : phi` through T (maps built for the 32 x 24 tile), writes phi_out.
 // part_max != NULL: also per-CTA maxima of the input's red-cell residual; *nparts receives their count.
+// Returns the number of kernels launched (2 when the images of the output are a pass of their own), or -1.
 static inline int launch_t2_sweep(const TmaLevelMaps& T, bool in_is_phi2, double* phi_out, const LevelDev& L, int sms, cudaStream_t s,
                                   double* part_max = nullptr, int max_parts = 0, int* nparts = nullptr)
 {
@@ -505,5 +513,13 @@ static inline int launch_t2_sweep(const TmaLevelMaps& T, bool in_is_phi2, double
         k_rbgs_t2<MAC_T2_LA, true><<<grid, dim3(LN, TYE), sm, s>>>(tin, T.rhs, T.ax, T.ay, T.az, L, phi_out, plan, part_max);
     } else
         k_rbgs_t2<MAC_T2_LA, false><<<grid, dim3(LN, TYE), sm, s>>>(tin, T.rhs, T.ax, T.ay, T.az, L, phi_out, plan, nullptr);
-    return cudaPeekAtLastError() == cudaSuccess ? 0 : -1;
+    int launches = 1;
+    if (!plan.images && (L.gx || L.gy)) {                   // the images of the output, as a pass of their own
+        LevelDev O = L;
+        O.phi = phi_out;
+        const int per_plane = 2 * L.gx * (L.ny + 1 + 2 * L.gy) + 2 * L.gy * (L.nx + 1);
+        k_fill_ghosts<<<dim3((per_plane + 255) / 256, L.nz + 1), 256, 0, s>>>(O, 1);
+        ++launches;
+    }
+    return cudaPeekAtLastError() == cudaSuccess ? launches : -1;
 }

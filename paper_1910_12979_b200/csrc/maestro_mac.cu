@@ -532,10 +532,10 @@ int do_sweep2(maestro_mac_handle* H, int l, cudaStream_t s, int* norm_parts = nu
     const bool timed = l == 0 && H->sm_ev && H->sm_used < kSmoothEvents;
     if (l == 0) ++H->sm_launches;
     if (timed) CUDA_OK(cudaEventRecord(H->sm_ev[2 * H->sm_used], s));
-    if (launch_t2_sweep(Lv.tma[2], Lv.phi != Lv.phi_a, Lv.phi2, dev_level(H, l), H->sms, s, norm_parts ? H->part_max : nullptr,
-                        kMaxParts, norm_parts) != 0)
-        return MAESTRO_MAC_ERR_CUDA;
-    ++H->launches;
+    const int nl = launch_t2_sweep(Lv.tma[2], Lv.phi != Lv.phi_a, Lv.phi2, dev_level(H, l), H->sms, s, norm_parts ? H->part_max : nullptr,
+                                   kMaxParts, norm_parts);
+    if (nl < 0) return MAESTRO_MAC_ERR_CUDA;
+    H->launches += nl;
     if (swap) { double* t = Lv.phi; Lv.phi = Lv.phi2; Lv.phi2 = t; }
     if (timed) { CUDA_OK(cudaEventRecord(H->sm_ev[2 * H->sm_used + 1], s)); ++H->sm_used; H->sm_sweeps += 2; }
     return MAESTRO_MAC_OK;
