@@ -382,20 +382,33 @@ constexpr unsigned kTx = (TY + 2) * BW * 8 + (TY + 1) * BW * 8 + TY * TX * 8;   
 static_assert((TY + 2) * BW * 8 <= kPhi && (TY + 1) * BW * 8 <= kSig, "stage layout");
 }  // namespace nodm
 
+// Work decomposition of one launch (host: nod_march_plan), as for the two-sweep smoother of the MAC solve: the first
+// nfull tiles (whole waves of blocks) march every plane, the remaining tiles are cut into nsplit z-chunks each so that
+// the last, partial wave spreads over every SM (257^3 nodes are 297 tiles of 32 x 8 on 296 block slots: uniform
+// chunks need 8 rounds of 37 planes, the mixed plan one round of 257 plus one of 16).
+struct NodPlan { int tiles_x, tiles, nfull, nsplit, zchunk, ncta; };
+
 template <int MODE>
 __global__ void __launch_bounds__(256, 2)
 k_nod_march(const __grid_constant__ CUtensorMap tm_phi, const __grid_constant__ CUtensorMap tm_sig,
             const __grid_constant__ CUtensorMap tm_rhs, NodLevel L, const double* __restrict__ pin, double* __restrict__ out,
-            double* __restrict__ part_max, int zchunk)
+            double* __restrict__ part_max, NodPlan plan)
 {
     using namespace nodm;
     using tma::mbar_init; using tma::mbar_expect_tx; using tma::mbar_wait; using tma::tma_load_3d; using tma::smem_u32;
     __shared__ __align__(128) unsigned char ring[NS * kStage];
     __shared__ __align__(8) unsigned long long bars[NS];
     const int tx = threadIdx.x, ty = threadIdx.y, tid = tx + TX * ty;
-    const int x0 = blockIdx.x * TX, y0 = blockIdx.y * TY;
+    int tile = blockIdx.x, k0 = 0, k1 = L.nz + 1;
+    if (tile >= plan.nfull) {
+        const int q = tile - plan.nfull, rem = plan.tiles - plan.nfull, c = q / rem;
+        tile = plan.nfull + (q - c * rem);
+        k0 = c * plan.zchunk;
+        k1 = min(k0 + plan.zchunk, L.nz + 1);
+    }
+    const int tby = tile / plan.tiles_x;
+    const int x0 = (tile - tby * plan.tiles_x) * TX, y0 = tby * TY;
     const int i = x0 + tx, j = y0 + ty;
-    const int k0 = blockIdx.z * zchunk, k1 = min(k0 + zchunk, L.nz + 1);
     int kxy = 3;                                                  // lateral kind: 0 unknown, 1 OUTFLOW, 2 duplicate, 3 outside
     if (i <= L.nx && j <= L.ny) {
         const int ka = nod_axis_kind(L, 0, i), kb = nod_axis_kind(L, 1, j);
@@ -500,7 +513,7 @@ k_nod_march(const __grid_constant__ CUtensorMap tm_phi, const __grid_constant__ 
         if (tid == 0) {
             double m = sh[0];
             for (int qq = 1; qq < 8; ++qq) m = nanmax(m, sh[qq]);
-            part_max[blockIdx.x + gridDim.x * (blockIdx.y + gridDim.y * blockIdx.z)] = m;
+            part_max[blockIdx.x] = m;
         }
     }
 }

@@ -44,24 +44,30 @@ void nod_dims_red(int ex, int ey, int ez, dim3* grid, dim3* block, int* zper)
     *zper = zp;
 }
 
-// grid of the z-marching operator pass (k_nod_march, 32 x 8 node tiles, two blocks per SM): the chunk count that
-// minimises waves x (planes per chunk + the planes a chunk loads directly), chunks of at least 16 planes, and at most
-// kMaxParts blocks (one partial maximum each)
-dim3 nod_march_grid(const maestro_mac_handle* H, const NodLevel& L, int* zchunk)
+// plan of the z-marching operator pass (k_nod_march, 32 x 8 node tiles, two blocks per SM): whole waves of tiles march
+// every plane, the tiles of the last partial wave are cut into z-chunks (of at least 16 planes); the combination that
+// minimises rounds x (planes per chunk + the planes a chunk loads directly); at most kMaxParts blocks
+NodPlan nod_march_plan(const maestro_mac_handle* H, const NodLevel& L)
 {
-    const int tx = (L.nx + 1 + 31) / 32, ty = (L.ny + 1 + 7) / 8, nzn = L.nz + 1;
-    const long slots = 2L * H->sms;
-    const int maxchunk = nzn >= 32 ? nzn / 16 : 1;
+    NodPlan P;
+    P.tiles_x = (L.nx + 1 + 31) / 32;
+    P.tiles = P.tiles_x * ((L.ny + 1 + 7) / 8);
+    const int nzn = L.nz + 1, S = 2 * H->sms, maxchunk = nzn >= 32 ? nzn / 16 : 1;
     long best = -1;
-    int bz = nzn;
-    for (int n = 1; n <= maxchunk; ++n) {
-        const int zc = (nzn + n - 1) / n, nn = (nzn + zc - 1) / zc;
-        if ((long)tx * ty * nn > kMaxParts) break;
-        const long cost = (((long)tx * ty * nn + slots - 1) / slots) * (zc + 4);
-        if (best < 0 || cost < best) { best = cost; bz = zc; }
+    P.nfull = 0; P.nsplit = 1;
+    for (int full = 0; full <= (P.tiles / S) * S; full += S) {
+        const int rem = P.tiles - full;
+        for (int n = 1; n <= maxchunk; ++n) {
+            const int zc = (nzn + n - 1) / n, nn = (nzn + zc - 1) / zc;
+            if ((long)full + (long)rem * nn > kMaxParts) break;
+            const long cost = (long)(full / S) * (nzn + 4) + (((long)rem * nn + S - 1) / S) * (zc + 4);
+            if (best < 0 || cost < best) { best = cost; P.nfull = full; P.nsplit = rem > 0 ? nn : 1; }
+            if (rem == 0) break;
+        }
     }
-    *zchunk = bz;
-    return dim3(tx, ty, (nzn + bz - 1) / bz);
+    P.zchunk = (nzn + P.nsplit - 1) / P.nsplit;
+    P.ncta = P.nfull + (P.tiles - P.nfull) * P.nsplit;
+    return P;
 }
 
 // folds nb block partials into scal[off] (sum) and scal[off + 1] (max)
@@ -157,15 +163,15 @@ int nod_do_rhs(maestro_mac_handle* H, const double* u, const double* v, const do
 int nod_do_jacobi(maestro_mac_handle* H, int l, cudaStream_t s, int* norm_parts = nullptr, bool swap = true)
 {
     const NodLevel L = dev_nod(H, l);
-    int zchunk;
-    const dim3 g = nod_march_grid(H, L, &zchunk);
+    const NodPlan plan = nod_march_plan(H, L);
+    const dim3 g(plan.ncta, 1, 1);
     const NodHost& N = H->nod[l];
     const CUtensorMap& tin = N.phi == N.phi_a ? N.tm_phi : N.tm_phi2;
     if (norm_parts) {
-        *norm_parts = (int)(g.x * g.y * g.z);
-        k_nod_march<NOD_JACOBI | NOD_NORM><<<g, dim3(32, 8), 0, s>>>(tin, N.tm_sig, N.tm_rhs, L, L.phi, L.phi2, H->part_max, zchunk);
+        *norm_parts = plan.ncta;
+        k_nod_march<NOD_JACOBI | NOD_NORM><<<g, dim3(32, 8), 0, s>>>(tin, N.tm_sig, N.tm_rhs, L, L.phi, L.phi2, H->part_max, plan);
     } else
-        k_nod_march<NOD_JACOBI><<<g, dim3(32, 8), 0, s>>>(tin, N.tm_sig, N.tm_rhs, L, L.phi, L.phi2, nullptr, zchunk);
+        k_nod_march<NOD_JACOBI><<<g, dim3(32, 8), 0, s>>>(tin, N.tm_sig, N.tm_rhs, L, L.phi, L.phi2, nullptr, plan);
     LAUNCHED(H);
     if (swap) { double* t = H->nod[l].phi; H->nod[l].phi = H->nod[l].phi2; H->nod[l].phi2 = t; }
     return MAESTRO_MAC_OK;
@@ -185,10 +191,9 @@ int nod_do_residual_restrict(maestro_mac_handle* H, int l, cudaStream_t s)
 {
     const NodLevel F = dev_nod(H, l), C = dev_nod(H, l + 1);
     dim3 g, b;
-    int zchunk;
-    g = nod_march_grid(H, F, &zchunk);
+    const NodPlan plan = nod_march_plan(H, F);
     const NodHost& N = H->nod[l];
-    k_nod_march<NOD_RESID><<<g, dim3(32, 8), 0, s>>>(N.phi == N.phi_a ? N.tm_phi : N.tm_phi2, N.tm_sig, N.tm_rhs, F, F.phi, F.phi2, nullptr, zchunk);
+    k_nod_march<NOD_RESID><<<dim3(plan.ncta, 1, 1), dim3(32, 8), 0, s>>>(N.phi == N.phi_a ? N.tm_phi : N.tm_phi2, N.tm_sig, N.tm_rhs, F, F.phi, F.phi2, nullptr, plan);
     LAUNCHED(H);
     nod_dims(C.nx + 1, C.ny + 1, C.nz + 1, &g, &b);
     k_nod_restrict<<<g, b, 0, s>>>(F, C, F.phi2);
@@ -238,13 +243,12 @@ int nod_do_vcycle(maestro_mac_handle* H, cudaStream_t s, int pre_done = 0)
 int nod_do_residual_norm(maestro_mac_handle* H, int l, cudaStream_t s)
 {
     const NodLevel L = dev_nod(H, l);
-    int zchunk;
-    const dim3 g = nod_march_grid(H, L, &zchunk);
+    const NodPlan plan = nod_march_plan(H, L);
     const NodHost& N = H->nod[l];
-    k_nod_march<NOD_RESID | NOD_NORM><<<g, dim3(32, 8), 0, s>>>(N.phi == N.phi_a ? N.tm_phi : N.tm_phi2, N.tm_sig, N.tm_rhs, L, L.phi, nullptr,
-                                                                H->part_max, zchunk);
+    k_nod_march<NOD_RESID | NOD_NORM><<<dim3(plan.ncta, 1, 1), dim3(32, 8), 0, s>>>(N.phi == N.phi_a ? N.tm_phi : N.tm_phi2, N.tm_sig, N.tm_rhs, L,
+                                                                                    L.phi, nullptr, H->part_max, plan);
     LAUNCHED(H);
-    return nod_fold(H, (int)(g.x * g.y * g.z), 3, s);
+    return nod_fold(H, plan.ncta, 3, s);
 }
 
 int nod_do_correct(maestro_mac_handle* H, const double* phi, const double* rho0, const double* rho, double* u, double* v,
