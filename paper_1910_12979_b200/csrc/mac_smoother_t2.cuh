@@ -474,7 +474,7 @@ static inline t2::T2Plan t2_plan(const LevelDev& L, int sms)
     t2::T2Plan P;
     P.tiles_x = (L.nx + 1 + t2::kTX - 1) / t2::kTX;                   // tile t finishes columns [26 t - 1, 26 t + 25)
     P.tiles = P.tiles_x * ((L.ny + t2::kTY - 1) / t2::kTY);
-    const int S = sms, maxchunk = L.nz >= 32 ? L.nz / 16 : 1;
+    const int S = sms, maxchunk = L.nz >= 8 ? L.nz / 4 : 1;                 // chunks of at least 4 planes
     // cost in marching steps of the slowest SM: rounds x (planes per chunk + the 6 redone planes + pipeline fill)
     long best = -1;
     P.nfull = 0; P.nsplit = 1;

@@ -52,7 +52,7 @@ NodPlan nod_march_plan(const maestro_mac_handle* H, const NodLevel& L)
     NodPlan P;
     P.tiles_x = (L.nx + 1 + 31) / 32;
     P.tiles = P.tiles_x * ((L.ny + 1 + 7) / 8);
-    const int nzn = L.nz + 1, S = 2 * H->sms, maxchunk = nzn >= 32 ? nzn / 16 : 1;
+    const int nzn = L.nz + 1, S = 2 * H->sms, maxchunk = nzn >= 16 ? nzn / 8 : 1;
     long best = -1;
     P.nfull = 0; P.nsplit = 1;
     for (int full = 0; full <= (P.tiles / S) * S; full += S) {
