@@ -297,7 +297,7 @@ static inline int tma_smoother_configure()
 static inline void tma_pick_chunks(int tiles, int nz, int slots, int* nchunk_out, int* zchunk_out)
 {
     long best = -1; int bn = 1;
-    const int maxchunk = nz >= 32 ? nz / 16 : 1;
+    const int maxchunk = nz >= 16 ? nz / 8 : 1;
     for (int n = 1; n <= maxchunk; ++n) {
         const int zc = (nz + n - 1) / n;
         const int nn = (nz + zc - 1) / zc;
