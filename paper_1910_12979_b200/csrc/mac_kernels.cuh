@@ -134,8 +134,8 @@ __device__ __forceinline__ void block_reduce_store(double s, double m, double* _
 // out[0] = sum of part_sum, out[1] = nanmax of part_max
 __global__ void __launch_bounds__(1024)
 k_reduce_final(const double* __restrict__ part_sum, const double* __restrict__ part_max, int n,
-               double* __restrict__ out)
-{
+               double* __restrict__ out, double* __restrict__ host_out = nullptr)
+{   // host_out: mapped pinned memory that receives the two values as well (what the host reads after its synchronise)
     double s = 0.0, m = 0.0;
     for (int q = threadIdx.x; q < n; q += blockDim.x) { s += part_sum[q]; m = nanmax(m, part_max[q]); }
     __shared__ double sh_s[32], sh_m[32];
@@ -148,7 +148,10 @@ k_reduce_final(const double* __restrict__ part_sum, const double* __restrict__ p
         m = sh_m[threadIdx.x];
         s = warp_sum(s);
         m = warp_nanmax(m);
-        if (threadIdx.x == 0) { out[0] = s; out[1] = m; }
+        if (threadIdx.x == 0) {
+            out[0] = s; out[1] = m;
+            if (host_out) { host_out[0] = s; host_out[1] = m; __threadfence_system(); }
+        }
     }
 }
 

@@ -1055,10 +1055,12 @@ extern "C" int maestro_mac_project(maestro_mac_handle* H, const double* beta0, c
                 if (spec) {
                     int nparts = 0;
                     if ((rc = ride2 ? do_sweep2(H, 0, s, &nparts, false) : do_sweep(H, 0, s, &nparts, false)) != 0) return rc;
-                    k_reduce_final<<<1, 1024, 0, s>>>(H->part_sum, H->part_max, nparts, H->scal + 3);
+                    k_reduce_final<<<1, 1024, 0, s>>>(H->part_sum, H->part_max, nparts, H->scal + 3, H->host_scal_dev + 3);   // (published too)
                     LAUNCHED(H);
-                } else if ((rc = do_residual_norm(H, 0, s)) != 0) return rc;
-                if (publish_scal(H, 4, 1, s) != 0) return MAESTRO_MAC_ERR_CUDA;
+                } else {
+                    if ((rc = do_residual_norm(H, 0, s)) != 0) return rc;
+                    if (publish_scal(H, 4, 1, s) != 0) return MAESTRO_MAC_ERR_CUDA;
+                }
                 CUDA_OK(cudaStreamSynchronize(s));
                 st.res_norm_inf = H->host_scal[4];
                 const double rel = st.res_norm_inf / st.rhs_norm_inf;
