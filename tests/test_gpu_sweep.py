@@ -53,3 +53,30 @@ def test_sizes_and_boundary_sets(oracle, mac, k, case):
     assert got["stats"]["cycles"] == ref["stats"]["cycles"]
     for key in ("phi", "u", "v", "w"):
         assert rel_l2(got[key], ref[key]) <= E2E_TOL, key
+
+
+NODAL_SIZES = [(40, 24, 56), (72, 72, 72), (64, 32, 16), (128, 64, 32), (160, 32, 32), (24, 40, 8)]
+NODAL_CASES = list(enumerate(itertools.product(NODAL_SIZES, BCS)))
+
+
+@pytest.mark.parametrize("k,case", NODAL_CASES, ids=[f"nodal-{n[0]}x{n[1]}x{n[2]}-bc{q % len(BCS)}" for q, (n, _) in NODAL_CASES])
+def test_nodal_sizes_and_boundary_sets(oracle, mac, k, case):
+    """The same grid for the end-of-step nodal projection (mixed whole-column / z-chunk plans of k_nod_march on ragged
+    node counts n + 1)."""
+    import test_gpu_nodal as TN
+    from oracle import nodal_oracle
+    nodal_oracle.lib()
+    n, (lo, hi) = case
+    wl = W.mixed_bc_case(n=n, bc_lo=lo, bc_hi=hi, seed=300 + k, geometry=W.SPHERICAL if k % 2 else W.PLANAR)
+    h = 1.0 / max(n)
+    wl.dx = (h, h, h)
+    if wl.geometry == W.PLANAR:
+        wl.dr = h
+    ref = TN.oracle_project(nodal_oracle, wl)
+    got = TN.gpu_project(mac, wl)
+    if got["stats"]["cycles"] != ref["stats"]["cycles"]:
+        got = TN.gpu_project(mac, wl, rel_tol=0.0, max_cycles=ref["stats"]["cycles"])
+    assert got["status"] == ref["status"] == 0
+    assert got["stats"]["cycles"] == ref["stats"]["cycles"]
+    for key in ("phi", "u", "v", "w"):
+        assert rel_l2(got[key], ref[key]) <= E2E_TOL, key
