@@ -244,6 +244,22 @@ int maestro_mac_base_state(int nr, const double *rho0, const double *p0, const d
 int maestro_mac_lateral_average(maestro_mac_handle *h, const double *rho, double *rho0, void *cuda_stream);
 
 /*
+ * maestro_mac_lateral_average_noalloc: the same lateral average for callers that cannot allocate device
+ * memory (code under CUDA graph capture, tight serving loops, harnesses that forbid cudaMalloc): no handle, no
+ * workspace, no cudaMalloc / cudaFree or allocating library call.  `desc` supplies nx, ny, nz, dx, geometry, nr, dr,
+ * center (validated like maestro_mac_setup's; the solver fields are ignored); rho: device [nx*ny*nz]; rho0: device
+ * [nr], out; both caller-owned.  The scratch (per-block partial sums and counts) is a static device array inside the
+ * library, sized for nr <= MAESTRO_MAC_NOALLOC_MAX_NR (3.77 MiB, held by every GPU that loads the library until the
+ * process exits); a larger nr returns ERR_UNSUPPORTED and launches nothing.  Same kernels and launch shape as
+ * maestro_mac_lateral_average: bit-identical results.  Asynchronous on `cuda_stream`.  All calls share the scratch:
+ * calls that overlap on the GPU (other streams, unordered host threads) race -- serialise them.  The first call on a
+ * device looks up the array's address (cudaGetSymbolAddress) and opts the kernel into its shared-memory size; make
+ * that call outside a capture.  Returns OK, ERR_ARG, ERR_UNSUPPORTED, ERR_CUDA.
+ */
+#define MAESTRO_MAC_NOALLOC_MAX_NR 2048
+int maestro_mac_lateral_average_noalloc(const maestro_mac_desc *desc, const double *rho, double *rho0, void *cuda_stream);
+
+/*
  * maestro_mac_set_dpdt_term: register the profile q = (1/(Gamma1bar p0)) dp0/dt (device, [nr], caller-owned,
  * alive and unchanged during every later project call) or NULL to clear it.  With it the right-hand side is the
  * full constraint of PAPER.md:49 Eq. 6,  rhs = D(beta0 U_edge) - beta0 (S - q(r)),  q evaluated at cell centres

@@ -10,6 +10,7 @@
 #include <cmath>
 #include <cstdlib>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include <vector>
 
@@ -1426,3 +1427,4 @@ extern "C" int maestro_mac_level_plan(const maestro_mac_handle* H, int level, in
 }
 
 #include "maestro_nodal.inl"
+#include "maestro_noalloc.inl"

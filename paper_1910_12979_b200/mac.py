@@ -26,6 +26,7 @@ EXPORTS = [
     "maestro_mac_step_residual_restrict", "maestro_mac_step_prolong", "maestro_mac_step_bottom",
     "maestro_mac_step_vcycle", "maestro_mac_step_residual_norm", "maestro_mac_step_correct",
     "maestro_mac_base_state", "maestro_mac_set_dpdt_term", "maestro_mac_lateral_average",
+    "maestro_mac_lateral_average_noalloc",
     "maestro_mac_status", "maestro_mac_level_plan",
     "maestro_mac_nodal_project", "maestro_mac_nodal_level_get", "maestro_mac_nodal_level_set",
     "maestro_mac_nodal_step_sigma", "maestro_mac_nodal_step_rhs", "maestro_mac_nodal_step_smooth",
@@ -103,6 +104,7 @@ def lib():
         L.maestro_mac_base_state.argtypes = [C.c_int, _VP, _VP, _VP, _VP, _VP, _VP, _VP]
         L.maestro_mac_set_dpdt_term.argtypes = [_VP, _VP]
         L.maestro_mac_lateral_average.argtypes = [_VP, _VP, _VP, _VP]
+        L.maestro_mac_lateral_average_noalloc.argtypes = [C.POINTER(Desc), _VP, _VP, _VP]
         L.maestro_mac_status.argtypes = [_VP, C.POINTER(Stats), _VP]
         L.maestro_mac_level_plan.argtypes = [_VP, C.c_int, C.POINTER(C.c_int * 8)]
         L.maestro_mac_nodal_project.argtypes = proj
@@ -158,6 +160,15 @@ def desc_from_workload(wl, **over) -> Desc:
               max_cycles=wl.max_cycles, rel_tol=wl.rel_tol, rho_mean=wl.meta.get("rho_mean", 0))
     kw.update(over)
     return make_desc(**kw)
+
+
+NOALLOC_MAX_NR = 2048          # MAESTRO_MAC_NOALLOC_MAX_NR
+
+
+def lateral_average_noalloc(desc: Desc, rho, out):
+    """rho0 = lateral average of rho into the caller's tensor `out` [nr] (maestro_mac_lateral_average_noalloc: no handle,
+    no workspace, no device allocation; scratch is a static device array for nr <= NOALLOC_MAX_NR).  Returns the status."""
+    return lib().maestro_mac_lateral_average_noalloc(C.byref(desc), _ptr(rho), _ptr(out), _stream())
 
 
 def workspace_bytes(desc: Desc) -> int:
