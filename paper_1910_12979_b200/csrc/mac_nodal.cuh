@@ -654,6 +654,114 @@ __device__ __forceinline__ NodBottomIdx nod_bottom_idx(const NodLevel& L, int c)
     return B;
 }
 
+// The usual bottom (5^3 = 125 nodes): ONE node per thread.  The thread keeps its row of the operator in registers -- the
+// 27 products -w[class] T(dx,dy,dz) and the storage indices of the 27 neighbours (coefficient 0 and its own index where
+// there is no such node or it is an OUTFLOW node) -- and every vector entry as a scalar; a matrix-vector product is 27
+// shared-memory reads of the operand, not the index arithmetic and sigma loads of nod_operator_generic.  Same
+// algorithm, stopping rule and exits as k_nod_bottom.  Needs nb <= 128 and a node layout of at most kNodSmallMax entries.
+constexpr int kNodSmallMax = 1024;
+
+__global__ void __launch_bounds__(128)
+k_nod_bottom_small(NodLevel L, int maxit, double tol, int singular, int* __restrict__ iters_accum)
+{
+    __shared__ double sh[64];
+    __shared__ double opd[kNodSmallMax];               // the operand of a product, in the level's node layout
+    const int nb = (L.nx + 1) * (L.ny + 1) * (L.nz + 1), nt = blockDim.x, tid = threadIdx.x;
+    const bool has = tid < nb;
+    const NodBottomIdx B = nod_bottom_idx(L, has ? tid : 0);
+    const bool active = has && B.active;
+    const int q = (int)B.q;
+    double cf[27];
+    int ix[27];
+#pragma unroll
+    for (int n = 0; n < 27; ++n) { cf[n] = 0.0; ix[n] = q; }
+    if (active) {
+        const NodAxis X = nod_axis(L, 0, B.i), Y = nod_axis(L, 1, B.j), Z = nod_axis(L, 2, B.k);
+        double sg[2][2][2];
+#pragma unroll
+        for (int c = 0; c < 2; ++c)
+#pragma unroll
+            for (int b = 0; b < 2; ++b)
+#pragma unroll
+                for (int a = 0; a < 2; ++a) {
+                    const bool ok = X.cl[a] >= 0 && Y.cl[b] >= 0 && Z.cl[c] >= 0;
+                    sg[c][b][a] = ok ? __ldg(L.sigma + nod_cidx(L, X.cl[a], Y.cl[b], Z.cl[c])) : 0.0;
+                }
+#pragma unroll
+        for (int c = 0; c < 3; ++c)
+#pragma unroll
+            for (int b = 0; b < 3; ++b)
+#pragma unroll
+                for (int a = 0; a < 3; ++a) {
+                    // T: sigma summed over the cells that contain the node and this neighbour (offset 0: both cells of the axis)
+                    double t = 0.0;
+#pragma unroll
+                    for (int cc = 0; cc < 2; ++cc)
+#pragma unroll
+                        for (int bb = 0; bb < 2; ++bb)
+#pragma unroll
+                            for (int aa = 0; aa < 2; ++aa) {
+                                const bool in = (a == 1 || aa == (a >> 1)) && (b == 1 || bb == (b >> 1)) && (c == 1 || cc == (c >> 1));
+                                if (in) t += sg[cc][bb][aa];
+                            }
+                    const int cls = (a != 1 ? 1 : 0) | (b != 1 ? 2 : 0) | (c != 1 ? 4 : 0);
+                    const bool ok = X.nd[a] >= 0 && Y.nd[b] >= 0 && Z.nd[c] >= 0;
+                    const int n = a + 3 * (b + 3 * c);
+                    if (ok) { cf[n] = -L.w[cls] * t; ix[n] = (int)nod_idx(L, X.nd[a], Y.nd[b], Z.nd[c]); }
+                }
+    }
+    auto matvec = [&](double y) -> double {            // (the operand entries of OUTFLOW nodes and duplicates are 0 by construction)
+        group_sync(nt);
+        if (has) opd[q] = y;
+        group_sync(nt);
+        double acc = 0.0;
+#pragma unroll
+        for (int n = 0; n < 27; ++n) acc = fma(cf[n], opd[ix[n]], acc);
+        return active ? acc : 0.0;
+    };
+    const double f = active ? L.rhs[q] : 0.0;
+    const Dot2 q0 = block_dot2(active ? 1.0 : 0.0, f, sh, nt);
+    const double nunk = q0.a, fm = singular ? q0.b / q0.a : 0.0;
+    double x = 0.0, r = active ? f - fm : 0.0, rhat = r, pv = 0.0, v = 0.0, sv = 0.0, tv = 0.0;
+    double rr = block_dot2(r * r, 0.0, sh, nt).a;
+    const double bnorm2 = rr;
+    int it = 0;
+    if (bnorm2 > 0.0 && bnorm2 == bnorm2) {
+        const double stop2 = tol * tol * bnorm2;
+        double rho = rr, rho_old = 1.0, alpha = 1.0, omega = 1.0;
+        while (it < maxit && rr > stop2) {
+            if (rho == 0.0) break;
+            const double beta = it == 0 ? 0.0 : (rho / rho_old) * (alpha / omega);
+            pv = r + beta * (pv - omega * v);
+            v = matvec(pv);
+            const double d = block_dot2(rhat * v, 0.0, sh, nt).a;
+            if (d == 0.0) break;
+            alpha = rho / d;
+            sv = r - alpha * v;
+            const double ss = block_dot2(sv * sv, 0.0, sh, nt).a;
+            ++it;
+            if (ss <= stop2) { x += alpha * pv; rr = ss; break; }
+            tv = matvec(sv);
+            Dot2 qd = block_dot2(tv * sv, tv * tv, sh, nt);
+            if (qd.b == 0.0) { x += alpha * pv; break; }
+            omega = qd.a / qd.b;
+            x += alpha * pv + omega * sv;
+            r = sv - omega * tv;
+            qd = block_dot2(r * r, rhat * r, sh, nt);
+            rr = qd.a;
+            rho_old = rho;
+            rho = qd.b;
+            if (omega == 0.0) break;
+        }
+    }
+    if (singular) {                                    // zero plain mean over the unknowns (N8)
+        const double xm = block_dot2(active ? x : 0.0, 0.0, sh, nt).a / nunk;
+        if (active) x -= xm;
+    }
+    if (has) L.phi[q] = active ? x : 0.0;
+    if (tid == 0 && iters_accum) *iters_accum += it;
+}
+
 __global__ void __launch_bounds__(1024)
 k_nod_bottom(NodLevel L, double* __restrict__ vec0, long long vstride, int maxit, double tol, int singular,
              int* __restrict__ iters_accum)

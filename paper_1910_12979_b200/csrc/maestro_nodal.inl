@@ -217,6 +217,11 @@ int nod_do_bottom(maestro_mac_handle* H, cudaStream_t s)
     const int l = H->nlev - 1;
     const int nb = (int)H->nod[l].nnode;
     const int threads = nb >= 1024 ? 1024 : ((nb + 31) / 32) * 32;
+    if (nb <= 128 && H->nod[l].anode <= (size_t)kNodSmallMax) {      // one node per thread, its operator row in registers
+        k_nod_bottom_small<<<1, threads, 0, s>>>(dev_nod(H, l), H->d.bottom_max_iter, H->d.bottom_rel_tol, H->singular, H->flags + 1);
+        LAUNCHED(H);
+        return MAESTRO_MAC_OK;
+    }
     k_nod_bottom<<<1, threads, 0, s>>>(dev_nod(H, l), H->nod_vecs + H->nod[l].onode, (long long)H->nod[l].anode, H->d.bottom_max_iter,
                                       H->d.bottom_rel_tol, H->singular, H->flags + 1);
     LAUNCHED(H);
