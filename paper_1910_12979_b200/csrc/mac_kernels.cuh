@@ -225,6 +225,20 @@ k_shift_mean(LevelDev L, double* __restrict__ a, const double* __restrict__ scal
     block_reduce_store(s, m, part_sum, part_max, blockIdx.x);
 }
 
+// pub = a - scal[0]/count: the mean removal of k_shift_mean written straight into the caller's array (public cell
+// layout idx = i + nx (j + ny k)) instead of in place -- the zero-mean phi the call returns, in one pass
+__global__ void __launch_bounds__(256)
+k_shift_mean_out(LevelDev L, const double* __restrict__ a, const double* __restrict__ scal, double inv_count, double* __restrict__ pub)
+{
+    const double c = scal[0] * inv_count;
+    const int nrows = L.ny * L.nz;
+    for (int row = blockIdx.x; row < nrows; row += gridDim.x) {
+        const double* __restrict__ p = a + cidx(L, 0, row % L.ny, row / L.ny);
+        double* __restrict__ o = pub + (size_t)L.nx * row;
+        for (int i = threadIdx.x; i < L.nx; i += blockDim.x) o[i] = p[i] - c;
+    }
+}
+
 __global__ void __launch_bounds__(256)
 k_sum(LevelDev L, const double* __restrict__ a, double* __restrict__ part_sum, double* __restrict__ part_max)
 {

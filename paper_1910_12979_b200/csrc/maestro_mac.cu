@@ -1080,19 +1080,20 @@ extern "C" int maestro_mac_project(maestro_mac_handle* H, const double* beta0, c
         }
     }
     CUDA_OK(cudaEventRecord(H->ev[2], s));
-    if (!trivial && result != MAESTRO_MAC_ERR_NONFINITE) {
-        if (H->singular) {   // A10: zero-mean phi
+    // A10: the phi a singular problem returns has zero mean.  The correction takes differences of phi only (a singular
+    // problem has no OUTFLOW face), so it runs on the iterate as it stands and the mean is removed while phi is written
+    // to the caller's array -- one pass instead of an in-place shift plus a copy, and none at all when phi == NULL.
+    const bool solved = !trivial && result != MAESTRO_MAC_ERR_NONFINITE;
+    if (solved && (rc = do_correct(H, H->lev[0].phi, rho0, rho, u, v, w, s)) != 0) return rc;
+    if (phi) {
+        if (solved && H->singular) {
             k_sum<<<H->red_blocks, 256, 0, s>>>(dev_level(H, 0), H->lev[0].phi, H->part_sum, H->part_max);
             LAUNCHED(H);
             k_reduce_final<<<1, 1024, 0, s>>>(H->part_sum, H->part_max, H->red_blocks, H->scal + 6);
             LAUNCHED(H);
-            k_shift_mean<<<H->red_blocks, 256, 0, s>>>(dev_level(H, 0), H->lev[0].phi, H->scal + 6, 1.0 / (double)L0.ncell, H->part_sum, H->part_max);
+            k_shift_mean_out<<<H->red_blocks, 256, 0, s>>>(dev_level(H, 0), H->lev[0].phi, H->scal + 6, 1.0 / (double)L0.ncell, phi);
             LAUNCHED(H);
-        }
-        if ((rc = do_correct(H, H->lev[0].phi, rho0, rho, u, v, w, s)) != 0) return rc;
-    }
-    if (phi) {
-        if (L0.gx == 0 && L0.gy == 0) {
+        } else if (L0.gx == 0 && L0.gy == 0) {
             CUDA_OK(cudaMemcpyAsync(phi, L0.phi, L0.ncell * sizeof(double), cudaMemcpyDeviceToDevice, s));
         } else {
             dim3 g, b;
