@@ -526,7 +526,23 @@ k_nod_restrict(NodLevel F, NodLevel C, const double* __restrict__ res)
     const int I = blockIdx.x * blockDim.x + threadIdx.x, J = blockIdx.y * blockDim.y + threadIdx.y, K = blockIdx.z;
     if (I > C.nx || J > C.ny) return;
     double s = 0.0;
-    if (nod_kind(C, I, J, K) == 0) {
+    if (I >= 1 && I < C.nx && J >= 1 && J < C.ny && K >= 1 && K < C.nz) {
+        // interior coarse node (an unknown whatever the boundary types): its 27 fine nodes 2T - 1 .. 2T + 1 exist and need
+        // no wrap -- constant offsets from one base pointer, the same terms in the same order as the general path below
+        const double* __restrict__ p = res + nod_idx(F, 2 * I, 2 * J, 2 * K);
+        const long long sy = F.NX, sz = sy * F.NY;
+#pragma unroll
+        for (int c = -1; c <= 1; ++c)
+#pragma unroll
+            for (int b = -1; b <= 1; ++b) {
+                const double* __restrict__ r = p + b * sy + c * sz;
+                const double wr = (b != 0 ? 0.5 : 1.0) * (c != 0 ? 0.5 : 1.0);
+                s += (0.5 * wr) * r[-1];
+                s += wr * r[0];
+                s += (0.5 * wr) * r[1];
+            }
+        s *= 0.125;
+    } else if (nod_kind(C, I, J, K) == 0) {
         int fi[3], fj[3], fk[3];
 #pragma unroll
         for (int o = 0; o < 3; ++o) {                 // fine node 2 T + (o - 1) per axis, wrapped, or -2
@@ -565,6 +581,37 @@ k_nod_prolong_add2(NodLevel F, NodLevel C)
     const int I = blockIdx.x * blockDim.x + threadIdx.x, J = blockIdx.y * blockDim.y + threadIdx.y, K = blockIdx.z;
     if (I > C.nx || J > C.ny) return;
     double e[2][2][2];
+    // interior: the 8 coarse corners have indices in [1, n - 1] (unknowns, no wrap) and the 8 fine nodes indices in
+    // [2, 2n - 3] (unknowns without periodic images): plain loads and stores, the same sums as the general path
+    const bool fast = I >= 1 && I + 1 < C.nx && J >= 1 && J + 1 < C.ny && K >= 1 && K + 1 < C.nz;
+    if (fast) {
+        const double* __restrict__ ce = C.phi + nod_idx(C, I, J, K);
+        const long long sy = C.NX, sz = sy * C.NY;
+#pragma unroll
+        for (int c = 0; c < 2; ++c)
+#pragma unroll
+            for (int b = 0; b < 2; ++b) { e[c][b][0] = ce[b * sy + c * sz]; e[c][b][1] = ce[1 + b * sy + c * sz]; }
+        double2* const fp = reinterpret_cast<double2*>(F.phi + nod_idx(F, 2 * I, 2 * J, 2 * K));   // node 2I sits at an even entry of its row
+        const long long fy = F.NX / 2, fz = fy * F.NY;
+#pragma unroll
+        for (int c = 0; c < 2; ++c)
+#pragma unroll
+            for (int b = 0; b < 2; ++b) {
+                double s0 = 0.0, s1 = 0.0;
+                for (int cc = 0; cc <= c; ++cc)
+                    for (int bb = 0; bb <= b; ++bb) {
+                        s0 += e[cc][bb][0];
+                        s1 += e[cc][bb][0];
+                        s1 += e[cc][bb][1];
+                    }
+                const double wt = (b ? 0.5 : 1.0) * (c ? 0.5 : 1.0);
+                double2 v = fp[b * fy + c * fz];
+                v.x += wt * s0;
+                v.y += (0.5 * wt) * s1;
+                fp[b * fy + c * fz] = v;
+            }
+        return;
+    }
 #pragma unroll
     for (int c = 0; c < 2; ++c)
 #pragma unroll
