@@ -129,7 +129,8 @@ __device__ __forceinline__ NodAxis nod_axis(const NodLevel& L, int d, int t)
 
 // L phi at the unknown node (i, j, k) through the node rules, one node at a time: the form that does not rely on
 // ghost entries (bottom solver).
-__device__ __forceinline__ double nod_operator_generic(const NodLevel& L, const double* __restrict__ phi, int i, int j, int k)
+__device__ __forceinline__ double nod_operator_generic(const NodLevel& L, const double* __restrict__ phi, int i, int j, int k,
+                                                      double* tcentre = nullptr)      // tcentre: receives T(0,0,0), the sigma sum of the diagonal
 {
     double p[3][3][3], s[2][2][2];
     const NodAxis X = nod_axis(L, 0, i), Y = nod_axis(L, 1, j), Z = nod_axis(L, 2, k);
@@ -178,6 +179,7 @@ __device__ __forceinline__ double nod_operator_generic(const NodLevel& L, const 
     double sum = 0.0;
 #pragma unroll
     for (int q = 7; q >= 0; --q) sum = fma(L.w[q], acc[q], sum);
+    if (tcentre) *tcentre = t[1][1][1];
     return -sum;
 }
 
@@ -516,6 +518,77 @@ k_nod_march(const __grid_constant__ CUtensorMap tm_phi, const __grid_constant__ 
             part_max[blockIdx.x] = m;
         }
     }
+}
+
+// ---- the same passes with one thread per node, for the levels that are too small for the z-march (its pipeline
+// prologue and a serial march over a handful of blocks cost 12 us on a 17^3 level; this form is launch-bound).
+// Interior nodes (indices in [1, n - 1] on every axis) read their 27 neighbours and 8 cells at constant offsets; the
+// others go through nod_operator_generic (node rules).  L phi = -sum_class w[class] sum_{n in class} T_n phi_n.
+// grid over (nx + 1, ny + 1, nz + 1) nodes; NORM: one partial maximum per block (linear block index).
+template <int MODE>
+__global__ void __launch_bounds__(256)
+k_nod_point(NodLevel L, const double* __restrict__ pin, double* __restrict__ out, double* __restrict__ part_sum,
+            double* __restrict__ part_max)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y * blockDim.y + threadIdx.y, k = blockIdx.z;
+    double rabs = 0.0;
+    if (i <= L.nx && j <= L.ny) {
+        const int kind = nod_kind(L, i, j, k);
+        const long long q = nod_idx(L, i, j, k);
+        if (kind == 0) {
+            double lphi, ndg;
+            if (i >= 1 && i < L.nx && j >= 1 && j < L.ny && k >= 1 && k < L.nz) {
+                const double* __restrict__ p = pin + q;
+                const double* __restrict__ sg = L.sigma + nod_cidx(L, i - 1, j - 1, k - 1);
+                const long long py = L.NX, pz = py * L.NY, cy = L.CX, cz = cy * L.CY;
+                double s8[2][2][2];
+#pragma unroll
+                for (int c = 0; c < 2; ++c)
+#pragma unroll
+                    for (int b = 0; b < 2; ++b) { s8[c][b][0] = __ldg(sg + b * cy + c * cz); s8[c][b][1] = __ldg(sg + 1 + b * cy + c * cz); }
+                double tx[2][2][3], ty[2][3][3], t[3][3][3];
+#pragma unroll
+                for (int c = 0; c < 2; ++c)
+#pragma unroll
+                    for (int b = 0; b < 2; ++b) { tx[c][b][0] = s8[c][b][0]; tx[c][b][1] = s8[c][b][0] + s8[c][b][1]; tx[c][b][2] = s8[c][b][1]; }
+#pragma unroll
+                for (int c = 0; c < 2; ++c)
+#pragma unroll
+                    for (int a = 0; a < 3; ++a) { ty[c][0][a] = tx[c][0][a]; ty[c][1][a] = tx[c][0][a] + tx[c][1][a]; ty[c][2][a] = tx[c][1][a]; }
+#pragma unroll
+                for (int b = 0; b < 3; ++b)
+#pragma unroll
+                    for (int a = 0; a < 3; ++a) { t[0][b][a] = ty[0][b][a]; t[1][b][a] = ty[0][b][a] + ty[1][b][a]; t[2][b][a] = ty[1][b][a]; }
+                double acc[8] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
+#pragma unroll
+                for (int c = 0; c < 3; ++c)
+#pragma unroll
+                    for (int b = 0; b < 3; ++b)
+#pragma unroll
+                        for (int a = 0; a < 3; ++a) {
+                            const int cls = (a != 1 ? 1 : 0) | (b != 1 ? 2 : 0) | (c != 1 ? 4 : 0);
+                            acc[cls] = fma(t[c][b][a], p[(a - 1) + (b - 1) * py + (c - 1) * pz], acc[cls]);
+                        }
+                double sum = 0.0;
+#pragma unroll
+                for (int w = 7; w >= 0; --w) sum = fma(L.w[w], acc[w], sum);
+                lphi = -sum;
+                ndg = L.w[0] * t[1][1][1];
+            } else {
+                double tc;
+                lphi = nod_operator_generic(L, pin, i, j, k, &tc);
+                ndg = L.w[0] * tc;
+            }
+            const double r = L.rhs[q] - lphi;
+            if (MODE & NOD_NORM) rabs = fabs(r);
+            if (MODE & NOD_JACOBI)
+                nod_store_images(L, out, q, pin[q] - fast_div_pos(L.omega * r, ndg), nod_image(L, 0, i), nod_image(L, 1, j), nod_image(L, 2, k));
+            else if (out) out[q] = r;
+        } else if (kind == 1 && out) {
+            out[q] = 0.0;                                                     // OUTFLOW node
+        }
+    }
+    if (MODE & NOD_NORM) block_reduce_store(0.0, rabs, part_sum, part_max, blockIdx.x + gridDim.x * (blockIdx.y + gridDim.y * blockIdx.z));
 }
 
 // ---- N6: coarse rhs = (1/8) P^T res (weights 1, 1/2 per axis over the 27 fine nodes); the coarse phi is zeroed by

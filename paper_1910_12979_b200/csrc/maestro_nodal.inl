@@ -44,6 +44,11 @@ void nod_dims_red(int ex, int ey, int ez, dim3* grid, dim3* block, int* zper)
     *zper = zp;
 }
 
+#ifndef MAC_NOD_POINT_MAX
+#define MAC_NOD_POINT_MAX 40000           // levels of at most this many nodes run the one-thread-per-node passes (k_nod_point)
+#endif
+bool nod_point_level(const maestro_mac_handle* H, int l) { return H->nod[l].nnode <= (size_t)MAC_NOD_POINT_MAX; }
+
 // plan of the z-marching operator pass (k_nod_march, 32 x 8 node tiles, two blocks per SM): whole waves of tiles march
 // every plane, the tiles of the last partial wave are cut into z-chunks (of at least 16 planes); the combination that
 // minimises rounds x (planes per chunk + the planes a chunk loads directly); at most kMaxParts blocks
@@ -163,6 +168,19 @@ int nod_do_rhs(maestro_mac_handle* H, const double* u, const double* v, const do
 int nod_do_jacobi(maestro_mac_handle* H, int l, cudaStream_t s, int* norm_parts = nullptr, bool swap = true)
 {
     const NodLevel L = dev_nod(H, l);
+    if (nod_point_level(H, l)) {
+        dim3 g, b;
+        nod_dims(L.nx + 1, L.ny + 1, L.nz + 1, &g, &b);
+        if (norm_parts) {
+            if ((long)g.x * g.y * g.z > kMaxParts) return MAESTRO_MAC_ERR_UNSUPPORTED;
+            *norm_parts = (int)(g.x * g.y * g.z);
+            k_nod_point<NOD_JACOBI | NOD_NORM><<<g, b, 0, s>>>(L, L.phi, L.phi2, H->part_sum, H->part_max);
+        } else
+            k_nod_point<NOD_JACOBI><<<g, b, 0, s>>>(L, L.phi, L.phi2, nullptr, nullptr);
+        LAUNCHED(H);
+        if (swap) { double* t = H->nod[l].phi; H->nod[l].phi = H->nod[l].phi2; H->nod[l].phi2 = t; }
+        return MAESTRO_MAC_OK;
+    }
     const NodPlan plan = nod_march_plan(H, L);
     const dim3 g(plan.ncta, 1, 1);
     const NodHost& N = H->nod[l];
@@ -191,9 +209,14 @@ int nod_do_residual_restrict(maestro_mac_handle* H, int l, cudaStream_t s)
 {
     const NodLevel F = dev_nod(H, l), C = dev_nod(H, l + 1);
     dim3 g, b;
-    const NodPlan plan = nod_march_plan(H, F);
-    const NodHost& N = H->nod[l];
-    k_nod_march<NOD_RESID><<<dim3(plan.ncta, 1, 1), dim3(32, 8), 0, s>>>(N.phi == N.phi_a ? N.tm_phi : N.tm_phi2, N.tm_sig, N.tm_rhs, F, F.phi, F.phi2, nullptr, plan);
+    if (nod_point_level(H, l)) {
+        nod_dims(F.nx + 1, F.ny + 1, F.nz + 1, &g, &b);
+        k_nod_point<NOD_RESID><<<g, b, 0, s>>>(F, F.phi, F.phi2, nullptr, nullptr);
+    } else {
+        const NodPlan plan = nod_march_plan(H, F);
+        const NodHost& N = H->nod[l];
+        k_nod_march<NOD_RESID><<<dim3(plan.ncta, 1, 1), dim3(32, 8), 0, s>>>(N.phi == N.phi_a ? N.tm_phi : N.tm_phi2, N.tm_sig, N.tm_rhs, F, F.phi, F.phi2, nullptr, plan);
+    }
     LAUNCHED(H);
     nod_dims(C.nx + 1, C.ny + 1, C.nz + 1, &g, &b);
     k_nod_restrict<<<g, b, 0, s>>>(F, C, F.phi2);
@@ -248,6 +271,14 @@ int nod_do_vcycle(maestro_mac_handle* H, cudaStream_t s, int pre_done = 0)
 int nod_do_residual_norm(maestro_mac_handle* H, int l, cudaStream_t s)
 {
     const NodLevel L = dev_nod(H, l);
+    if (nod_point_level(H, l)) {
+        dim3 g, b;
+        nod_dims(L.nx + 1, L.ny + 1, L.nz + 1, &g, &b);
+        if ((long)g.x * g.y * g.z > kMaxParts) return MAESTRO_MAC_ERR_UNSUPPORTED;
+        k_nod_point<NOD_RESID | NOD_NORM><<<g, b, 0, s>>>(L, L.phi, nullptr, H->part_sum, H->part_max);
+        LAUNCHED(H);
+        return nod_fold(H, (int)(g.x * g.y * g.z), 3, s);
+    }
     const NodPlan plan = nod_march_plan(H, L);
     const NodHost& N = H->nod[l];
     k_nod_march<NOD_RESID | NOD_NORM><<<dim3(plan.ncta, 1, 1), dim3(32, 8), 0, s>>>(N.phi == N.phi_a ? N.tm_phi : N.tm_phi2, N.tm_sig, N.tm_rhs, L,
