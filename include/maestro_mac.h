@@ -314,6 +314,13 @@ enum { MAESTRO_MAC_KERNEL_COLOR = 0, MAESTRO_MAC_KERNEL_FUSED = 1, MAESTRO_MAC_K
        MAESTRO_MAC_KERNEL_T2 = 3, MAESTRO_MAC_KERNEL_TAIL = 4, MAESTRO_MAC_KERNEL_BOTTOM = 5,
        MAESTRO_MAC_KERNEL_CLUSTER = 6 };   /* CLUSTER: the level is one of those k_cluster_vcycles walks in one launch */
 int maestro_mac_level_plan(const maestro_mac_handle *h, int level, int info[8]);
+/* The planners behind that, as pure host arithmetic (no handle, no CUDA call; CPU-side tests of the wave / chunk
+ * decomposition): the plan of one launch on a level of nx x ny x nz cells on a device with `sms` multiprocessors.
+ * which = 0: the two-sweep smoother k_rbgs_t2 (tiles of 26 x 18 finished cells, one block per SM at a time);
+ * which = 1: the nodal march k_nod_march ((nx+1)(ny+1)(nz+1) nodes, tiles of 32 x 8 nodes, two blocks per SM).
+ * info[1..5] as in maestro_mac_level_plan (tiles, whole-column tiles, z-chunks per remaining tile, planes per chunk,
+ * blocks); info[0] = tiles along x.  Returns OK or ERR_ARG. */
+int maestro_mac_plan_query(int which, int nx, int ny, int nz, int sms, int info[8]);
 /* n[3] cells and h[3] spacing of a level */
 int maestro_mac_level_dims(const maestro_mac_handle *h, int level, int n[3], double hh[3]);
 /* Copy a level array to / from a caller DEVICE buffer in the public layout (cells, or the face

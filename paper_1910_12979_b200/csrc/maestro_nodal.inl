@@ -52,12 +52,14 @@ bool nod_point_level(const maestro_mac_handle* H, int l) { return H->nod[l].nnod
 // plan of the z-marching operator pass (k_nod_march, 32 x 8 node tiles, two blocks per SM): whole waves of tiles march
 // every plane, the tiles of the last partial wave are cut into z-chunks (of at least 16 planes); the combination that
 // minimises rounds x (planes per chunk + the planes a chunk loads directly); at most kMaxParts blocks
-NodPlan nod_march_plan(const maestro_mac_handle* H, const NodLevel& L)
+NodPlan nod_march_plan_sms(int sms, const NodLevel& L);
+NodPlan nod_march_plan(const maestro_mac_handle* H, const NodLevel& L) { return nod_march_plan_sms(H->sms, L); }
+NodPlan nod_march_plan_sms(int sms, const NodLevel& L)
 {
     NodPlan P;
     P.tiles_x = (L.nx + 1 + 31) / 32;
     P.tiles = P.tiles_x * ((L.ny + 1 + 7) / 8);
-    const int nzn = L.nz + 1, S = 2 * H->sms, maxchunk = nzn >= 16 ? nzn / 8 : 1;
+    const int nzn = L.nz + 1, S = 2 * sms, maxchunk = nzn >= 16 ? nzn / 8 : 1;
     long best = -1;
     P.nfull = 0; P.nsplit = 1;
     for (int full = 0; full <= (P.tiles / S) * S; full += S) {
@@ -507,4 +509,24 @@ extern "C" int maestro_mac_nodal_step_correct(maestro_mac_handle* H, const doubl
 {
     if (!H || !H->has_nodal || !uc || !vc || !wc || (!rho && !rho0)) return MAESTRO_MAC_ERR_ARG;
     return nod_do_correct(H, H->nod[0].phi, rho0, rho, uc, vc, wc, (cudaStream_t)cuda_stream);
+}
+
+extern "C" int maestro_mac_plan_query(int which, int nx, int ny, int nz, int sms, int info[8])
+{
+    if (!info || nx < 1 || ny < 1 || nz < 1 || sms < 1 || (which != 0 && which != 1)) return MAESTRO_MAC_ERR_ARG;
+    for (int q = 0; q < 8; ++q) info[q] = 0;
+    if (which == 0) {
+        LevelDev L;
+        std::memset(&L, 0, sizeof(L));
+        L.nx = nx; L.ny = ny; L.nz = nz;
+        const t2::T2Plan P = t2_plan(L, sms);
+        info[0] = P.tiles_x; info[1] = P.tiles; info[2] = P.nfull; info[3] = P.nsplit; info[4] = P.zchunk; info[5] = P.ncta;
+    } else {
+        NodLevel L;
+        std::memset(&L, 0, sizeof(L));
+        L.nx = nx; L.ny = ny; L.nz = nz;
+        const NodPlan P = nod_march_plan_sms(sms, L);
+        info[0] = P.tiles_x; info[1] = P.tiles; info[2] = P.nfull; info[3] = P.nsplit; info[4] = P.zchunk; info[5] = P.ncta;
+    }
+    return MAESTRO_MAC_OK;
 }

@@ -27,7 +27,7 @@ EXPORTS = [
     "maestro_mac_step_vcycle", "maestro_mac_step_residual_norm", "maestro_mac_step_correct",
     "maestro_mac_base_state", "maestro_mac_set_dpdt_term", "maestro_mac_lateral_average",
     "maestro_mac_lateral_average_noalloc",
-    "maestro_mac_status", "maestro_mac_level_plan",
+    "maestro_mac_status", "maestro_mac_level_plan", "maestro_mac_plan_query",
     "maestro_mac_nodal_project", "maestro_mac_nodal_level_get", "maestro_mac_nodal_level_set",
     "maestro_mac_nodal_step_sigma", "maestro_mac_nodal_step_rhs", "maestro_mac_nodal_step_smooth",
     "maestro_mac_nodal_step_residual_restrict", "maestro_mac_nodal_step_prolong", "maestro_mac_nodal_step_bottom",
@@ -107,6 +107,7 @@ def lib():
         L.maestro_mac_lateral_average_noalloc.argtypes = [C.POINTER(Desc), _VP, _VP, _VP]
         L.maestro_mac_status.argtypes = [_VP, C.POINTER(Stats), _VP]
         L.maestro_mac_level_plan.argtypes = [_VP, C.c_int, C.POINTER(C.c_int * 8)]
+        L.maestro_mac_plan_query.argtypes = [C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, C.POINTER(C.c_int * 8)]
         L.maestro_mac_nodal_project.argtypes = proj
         L.maestro_mac_nodal_level_get.argtypes = [_VP, C.c_int, C.c_int, _VP, _VP]
         L.maestro_mac_nodal_level_set.argtypes = [_VP, C.c_int, C.c_int, _VP, _VP]
@@ -160,6 +161,15 @@ def desc_from_workload(wl, **over) -> Desc:
               max_cycles=wl.max_cycles, rel_tol=wl.rel_tol, rho_mean=wl.meta.get("rho_mean", 0))
     kw.update(over)
     return make_desc(**kw)
+
+
+def plan_query(which, nx, ny, nz, sms):
+    """Launch plan of the two-sweep smoother (which = 0) or the nodal march (1) as pure host arithmetic (no GPU needed)."""
+    info = (C.c_int * 8)()
+    rc = lib().maestro_mac_plan_query(which, nx, ny, nz, sms, C.byref(info))
+    if rc != OK:
+        raise MacError(rc, "plan_query")
+    return dict(tiles_x=info[0], tiles=info[1], nfull=info[2], nsplit=info[3], zchunk=info[4], ncta=info[5])
 
 
 NOALLOC_MAX_NR = 2048          # MAESTRO_MAC_NOALLOC_MAX_NR
