@@ -433,14 +433,18 @@ k_prolong_add(LevelDev F, LevelDev C, int prolongation)
 // written as four 16-byte x pairs, so a warp moves 512 contiguous bytes per row.  Interpolation is
 // done axis by axis in the order x, y, z, i.e. the expression tree of k_prolong_add.
 __global__ void __launch_bounds__(256, 4)
-k_prolong_add2(LevelDev F, LevelDev C, int prolongation)
+k_prolong_add2(LevelDev F, LevelDev C, int prolongation, double* fout)
 {
     const int I = blockIdx.x * blockDim.x + threadIdx.x;
     const int J = blockIdx.y * blockDim.y + threadIdx.y;
     const int K = blockIdx.z;
     if (I >= C.nx || J >= C.ny) return;
     // the eight children, requested first: their HBM latency overlaps the (cache-resident) coarse reads below
-    double2* const fp = reinterpret_cast<double2*>(F.phi + cidx(F, 2 * I, 2 * J, 2 * K));
+    // fout: the array that receives phi + P e (same layout as F.phi; F.phi itself for the in-place form).  Out of place
+    // (the level's ping-pong partner) the pass is two plain streams instead of a read-modify-write of the same lines.
+    const size_t fo = cidx(F, 2 * I, 2 * J, 2 * K);
+    const double2* const fp = reinterpret_cast<const double2*>(F.phi + fo);
+    double2* const fq = reinterpret_cast<double2*>(fout + fo);
     const long long frow = F.cx / 2, fpl = (long long)F.cx * F.ry / 2;      // strides in double2 (cx is even here)
     double2 fv[2][2];
 #pragma unroll
@@ -498,7 +502,7 @@ k_prolong_add2(LevelDev F, LevelDev C, int prolongation)
     for (int dk = 0; dk < 2; ++dk)
 #pragma unroll
         for (int dj = 0; dj < 2; ++dj) {
-            double2* p = fp + dk * fpl + dj * frow;
+            double2* p = fq + dk * fpl + dj * frow;
             double2 v = fv[dk][dj];
             v.x += out[dk][dj][0];
             v.y += out[dk][dj][1];

@@ -587,8 +587,14 @@ int do_prolong(maestro_mac_handle* H, int l, cudaStream_t s)
     if (H->d.smoother != 1 && (F.nx & 1) == 0) {             // bandwidth form: one thread per coarse cell
         LevelDev C = dev_level(H, l + 1);
         dims3(C.nx, C.ny, C.nz, &g, &b);
-        k_prolong_add2<<<g, b, 0, s>>>(F, C, H->d.prolongation);
+#ifdef MAC_PROLONG_INPLACE
+        k_prolong_add2<<<g, b, 0, s>>>(F, C, H->d.prolongation, F.phi);
         LAUNCHED(H);
+#else
+        k_prolong_add2<<<g, b, 0, s>>>(F, C, H->d.prolongation, F.phi2);      // phi + P e into the ping-pong partner, then swap
+        LAUNCHED(H);
+        { double* t = H->lev[l].phi; H->lev[l].phi = H->lev[l].phi2; H->lev[l].phi2 = t; }
+#endif
         return MAESTRO_MAC_OK;
     }
     dims3(F.nx, F.ny, F.nz, &g, &b);
